@@ -366,24 +366,26 @@ def make_config(k, seed=0, scale=1):
 
 
 def dense_state(kind, cells, seed=1, max_angle=0.05, jitter=0.02, spacing=None):
-    """P2: dense near-aligned lattices in which ~1/3 of the pairs interact through many terms."""
+    """P2: dense near-aligned lattices in which many pairs interact through many terms.  Default
+    spacings were chosen (with the oracle, offline) so that U/N is a few epsilon: in contact, nothing overlapping.
+    `cells` must be large enough that every box edge is >= 2 r_cut (4 for the 3D kinds, 4 for the 2D kinds)."""
     if kind == "squares":
-        return lattice_state(2, [square(1.0, 0.15)], (cells, cells), spacing or 1.30, seed=seed, jitter=jitter,
+        return lattice_state(2, [square(1.0, 0.15)], (cells, cells), spacing or 1.34, seed=seed, jitter=jitter,
                              orient="small", max_angle=max_angle, name="dense_squares")
     if kind == "pentagons":
-        return lattice_state(2, [regular_polygon(5, 0.5, 0.05)], (cells, cells), spacing or 0.96, seed=seed,
+        return lattice_state(2, [regular_polygon(5, 0.5, 0.05)], (cells, cells), spacing or 1.055, seed=seed,
                              jitter=jitter / 2, orient="small", max_angle=max_angle, triangular=False,
                              name="dense_pentagons")
     if kind == "cubes":
-        return lattice_state(3, [cube(1.0, 0.15)], (cells,) * 3, spacing or 1.30, seed=seed, jitter=jitter,
+        return lattice_state(3, [cube(1.0, 0.15)], (cells,) * 3, spacing or 1.34, seed=seed, jitter=jitter,
                              orient="small", max_angle=max_angle, name="dense_cubes")
     if kind == "octahedra":
         # aligned octahedra (R = 0.5) touch vertex to vertex along the axes at spacing 1.0 + r*
-        return lattice_state(3, [octahedron(0.5, 0.075)], (cells,) * 3, spacing or 1.14, seed=seed, jitter=jitter,
+        return lattice_state(3, [octahedron(0.5, 0.075)], (cells,) * 3, spacing or 1.18, seed=seed, jitter=jitter,
                              orient="small", max_angle=max_angle, name="dense_octahedra")
     if kind == "mixed":
         return lattice_state(3, [truncated_icosahedron(0.5, 0.05), tetrahedron(0.5, 0.05)], (cells,) * 3,
-                             spacing or 1.06, seed=seed, jitter=jitter / 2, orient="random",
+                             spacing or 1.08, seed=seed, jitter=jitter / 2, orient="random",
                              shape_fractions=(0.5, 0.5), name="dense_mixed")
     raise ValueError(kind)
 

@@ -150,12 +150,24 @@ def neighbors(state, r_cut=None, subset=None, stride=64):
         stride = mx
 
 
+def _check_min_image(state, tab):
+    """The all-pairs minimum-image sum equals the periodic sum only if no interaction reaches beyond half a box
+    edge (reading R9): reach = max (R_i + R_j + 2^(1/6) (rho_i + rho_j))."""
+    rad = [np.sqrt((np.asarray(s["verts"]) ** 2).sum(1).max()) for s in tab.shapes]
+    reach = max(a + b + 2 ** (1 / 6) * (sa["rounding"] + sb["rounding"])
+                for a, sa in zip(rad, tab.shapes) for b, sb in zip(rad, tab.shapes))
+    box = np.asarray(state["box"], dtype=np.float64)
+    if np.any(box[:state["dim"]] < 2 * reach):
+        raise ValueError("box edge %s < 2 x interaction reach %g: minimum image invalid" % (box, reach))
+
+
 def compute(state, subset=None, use_reject=True, eps_par=DEFAULT_EPS_PAR, pos=None, quat=None):
     """Per-particle force+energy (rows,4), torque (rows,4), virial (rows,6), counters(5) by the definition."""
     tab = state.get("_tab") or ShapeTable(state["shapes"])
     pos = _f64(state["pos"] if pos is None else pos)
     quat = _f64(state["quat"] if quat is None else quat)
     n = len(pos)
+    _check_min_image(state, tab)
     sub = None if subset is None else np.ascontiguousarray(subset, dtype=np.int32)
     rows = n if sub is None else len(sub)
     f, t, w = np.zeros((rows, 4)), np.zeros((rows, 4)), np.zeros((rows, 6))
