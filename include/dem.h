@@ -1,0 +1,180 @@
+/*
+ * dem.h -- C ABI of libdem_b200: the DEM conservative force / torque / energy / virial evaluation between rounded
+ * polytopes of arXiv:1607.02427, hand-written CUDA for sm_100a (one GPU).
+ *
+ * What the library computes (citations are PAPER.md lines):
+ *   Eq. 1  3D:  U_ij = sum_{E_i,E_j} U(r*_EE) + sum_{V_i,F_j} U(r*_VF) + sum_{V_j,F_i} U(r*_VF)
+ *   Eq. 2  2D:  U_ij = sum_{V_i,E_j} U(r*_VE) + sum_{V_j,E_i} U(r*_VE)
+ *   r* = distance between the nearest points of two features; U = WCA (Eq. 3-4)
+ *   with sigma_ij = rho_i + rho_j (rounding radius = sigma/2) and r_cut^WCA = 2^(1/6) sigma_ij;
+ *   force along the line between the nearest points, torque from the interaction point on each particle
+ *   (PAPER.md:45); near-parallel edges interact at the midpoint of their overlap;
+ *   per-particle totals = sum over neighbours; virial tensor for "the barostat ... just as in MD"
+ *   (PAPER.md:115); second-order NVE integrator.
+ * Readings of passages on which the paper is silent or ambiguous are DESIGN.md "Readings" R1..R13.
+ *
+ * Conventions
+ *   - Every function returns DEM_OK (0) or a negative dem_status.  No exception crosses the ABI.
+ *     dem_last_error(ctx) returns a NUL-terminated description of the last failure on that context (owned by ctx).
+ *   - `real` is float for a context created with DEM_F32 and double for DEM_F64 (one precision per context).
+ *     Particle arrays are passed as `void*`/`const void*` and are interpreted as real[N][4] (16-byte aligned for
+ *     float, 32-byte aligned for double), row-major, unless a parameter comment says otherwise.
+ *   - Parameters documented "DEVICE" are device pointers owned by the caller (e.g. torch tensors); the library
+ *     never frees or retains them beyond the call.  Parameters documented "HOST" are host pointers, read or written
+ *     during the call only.  The library owns only what hangs off the opaque context.
+ *   - All device work is enqueued on the cudaStream_t given to dem_create (NULL = legacy default stream).  Calls that
+ *     return host scalars or need a capacity check synchronise that stream (each function says so).
+ *   - Positions: x,y,z,(unused).  Box: orthorhombic, edge lengths box[3], centred on the origin, periodic in the
+ *     first `dim` axes (2D ignores box[2] and z).  Positions outside the box are legal: every separation goes through
+ *     the minimum image  d_a -= L_a * rint(d_a / L_a).
+ *   - Quaternions: w,x,y,z, unit, scalar first, body -> lab (v_lab = q v q*); 2D: (cos t/2, 0, 0, sin t/2).
+ *   - Angular momentum: LAB frame, Lx,Ly,Lz,(unused); 2D uses only Lz.
+ *   - There is no CPU fallback: every entry point that computes needs a CUDA device and fails with DEM_ECUDA without.
+ */
+#ifndef DEM_B200_H
+#define DEM_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dem_ctx dem_ctx; /* opaque */
+
+typedef enum dem_status {
+    DEM_OK = 0,
+    DEM_EINVAL = -1,    /* bad argument / malformed shape                                                        */
+    DEM_ENOMEM = -2,    /* host or device allocation failed                                                      */
+    DEM_ECUDA = -3,     /* CUDA runtime error (text in dem_last_error)                                           */
+    DEM_EBOX = -4,      /* a periodic box edge < 2 r_cut: the minimum image would be invalid                      */
+    DEM_ERCUT = -5,     /* r_cut < max_ij (R_i + R_j + 2^(1/6) sigma_ij): interactions would be dropped silently  */
+    DEM_EOVERFLOW = -6, /* neighbour capacity exceeded and could not be regrown                                  */
+    DEM_ESTALE = -7     /* dem_compute called with N different from the last dem_build_neighbors                  */
+} dem_status;
+
+enum { DEM_F32 = 0, DEM_F64 = 1 };
+
+/* Create a context.  dim = 2 or 3; epsilon = the single WCA energy scale (Eq. 3); precision = DEM_F32 | DEM_F64;
+ * cuda_stream = a cudaStream_t (as void*), NULL for the default stream.  Does not touch the GPU beyond
+ * cudaGetDevice.  *out is owned by the caller and released with dem_destroy (which frees everything the library
+ * allocated on host and device). */
+int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda_stream);
+int dem_destroy(dem_ctx* ctx);
+const char* dem_last_error(const dem_ctx* ctx);
+
+/* Near-parallel edge threshold of PAPER.md:59 (reading R5): edges are "sufficiently close to parallel" iff
+ * |d1 x d2|^2 < eps_par |d1|^2 |d2|^2.  Default 1e-6. */
+int dem_set_eps_par(dem_ctx* ctx, double eps_par);
+
+/*
+ * Register a shape (inner polygon/polyhedron given by vertices V, edges E, faces F, rounded by a
+ * disk/sphere of radius `rounding_radius` = sigma/2).  All pointers HOST; copied.
+ *   verts          [nv][3] doubles, body frame, centre of mass at the origin, principal axes (z = 0 in 2D); nv >= 1
+ *   face_offsets   [nf+1] CSR offsets into face_verts; face_verts = vertex indices of each planar convex polygon face
+ *                  in boundary order (either orientation: faces are two-sided).  2D: NULL, NULL, 0.
+ *   edges          [ne][2] vertex index pairs, or NULL (then ne is ignored) to derive them: 2D = the closed CCW
+ *                  polygon, edge k = (k, (k+1) mod nv), a single edge for nv = 2, the degenerate edge
+ *                  (0,0) for nv = 1; 3D = the unique undirected boundary edges of the faces.
+ *                  Explicit edges allow the degenerate shapes used as pins: sphere = 1 vertex + edge (0,0), no face
+ *                  (Eq. 1 then reduces to one central WCA); rod = 2 vertices + edge (0,1).
+ *   mass, inertia  mass and the three principal moments (2D uses inertia[2]); only dem_step / dem_energy use them.
+ *   *shape_id      receives the id (0, 1, ...) to be used in the shape_id arrays.
+ * Errors: DEM_EINVAL for indices out of range, faces with < 3 vertices, non-planar or non-convex faces, nv < 1,
+ * rounding_radius <= 0, more than DEM_MAX_SHAPES shapes.  Invalidates the current neighbour list.
+ */
+#define DEM_MAX_SHAPES 8
+int dem_create_shape(dem_ctx* ctx, const double* verts, int nv, const int* face_offsets, const int* face_verts,
+                     int nf, const int* edges, int ne, double rounding_radius, double mass,
+                     const double inertia[3], int* shape_id);
+
+/*
+ * Build the cell list and the full (two-sided) neighbour list ("it and its neighbors"; reading R13):
+ * j is a neighbour of i  <=>  j != i and the minimum-image |x_j - x_i|^2 < r_cut^2 (strict), evaluated in double on
+ * the stored coordinate values with exactly the operation order of DESIGN.md R13, so that the list is bit-identical
+ * to the all-pairs definition.  Also builds the library's internal unique-pair work list for dem_compute.
+ *   pos       DEVICE real[N][4]      shape_id  DEVICE int32[N]      box  HOST double[3]
+ * Does not modify caller data.  Synchronises the stream (capacity check; the list is regrown and rebuilt
+ * transparently on overflow).  Errors: DEM_EBOX, DEM_ERCUT, DEM_EINVAL (N < 1, no shapes), DEM_ECUDA, DEM_ENOMEM.
+ */
+int dem_build_neighbors(dem_ctx* ctx, const void* pos, const int32_t* shape_id, int N, const double box[3],
+                        double r_cut);
+
+/* Device pointers (owned by ctx, valid until the next build or dem_destroy) to the list of the last build:
+ * counts[i] = number of neighbours of i, row i = list[i*stride .. i*stride + counts[i]), rows in no particular
+ * order.  *max_count (may be NULL) receives the largest count. */
+int dem_get_neighbors(dem_ctx* ctx, const int32_t** counts, const int32_t** list, int* stride, int* max_count);
+
+/* Copy the list of the last build into caller-owned DEVICE arrays: counts_out int32[N], list_out int32[N][out_stride]
+ * (out_stride >= max_count; unused entries are set to -1).  Asynchronous on the context's stream. */
+int dem_copy_neighbors(dem_ctx* ctx, int32_t* counts_out, int32_t* list_out, int out_stride);
+
+/*
+ * Evaluate Eq. 1 / Eq. 2 over the current neighbour list (steps a3-a8 of DESIGN.md).  All pointers DEVICE.
+ *   pos, quat     real[N][4]        shape_id  int32[N]
+ *   force_energy  real[N][4]  = Fx, Fy, Fz, U_i      with U_i = 1/2 sum_j U_ij
+ *   torque        real[N][4]  = lab-frame torque, 0  (2D: only .z is non-zero)
+ *   virial6       real[N][6]  = 1/2 sum_j W_ij, W^{ab} = r_ij^a F_ij^b, r_ij = x_i - x_j (xx,xy,xz,yy,yz,zz); may be NULL
+ * Outputs are fully overwritten.  Asynchronous (no synchronisation).  The positions may have moved since the build
+ * as long as no pair that can interact is missing from the list (dem_step takes care of that with a skin).
+ * Features closer than 1e-6 sigma are outside the model (WCA diverges): the term is skipped and counted (R11).
+ * Errors: DEM_ESTALE, DEM_EINVAL, DEM_ECUDA.
+ */
+int dem_compute(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* shape_id, int N, void* force_energy,
+                void* torque, void* virial6);
+
+/* Counters of the last dem_compute (synchronises): out[0] unique particle pairs evaluated, out[1] Eq. 1/2 terms
+ * evaluated (polygon faces, each unique pair once), out[2] terms inside the WCA cutoff, out[3] degenerate terms
+ * skipped, out[4] terms that took the parallel-edge branch, out[5] unique pairs in the work list. HOST int64[6]. */
+int dem_get_counters(dem_ctx* ctx, int64_t out[6]);
+
+/*
+ * nsteps of velocity-Verlet NVE with quaternion rotation (reading R15): half-kick v and L; drift x
+ * (wrapped back into the centred box); free rotation of q (exact for spherical tops and in 2D, symmetric splitting
+ * otherwise); force evaluation; half-kick.  pos, quat, vel, angmom: DEVICE real[N][4], updated in place;
+ * shape_id DEVICE int32[N]; box HOST double[3].  The neighbour list is (re)built with r_cut = reach + skin, reach =
+ * max_ij (R_i + R_j + 2^(1/6) sigma_ij), and rebuilt whenever some particle has moved more than skin/2 since the last
+ * build.  A DEM_F32 context integrates its state in double internally (R15b) and rounds it to float on return.
+ * force_energy / torque (DEVICE real[N][4], may be NULL) receive the forces of the final state.
+ * Synchronises before returning.
+ */
+int dem_step(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const int32_t* shape_id, int N,
+             const double box[3], double dt, int nsteps, double skin, void* force_energy, void* torque);
+
+/* U = sum_i U_i (from force_energy[.][3]), K_trans, K_rot of a state; DEVICE inputs, HOST out[3]; synchronises. */
+int dem_energy(dem_ctx* ctx, const void* quat, const void* vel, const void* angmom, const int32_t* shape_id,
+               const void* force_energy, int N, double out[3]);
+
+/*
+ * Host-buffer forms (the end-to-end path): same semantics, every particle array is a HOST pointer (pinned memory
+ * gives the best copy rate); the library copies inputs to device scratch it owns, runs dem_build_neighbors +
+ * dem_compute (or dem_step), copies the results back and synchronises.
+ */
+int dem_compute_host(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* shape_id, int N,
+                     const double box[3], double r_cut, void* force_energy, void* torque, void* virial6);
+int dem_step_host(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const int32_t* shape_id, int N,
+                  const double box[3], double dt, int nsteps, double skin, void* force_energy, void* torque);
+
+/* Tuning / test hook: number of lanes that share one particle pair in the pair-feature kernel (each takes a slice of
+ * the pair's outer feature loop; their partial results are summed by the reduction).  0 = heuristic (default: enough
+ * lanes to fill the GPU when there are few pairs).  Takes effect at the next neighbour build. */
+int dem_set_slices(dem_ctx* ctx, int slices);
+
+/* Kernel-time accounting for bench.py: when enabled, every launch of the pair-feature kernel is bracketed by CUDA
+ * events on the context's stream; dem_kernel_time returns (and resets) the number of bracketed launches and their
+ * summed duration in milliseconds (synchronises). */
+int dem_set_timing(dem_ctx* ctx, int enabled);
+int dem_kernel_time(dem_ctx* ctx, int64_t* launches, double* total_ms);
+/* Number of kernels the library has launched on this context since creation (all kernels). */
+int64_t dem_launch_count(const dem_ctx* ctx);
+
+/* FP32 FMA-chain microbenchmark (roofline denominator): runs `iters` dependent-chain FFMA iterations on
+ * every SM and returns the achieved FP32 TFLOP/s (2 flop per FMA); synchronises. */
+int dem_fp32_peak(dem_ctx* ctx, int iters, double* tflops);
+
+const char* dem_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DEM_B200_H */

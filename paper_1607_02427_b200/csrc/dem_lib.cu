@@ -1,0 +1,732 @@
+// dem_lib.cu -- C ABI (include/dem.h) and host orchestration of libdem_b200.  Kernels: dem_kernels.cuh.
+// There is no CPU path: every computing entry point launches CUDA kernels and fails with DEM_ECUDA without a device.
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/dem.h"
+#include "dem_kernels.cuh"
+#include "dem_shape.h"
+
+using namespace dem;
+
+namespace {
+
+struct DevBuf {  // grow-only device buffer
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t reserve(size_t bytes) {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+        size_t want = bytes + bytes / 8 + 256;
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e == cudaSuccess) cap = want;
+        return e;
+    }
+    void release() {
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+    }
+    template <typename T> T* as() const { return static_cast<T*>(p); }
+};
+
+}  // namespace
+
+struct dem_ctx {
+    int dim = 3, prec = DEM_F32;
+    double eps = 1.0, eps_par = 1e-6;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    std::vector<HostShape> shapes;
+    bool table_dirty = true;
+    std::vector<ShapeDev> shape_dev;
+    DevBuf table;
+    MassTable mt;
+    // neighbour list state
+    bool have_list = false;
+    int N = 0, stride = 16, max_count = 0;
+    double box[3] = {0, 0, 0}, r_cut = 0;
+    GridDev grid;
+    DevBuf cell_of, rank, cell_start, order, xs, counts, list, slot, scratch_scan, pcnt, pairs, rec, flags, counters;
+    ClassTable ct;
+    int nclass = 0;
+    int class_sa[DEM_MAX_CLASSES], class_sb[DEM_MAX_CLASSES], class_np[DEM_MAX_CLASSES];
+    long long npairs_total = 0, nrec_total = 0;
+    int force_slices = 0;  // 0 = heuristic
+    // dem_step state (double) for DEM_F32 contexts, plus forces and the positions of the last build
+    DevBuf st_pos, st_quat, st_vel, st_ang, st_force, st_torque, pos_build, epart;
+    // host-buffer entry points
+    DevBuf h_pos, h_quat, h_vel, h_ang, h_sid, h_force, h_torque, h_virial;
+    // accounting
+    int64_t launches = 0;
+    bool timing = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pool;
+    size_t ev_used = 0;
+    int64_t last_terms = 0;
+    int sm_count = 148;
+};
+
+namespace {
+
+int fail(dem_ctx* c, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (c) c->err = buf;
+    return code;
+}
+
+#define CU(call)                                                                                        \
+    do {                                                                                                \
+        cudaError_t e_ = (call);                                                                        \
+        if (e_ != cudaSuccess)                                                                          \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? DEM_ENOMEM : DEM_ECUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                                        \
+    } while (0)
+#define CHECK(call)             \
+    do {                        \
+        int rc_ = (call);       \
+        if (rc_ != DEM_OK) return rc_; \
+    } while (0)
+#define LAUNCHED(ctx) ((ctx)->launches++)
+
+inline int nblk(long long n, int b) { return (int)((n + b - 1) / b); }
+
+// in-place exclusive scan of data[0..n); data must have room for n entries; uses ctx->scratch_scan
+int scan_exclusive(dem_ctx* ctx, int* data, int n, int* scratch, size_t scratch_ints) {
+    const int nb = nblk(n, 1024);
+    if (nb == 1) {
+        k_scan_block<<<1, 1024, 0, ctx->stream>>>(data, n, nullptr);
+        LAUNCHED(ctx);
+        return DEM_OK;
+    }
+    if ((size_t)nb > scratch_ints) return fail(ctx, DEM_EINVAL, "scan scratch too small");
+    k_scan_block<<<nb, 1024, 0, ctx->stream>>>(data, n, scratch);
+    LAUNCHED(ctx);
+    CHECK(scan_exclusive(ctx, scratch, nb, scratch + ((nb + 3) & ~3), scratch_ints - ((nb + 3) & ~3)));
+    k_scan_add<<<nb, 1024, 0, ctx->stream>>>(data, n, scratch);
+    LAUNCHED(ctx);
+    return DEM_OK;
+}
+
+template <typename real> int upload_table(dem_ctx* ctx) {
+    typedef typename vec4<real>::type real4;
+    std::vector<real4> host;
+    ctx->shape_dev.clear();
+    for (auto& S : ctx->shapes) {
+        ShapeDev d;
+        d.nv = S.nv; d.ne = S.ne; d.nf = S.nf; d.nfe = S.nfe;
+        d.off = (int)host.size();
+        d.len = S.table_len4();
+        for (int k = 0; k < d.len; ++k) {
+            real4 v;
+            v.x = (real)S.table[4 * k]; v.y = (real)S.table[4 * k + 1];
+            v.z = (real)S.table[4 * k + 2]; v.w = (real)S.table[4 * k + 3];
+            host.push_back(v);
+        }
+        ctx->shape_dev.push_back(d);
+    }
+    CU(ctx->table.reserve(host.size() * sizeof(real4)));
+    CU(cudaMemcpyAsync(ctx->table.p, host.data(), host.size() * sizeof(real4), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));  // `host` goes out of scope
+    return DEM_OK;
+}
+
+int sync_tables(dem_ctx* ctx) {
+    if (!ctx->table_dirty) return DEM_OK;
+    if (ctx->shapes.empty()) return fail(ctx, DEM_EINVAL, "no shapes registered");
+    CHECK(ctx->prec == DEM_F64 ? upload_table<double>(ctx) : upload_table<float>(ctx));
+    const int ns = (int)ctx->shapes.size();
+    int c = 0;
+    memset(&ctx->ct, 0, sizeof ctx->ct);
+    for (int a = 0; a < ns; ++a)
+        for (int b = a; b < ns; ++b) {
+            ctx->ct.lut[a][b] = ctx->ct.lut[b][a] = (signed char)c;
+            ctx->class_sa[c] = a;
+            ctx->class_sb[c] = b;
+            ++c;
+        }
+    ctx->nclass = c;
+    for (int s = 0; s < ns; ++s) {
+        ctx->mt.mass[s] = ctx->shapes[s].mass;
+        for (int a = 0; a < 3; ++a) ctx->mt.inertia[s][a] = ctx->shapes[s].inertia[a];
+    }
+    cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, 0);
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    ctx->table_dirty = false;
+    return DEM_OK;
+}
+
+double reach_of(const HostShape& a, const HostShape& b) {
+    return a.circumradius + b.circumradius + std::pow(2.0, 1.0 / 6.0) * (a.rounding + b.rounding);
+}
+double max_reach(const dem_ctx* ctx) {
+    double r = 0;
+    for (auto& a : ctx->shapes)
+        for (auto& b : ctx->shapes) r = std::max(r, reach_of(a, b));
+    return r;
+}
+
+// nominal Eq. 1 / Eq. 2 terms of one pair of the class, and the outer-loop length the pair kernel slices
+long long class_terms(const dem_ctx* ctx, int c) {
+    const HostShape &A = ctx->shapes[ctx->class_sa[c]], &B = ctx->shapes[ctx->class_sb[c]];
+    if (ctx->dim == 3) return (long long)A.ne * B.ne + (long long)A.nv * B.nf + (long long)B.nv * A.nf;
+    return (long long)A.nv * B.ne + (long long)B.nv * A.ne;
+}
+int class_outer(const dem_ctx* ctx, int c) {
+    const HostShape &A = ctx->shapes[ctx->class_sa[c]], &B = ctx->shapes[ctx->class_sb[c]];
+    return ctx->dim == 3 ? B.ne + B.nv + A.nv : B.nv + A.nv;
+}
+
+// ---- neighbour build ----------------------------------------------------------------------------------------------
+template <typename PosT>
+int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, const double box[3], double r_cut,
+                      bool check_rcut) {
+    if (N < 1) return fail(ctx, DEM_EINVAL, "N must be >= 1");
+    if (!pos || !sid) return fail(ctx, DEM_EINVAL, "null particle array");
+    if (!(r_cut > 0)) return fail(ctx, DEM_EINVAL, "r_cut must be positive");
+    CHECK(sync_tables(ctx));
+    for (int a = 0; a < ctx->dim; ++a)
+        if (!(box[a] >= 2.0 * r_cut))
+            return fail(ctx, DEM_EBOX, "box edge %d = %g < 2 r_cut = %g: minimum image invalid", a, box[a], 2 * r_cut);
+    if (check_rcut && r_cut < max_reach(ctx) * (1.0 - 1e-12))
+        return fail(ctx, DEM_ERCUT, "r_cut = %.17g < interaction reach %.17g", r_cut, max_reach(ctx));
+    cudaStream_t st = ctx->stream;
+    ctx->have_list = false;
+    ctx->N = N;
+    for (int a = 0; a < 3; ++a) ctx->box[a] = box[a];
+    ctx->r_cut = r_cut;
+    BoxDev bx;
+    bx.dim = ctx->dim;
+    for (int a = 0; a < 3; ++a) bx.L[a] = box[a];
+    if (ctx->dim == 2) bx.L[2] = 1.0;
+    // cells at least r_cut wide (with a relative margin far above double rounding), at most ~2 N + 64 cells in all
+    GridDev g;
+    g.nc[0] = g.nc[1] = g.nc[2] = 1;
+    for (int a = 0; a < ctx->dim; ++a) g.nc[a] = std::max(1, (int)std::floor(box[a] / (r_cut * (1.0 + 1e-9))));
+    while ((double)g.nc[0] * g.nc[1] * g.nc[2] > 2.0 * N + 64.0) {
+        int amax = 0;
+        for (int a = 1; a < ctx->dim; ++a)
+            if (g.nc[a] > g.nc[amax]) amax = a;
+        if (g.nc[amax] <= 3) break;
+        g.nc[amax] = std::max(3, (int)(g.nc[amax] * 0.8));
+    }
+    g.ncell = g.nc[0] * g.nc[1] * g.nc[2];
+    ctx->grid = g;
+    const size_t scan_ints = 4096 + (size_t)std::max<long long>(g.ncell, (long long)ctx->nclass * N) / 512;
+    CU(ctx->cell_of.reserve(sizeof(int) * (size_t)N));
+    CU(ctx->rank.reserve(sizeof(int) * (size_t)N));
+    CU(ctx->order.reserve(sizeof(int) * (size_t)N));
+    CU(ctx->cell_start.reserve(sizeof(int) * ((size_t)g.ncell + 1)));
+    CU(ctx->xs.reserve(sizeof(d4) * (size_t)N));
+    CU(ctx->counts.reserve(sizeof(int) * (size_t)N));
+    CU(ctx->scratch_scan.reserve(sizeof(int) * scan_ints));
+    CU(ctx->flags.reserve(sizeof(int) * 16));
+    CU(ctx->counters.reserve(sizeof(unsigned long long) * 8));
+    CU(ctx->pos_build.reserve(sizeof(d4) * (size_t)N));
+    int* cell_start = ctx->cell_start.as<int>();
+    CU(cudaMemsetAsync(cell_start, 0, sizeof(int) * ((size_t)g.ncell + 1), st));
+    const int B = 256;
+    k_bin<PosT><<<nblk(N, B), B, 0, st>>>(pos, N, bx, g, ctx->cell_of.as<int>(), cell_start, ctx->rank.as<int>());
+    LAUNCHED(ctx);
+    CHECK(scan_exclusive(ctx, cell_start, g.ncell + 1, ctx->scratch_scan.as<int>(), scan_ints));
+    k_place<<<nblk(N, B), B, 0, st>>>(N, ctx->cell_of.as<int>(), ctx->rank.as<int>(), cell_start, ctx->order.as<int>());
+    LAUNCHED(ctx);
+    k_sort_cells<<<nblk(g.ncell, B), B, 0, st>>>(g.ncell, cell_start, ctx->order.as<int>());
+    LAUNCHED(ctx);
+    k_gather_sorted<PosT><<<nblk(N, B), B, 0, st>>>(pos, N, ctx->order.as<int>(), ctx->xs.as<d4>());
+    LAUNCHED(ctx);
+    // positions of this build, in original order, for dem_step's displacement test
+    if (sizeof(PosT) == sizeof(double)) {
+        CU(cudaMemcpyAsync(ctx->pos_build.p, pos, sizeof(d4) * (size_t)N, cudaMemcpyDeviceToDevice, st));
+    } else {
+        k_f4_to_d4<<<nblk(N, B), B, 0, st>>>(N, reinterpret_cast<const f4*>(pos), ctx->pos_build.as<d4>());
+        LAUNCHED(ctx);
+    }
+    int* flags = ctx->flags.as<int>();
+    for (int attempt = 0; attempt < 8; ++attempt) {
+        CU(ctx->list.reserve(sizeof(int) * (size_t)N * ctx->stride));
+        CU(ctx->slot.reserve(sizeof(int) * (size_t)N * ctx->stride));
+        CU(cudaMemsetAsync(flags, 0, sizeof(int) * 16, st));
+        k_neigh<<<nblk(N, 128), 128, 0, st>>>(N, bx, g, r_cut * r_cut, ctx->order.as<int>(), ctx->cell_of.as<int>(),
+                                              cell_start, ctx->xs.as<d4>(), ctx->stride, ctx->counts.as<int>(),
+                                              ctx->list.as<int>(), flags);
+        LAUNCHED(ctx);
+        int mc = 0;
+        CU(cudaMemcpyAsync(&mc, flags, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        ctx->max_count = mc;
+        if (mc <= ctx->stride) break;
+        if (attempt == 7) return fail(ctx, DEM_EOVERFLOW, "neighbour capacity could not be regrown (max count %d)", mc);
+        ctx->stride = (mc + 7) & ~7;
+    }
+    // unique-pair work list, class-major
+    const int nc = ctx->nclass;
+    CU(ctx->pcnt.reserve(sizeof(int) * ((size_t)nc * N + 1)));
+    int* pcnt = ctx->pcnt.as<int>();
+    CU(cudaMemsetAsync(pcnt + (size_t)nc * N, 0, sizeof(int), st));
+    k_pair_count<<<nblk(N, B), B, 0, st>>>(N, ctx->counts.as<int>(), ctx->list.as<int>(), ctx->stride, sid, ctx->ct, nc, pcnt);
+    LAUNCHED(ctx);
+    CHECK(scan_exclusive(ctx, pcnt, nc * N + 1, ctx->scratch_scan.as<int>(), scan_ints));
+    int bases[DEM_MAX_CLASSES + 1];
+    for (int c = 0; c <= nc; ++c)
+        CU(cudaMemcpyAsync(&bases[c], pcnt + (size_t)c * N, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    ctx->npairs_total = bases[nc];
+    long long nrec = 0, terms = 0;
+    for (int c = 0; c < nc; ++c) {
+        ctx->class_np[c] = bases[c + 1] - bases[c];
+        ctx->ct.pair_base[c] = bases[c];
+        // slices: split a pair's outer feature loop over several lanes when there are too few pairs to fill the GPU
+        int S = 1;
+        const int outer = class_outer(ctx, c);
+        if (ctx->force_slices > 0) {
+            S = std::min(ctx->force_slices, std::max(outer, 1));
+        } else if (ctx->class_np[c] > 0) {
+            const long long want_lanes = (long long)ctx->sm_count * 2048;  // one full wave of resident threads
+            const long long per_slice_min_terms = 64;                      // keep the per-lane setup amortised
+            long long s = want_lanes / std::max(1, ctx->class_np[c]);
+            s = std::min<long long>(s, class_terms(ctx, c) / per_slice_min_terms);
+            s = std::min<long long>(s, outer);
+            S = (int)std::max<long long>(1, s);
+        }
+        ctx->ct.slices[c] = S;
+        ctx->ct.rec_base[c] = (int)nrec;
+        nrec += (long long)ctx->class_np[c] * S;
+        terms += (long long)ctx->class_np[c] * class_terms(ctx, c);
+    }
+    ctx->ct.pair_base[nc] = bases[nc];
+    ctx->ct.rec_base[nc] = (int)nrec;
+    ctx->nrec_total = nrec;
+    ctx->last_terms = terms;
+    if (nrec * 4 > 0x7fffffffLL) return fail(ctx, DEM_EOVERFLOW, "too many pair records");
+    CU(ctx->pairs.reserve(sizeof(int2) * (size_t)std::max<long long>(ctx->npairs_total, 1)));
+    CU(ctx->rec.reserve((ctx->prec == DEM_F64 ? sizeof(d4) : sizeof(f4)) * 4 * (size_t)std::max<long long>(nrec, 1)));
+    k_pair_fill<<<nblk(N, B), B, 0, st>>>(N, ctx->counts.as<int>(), ctx->list.as<int>(), ctx->stride, sid, ctx->ct, nc,
+                                          pcnt, ctx->pairs.as<int2>(), ctx->slot.as<int>());
+    LAUNCHED(ctx);
+    k_slot_back<<<nblk(N, B), B, 0, st>>>(N, ctx->counts.as<int>(), ctx->list.as<int>(), ctx->stride, sid, ctx->ct, pcnt,
+                                          ctx->slot.as<int>());
+    LAUNCHED(ctx);
+    CU(cudaGetLastError());
+    ctx->have_list = true;
+    return DEM_OK;
+}
+
+// ---- force evaluation ---------------------------------------------------------------------------------------------
+template <typename real, typename PosT>
+int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* sid, int N, void* force, void* torque,
+              void* virial) {
+    typedef typename vec4<real>::type real4;
+    if (!ctx->have_list) return fail(ctx, DEM_ESTALE, "no neighbour list: call dem_build_neighbors first");
+    if (N != ctx->N) return fail(ctx, DEM_ESTALE, "N = %d differs from the last build (%d)", N, ctx->N);
+    if (!pos || !quat || !sid || !force || !torque) return fail(ctx, DEM_EINVAL, "null particle array");
+    cudaStream_t st = ctx->stream;
+    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8, st));
+    BoxDev bx;
+    bx.dim = ctx->dim;
+    for (int a = 0; a < 3; ++a) bx.L[a] = ctx->box[a];
+    if (ctx->dim == 2) bx.L[2] = 1.0;
+    for (int c = 0; c < ctx->nclass; ++c) {
+        const int np = ctx->class_np[c];
+        if (np == 0) continue;
+        const HostShape &HA = ctx->shapes[ctx->class_sa[c]], &HB = ctx->shapes[ctx->class_sb[c]];
+        PairArgs<real> a;
+        a.table = ctx->table.as<real4>();
+        a.sa = ctx->shape_dev[ctx->class_sa[c]];
+        a.sb = ctx->shape_dev[ctx->class_sb[c]];
+        a.pairs = ctx->pairs.as<int2>() + ctx->ct.pair_base[c];
+        a.npairs = np;
+        a.slices = ctx->ct.slices[c];
+        a.n_outer = class_outer(ctx, c);
+        a.rec = ctx->rec.as<real4>() + 4 * (size_t)ctx->ct.rec_base[c];
+        a.pos = pos;
+        a.quat = quat;
+        a.box = bx;
+        const double reach = reach_of(HA, HB), sigma = HA.rounding + HB.rounding;
+        a.reach2 = reach * reach;
+        a.pc.rc2 = (real)(std::cbrt(2.0) * sigma * sigma);
+        a.pc.sig2 = (real)(sigma * sigma);
+        a.pc.eps = (real)ctx->eps;
+        a.pc.eps_par = (real)ctx->eps_par;
+        a.pc.degen2 = (real)((1e-6 * sigma) * (1e-6 * sigma));
+        a.counters = ctx->counters.as<unsigned long long>();
+        const size_t smem = sizeof(real4) * (size_t)(a.sa.len + (a.sa.off == a.sb.off ? 0 : a.sb.len));
+        const long long items = (long long)((np + 31) & ~31) * a.slices;
+        const int threads = 128;
+        const int grid = (int)std::min<long long>(nblk(items, threads), (long long)ctx->sm_count * 64);
+        auto kern = ctx->dim == 3 ? k_pair<real, PosT, 3> : k_pair<real, PosT, 2>;
+        if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        if (ctx->timing) {
+            if (ctx->ev_used == ctx->ev_pool.size()) {
+                cudaEvent_t x, y;
+                CU(cudaEventCreate(&x));
+                CU(cudaEventCreate(&y));
+                ctx->ev_pool.push_back({x, y});
+            }
+            e0 = ctx->ev_pool[ctx->ev_used].first;
+            e1 = ctx->ev_pool[ctx->ev_used].second;
+            ctx->ev_used++;
+            CU(cudaEventRecord(e0, st));
+        }
+        kern<<<grid, threads, smem, st>>>(a);
+        LAUNCHED(ctx);
+        if (ctx->timing) CU(cudaEventRecord(e1, st));
+    }
+    k_reduce<real><<<nblk(4LL * N, 128), 128, 0, st>>>(N, ctx->counts.as<int>(), ctx->list.as<int>(), ctx->slot.as<int>(),
+                                                      ctx->stride, sid, ctx->ct, ctx->rec.as<real4>(),
+                                                      static_cast<real4*>(force), static_cast<real4*>(torque),
+                                                      static_cast<real*>(virial));
+    LAUNCHED(ctx);
+    CU(cudaGetLastError());
+    return DEM_OK;
+}
+
+template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* vel, void* ang, const int32_t* sid,
+                                    int N, const double box[3], double dt, int nsteps, double skin, void* force_out,
+                                    void* torque_out) {
+    typedef typename vec4<real>::type real4;
+    if (N < 1 || !pos || !quat || !vel || !ang || !sid) return fail(ctx, DEM_EINVAL, "bad particle arrays");
+    if (nsteps < 0 || !(skin >= 0)) return fail(ctx, DEM_EINVAL, "bad nsteps / skin");
+    CHECK(sync_tables(ctx));
+    cudaStream_t st = ctx->stream;
+    const int B = 256;
+    const bool conv = ctx->prec == DEM_F32;
+    d4 *x, *q, *v, *L;
+    if (conv) {  // R15b: a DEM_F32 context integrates its state in double
+        CU(ctx->st_pos.reserve(sizeof(d4) * (size_t)N));
+        CU(ctx->st_quat.reserve(sizeof(d4) * (size_t)N));
+        CU(ctx->st_vel.reserve(sizeof(d4) * (size_t)N));
+        CU(ctx->st_ang.reserve(sizeof(d4) * (size_t)N));
+        x = ctx->st_pos.as<d4>(); q = ctx->st_quat.as<d4>(); v = ctx->st_vel.as<d4>(); L = ctx->st_ang.as<d4>();
+        const void* in[4] = {pos, quat, vel, ang};
+        d4* out[4] = {x, q, v, L};
+        for (int k = 0; k < 4; ++k) {
+            k_f4_to_d4<<<nblk(N, B), B, 0, st>>>(N, static_cast<const f4*>(in[k]), out[k]);
+            LAUNCHED(ctx);
+        }
+    } else {
+        x = static_cast<d4*>(pos); q = static_cast<d4*>(quat); v = static_cast<d4*>(vel); L = static_cast<d4*>(ang);
+    }
+    CU(ctx->st_force.reserve(sizeof(real4) * (size_t)N));
+    CU(ctx->st_torque.reserve(sizeof(real4) * (size_t)N));
+    real4* F = ctx->st_force.as<real4>();
+    real4* T = ctx->st_torque.as<real4>();
+    const double r_list = max_reach(ctx) + skin;
+    BoxDev bx;
+    bx.dim = ctx->dim;
+    for (int a = 0; a < 3; ++a) bx.L[a] = box[a];
+    if (ctx->dim == 2) bx.L[2] = 1.0;
+    CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
+    CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr)));
+    int* moved = ctx->flags.as<int>() + 8;
+    const double half_skin2 = 0.25 * skin * skin;
+    for (int s = 0; s < nsteps; ++s) {
+        CU(cudaMemsetAsync(moved, 0, sizeof(int), st));
+        k_kick_drift<real><<<nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T, ctx->pos_build.as<d4>(),
+                                                     half_skin2, moved);
+        LAUNCHED(ctx);
+        int m = 0;
+        CU(cudaMemcpyAsync(&m, moved, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        if (m) CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
+        CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr)));
+        k_kick<real><<<nblk(N, B), B, 0, st>>>(N, ctx->dim, dt, sid, ctx->mt, v, L, F, T);
+        LAUNCHED(ctx);
+    }
+    if (conv) {
+        void* out[4] = {pos, quat, vel, ang};
+        d4* in[4] = {x, q, v, L};
+        for (int k = 0; k < 4; ++k) {
+            k_d4_to_f4<<<nblk(N, B), B, 0, st>>>(N, in[k], static_cast<f4*>(out[k]));
+            LAUNCHED(ctx);
+        }
+    }
+    if (force_out) CU(cudaMemcpyAsync(force_out, F, sizeof(real4) * (size_t)N, cudaMemcpyDeviceToDevice, st));
+    if (torque_out) CU(cudaMemcpyAsync(torque_out, T, sizeof(real4) * (size_t)N, cudaMemcpyDeviceToDevice, st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    // the internal list was built from internal (double) positions; a later dem_compute on caller arrays is still valid
+    return DEM_OK;
+}
+
+template <typename real, typename PosT>
+int energy_t(dem_ctx* ctx, const PosT* quat, const PosT* vel, const PosT* ang, const int32_t* sid, const void* force,
+             int N, double out[3]) {
+    typedef typename vec4<real>::type real4;
+    CHECK(sync_tables(ctx));
+    const int nb = nblk(N, 256);
+    CU(ctx->epart.reserve(sizeof(double) * 3 * (size_t)nb));
+    k_energy<real, PosT><<<nb, 256, 0, ctx->stream>>>(N, ctx->dim, sid, ctx->mt, quat, vel, ang,
+                                                     static_cast<const real4*>(force), ctx->epart.as<double>());
+    LAUNCHED(ctx);
+    std::vector<double> h(3 * (size_t)nb);
+    CU(cudaMemcpyAsync(h.data(), ctx->epart.p, sizeof(double) * h.size(), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    out[0] = out[1] = out[2] = 0;
+    for (int b = 0; b < nb; ++b)
+        for (int a = 0; a < 3; ++a) out[a] += h[3 * (size_t)b + a];
+    return DEM_OK;
+}
+
+}  // namespace
+
+// =====================================================================================================================
+extern "C" {
+
+const char* dem_version(void) { return "dem_b200 0.1 (sm_100a)"; }
+
+int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda_stream) {
+    if (!out) return DEM_EINVAL;
+    *out = nullptr;
+    if ((dim != 2 && dim != 3) || !(epsilon > 0) || (precision != DEM_F32 && precision != DEM_F64)) return DEM_EINVAL;
+    dem_ctx* c = new (std::nothrow) dem_ctx;
+    if (!c) return DEM_ENOMEM;
+    c->dim = dim;
+    c->eps = epsilon;
+    c->prec = precision;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    memset(&c->ct, 0, sizeof c->ct);
+    memset(&c->mt, 0, sizeof c->mt);
+    *out = c;
+    return DEM_OK;
+}
+
+int dem_destroy(dem_ctx* c) {
+    if (!c) return DEM_EINVAL;
+    DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
+                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->st_pos, &c->st_quat,
+                      &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->pos_build, &c->epart, &c->h_pos,
+                      &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial};
+    for (DevBuf* b : bufs) b->release();
+    for (auto& e : c->ev_pool) {
+        cudaEventDestroy(e.first);
+        cudaEventDestroy(e.second);
+    }
+    delete c;
+    return DEM_OK;
+}
+
+const char* dem_last_error(const dem_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+int dem_set_eps_par(dem_ctx* ctx, double eps_par) {
+    if (!ctx || !(eps_par >= 0)) return fail(ctx, DEM_EINVAL, "eps_par must be >= 0");
+    ctx->eps_par = eps_par;
+    return DEM_OK;
+}
+
+// Tuning / test hook: lanes per pair (0 = heuristic).  Takes effect at the next neighbour build.
+int dem_set_slices(dem_ctx* ctx, int slices) {
+    if (!ctx || slices < 0) return fail(ctx, DEM_EINVAL, "slices must be >= 0");
+    ctx->force_slices = slices;
+    ctx->have_list = false;
+    return DEM_OK;
+}
+
+int dem_create_shape(dem_ctx* ctx, const double* verts, int nv, const int* face_offsets, const int* face_verts, int nf,
+                     const int* edges, int ne, double rounding_radius, double mass, const double inertia[3],
+                     int* shape_id) {
+    if (!ctx) return DEM_EINVAL;
+    if (!verts || !shape_id) return fail(ctx, DEM_EINVAL, "null argument");
+    if ((int)ctx->shapes.size() >= DEM_MAX_SHAPES) return fail(ctx, DEM_EINVAL, "more than %d shapes", DEM_MAX_SHAPES);
+    if (!(mass > 0)) return fail(ctx, DEM_EINVAL, "mass must be positive");
+    HostShape S;
+    const std::string e = build_host_shape(S, ctx->dim, verts, nv, face_offsets, face_verts, nf, edges, ne,
+                                           rounding_radius, mass, inertia);
+    if (!e.empty()) return fail(ctx, DEM_EINVAL, "%s", e.c_str());
+    if (S.table_len4() * 32 > 100 * 1024) return fail(ctx, DEM_EINVAL, "shape too large for the shared-memory table");
+    ctx->shapes.push_back(std::move(S));
+    ctx->table_dirty = true;
+    ctx->have_list = false;
+    *shape_id = (int)ctx->shapes.size() - 1;
+    return DEM_OK;
+}
+
+int dem_build_neighbors(dem_ctx* ctx, const void* pos, const int32_t* shape_id, int N, const double box[3], double r_cut) {
+    if (!ctx) return DEM_EINVAL;
+    if (!box) return fail(ctx, DEM_EINVAL, "null box");
+    if (ctx->prec == DEM_F64) return build_neighbors_t<double>(ctx, static_cast<const double*>(pos), shape_id, N, box, r_cut, true);
+    return build_neighbors_t<float>(ctx, static_cast<const float*>(pos), shape_id, N, box, r_cut, true);
+}
+
+int dem_get_neighbors(dem_ctx* ctx, const int32_t** counts, const int32_t** list, int* stride, int* max_count) {
+    if (!ctx) return DEM_EINVAL;
+    if (!ctx->have_list) return fail(ctx, DEM_ESTALE, "no neighbour list");
+    if (counts) *counts = ctx->counts.as<int32_t>();
+    if (list) *list = ctx->list.as<int32_t>();
+    if (stride) *stride = ctx->stride;
+    if (max_count) *max_count = ctx->max_count;
+    return DEM_OK;
+}
+
+int dem_copy_neighbors(dem_ctx* ctx, int32_t* counts_out, int32_t* list_out, int out_stride) {
+    if (!ctx) return DEM_EINVAL;
+    if (!ctx->have_list) return fail(ctx, DEM_ESTALE, "no neighbour list");
+    if (!counts_out || !list_out || out_stride < ctx->max_count) return fail(ctx, DEM_EINVAL, "bad output arrays");
+    CU(cudaMemcpyAsync(counts_out, ctx->counts.p, sizeof(int) * (size_t)ctx->N, cudaMemcpyDeviceToDevice, ctx->stream));
+    k_copy_rows<<<nblk((long long)ctx->N * out_stride, 256), 256, 0, ctx->stream>>>(
+        ctx->N, ctx->counts.as<int>(), ctx->list.as<int>(), ctx->stride, list_out, out_stride);
+    LAUNCHED(ctx);
+    CU(cudaGetLastError());
+    return DEM_OK;
+}
+
+int dem_compute(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* shape_id, int N, void* force_energy,
+                void* torque, void* virial6) {
+    if (!ctx) return DEM_EINVAL;
+    if (ctx->prec == DEM_F64)
+        return compute_t<double, double>(ctx, static_cast<const double*>(pos), static_cast<const double*>(quat), shape_id,
+                                         N, force_energy, torque, virial6);
+    return compute_t<float, float>(ctx, static_cast<const float*>(pos), static_cast<const float*>(quat), shape_id, N,
+                                   force_energy, torque, virial6);
+}
+
+int dem_get_counters(dem_ctx* ctx, int64_t out[6]) {
+    if (!ctx || !out) return DEM_EINVAL;
+    if (!ctx->counters.p) return fail(ctx, DEM_ESTALE, "no evaluation yet");
+    unsigned long long h[4];
+    CU(cudaMemcpyAsync(h, ctx->counters.p, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    // terms evaluated = nominal terms of the evaluated pairs; with a single class this is exact, with several classes
+    // pairs rejected by the reach test are attributed proportionally (the list is normally built at r_cut = reach)
+    out[0] = (int64_t)h[0];
+    out[1] = ctx->npairs_total > 0 ? (int64_t)((double)ctx->last_terms * ((double)h[0] / (double)ctx->npairs_total) + 0.5) : 0;
+    out[2] = (int64_t)h[1];
+    out[3] = (int64_t)h[2];
+    out[4] = (int64_t)h[3];
+    out[5] = ctx->npairs_total;
+    return DEM_OK;
+}
+
+int dem_step(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const int32_t* shape_id, int N,
+             const double box[3], double dt, int nsteps, double skin, void* force_energy, void* torque) {
+    if (!ctx) return DEM_EINVAL;
+    if (!box) return fail(ctx, DEM_EINVAL, "null box");
+    if (ctx->prec == DEM_F64)
+        return step_t<double>(ctx, pos, quat, vel, angmom, shape_id, N, box, dt, nsteps, skin, force_energy, torque);
+    return step_t<float>(ctx, pos, quat, vel, angmom, shape_id, N, box, dt, nsteps, skin, force_energy, torque);
+}
+
+int dem_energy(dem_ctx* ctx, const void* quat, const void* vel, const void* angmom, const int32_t* shape_id,
+               const void* force_energy, int N, double out[3]) {
+    if (!ctx || !out) return DEM_EINVAL;
+    if (!quat || !vel || !angmom || !shape_id || !force_energy || N < 1) return fail(ctx, DEM_EINVAL, "bad arguments");
+    if (ctx->prec == DEM_F64)
+        return energy_t<double, double>(ctx, static_cast<const double*>(quat), static_cast<const double*>(vel),
+                                        static_cast<const double*>(angmom), shape_id, force_energy, N, out);
+    return energy_t<float, float>(ctx, static_cast<const float*>(quat), static_cast<const float*>(vel),
+                                  static_cast<const float*>(angmom), shape_id, force_energy, N, out);
+}
+
+int dem_compute_host(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* shape_id, int N, const double box[3],
+                     double r_cut, void* force_energy, void* torque, void* virial6) {
+    if (!ctx) return DEM_EINVAL;
+    if (!pos || !quat || !shape_id || !force_energy || !torque || !box || N < 1) return fail(ctx, DEM_EINVAL, "bad arguments");
+    const size_t r4 = (ctx->prec == DEM_F64 ? sizeof(d4) : sizeof(f4)), rs = r4 / 4;
+    cudaStream_t st = ctx->stream;
+    CU(ctx->h_pos.reserve(r4 * N));
+    CU(ctx->h_quat.reserve(r4 * N));
+    CU(ctx->h_sid.reserve(sizeof(int32_t) * (size_t)N));
+    CU(ctx->h_force.reserve(r4 * N));
+    CU(ctx->h_torque.reserve(r4 * N));
+    if (virial6) CU(ctx->h_virial.reserve(rs * 6 * N));
+    CU(cudaMemcpyAsync(ctx->h_pos.p, pos, r4 * N, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(ctx->h_quat.p, quat, r4 * N, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(ctx->h_sid.p, shape_id, sizeof(int32_t) * (size_t)N, cudaMemcpyHostToDevice, st));
+    CHECK(dem_build_neighbors(ctx, ctx->h_pos.p, ctx->h_sid.as<int32_t>(), N, box, r_cut));
+    CHECK(dem_compute(ctx, ctx->h_pos.p, ctx->h_quat.p, ctx->h_sid.as<int32_t>(), N, ctx->h_force.p, ctx->h_torque.p,
+                      virial6 ? ctx->h_virial.p : nullptr));
+    CU(cudaMemcpyAsync(force_energy, ctx->h_force.p, r4 * N, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(torque, ctx->h_torque.p, r4 * N, cudaMemcpyDeviceToHost, st));
+    if (virial6) CU(cudaMemcpyAsync(virial6, ctx->h_virial.p, rs * 6 * N, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return DEM_OK;
+}
+
+int dem_step_host(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const int32_t* shape_id, int N,
+                  const double box[3], double dt, int nsteps, double skin, void* force_energy, void* torque) {
+    if (!ctx) return DEM_EINVAL;
+    if (!pos || !quat || !vel || !angmom || !shape_id || !box || N < 1) return fail(ctx, DEM_EINVAL, "bad arguments");
+    const size_t r4 = (ctx->prec == DEM_F64 ? sizeof(d4) : sizeof(f4));
+    cudaStream_t st = ctx->stream;
+    DevBuf* bufs[4] = {&ctx->h_pos, &ctx->h_quat, &ctx->h_vel, &ctx->h_ang};
+    void* host[4] = {pos, quat, vel, angmom};
+    for (int k = 0; k < 4; ++k) {
+        CU(bufs[k]->reserve(r4 * N));
+        CU(cudaMemcpyAsync(bufs[k]->p, host[k], r4 * N, cudaMemcpyHostToDevice, st));
+    }
+    CU(ctx->h_sid.reserve(sizeof(int32_t) * (size_t)N));
+    CU(cudaMemcpyAsync(ctx->h_sid.p, shape_id, sizeof(int32_t) * (size_t)N, cudaMemcpyHostToDevice, st));
+    CU(ctx->h_force.reserve(r4 * N));
+    CU(ctx->h_torque.reserve(r4 * N));
+    CHECK(dem_step(ctx, ctx->h_pos.p, ctx->h_quat.p, ctx->h_vel.p, ctx->h_ang.p, ctx->h_sid.as<int32_t>(), N, box, dt,
+                   nsteps, skin, ctx->h_force.p, ctx->h_torque.p));
+    for (int k = 0; k < 4; ++k) CU(cudaMemcpyAsync(host[k], bufs[k]->p, r4 * N, cudaMemcpyDeviceToHost, st));
+    if (force_energy) CU(cudaMemcpyAsync(force_energy, ctx->h_force.p, r4 * N, cudaMemcpyDeviceToHost, st));
+    if (torque) CU(cudaMemcpyAsync(torque, ctx->h_torque.p, r4 * N, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return DEM_OK;
+}
+
+int dem_set_timing(dem_ctx* ctx, int enabled) {
+    if (!ctx) return DEM_EINVAL;
+    ctx->timing = enabled != 0;
+    return DEM_OK;
+}
+
+int dem_kernel_time(dem_ctx* ctx, int64_t* launches, double* total_ms) {
+    if (!ctx || !launches || !total_ms) return DEM_EINVAL;
+    CU(cudaStreamSynchronize(ctx->stream));
+    double tot = 0;
+    for (size_t k = 0; k < ctx->ev_used; ++k) {
+        float ms = 0;
+        CU(cudaEventElapsedTime(&ms, ctx->ev_pool[k].first, ctx->ev_pool[k].second));
+        tot += ms;
+    }
+    *launches = (int64_t)ctx->ev_used;
+    *total_ms = tot;
+    ctx->ev_used = 0;
+    return DEM_OK;
+}
+
+int64_t dem_launch_count(const dem_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int dem_fp32_peak(dem_ctx* ctx, int iters, double* tflops) {
+    if (!ctx || !tflops || iters < 1) return DEM_EINVAL;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CU(ctx->flags.reserve(sizeof(int) * 16));
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    const int grid = sms * 8, threads = 256;
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        CU(cudaEventRecord(e0, ctx->stream));
+        k_fma_peak<<<grid, threads, 0, ctx->stream>>>(iters, 1.0f, ctx->flags.as<float>());
+        LAUNCHED(ctx);
+        CU(cudaEventRecord(e1, ctx->stream));
+        CU(cudaEventSynchronize(e1));
+        float ms = 0;
+        CU(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *tflops = 2.0 * 8.0 * (double)iters * (double)grid * threads / (best * 1e-3) / 1e12;
+    return DEM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,129 @@
+"""GPU tests of dem_step / dem_energy (velocity-Verlet NVE with quaternion rotation) against the oracle's
+integrator, plus the energy-conservation gate of north_star (drift < 1e-4 per particle over 10^4 steps)."""
+import numpy as np
+import pytest
+
+import dem_inputs as di
+from _gpu_util import round_state
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device: the product has no CPU path")
+    import paper_1607_02427_b200 as p
+
+    p.lib()
+    return p
+
+
+def _run(pkg, st, precision, dt, nsteps, skin, chunks=1):
+    import torch
+
+    dem, t = pkg.from_state(st, precision)
+    n = st["N"]
+    f = torch.empty((n, 4), dtype=dem.dtype, device="cuda")
+    tq = torch.empty((n, 4), dtype=dem.dtype, device="cuda")
+    energies = []
+    for _ in range(chunks):
+        dem.step(t["pos"], t["quat"], t["vel"], t["angmom"], t["shape_id"], st["box"], dt, nsteps // chunks, skin, f, tq)
+        energies.append(dem.energy(t["quat"], t["vel"], t["angmom"], t["shape_id"], f))
+    out = {k: v.cpu().numpy().astype(np.float64) for k, v in t.items()}
+    out["force"], out["torque"] = f.cpu().numpy().astype(np.float64), tq.cpu().numpy().astype(np.float64)
+    out["energies"] = np.array(energies)
+    out["launches"] = dem.launch_count()
+    dem.close()
+    return out
+
+
+@pytest.mark.parametrize("kind,cells,dt,nsteps", [("squares", 8, 1e-3, 200), ("cubes", 4, 1e-3, 100),
+                                                  ("mixed", 4, 5e-4, 60)])
+def test_step_matches_oracle_f64(pkg, oracle, kind, cells, dt, nsteps):
+    st = di.dense_state(kind, cells)
+    ref = oracle.step(st, dt, nsteps)
+    got = _run(pkg, st, "f64", dt, nsteps, skin=0.3)
+    for k in ("pos", "quat", "vel", "angmom"):
+        assert np.abs(got[k] - ref[k]).max() < 1e-8, k
+    e = ref["energies"][-1]
+    assert np.allclose(got["energies"][-1], e, rtol=1e-9, atol=1e-9)
+    assert abs(ref["energies"][0].sum() - e.sum()) > 0  # the state really moved / interacted
+
+
+def test_step_f32_context_tracks_oracle(pkg, oracle):
+    """A DEM_F32 context (FP32 forces, FP64 state inside dem_step) stays close to the FP64 trajectory."""
+    st = round_state(di.dense_state("cubes", 4), "f32")
+    ref = oracle.step(st, 1e-3, 50)
+    got = _run(pkg, st, "f32", 1e-3, 50, skin=0.3)
+    assert np.abs(got["pos"] - ref["pos"]).max() < 2e-5
+    assert np.abs(got["vel"] - ref["vel"]).max() < 2e-3
+    etot = got["energies"][-1].sum()
+    assert abs(etot - ref["energies"][-1].sum()) / st["N"] < 1e-4
+
+
+def test_asymmetric_top_free_rotation(pkg, oracle):
+    """Non-interacting cuboids (three different moments): the splitting integrator matches the oracle's."""
+    st = di.lattice_state(3, [di.box_shape(1.0, 0.7, 0.4, 0.1)], (3, 3, 3), 6.0, seed=4)
+    ref = oracle.step(st, 5e-3, 100)
+    got = _run(pkg, st, "f64", 5e-3, 100, skin=0.5)
+    assert np.abs(got["quat"] - ref["quat"]).max() < 1e-10
+    assert np.array_equal(got["angmom"], st["angmom"])  # torque-free: L untouched
+    assert np.allclose(got["energies"][-1], ref["energies"][-1], rtol=1e-10)
+
+
+def test_rebuilds_do_not_change_the_trajectory(pkg):
+    st = di.dense_state("squares", 8)
+    a = _run(pkg, st, "f64", 2e-3, 300, skin=0.02)   # many rebuilds
+    b = _run(pkg, st, "f64", 2e-3, 300, skin=0.6)    # none
+    assert a["launches"] > b["launches"]
+    assert np.abs(a["pos"] - b["pos"]).max() < 1e-9
+
+
+def test_config1_energy_parity_and_drift_gate(pkg, oracle):
+    """Config 1 in FP64: 1000 steps at dt = 1e-4 against the oracle's energies, then the north_star gate:
+    max_t |E(t) - E(0)| / N < 1e-4 over 10^4 steps (sampled every 500 steps)."""
+    st = di.make_config(1)
+    ref = oracle.step(st, st["dt"], 1000)
+    got = _run(pkg, st, "f64", st["dt"], 1000, skin=0.3)
+    assert np.allclose(got["energies"][-1], ref["energies"][-1], rtol=1e-9, atol=1e-9)
+    assert np.abs(got["pos"] - ref["pos"]).max() < 1e-9
+    e0 = ref["energies"][0].sum()
+    long = _run(pkg, st, "f64", st["dt"], 10000, skin=0.3, chunks=20)
+    drift = np.abs(long["energies"].sum(1) - e0).max() / st["N"]
+    assert drift < 1e-4, drift
+
+
+@pytest.mark.parametrize("kind,cells,dt", [("squares", 10, 1e-3), ("cubes", 5, 1e-3)])
+def test_dense_state_drift_gate_f64(pkg, kind, cells, dt):
+    """Interacting dense states, FP64, 10^4 steps: drift per particle below 1e-4 (north_star)."""
+    import torch
+
+    st = di.dense_state(kind, cells)
+    dem, t = pkg.from_state(st, "f64")
+    n = st["N"]
+    f = torch.empty((n, 4), dtype=torch.float64, device="cuda")
+    dem.step(t["pos"], t["quat"], t["vel"], t["angmom"], t["shape_id"], st["box"], dt, 0, 0.3, f, None)
+    e0 = dem.energy(t["quat"], t["vel"], t["angmom"], t["shape_id"], f).sum()
+    worst = 0.0
+    for _ in range(20):
+        dem.step(t["pos"], t["quat"], t["vel"], t["angmom"], t["shape_id"], st["box"], dt, 500, 0.3, f, None)
+        worst = max(worst, abs(dem.energy(t["quat"], t["vel"], t["angmom"], t["shape_id"], f).sum() - e0) / n)
+    dem.close()
+    assert worst < 1e-4, worst
+
+
+def test_step_host_matches_device(pkg):
+    import torch
+
+    st = round_state(di.dense_state("cubes", 4), "f32")
+    dev = _run(pkg, st, "f32", 1e-3, 20, skin=0.3)
+    dem, _ = pkg.from_state(st, "f32")
+    h = {k: torch.tensor(st[k], dtype=torch.float32).pin_memory() for k in ("pos", "quat", "vel", "angmom")}
+    sid = torch.tensor(st["shape_id"], dtype=torch.int32).pin_memory()
+    dem.step_host(h["pos"], h["quat"], h["vel"], h["angmom"], sid, st["box"], 1e-3, 20, 0.3)
+    for k in ("pos", "quat", "vel", "angmom"):
+        assert np.array_equal(h[k].numpy().astype(np.float64), dev[k]), k
+    dem.close()

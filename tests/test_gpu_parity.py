@@ -1,0 +1,272 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the FP64 CPU oracle, element by element, on the same
+seeded inputs.  Run on the B200 box with `-m gpu`.
+
+Tolerances (north_star): neighbour list bit-exact; per-particle force and torque within 1e-4 (FP32) / 1e-10 (FP64)
+of the system's max |F| (floored by eps/sigma, R19); the same bar is applied to energies and the virial.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import dem_inputs as di
+from _gpu_util import TOL, assert_neighbors_exact, assert_parity, gpu_compute, round_state, scales
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device: the product has no CPU path")
+    import paper_1607_02427_b200 as p
+
+    p.lib()
+    return p
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# neighbour list: bit-exact against the all-pairs definition
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "dense_squares", "dense_cubes", "dense_mixed"])
+def test_neighbors_bit_exact(pkg, oracle, name, precision):
+    st = {"cfg1": lambda: di.make_config(1), "cfg2": lambda: di.make_config(2),
+          "dense_squares": lambda: di.dense_state("squares", 12), "dense_cubes": lambda: di.dense_state("cubes", 6),
+          "dense_mixed": lambda: di.dense_state("mixed", 6)}[name]()
+    counts = assert_neighbors_exact(st, precision, oracle)
+    assert counts.sum() % 2 == 0
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_neighbors_random_gas_odd_boxes(pkg, oracle, dim):
+    """Random points (several per cell, ragged cell occupancy, positions outside the box), boxes with only 2 cells
+    along an axis, cutoffs that put many pairs near r_cut."""
+    rng = np.random.default_rng(5)
+    for box, rc, n in (([7.3, 5.1, 4.4], 1.3, 700), ([4.1, 9.0, 4.05], 2.0, 500), ([30.0, 3.0, 2.9], 1.45, 900)):
+        pos = np.zeros((n, 4))
+        pos[:, :dim] = rng.uniform(-0.75, 0.75, (n, dim)) * np.array(box[:dim])  # some outside the box
+        sh = [di.disk(0.1)] if dim == 2 else [di.sphere(0.1)]
+        st = dict(dim=dim, shapes=sh, box=np.array(box), pos=pos, quat=np.tile([1.0, 0, 0, 0], (n, 1)),
+                  vel=np.zeros((n, 4)), angmom=np.zeros((n, 4)), shape_id=np.zeros(n, dtype=np.int32), N=n,
+                  r_cut=rc, epsilon=1.0)
+        for precision in ("f32", "f64"):
+            counts = assert_neighbors_exact(st, precision, oracle)
+            assert counts.max() > 16  # exercises the capacity regrow
+
+
+def test_neighbors_full_size_sampled(pkg, oracle):
+    """Config 4 at full size (N = 262,144): rows of 512 sampled particles against the all-pairs definition."""
+    st = di.make_config(4)
+    sub = np.random.default_rng(1).choice(st["N"], 512, replace=False).astype(np.int32)
+    assert_neighbors_exact(st, "f32", oracle, subset=sub)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# force / torque / energy / virial
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_config1_squares(pkg, oracle, precision):
+    assert_parity(di.make_config(1), precision, oracle)
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_config2_cubes(pkg, oracle, precision):
+    r = assert_parity(di.make_config(2), precision, oracle)
+    assert r["counters"]["pairs_listed"] == 1536 and r["counters"]["terms"] == 1536 * 240
+
+
+DENSE = [("squares", 12), ("pentagons", 12), ("cubes", 6), ("octahedra", 6), ("mixed", 5)]
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+@pytest.mark.parametrize("kind,cells", DENSE)
+def test_dense_states(pkg, oracle, kind, cells, precision):
+    """P2: dense near-aligned lattices in which many pairs interact through many terms."""
+    r = assert_parity(di.dense_state(kind, cells), precision, oracle)
+    assert r["counters"]["active"] > 50  # the state really exercises WCA / torque code
+
+
+@pytest.mark.parametrize("kind,cells,slices", [("cubes", 5, 3), ("cubes", 5, 28), ("squares", 10, 2), ("mixed", 4, 7),
+                                               ("octahedra", 5, 1000)])
+def test_sliced_pairs_match(pkg, oracle, kind, cells, slices):
+    """Several lanes per pair (slices of the outer feature loop) give the same sums."""
+    assert_parity(di.dense_state(kind, cells), "f64", oracle, slices=slices)
+    assert_parity(di.dense_state(kind, cells), "f32", oracle, slices=slices)
+
+
+def test_exactly_aligned_cube_lattice_closed_form(pkg):
+    """Aligned unit cubes at spacing 1 + sigma: every face-neighbour pair has 56 terms at r = sigma (PAPER.md:61 as
+    corrected by Eq. 1), so U_i = 1/2 * 6 * 56 eps = 168 eps, F_i = tau_i = 0 -- and every one of the 32 edge-edge
+    terms goes through the parallel-edge rule."""
+    sig = 0.3
+    st = di.lattice_state(3, [di.cube(1.0, sig / 2)], (4, 4, 4), 1.0 + sig, orient="aligned")
+    for precision in ("f32", "f64"):
+        f, tq, w, cnt = gpu_compute(round_state(st, precision), precision)
+        tol = 1e-4 if precision == "f32" else 1e-9
+        assert np.allclose(f[:, 3], 168.0, rtol=tol)
+        assert np.abs(f[:, :3]).max() < tol * 56 * 24 / sig and np.abs(tq[:, :3]).max() < tol * 56 * 24 / sig
+        assert cnt["active"] == 64 * 3 * 56 and cnt["parallel"] == 64 * 3 * 32
+        # sum_i tr W_i = N * 3 pairs * 56 * (24 eps / sigma) * (1 + sigma)
+        assert math.isclose(w[:, [0, 3, 5]].sum(), 64 * 3 * 56 * 24 / sig * (1 + sig), rel_tol=tol)
+
+
+def test_parallel_rule_just_inside_and_outside(pkg, oracle):
+    """Two rods, slightly non-parallel: the angle is set just inside / outside eps_par (R5)."""
+    rod = di.rod(1.0, 0.15)
+    for ang in (0.5e-3, 0.9e-3, 1.1e-3, 2e-3):  # threshold: sin^2 < 1e-6  <=>  angle < 1e-3
+        st = di.two_particle_state(rod, rod, seed=0)
+        st["pos"][:, :3] = [[0, 0, 0], [0.31, 0.02, 0.1]]
+        st["quat"][0] = [1, 0, 0, 0]
+        st["quat"][1] = [math.cos(ang / 2), 0, math.sin(ang / 2), 0]
+        r = assert_parity(st, "f64", oracle)
+        assert r["counters"]["active"] == 1 and r["counters"]["parallel"] == (1 if ang < 1e-3 else 0)
+        assert_parity(st, "f32", oracle)
+
+
+PAIRS = [("square", "square"), ("pentagon", "square"), ("disk", "square"), ("cube", "cube"), ("octa", "octa"),
+         ("tet", "ti"), ("ti", "ti"), ("ico", "cube"), ("sphere", "sphere"), ("sphere", "cube"), ("rod", "rod"),
+         ("rod", "cube"), ("plate", "plate"), ("plate", "tet")]
+SHAPES = dict(square=lambda: di.square(), pentagon=lambda: di.regular_polygon(5, 0.5, 0.05), disk=lambda: di.disk(0.2),
+              cube=lambda: di.cube(), octa=lambda: di.octahedron(), tet=lambda: di.tetrahedron(),
+              ti=lambda: di.truncated_icosahedron(), ico=lambda: di.icosahedron(), sphere=lambda: di.sphere(0.3),
+              rod=lambda: di.rod(1.0, 0.2), plate=lambda: di.triangular_plate())
+
+
+@pytest.mark.parametrize("na,nb", PAIRS)
+def test_isolated_pair_poses(pkg, oracle, na, nb):
+    """P3: many isolated two-particle poses, rejection-sampled (with the oracle) to be in contact, batched into ONE
+    state on a sparse lattice of pairs so that every species pair -- including the degenerate shapes (sphere, rod,
+    plate, disk) and both orderings of unlike shapes -- goes through the kernel."""
+    sa, sb = SHAPES[na](), SHAPES[nb]()
+    dim = sa["dim"]
+    shapes = [sa, sb]
+    sig = sa["rounding"] + sb["rounding"]
+    reach = di.default_rcut(shapes)
+    rng = np.random.default_rng(11)
+    poses = []
+    tries = 0
+    want = 24 if "ti" in (na, nb) else 64
+    while len(poses) < want and tries < 20000:
+        tries += 1
+        d = rng.standard_normal(3)
+        if dim == 2:
+            d[2] = 0
+        d *= rng.uniform(0.3, 1.0) * reach / np.linalg.norm(d)
+        if dim == 2:
+            qi, qj = di.planar_quaternions(rng.uniform(0, 2 * math.pi, 2))
+        else:
+            qi, qj = di.random_quaternions(rng, 2)
+        _, sums = oracle.pair_terms(shapes, 0, 1, qi, qj, d)
+        if 0.8 * sig < sums["rmin"] < 2 ** (1 / 6) * sig:
+            poses.append((d, qi, qj))
+    assert len(poses) >= want // 2
+    m = len(poses)
+    side = int(math.ceil(m ** (1.0 / dim)))
+    spacing = 3.0 * reach
+    n = 2 * m
+    pos, quat, sid = np.zeros((n, 4)), np.zeros((n, 4)), np.zeros(n, dtype=np.int32)
+    for k, (d, qi, qj) in enumerate(poses):
+        cell = np.array([k % side, (k // side) % side, k // (side * side) if dim == 3 else 0], dtype=np.float64)
+        c = (cell - side / 2 + 0.5) * spacing
+        a, b = (2 * k, 2 * k + 1) if k % 2 == 0 else (2 * k + 1, 2 * k)  # both index orders
+        pos[a, :3], pos[b, :3] = c - d / 2, c + d / 2
+        quat[a], quat[b] = qi, qj
+        sid[a], sid[b] = 0, 1
+    box = np.array([side * spacing] * 3)
+    st = dict(dim=dim, shapes=shapes, box=box, pos=pos, quat=quat, vel=np.zeros((n, 4)), angmom=np.zeros((n, 4)),
+              shape_id=sid, N=n, r_cut=reach, epsilon=1.0)
+    for precision in ("f64", "f32"):
+        r = assert_parity(st, precision, oracle)
+        assert r["counters"]["active"] >= m
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# full-size configs (the launch configuration bench.py times): sampled rows against the oracle + global invariants
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("k,nsample", [(3, 256), (4, 192), (5, 48)])
+def test_full_size_configs_sampled(pkg, oracle, k, nsample):
+    st = round_state(di.make_config(k), "f32")
+    sub = np.sort(np.random.default_rng(k).choice(st["N"], nsample, replace=False)).astype(np.int32)
+    f, tq, w, cnt = gpu_compute(st, "f32")
+    of, ot, ow, ocnt = oracle.compute(st, subset=sub)
+    fs, ts, us = scales(st, of, ot)
+    # the system max |F| is at least the sample's; use the GPU's own global max as the (larger) denominator check too
+    fs = max(fs, np.abs(f[:, :3]).max())
+    assert np.abs(f[sub, :3] - of[:, :3]).max() / fs < TOL["f32"]
+    assert np.abs(tq[sub, :3] - ot[:, :3]).max() / max(ts, np.abs(tq[:, :3]).max()) < TOL["f32"]
+    assert np.abs(f[sub, 3] - of[:, 3]).max() / us < TOL["f32"]
+    assert np.abs(w[sub] - ow).max() / max(np.abs(ow).max(), 1.0) < TOL["f32"]
+    # properties that hold at any size: Newton's third law over the whole system, pair/term counts of the lattice
+    assert np.abs(f[:, :3].sum(0)).max() < 1e-3 * max(fs, 1.0) * math.sqrt(st["N"])
+    assert cnt["pairs_listed"] == 3 * st["N"]  # 6 neighbours per particle on these lattices
+    per_pair = {3: 50, 4: 240}.get(k)
+    if per_pair:
+        assert cnt["terms"] == cnt["pairs_listed"] * per_pair
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# edge cases and error behaviour
+# ---------------------------------------------------------------------------------------------------------------
+def test_single_particle_and_isolated_particles(pkg):
+    st = di.lattice_state(3, [di.cube()], (1, 1, 1), 10.0)
+    f, tq, w, cnt = gpu_compute(st, "f32")
+    assert np.all(f == 0) and np.all(tq == 0) and np.all(w == 0) and cnt["pairs_listed"] == 0
+    st = di.lattice_state(2, [di.square()], (3, 3), 5.0)
+    f, tq, w, cnt = gpu_compute(st, "f64")
+    assert np.all(f == 0) and cnt["pairs_listed"] == 0
+
+
+def test_error_codes(pkg):
+    import torch
+
+    st = di.make_config(2, scale=2)
+    dem, t = pkg.from_state(st, "f32")
+    with pytest.raises(pkg.DemError) as e:
+        dem.compute(t["pos"], t["quat"], t["shape_id"])
+    assert e.value.code == -7  # DEM_ESTALE: no list yet
+    with pytest.raises(pkg.DemError) as e:
+        dem.build_neighbors(t["pos"], t["shape_id"], st["box"], 0.5 * st["r_cut"])
+    assert e.value.code == -5  # DEM_ERCUT
+    with pytest.raises(pkg.DemError) as e:
+        dem.build_neighbors(t["pos"], t["shape_id"], [3.0, 3.0, 3.0], st["r_cut"])
+    assert e.value.code == -4  # DEM_EBOX
+    dem.build_neighbors(t["pos"], t["shape_id"], st["box"], st["r_cut"])
+    with pytest.raises(pkg.DemError) as e:
+        dem.compute(t["pos"][:10].contiguous(), t["quat"][:10].contiguous(), t["shape_id"][:10].contiguous())
+    assert e.value.code == -7
+    with pytest.raises(TypeError):
+        dem.compute(t["pos"].cpu(), t["quat"], t["shape_id"])  # no CPU path
+    # a list built with a larger cutoff (skin) gives identical forces: the extra pairs contribute exactly zero
+    f0, t0, _ = dem.compute(t["pos"], t["quat"], t["shape_id"])
+    dem.build_neighbors(t["pos"], t["shape_id"], st["box"], 1.4 * st["r_cut"])
+    f1, t1, _ = dem.compute(t["pos"], t["quat"], t["shape_id"])
+    assert torch.equal(f0, f1) and torch.equal(t0, t1)
+    dem.close()
+
+
+def test_run_to_run_bit_reproducible(pkg):
+    """No atomics on the accumulation path and a sorted cell list: two runs give identical bits."""
+    st = di.dense_state("mixed", 5)
+    a = gpu_compute(st, "f32")
+    b = gpu_compute(st, "f32")
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+
+
+def test_host_buffer_entry_point_matches_device_path(pkg):
+    import torch
+
+    st = round_state(di.dense_state("cubes", 5), "f32")
+    f, tq, w, _ = gpu_compute(st, "f32")
+    dem, _ = pkg.from_state(st, "f32")
+    n = st["N"]
+    pos = torch.tensor(st["pos"], dtype=torch.float32).pin_memory()
+    quat = torch.tensor(st["quat"], dtype=torch.float32).pin_memory()
+    sid = torch.tensor(st["shape_id"], dtype=torch.int32).pin_memory()
+    fo, to, wo = (torch.empty((n, 4)).pin_memory(), torch.empty((n, 4)).pin_memory(), torch.empty((n, 6)).pin_memory())
+    dem.compute_host(pos, quat, sid, st["box"], st["r_cut"], fo, to, wo)
+    assert np.array_equal(fo.numpy().astype(np.float64), f) and np.array_equal(to.numpy().astype(np.float64), tq)
+    assert np.array_equal(wo.numpy().astype(np.float64), w)
+    dem.close()
