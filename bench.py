@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the DEM hot path (arXiv:1607.02427) on B200, one JSON line on stdout.
+
+A "step" is one NVE time step of the whole hot path (neighbour-list upkeep, pair-feature kernel, per-particle
+reduction, integrator) over one synthetic configuration of BASELINE.json.  Default workload at N = 1: config 4
+(3D rounded octahedra, N = 262,144, fp32, dt = 2e-4), the largest single-GPU 3D NVE configuration.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg3|cfg4|cfg5|cfg2]
+
+metric  = particle-timesteps/s (BASELINE.json); feature-pair evaluations/s are reported beside it.
+value   = N_particles * K / (device time of dem_step(nsteps=K)), state resident in HBM, max over ranks.
+e2e     = the same metric through dem_step_host (HOST buffers: every step copies the state host->device and back).
+roofline= the pair-feature kernel (dominant): algorithmic FP32 flops per launch / its CUDA-event time, against the
+          FP32 peak 148 SM x 128 lanes x 2 x clocks.max.sm.
+cpu_baseline = the FP64 oracle (oracle/dem_oracle.c, as it stands) timed on this box's host cores on a bounded sample.
+`--impl reference` times the oracle as the reference arm (this tier has no reference implementation to install).
+With --gpus N > 1 (torchrun) every rank runs an independent replica of the workload (the path does not shard:
+DESIGN.md "Multi-GPU"): weak scaling, no data-path collective, one MAX all-reduce of the elapsed time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import dem_inputs as di  # noqa: E402
+
+WORKLOADS = {"cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}
+SKIN = {2: 0.3, 3: 0.2, 4: 0.3, 5: 0.3}
+L2_FLUSH_BYTES = 256 << 20
+
+# Algorithmic FP32 flop per Eq. 1 / Eq. 2 term of the formulation in csrc/dem_math.cuh (FMA = 2)
+FLOP_VE_2D = 15           # point - segment, 2D
+FLOP_EE = 81              # segment - segment (skew path)
+FLOP_VF_FACE = 22         # projection on the face frame + combine
+FLOP_VF_EDGE = 19         # per boundary edge of the face
+
+
+def pair_flops(dim, a, b):
+    """Algorithmic flop of one unique pair with shapes a (first) and b (second)."""
+    if dim == 2:
+        return FLOP_VE_2D * (len(a["verts"]) * len(b["edges"]) + len(b["verts"]) * len(a["edges"]))
+    fa = sum(FLOP_VF_FACE + FLOP_VF_EDGE * len(f) for f in a["faces"])
+    fb = sum(FLOP_VF_FACE + FLOP_VF_EDGE * len(f) for f in b["faces"])
+    return FLOP_EE * len(a["edges"]) * len(b["edges"]) + len(a["verts"]) * fb + len(b["verts"]) * fa
+
+
+def pair_terms(dim, a, b):
+    if dim == 2:
+        return len(a["verts"]) * len(b["edges"]) + len(b["verts"]) * len(a["edges"])
+    return len(a["edges"]) * len(b["edges"]) + len(a["verts"]) * len(b["faces"]) + len(b["verts"]) * len(a["faces"])
+
+
+def class_pair_counts(st, counts, rows):
+    """Unique neighbour pairs per (shape, shape) class from the neighbour list (host-side bookkeeping for the flop
+    count only)."""
+    sid = st["shape_id"]
+    ns = len(st["shapes"])
+    out = np.zeros((ns, ns), dtype=np.int64)
+    i = np.repeat(np.arange(len(sid)), rows.shape[1])
+    j = rows.reshape(-1)
+    ok = (j >= 0) & (j > i)
+    a, b = sid[i[ok]], sid[j[ok]]
+    lo, hi = np.minimum(a, b), np.maximum(a, b)
+    np.add.at(out, (lo, hi), 1)
+    return out
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.split(",") for r in open(self.f.name).read().strip().splitlines() if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+                power.append(float(r[2]))
+                for k, nm in enumerate(names):
+                    if r[3 + k].strip().lower().startswith("active"):
+                        reasons.add(nm)
+            except (ValueError, IndexError):
+                continue
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        load = [s for s, p in zip(sm, power) if p >= 0.5 * max(power)] or sm
+        return {"sm_mhz": statistics.median(load), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": max(power)}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        return json.load(open(path)), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def oracle_sample_rate(st, target_seconds, max_rows=None):
+    """Time the oracle (as it stands) on a bounded random sample of particles of the same workload: each sampled
+    particle costs what one particle costs in a full oracle force evaluation (all-pairs scan + every Eq. 1/2 term
+    of its neighbours).  Returns (particle-evaluations/s, threads, description)."""
+    from oracle import dem_oracle as orc
+
+    orc.build()
+    n = st["N"]
+    rng = np.random.default_rng(123)
+    probe = np.sort(rng.choice(n, min(n, 64), replace=False)).astype(np.int32)
+    tab = orc.ShapeTable(st["shapes"])
+    st = dict(st, _tab=tab)
+    t0 = time.perf_counter()
+    orc.compute(st, subset=probe)
+    per = (time.perf_counter() - t0) / len(probe)
+    rows = int(max(64, min(n, target_seconds / max(per, 1e-9))))
+    if max_rows:
+        rows = min(rows, max_rows)
+    sub = np.sort(rng.choice(n, rows, replace=False)).astype(np.int32)
+    t0 = time.perf_counter()
+    orc.compute(st, subset=sub)
+    dt = time.perf_counter() - t0
+    return rows / dt, orc.num_threads(), "%d of %d particles, one full force evaluation each (all-pairs O(N) scan + all feature pairs), fp64" % (rows, n), rows, sub
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    k = WORKLOADS[args.workload]
+    st = di.make_config(k)
+    from oracle import dem_oracle as orc
+
+    orc.build()
+    tab = orc.ShapeTable(st["shapes"])
+    st["_tab"] = tab
+    n = st["N"]
+    rng = np.random.default_rng(7)
+    probe = np.sort(rng.choice(n, min(n, 64), replace=False)).astype(np.int32)
+    t0 = time.perf_counter()
+    orc.compute(st, subset=probe)
+    per = (time.perf_counter() - t0) / len(probe)
+    budget = 150.0 / (args.steps + args.warmup)       # whole run within a few minutes
+    rows = int(max(16, min(n, budget / max(per, 1e-9))))
+    for _ in range(args.warmup):
+        orc.compute(st, subset=np.sort(rng.choice(n, rows, replace=False)).astype(np.int32))
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.compute(st, subset=np.sort(rng.choice(n, rows, replace=False)).astype(np.int32))
+    dt = time.perf_counter() - t0
+    value = rows * args.steps / dt
+    sample = "each step = one oracle force evaluation of %d of %d particles (all-pairs scan + all feature pairs), fp64" % (rows, n)
+    line = {"impl": "reference", "metric": "particle-timesteps/s", "value": value, "unit": "particle-timesteps/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": di.CONFIG_NAMES[k], "N": n},
+            "cpu_baseline": {"value": value, "unit": "particle-timesteps/s", "cores": orc.num_threads(),
+                             "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "particle-timesteps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-l2-flush", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_1607_02427_b200 as pkg
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    k = WORKLOADS[args.workload]
+    st = di.make_config(k, seed=rank)  # independent replica per rank
+    n, dt_step, skin = st["N"], st["dt"], SKIN[k]
+    dem, t = pkg.from_state(st, "f32")
+    if not args.no_l2_flush:
+        dem.set_l2_flush(L2_FLUSH_BYTES)
+    force = torch.empty((n, 4), dtype=torch.float32, device="cuda")
+    torque = torch.empty((n, 4), dtype=torch.float32, device="cuda")
+
+    def step(nsteps):
+        dem.step(t["pos"], t["quat"], t["vel"], t["angmom"], t["shape_id"], st["box"], dt_step, nsteps, skin, force, torque)
+
+    # ---- device-resident throughput ---------------------------------------------------------------------------
+    step(args.warmup)
+    dem.set_timing(True)
+    dem.kernel_time()
+    launches0 = dem.launch_count()
+    sampler = ClockSampler(local) if rank == 0 else None
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    step(args.steps)
+    e1.record()
+    barrier()
+    elapsed_ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if sampler else None
+    gpu_launches = dem.launch_count() - launches0
+    n_pair_launches, pair_ms = dem.kernel_time()
+    dem.set_timing(False)
+    cnt = dem.get_counters()
+    tm = torch.tensor([elapsed_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+    elapsed_ms = float(tm.item())
+    value = n * world * args.steps / (elapsed_ms * 1e-3)
+
+    # ---- roofline of the pair-feature kernel ---------------------------------------------------------------------
+    counts, rows = dem.get_neighbors()
+    cls = class_pair_counts(st, counts.cpu().numpy(), rows.cpu().numpy())
+    flops = sum(int(cls[a, b]) * pair_flops(st["dim"], st["shapes"][a], st["shapes"][b])
+                for a in range(len(st["shapes"])) for b in range(a, len(st["shapes"])))
+    terms = sum(int(cls[a, b]) * pair_terms(st["dim"], st["shapes"][a], st["shapes"][b])
+                for a in range(len(st["shapes"])) for b in range(a, len(st["shapes"])))
+    n_classes = int((cls > 0).sum())
+    evals = max(n_pair_launches // max(n_classes, 1), 1)          # force evaluations timed
+    kern_ms_per_eval = pair_ms / evals
+    peaks, peak_kind = measured_peaks()
+    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+    peak_tf = sm_count * 128 * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+    achieved_tf = flops / (kern_ms_per_eval * 1e-3) / 1e12
+    fma_measured = dem.fp32_peak(1 << 15)
+
+    # ---- end to end through the host-buffer entry point -------------------------------------------------------------
+    h = {kk: t[kk].cpu().pin_memory() for kk in ("pos", "quat", "vel", "angmom")}
+    hsid = t["shape_id"].cpu().pin_memory()
+    hf = torch.empty((n, 4), dtype=torch.float32).pin_memory()
+    dem.set_l2_flush(0)
+    for _ in range(3):
+        dem.step_host(h["pos"], h["quat"], h["vel"], h["angmom"], hsid, st["box"], dt_step, 1, skin, hf, None)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.e2e_steps):
+        dem.step_host(h["pos"], h["quat"], h["vel"], h["angmom"], hsid, st["box"], dt_step, 1, skin, hf, None)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = n * world * args.e2e_steps / float(te.item())
+    h2d = 4 * n * 16 + n * 4
+    d2h = 5 * n * 16
+
+    # ---- oracle on the host cores (rank 0, N = 1 only) ---------------------------------------------------------------
+    cpu_baseline = None
+    if rank == 0 and world == 1:
+        rate, cores, desc, _, _ = oracle_sample_rate(di.make_config(k, seed=rank), args.cpu_seconds)
+        cpu_baseline = {"value": rate, "unit": "particle-timesteps/s", "cores": cores, "kind": "oracle", "sample": desc}
+
+    if rank == 0:
+        line = {
+            "metric": "particle-timesteps/s", "value": value, "unit": "particle-timesteps/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": di.CONFIG_NAMES[k], "N": n, "dt": dt_step, "skin": skin,
+                       "parallelism": "replicas x%d" % world if world > 1 else "1 GPU",
+                       "l2": ("flushed before every step (256 MiB memset inside the timed region)"
+                              if not args.no_l2_flush else "not flushed (working set < L2)")},
+            "feature_pair_evals_per_s": terms * world * (args.steps + 1) / (elapsed_ms * 1e-3),
+            "feature_pairs_per_step": terms, "unique_pairs": int(cls.sum()), "active_terms_last_step": cnt["active"],
+            "roofline": {"bound": "alu", "kernel": "k_pair", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                         "frac": achieved_tf / peak_tf, "traffic": None,
+                         "peak_source": "%d SM x 128 FP32 lanes x 2 x %.0f MHz (clocks.max.sm, %s)" % (
+                             sm_count, float(peaks.get("sm_max_mhz", 1965.0)), peak_kind),
+                         "flops_per_launch": flops, "kernel_ms": kern_ms_per_eval, "launches_timed": n_pair_launches,
+                         "kernel_share_of_step": pair_ms / elapsed_ms,
+                         "fma_chain_measured_tflops": fma_measured},
+            "cpu_baseline": cpu_baseline,
+            "e2e": {"value": e2e_value, "unit": "particle-timesteps/s", "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "steps": args.e2e_steps},
+            "gpu_launches": gpu_launches, "clocks": clocks,
+        }
+        print(json.dumps(line))
+    dem.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -160,6 +160,10 @@ int dem_step_host(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, 
  * lanes to fill the GPU when there are few pairs).  Takes effect at the next neighbour build. */
 int dem_set_slices(dem_ctx* ctx, int slices);
 
+/* Benchmark hygiene: when bytes > 0, dem_step overwrites a scratch buffer of that size (larger than the 126 MB L2)
+ * before every time step, so that no step finds its inputs cached by the previous one.  0 (default) = off. */
+int dem_set_l2_flush(dem_ctx* ctx, int64_t bytes);
+
 /* Kernel-time accounting for bench.py: when enabled, every launch of the pair-feature kernel is bracketed by CUDA
  * events on the context's stream; dem_kernel_time returns (and resets) the number of bracketed launches and their
  * summed duration in milliseconds (synchronises). */

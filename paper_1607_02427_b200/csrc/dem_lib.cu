@@ -60,6 +60,8 @@ struct dem_ctx {
     int class_sa[DEM_MAX_CLASSES], class_sb[DEM_MAX_CLASSES], class_np[DEM_MAX_CLASSES];
     long long npairs_total = 0, nrec_total = 0;
     int force_slices = 0;  // 0 = heuristic
+    size_t l2_flush_bytes = 0;  // bench hygiene: overwrite this many bytes of scratch before every time step
+    DevBuf l2_scratch;
     // dem_step state (double) for DEM_F32 contexts, plus forces and the positions of the last build
     DevBuf st_pos, st_quat, st_vel, st_ang, st_force, st_torque, pos_build, epart;
     // host-buffer entry points
@@ -432,7 +434,9 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr)));
     int* moved = ctx->flags.as<int>() + 8;
     const double half_skin2 = 0.25 * skin * skin;
+    if (ctx->l2_flush_bytes) CU(ctx->l2_scratch.reserve(ctx->l2_flush_bytes));
     for (int s = 0; s < nsteps; ++s) {
+        if (ctx->l2_flush_bytes) CU(cudaMemsetAsync(ctx->l2_scratch.p, s & 0xff, ctx->l2_flush_bytes, st));
         CU(cudaMemsetAsync(moved, 0, sizeof(int), st));
         k_kick_drift<real><<<nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T, ctx->pos_build.as<d4>(),
                                                      half_skin2, moved);
@@ -508,7 +512,7 @@ int dem_destroy(dem_ctx* c) {
     DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
                       &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->st_pos, &c->st_quat,
                       &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->pos_build, &c->epart, &c->h_pos,
-                      &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial};
+                      &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();
     for (auto& e : c->ev_pool) {
         cudaEventDestroy(e.first);
@@ -676,6 +680,12 @@ int dem_step_host(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, 
     if (force_energy) CU(cudaMemcpyAsync(force_energy, ctx->h_force.p, r4 * N, cudaMemcpyDeviceToHost, st));
     if (torque) CU(cudaMemcpyAsync(torque, ctx->h_torque.p, r4 * N, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    return DEM_OK;
+}
+
+int dem_set_l2_flush(dem_ctx* ctx, int64_t bytes) {
+    if (!ctx || bytes < 0) return fail(ctx, DEM_EINVAL, "bytes must be >= 0");
+    ctx->l2_flush_bytes = (size_t)bytes;
     return DEM_OK;
 }
 

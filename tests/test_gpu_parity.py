@@ -99,8 +99,9 @@ def test_sliced_pairs_match(pkg, oracle, kind, cells, slices):
 
 def test_exactly_aligned_cube_lattice_closed_form(pkg):
     """Aligned unit cubes at spacing 1 + sigma: every face-neighbour pair has 56 terms at r = sigma (PAPER.md:61 as
-    corrected by Eq. 1), so U_i = 1/2 * 6 * 56 eps = 168 eps, F_i = tau_i = 0 -- and every one of the 32 edge-edge
-    terms goes through the parallel-edge rule."""
+    corrected by Eq. 1), so U_i = 1/2 * 6 * 56 eps = 168 eps, F_i = tau_i = 0.  Of the 32 edge-edge terms of a pair, the
+    4 facing-edge/facing-edge ones overlap and go through the parallel-midpoint rule; the 4 collinear
+    side-edge pairs are parallel without overlap and fall through to the general routine (R5)."""
     sig = 0.3
     st = di.lattice_state(3, [di.cube(1.0, sig / 2)], (4, 4, 4), 1.0 + sig, orient="aligned")
     for precision in ("f32", "f64"):
@@ -108,7 +109,7 @@ def test_exactly_aligned_cube_lattice_closed_form(pkg):
         tol = 1e-4 if precision == "f32" else 1e-9
         assert np.allclose(f[:, 3], 168.0, rtol=tol)
         assert np.abs(f[:, :3]).max() < tol * 56 * 24 / sig and np.abs(tq[:, :3]).max() < tol * 56 * 24 / sig
-        assert cnt["active"] == 64 * 3 * 56 and cnt["parallel"] == 64 * 3 * 32
+        assert cnt["active"] == 64 * 3 * 56 and cnt["parallel"] == 64 * 3 * 4
         # sum_i tr W_i = N * 3 pairs * 56 * (24 eps / sigma) * (1 + sigma)
         assert math.isclose(w[:, [0, 3, 5]].sum(), 64 * 3 * 56 * 24 / sig * (1 + sig), rel_tol=tol)
 
