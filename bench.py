@@ -40,11 +40,12 @@ WORKLOADS = {"cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}
 SKIN = {2: 0.3, 3: 0.2, 4: 0.3, 5: 0.3}
 L2_FLUSH_BYTES = 256 << 20
 
-# Algorithmic FP32 flop per Eq. 1 / Eq. 2 term of the formulation in csrc/dem_math.cuh (FMA = 2)
-FLOP_VE_2D = 15           # point - segment, 2D
-FLOP_EE = 81              # segment - segment (skew path)
-FLOP_VF_FACE = 22         # projection on the face frame + combine
-FLOP_VF_EDGE = 19         # per boundary edge of the face
+# Algorithmic FP32 flop per Eq. 1 / Eq. 2 term of the search formulation in csrc/dem_fast.cuh (FMA = 2, every other
+# arithmetic instruction = 1).  The rare candidate terms' scalar evaluation is not counted.
+FLOP_VE_2D = 15           # point - segment, 2D: side 4, along 4, over 1, excess 2, r^2 - rc^2 4
+FLOP_EE = 49              # segment - segment: r 3, b c f 15, nn num 4, rcp 1, s 1, t 4, s' 3, d 12, r^2 - rc^2 6
+FLOP_VF_FACE = 22         # projection on the face frame 18, h^2 - rc^2 2, inside select + add 2
+FLOP_VF_EDGE = 16         # per boundary edge of the face: side 4, along 4, over 1, excess 2, d^2 3, two minima 2
 
 
 def pair_flops(dim, a, b):

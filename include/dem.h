@@ -160,6 +160,14 @@ int dem_step_host(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, 
  * lanes to fill the GPU when there are few pairs).  Takes effect at the next neighbour build. */
 int dem_set_slices(dem_ctx* ctx, int slices);
 
+/* Which pair-feature kernel a DEM_F32 context runs.  DEM_KERNEL_SEARCH (default): the packed-FP32 contact search with
+ * cooperative evaluation of the candidate terms.  DEM_KERNEL_GENERIC: the fused scalar kernel
+ * that DEM_F64 contexts always use (every Eq. 1 / Eq. 2 term evaluated in place).  Both produce the same contributing
+ * terms; sums may differ in rounding order.  Takes effect at the next dem_compute / dem_step. */
+#define DEM_KERNEL_SEARCH 0
+#define DEM_KERNEL_GENERIC 1
+int dem_set_pair_kernel(dem_ctx* ctx, int which);
+
 /* Benchmark hygiene: when bytes > 0, dem_step overwrites a scratch buffer of that size (larger than the 126 MB L2)
  * before every time step, so that no step finds its inputs cached by the previous one.  0 (default) = off. */
 int dem_set_l2_flush(dem_ctx* ctx, int64_t bytes);

@@ -1,0 +1,563 @@
+// dem_fast.cuh -- the FP32 pair-feature kernel of libdem_b200 for sm_100a: packed contact search + cooperative
+// evaluation of the candidate terms.  (The generic k_pair of dem_kernels.cuh stays as the FP64 path.)
+//
+// The paper fuses the nearest-point search and the potential in one kernel and names the resulting register
+// pressure as its bottleneck, with "split contact search from force evaluation" as future work.  On
+// B200 the search is bound by FP32 issue slots, so it is written here with Blackwell's packed FP32 instructions
+// (FFMA2 / FADD2 / FMUL2, PTX fma.rn.f32x2): one lane carries TWO outer features of particle j in the halves of
+// 64-bit registers and sweeps them over the inner features of particle i, which it reads as warp-uniform shared-memory
+// broadcasts (FFMA2 takes a 32-bit register as a broadcast operand).  A packed instruction occupies the FMA pipe
+// for two cycles but takes ONE issue slot, which leaves the slots the clamps, minima, shared-memory loads and loop
+// control need (measured on B200: 8 FFMA2 + 8 FMNMX per 17.8 cycles against 8 FFMA + 4 FMNMX per 12.5).
+//
+//   search  : every Eq. 1 / Eq. 2 term gets its nearest-point distance r*^2
+//             from a branch-free packed formulation; the only output is one bit per packed evaluation,
+//             "some r*^2 < rc_search^2", shifted into a per-lane mask (sign bit of r^2 - rc_search^2, funnel shift).
+//   queue   : after each sweep the lanes of a warp append their flagged (outer, inner) term ids to a warp-private
+//             shared-memory queue (ballot ranks: deterministic order, no atomics).
+//   evaluate: whenever 32 candidates are queued the warp evaluates them TOGETHER, one term per lane, with the exact
+//             scalar routines of dem_math.cuh (parallel-edge rule R5, WCA, force, torque), and hands each
+//             contribution back to the lane that owns the pair with warp shuffles, in queue order.  Contact terms
+//             therefore cost one lane-evaluation each instead of one divergent warp-evaluation each.
+//
+// rc_search is the WCA cutoff plus a slack that covers FP32 rounding of the packed formulation and the error of its
+// segment-segment routine on near-parallel edges, so every term the scalar routine finds inside
+// the cutoff is a candidate; the scalar routine alone decides what contributes.
+#pragma once
+#include "dem_kernels.cuh"
+
+namespace dem {
+
+typedef unsigned long long u64;
+
+__device__ __forceinline__ u64 pk(float lo, float hi) {
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk(u64 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ u64 bc(float x) { return pk(x, x); }  // ptxas folds this into FFMA2's .F32 broadcast operand
+__device__ __forceinline__ u64 neg2(u64 v) {                     // folded into the operand's negate modifier
+    float lo, hi;
+    upk(v, lo, hi);
+    return pk(-lo, -hi);
+}
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
+    u64 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) {
+    u64 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ u64 add2(u64 a, u64 b) {
+    u64 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ float mul_sat(float a, float b) {
+    float r;
+    asm("mul.rn.sat.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
+    return r;
+}
+// shift the sign bit of v into the mask: bit set <=> v < 0
+__device__ __forceinline__ unsigned push_sign(unsigned mask, float v) { return __funnelshift_l(__float_as_uint(v), mask, 1); }
+
+#define DEM_QCAP 96        // 31 left over + at most 64 appended per round
+#define DEM_Q_INVALID 0xffffffffu
+enum { PH_EE = 0, PH_VF_OWN = 1, PH_VF_OTHER = 2, PH_VE_OWN = 3, PH_VE_OTHER = 4 };
+
+// what the cooperative evaluation needs, kept in shared memory (the hot loops hold their own copies in registers)
+struct FastShared {
+    ShapeView<float> A, B;
+    PairConst<float> pc;
+};
+
+__device__ __forceinline__ unsigned q_entry(int lane, int phase, int outer, int inner) {
+    return ((unsigned)lane << 27) | ((unsigned)phase << 24) | ((unsigned)outer << 12) | (unsigned)inner;
+}
+
+// ---- evaluate: up to 32 queued candidates, one per lane -----------------------------------------------------------------
+// q: this warp's queue (qn entries, the first cnt <= 32 are consumed and the rest moved to the front); sacc: this warp's
+// per-lane accumulators [7][32] = (F.xyz, T.xyz, u) in the owner's body frame; scnt: this warp's counters (active,
+// degenerate, parallel).  R*, t*: the CALLING lane's pose; the evaluating lane fetches its owner's with shuffles.
+// Contributions are added to the owner in queue order, so the result does not depend on scheduling.
+__device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* q, float* sacc, unsigned* scnt, int cnt, int qn,
+                                         float R0, float R1, float R2, float R3, float R4, float R5, float R6, float R7,
+                                         float R8, float t0, float t1, float t2) {
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const unsigned e = lane < cnt ? q[lane] : DEM_Q_INVALID;
+    const int rem = qn - cnt;
+    const unsigned v0 = lane < rem ? q[cnt + lane] : 0u, v1 = lane + 32 < rem ? q[cnt + 32 + lane] : 0u;
+    __syncwarp();
+    if (lane < rem) q[lane] = v0;
+    if (lane + 32 < rem) q[32 + lane] = v1;
+    __syncwarp();
+    const int owner = e == DEM_Q_INVALID ? lane : (int)(e >> 27);
+    float R[9], t[3];
+    R[0] = __shfl_sync(full, R0, owner); R[1] = __shfl_sync(full, R1, owner); R[2] = __shfl_sync(full, R2, owner);
+    R[3] = __shfl_sync(full, R3, owner); R[4] = __shfl_sync(full, R4, owner); R[5] = __shfl_sync(full, R5, owner);
+    R[6] = __shfl_sync(full, R6, owner); R[7] = __shfl_sync(full, R7, owner); R[8] = __shfl_sync(full, R8, owner);
+    t[0] = __shfl_sync(full, t0, owner); t[1] = __shfl_sync(full, t1, owner); t[2] = __shfl_sync(full, t2, owner);
+    PairAcc<float> loc;
+    loc.F[0] = loc.F[1] = loc.F[2] = loc.T[0] = loc.T[1] = loc.T[2] = loc.u = 0.f;
+    loc.nactive = loc.ndegen = loc.npar = 0u;
+    if (e != DEM_Q_INVALID) {
+        const int phase = (int)((e >> 24) & 7u), o = (int)((e >> 12) & 0xfffu), k = (int)(e & 0xfffu);
+        const ShapeView<float> A = fs->A, B = fs->B;
+        const PairConst<float> pc = fs->pc;
+        float p[3];
+        if (phase == PH_EE) {
+            float d2[3], ee, inv_e;
+            edge_to_i<float>(B, o, R, t, p, d2, ee, inv_e);
+            term_ee<float>(A, k, p[0], p[1], p[2], d2[0], d2[1], d2[2], ee, inv_e, pc, loc);
+        } else if (phase == PH_VF_OWN) {
+            const f4 v = B.V[o];
+            vertex_to_i<float>(v.x, v.y, v.z, R, t, p);
+            term_vf_own<float>(A, k, p[0], p[1], p[2], pc, loc);
+        } else if (phase == PH_VF_OTHER) {
+            const f4 v = A.V[o];
+            vertex_to_j<float>(v.x, v.y, v.z, R, t, p);
+            term_vf_other<float>(B, k, v.x, v.y, v.z, p[0], p[1], p[2], R, pc, loc);
+        } else if (phase == PH_VE_OWN) {
+            const f4 v = B.V[o];
+            vertex_to_i<float>(v.x, v.y, 0.f, R, t, p);
+            term_ve_own<float>(A, k, p[0], p[1], pc, loc);
+        } else {
+            const f4 v = A.V[o];
+            vertex_to_j<float>(v.x, v.y, 0.f, R, t, p);
+            term_ve_other<float>(B, k, v.x, v.y, p[0], p[1], R, pc, loc);
+        }
+    }
+    const unsigned na = __reduce_add_sync(full, loc.nactive), nd = __reduce_add_sync(full, loc.ndegen),
+                   np = __reduce_add_sync(full, loc.npar);
+    if (lane == 0) {
+        scnt[0] += na;
+        scnt[1] += nd;
+        scnt[2] += np;
+    }
+    unsigned act = __ballot_sync(full, loc.nactive != 0u);
+    while (act) {
+        const int s = __ffs(act) - 1;
+        act &= act - 1;
+        const int ow = __shfl_sync(full, owner, s);
+        const float fx = __shfl_sync(full, loc.F[0], s), fy = __shfl_sync(full, loc.F[1], s),
+                    fz = __shfl_sync(full, loc.F[2], s), tx = __shfl_sync(full, loc.T[0], s),
+                    ty = __shfl_sync(full, loc.T[1], s), tz = __shfl_sync(full, loc.T[2], s),
+                    uu = __shfl_sync(full, loc.u, s);
+        if (lane == ow) {
+            sacc[0 * 32 + lane] += fx; sacc[1 * 32 + lane] += fy; sacc[2 * 32 + lane] += fz;
+            sacc[3 * 32 + lane] += tx; sacc[4 * 32 + lane] += ty; sacc[5 * 32 + lane] += tz;
+            sacc[6 * 32 + lane] += uu;
+        }
+    }
+    __syncwarp();
+}
+
+// per-warp state of the search loops
+struct WarpCtx {
+    const FastShared* fs;
+    unsigned* q;
+    float* sacc;
+    unsigned* scnt;
+    int qn;    // queued candidates (warp-uniform)
+    int lane;
+};
+
+// ---- queue: append the candidates flagged in mask[] and evaluate while a full warp of them is waiting ------------------
+// mask[tau] bit (n - 1 - i) <=> the packed evaluation of inner feature k0 + i against outer features o0 + 2 tau and
+// o0 + 2 tau + 1 flagged a candidate (either half: both terms are queued, the scalar routine sorts them out).
+template <int T>
+__device__ __forceinline__ void push_and_drain(WarpCtx& w, int phase, const unsigned (&mask)[T], int n, int k0, int o0,
+                                               int o_end, const float* R, const float* t) {
+    const unsigned full = 0xffffffffu;
+    const unsigned lt = (1u << w.lane) - 1u;
+#pragma unroll
+    for (int tau = 0; tau < T; ++tau) {
+        unsigned m = mask[tau];
+        const int oa = o0 + 2 * tau, ob = oa + 1;
+        while (__any_sync(full, m != 0u)) {
+            const bool have = m != 0u;
+            const int bit = 31 - __clz((int)m);
+            const int k = k0 + (n - 1 - bit);
+            if (have) m &= ~(1u << bit);
+            const bool ha = have && oa < o_end, hb = have && ob < o_end;
+            const unsigned ba = __ballot_sync(full, ha), bb = __ballot_sync(full, hb);
+            const int na = __popc(ba);
+            if (ha) w.q[w.qn + __popc(ba & lt)] = q_entry(w.lane, phase, oa, k);
+            if (hb) w.q[w.qn + na + __popc(bb & lt)] = q_entry(w.lane, phase, ob, k);
+            w.qn += na + __popc(bb);
+            __syncwarp();
+            while (w.qn >= 32) {
+                drain_terms(w.fs, w.q, w.sacc, w.scnt, 32, w.qn, R[0], R[1], R[2], R[3], R[4], R[5], R[6], R[7], R[8],
+                            t[0], t[1], t[2]);
+                w.qn -= 32;
+            }
+        }
+    }
+}
+
+// ---- search: packed nearest-point distances ---------------------------------------------------------------------------
+// Segment-segment (first sum of Eq. 1): inner edge of i as scalars e0 = (p1, |d1|^2), e1 = (d1, 1/|d1|^2), parameter
+// s in [0,1]; two outer edges of j packed, unit directions d2, parameter t in [0, L2] (length units), np2 = -p2.
+// Closest points of the two lines from the normal equations, then the textbook clamp cascade with the second clamp of
+// s taken unconditionally (KKT: when t was not clamped it reproduces s).  Returns min over the two halves of
+// r^2 - rc_search^2.  Near-parallel edges (|d1 x d2|^2 -> 0) make s inaccurate but never out of [0,1], and t, s2 are
+// then exact for that s, so r is off by at most sin(angle) x edge length: covered by rc_search's slack.
+__device__ __forceinline__ float ee_eval(const f4 e0, const f4 e1, u64 np2x, u64 np2y, u64 np2z, u64 d2x, u64 d2y,
+                                         u64 d2z, float Llo, float Lhi, float nrc2) {
+    const u64 rx = add2(bc(e0.x), np2x), ry = add2(bc(e0.y), np2y), rz = add2(bc(e0.z), np2z);  // r = p1 - p2
+    const u64 b = fma2(bc(e1.z), d2z, fma2(bc(e1.y), d2y, mul2(bc(e1.x), d2x)));              // d1 . d2
+    const u64 c = fma2(bc(e1.z), rz, fma2(bc(e1.y), ry, mul2(bc(e1.x), rx)));                 // d1 . r
+    const u64 f = fma2(d2z, rz, fma2(d2y, ry, mul2(d2x, rx)));                                // d2 . r
+    const u64 nn = fma2(neg2(b), b, bc(e0.w));                                                // |d1|^2 - b^2
+    const u64 num = fma2(b, f, neg2(c));
+    float nl, nh, ul, uh;
+    upk(nn, nl, nh);
+    upk(num, ul, uh);
+    const u64 s = pk(mul_sat(ul, rcp(nl)), mul_sat(uh, rcp(nh)));
+    float xl, xh;
+    upk(fma2(b, s, f), xl, xh);
+    const u64 tt = pk(fminf(fmaxf(xl, 0.f), Llo), fminf(fmaxf(xh, 0.f), Lhi));
+    float yl, yh;
+    upk(fma2(b, tt, neg2(c)), yl, yh);
+    const u64 s2 = pk(mul_sat(yl, e1.w), mul_sat(yh, e1.w)), ntt = neg2(tt);
+    const u64 dx = fma2(ntt, d2x, fma2(s2, bc(e1.x), rx));
+    const u64 dy = fma2(ntt, d2y, fma2(s2, bc(e1.y), ry));
+    const u64 dz = fma2(ntt, d2z, fma2(s2, bc(e1.z), rz));
+    float lo, hi;
+    upk(fma2(dx, dx, fma2(dy, dy, fma2(dz, dz, bc(nrc2)))), lo, hi);
+    return fminf(lo, hi);
+}
+
+// One boundary edge (or 2D edge) e0 = (., ., ux, uy), e1 = (len, cs, cu, .) against two packed points (x, y):
+// side = u x q + cs (>= 0 on the inner side), along = u . q + cu, excess = max(-along, along - len, 0).
+__device__ __forceinline__ void edge2_eval(const f4 e0, const f4 e1, u64 x, u64 y, u64& side, u64& exc) {
+    side = fma2(bc(e0.z), y, fma2(bc(-e0.w), x, bc(e1.y)));
+    const u64 al = fma2(bc(e0.z), x, fma2(bc(e0.w), y, bc(e1.z)));
+    const u64 over = add2(al, bc(-e1.x));
+    float al_l, al_h, ov_l, ov_h;
+    upk(al, al_l, al_h);
+    upk(over, ov_l, ov_h);
+    exc = pk(fmaxf(fmaxf(-al_l, ov_l), 0.f), fmaxf(fmaxf(-al_h, ov_h), 0.f));
+}
+
+// Point against closed convex polygon face (R1/R2): two packed points against face header F[0..2] and its M boundary
+// edges.  r^2 = h^2 + (inside ? 0 : min over edges of side^2 + excess^2).  Updates mask[tau] for T packed point pairs.
+template <int T, int M>
+__device__ __forceinline__ void face_eval(const f4* __restrict__ F, const f4* __restrict__ FE, int m_rt, const u64 (&px)[T],
+                                          const u64 (&py)[T], const u64 (&pz)[T], float nrc2, unsigned (&mask)[T]) {
+    const f4 f0 = F[0], f1 = F[1], f2 = F[2];
+    u64 x[T], y[T], hh[T];
+    float smin_l[T], smin_h[T], dmin_l[T], dmin_h[T];
+#pragma unroll
+    for (int tau = 0; tau < T; ++tau) {
+        x[tau] = fma2(bc(f0.z), pz[tau], fma2(bc(f0.y), py[tau], fma2(bc(f0.x), px[tau], bc(f0.w))));
+        y[tau] = fma2(bc(f1.z), pz[tau], fma2(bc(f1.y), py[tau], fma2(bc(f1.x), px[tau], bc(f1.w))));
+        const u64 h = fma2(bc(f2.z), pz[tau], fma2(bc(f2.y), py[tau], fma2(bc(f2.x), px[tau], bc(f2.w))));
+        hh[tau] = fma2(h, h, bc(nrc2));
+        smin_l[tau] = smin_h[tau] = dmin_l[tau] = dmin_h[tau] = 1e30f;
+    }
+    const int mcount = M > 0 ? M : m_rt;
+#pragma unroll
+    for (int m = 0; m < mcount; ++m) {
+        const f4 e0 = FE[2 * m], e1 = FE[2 * m + 1];
+#pragma unroll
+        for (int tau = 0; tau < T; ++tau) {
+            u64 side, exc;
+            edge2_eval(e0, e1, x[tau], y[tau], side, exc);
+            float sl, sh, dl, dh;
+            upk(side, sl, sh);
+            upk(fma2(exc, exc, mul2(side, side)), dl, dh);
+            smin_l[tau] = fminf(smin_l[tau], sl);
+            smin_h[tau] = fminf(smin_h[tau], sh);
+            dmin_l[tau] = fminf(dmin_l[tau], dl);
+            dmin_h[tau] = fminf(dmin_h[tau], dh);
+        }
+    }
+#pragma unroll
+    for (int tau = 0; tau < T; ++tau) {
+        const u64 sel = pk(smin_l[tau] >= 0.f ? 0.f : dmin_l[tau], smin_h[tau] >= 0.f ? 0.f : dmin_h[tau]);
+        float lo, hi;
+        upk(add2(hh[tau], sel), lo, hi);
+        mask[tau] = push_sign(mask[tau], fminf(lo, hi));
+    }
+}
+
+// sweep T packed pairs of points over faces [f0, f1) of shape S (at most 32 faces: one mask bit each)
+template <int T>
+__device__ __forceinline__ void sweep_faces(const ShapeView<float>& S, int f0, int f1, const u64 (&px)[T], const u64 (&py)[T],
+                                            const u64 (&pz)[T], float nrc2, unsigned (&mask)[T]) {
+    for (int f = f0; f < f1; ++f) {
+        const f4* F = S.F + 4 * f;
+        const f4 f3 = F[3];
+        const int m0 = (int)f3.x, mc = (int)f3.y;
+        const f4* FE = S.FE + 2 * m0;
+        switch (mc) {
+            case 3: face_eval<T, 3>(F, FE, 3, px, py, pz, nrc2, mask); break;
+            case 4: face_eval<T, 4>(F, FE, 4, px, py, pz, nrc2, mask); break;
+            case 5: face_eval<T, 5>(F, FE, 5, px, py, pz, nrc2, mask); break;
+            case 6: face_eval<T, 6>(F, FE, 6, px, py, pz, nrc2, mask); break;
+            default: face_eval<T, 0>(F, FE, mc, px, py, pz, nrc2, mask); break;
+        }
+    }
+}
+
+// ---- the kernel ---------------------------------------------------------------------------------------------------------
+// One warp = 32 consecutive (pair, slice) items of one pair class (same shapes, same loop bounds).  TE / TV = packed
+// outer pairs per sweep for edges / vertices (2 TE outer edges, 2 TV outer vertices share every inner-feature load).
+template <typename PosT, int DIM, int TE, int TV>
+__global__ void __launch_bounds__(128, 3) k_pair_fast(const PairArgs<float> a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    FastShared* fs = reinterpret_cast<FastShared*>(smem_raw);
+    unsigned* queue = reinterpret_cast<unsigned*>(smem_raw + 256);  // 4 warps x DEM_QCAP
+    float* sacc_all = reinterpret_cast<float*>(queue + 4 * DEM_QCAP);  // 4 warps x 7 x 32
+    unsigned* scnt_all = reinterpret_cast<unsigned*>(sacc_all + 4 * 7 * 32);  // 4 warps x 4
+    f4* sm = reinterpret_cast<f4*>(scnt_all + 16);
+    static_assert(sizeof(FastShared) <= 256, "FastShared header");
+    // stage the shape-feature tables of the class (a1) into shared memory
+    const bool same = a.sa.off == a.sb.off;
+    for (int k = threadIdx.x; k < a.sa.len; k += blockDim.x) sm[k] = a.table[a.sa.off + k];
+    if (!same)
+        for (int k = threadIdx.x; k < a.sb.len; k += blockDim.x) sm[a.sa.len + k] = a.table[a.sb.off + k];
+    ShapeView<float> A, B;
+    A.nv = a.sa.nv; A.ne = a.sa.ne; A.nf = a.sa.nf;
+    A.V = sm; A.E = A.V + A.nv; A.F = A.E + 2 * A.ne; A.FE = A.F + 4 * A.nf; A.OE = A.FE + 2 * a.sa.nfe;
+    B.nv = a.sb.nv; B.ne = a.sb.ne; B.nf = a.sb.nf;
+    B.V = same ? sm : sm + a.sa.len; B.E = B.V + B.nv; B.F = B.E + 2 * B.ne; B.FE = B.F + 4 * B.nf;
+    B.OE = B.FE + 2 * a.sb.nfe;
+    if (threadIdx.x == 0) {
+        fs->A = A;
+        fs->B = B;
+        fs->pc = a.pc;
+    }
+    if (threadIdx.x < 16) scnt_all[threadIdx.x] = 0u;
+    __syncthreads();
+
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpCtx w;
+    w.fs = fs;
+    w.q = queue + warp * DEM_QCAP;
+    w.sacc = sacc_all + warp * 7 * 32;
+    w.scnt = scnt_all + warp * 4;
+    w.qn = 0;
+    w.lane = lane;
+    const float nrc2 = -a.rc2_search;
+    const int np_pad = (a.npairs + 31) & ~31;  // slices are warp-uniform
+    const long long n_wtiles = (long long)(np_pad >> 5) * a.slices;
+    unsigned c_eval = 0;
+    for (long long wt = (long long)blockIdx.x * 4 + warp; wt < n_wtiles; wt += (long long)gridDim.x * 4) {
+        const long long item = wt * 32 + lane;
+        const int slice = (int)(item / np_pad), p = (int)(item - (long long)slice * np_pad);
+        const bool in_list = p < a.npairs;
+        bool valid = false;
+        double d[3] = {0.0, 0.0, 0.0};
+        float Mi[9], R[9], t[3];
+        if (in_list) {
+            const int2 ij = a.pairs[p];
+            const d4 xi = load4d(static_cast<const PosT*>(a.pos), ij.x), xj = load4d(static_cast<const PosT*>(a.pos), ij.y);
+            d[0] = min_image_1(xi.x, xj.x, a.box.L[0]);
+            d[1] = min_image_1(xi.y, xj.y, a.box.L[1]);
+            d[2] = DIM == 3 ? min_image_1(xi.z, xj.z, a.box.L[2]) : 0.0;
+            valid = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] < a.reach2;
+            if (valid) {
+                const d4 qi = load4d(static_cast<const PosT*>(a.quat), ij.x), qj = load4d(static_cast<const PosT*>(a.quat), ij.y);
+                const double qa[4] = {qi.x, qi.y, qi.z, qi.w}, qb[4] = {qj.x, qj.y, qj.z, qj.w};
+                pair_pose<float>(qa, qb, d, Mi, R, t);
+            }
+        }
+        if (!valid) {  // lanes without work sweep a far-away dummy so that the warp stays converged
+#pragma unroll
+            for (int k = 0; k < 9; ++k) Mi[k] = R[k] = (k % 4 == 0) ? 1.f : 0.f;
+            t[0] = t[1] = 1.0e4f;
+            t[2] = DIM == 3 ? 1.0e4f : 0.f;
+        }
+        float out[10];
+#pragma unroll
+        for (int k = 0; k < 10; ++k) out[k] = 0.f;
+        if (__any_sync(full, valid)) {
+            c_eval += (valid && slice == 0) ? 1u : 0u;
+#pragma unroll
+            for (int k = 0; k < 7; ++k) w.sacc[k * 32 + lane] = 0.f;
+            const int ob = (int)((long long)slice * a.n_outer / a.slices);
+            const int oe = (int)((long long)(slice + 1) * a.n_outer / a.slices);
+            if (DIM == 3) {
+                const int oE = B.ne, oV = B.ne + B.nv;
+                // (1) first sum of Eq. 1: edges of j (outer, packed) against edges of i (inner)
+                for (int l0 = ob, le = min(oe, oE); l0 < le; l0 += 2 * TE) {
+                    for (int k0 = 0; k0 < A.ne; k0 += 32) {
+                        u64 np2x[TE], np2y[TE], np2z[TE], d2x[TE], d2y[TE], d2z[TE];
+                        float Llo[TE], Lhi[TE];
+#pragma unroll
+                        for (int tau = 0; tau < TE; ++tau) {
+                            const int la = min(l0 + 2 * tau, le - 1), lb = min(l0 + 2 * tau + 1, le - 1);
+                            const f4 a0 = B.OE[2 * la], a1 = B.OE[2 * la + 1], b0 = B.OE[2 * lb], b1 = B.OE[2 * lb + 1];
+                            float pa[3], pb[3];
+                            vertex_to_i<float>(a0.x, a0.y, a0.z, R, t, pa);
+                            vertex_to_i<float>(b0.x, b0.y, b0.z, R, t, pb);
+                            np2x[tau] = pk(-pa[0], -pb[0]);
+                            np2y[tau] = pk(-pa[1], -pb[1]);
+                            np2z[tau] = pk(-pa[2], -pb[2]);
+                            d2x[tau] = pk(R[0] * a1.x + R[1] * a1.y + R[2] * a1.z, R[0] * b1.x + R[1] * b1.y + R[2] * b1.z);
+                            d2y[tau] = pk(R[3] * a1.x + R[4] * a1.y + R[5] * a1.z, R[3] * b1.x + R[4] * b1.y + R[5] * b1.z);
+                            d2z[tau] = pk(R[6] * a1.x + R[7] * a1.y + R[8] * a1.z, R[6] * b1.x + R[7] * b1.y + R[8] * b1.z);
+                            Llo[tau] = a0.w;
+                            Lhi[tau] = b0.w;
+                        }
+                        const int k1 = min(k0 + 32, A.ne);
+                        unsigned mask[TE];
+#pragma unroll
+                        for (int tau = 0; tau < TE; ++tau) mask[tau] = 0u;
+                        for (int k = k0; k < k1; ++k) {
+                            const f4 e0 = A.E[2 * k], e1 = A.E[2 * k + 1];
+#pragma unroll
+                            for (int tau = 0; tau < TE; ++tau)
+                                mask[tau] = push_sign(mask[tau], ee_eval(e0, e1, np2x[tau], np2y[tau], np2z[tau], d2x[tau],
+                                                                         d2y[tau], d2z[tau], Llo[tau], Lhi[tau], nrc2));
+                        }
+                        unsigned any = 0u;
+#pragma unroll
+                        for (int tau = 0; tau < TE; ++tau) any |= mask[tau];
+                        if (__any_sync(full, any != 0u)) push_and_drain<TE>(w, PH_EE, mask, k1 - k0, k0, l0, le, R, t);
+                    }
+                }
+                // (2) third sum of Eq. 1: vertices of j (outer, packed, i's frame) against faces of i
+                for (int o0 = max(ob, oE) - oE, on = min(oe, oV) - oE; o0 < on; o0 += 2 * TV) {
+                    for (int f0 = 0; f0 < A.nf; f0 += 32) {
+                        u64 px[TV], py[TV], pz[TV];
+#pragma unroll
+                        for (int tau = 0; tau < TV; ++tau) {
+                            const f4 va = B.V[min(o0 + 2 * tau, on - 1)], vb = B.V[min(o0 + 2 * tau + 1, on - 1)];
+                            float pa[3], pb[3];
+                            vertex_to_i<float>(va.x, va.y, va.z, R, t, pa);
+                            vertex_to_i<float>(vb.x, vb.y, vb.z, R, t, pb);
+                            px[tau] = pk(pa[0], pb[0]);
+                            py[tau] = pk(pa[1], pb[1]);
+                            pz[tau] = pk(pa[2], pb[2]);
+                        }
+                        const int f1 = min(f0 + 32, A.nf);
+                        unsigned mask[TV];
+#pragma unroll
+                        for (int tau = 0; tau < TV; ++tau) mask[tau] = 0u;
+                        sweep_faces<TV>(A, f0, f1, px, py, pz, nrc2, mask);
+                        unsigned any = 0u;
+#pragma unroll
+                        for (int tau = 0; tau < TV; ++tau) any |= mask[tau];
+                        if (__any_sync(full, any != 0u)) push_and_drain<TV>(w, PH_VF_OWN, mask, f1 - f0, f0, o0, on, R, t);
+                    }
+                }
+                // (3) second sum of Eq. 1: vertices of i (outer, packed, j's frame) against faces of j
+                for (int o0 = max(ob, oV) - oV, on = min(oe, oV + A.nv) - oV; o0 < on; o0 += 2 * TV) {
+                    for (int f0 = 0; f0 < B.nf; f0 += 32) {
+                        u64 px[TV], py[TV], pz[TV];
+#pragma unroll
+                        for (int tau = 0; tau < TV; ++tau) {
+                            const f4 va = A.V[min(o0 + 2 * tau, on - 1)], vb = A.V[min(o0 + 2 * tau + 1, on - 1)];
+                            float pa[3], pb[3];
+                            vertex_to_j<float>(va.x, va.y, va.z, R, t, pa);
+                            vertex_to_j<float>(vb.x, vb.y, vb.z, R, t, pb);
+                            px[tau] = pk(pa[0], pb[0]);
+                            py[tau] = pk(pa[1], pb[1]);
+                            pz[tau] = pk(pa[2], pb[2]);
+                        }
+                        const int f1 = min(f0 + 32, B.nf);
+                        unsigned mask[TV];
+#pragma unroll
+                        for (int tau = 0; tau < TV; ++tau) mask[tau] = 0u;
+                        sweep_faces<TV>(B, f0, f1, px, py, pz, nrc2, mask);
+                        unsigned any = 0u;
+#pragma unroll
+                        for (int tau = 0; tau < TV; ++tau) any |= mask[tau];
+                        if (__any_sync(full, any != 0u)) push_and_drain<TV>(w, PH_VF_OTHER, mask, f1 - f0, f0, o0, on, R, t);
+                    }
+                }
+            } else {
+                // Eq. 2: vertices of j against edges of i (i's frame), then vertices of i against edges of j (j's frame)
+#pragma unroll
+                for (int side = 0; side < 2; ++side) {
+                    const ShapeView<float>& In = side == 0 ? A : B;    // owner of the inner edges
+                    const ShapeView<float>& Out = side == 0 ? B : A;   // owner of the outer vertices
+                    const int base = side == 0 ? 0 : B.nv;
+                    for (int o0 = max(ob, base) - base, on = min(oe, base + Out.nv) - base; o0 < on; o0 += 2 * TV) {
+                        for (int k0 = 0; k0 < In.ne; k0 += 32) {
+                            u64 px[TV], py[TV];
+#pragma unroll
+                            for (int tau = 0; tau < TV; ++tau) {
+                                const f4 va = Out.V[min(o0 + 2 * tau, on - 1)], vb = Out.V[min(o0 + 2 * tau + 1, on - 1)];
+                                float pa[3], pb[3];
+                                if (side == 0) {
+                                    vertex_to_i<float>(va.x, va.y, 0.f, R, t, pa);
+                                    vertex_to_i<float>(vb.x, vb.y, 0.f, R, t, pb);
+                                } else {
+                                    vertex_to_j<float>(va.x, va.y, 0.f, R, t, pa);
+                                    vertex_to_j<float>(vb.x, vb.y, 0.f, R, t, pb);
+                                }
+                                px[tau] = pk(pa[0], pb[0]);
+                                py[tau] = pk(pa[1], pb[1]);
+                            }
+                            const int k1 = min(k0 + 32, In.ne);
+                            unsigned mask[TV];
+#pragma unroll
+                            for (int tau = 0; tau < TV; ++tau) mask[tau] = 0u;
+                            for (int k = k0; k < k1; ++k) {
+                                const f4 e0 = In.E[2 * k], e1 = In.E[2 * k + 1];
+#pragma unroll
+                                for (int tau = 0; tau < TV; ++tau) {
+                                    u64 sd, exc;
+                                    edge2_eval(e0, e1, px[tau], py[tau], sd, exc);
+                                    float lo, hi;
+                                    upk(fma2(exc, exc, fma2(sd, sd, bc(nrc2))), lo, hi);
+                                    mask[tau] = push_sign(mask[tau], fminf(lo, hi));
+                                }
+                            }
+                            unsigned any = 0u;
+#pragma unroll
+                            for (int tau = 0; tau < TV; ++tau) any |= mask[tau];
+                            if (__any_sync(full, any != 0u))
+                                push_and_drain<TV>(w, side == 0 ? PH_VE_OWN : PH_VE_OTHER, mask, k1 - k0, k0, o0, on, R, t);
+                        }
+                    }
+                }
+            }
+            if (w.qn > 0) {
+                drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, R[0], R[1], R[2], R[3], R[4], R[5], R[6], R[7], R[8], t[0],
+                            t[1], t[2]);
+                w.qn = 0;
+            }
+            float F[3], T[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                F[k] = w.sacc[k * 32 + lane];
+                T[k] = w.sacc[(3 + k) * 32 + lane];
+            }
+            if (valid) pair_finish<float>(Mi, t, F, T, w.sacc[6 * 32 + lane], out);
+        }
+        if (in_list) {
+            f4* rec = a.rec + 4 * ((size_t)p * a.slices + slice);
+            f4 r0, r1, r2, r3;
+            r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
+            r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = (float)d[0];
+            r2.x = out[6]; r2.y = out[7]; r2.z = out[8]; r2.w = (float)d[1];
+            r3.x = (float)d[2]; r3.y = r3.z = r3.w = 0.f;
+            rec[0] = r0; rec[1] = r1; rec[2] = r2; rec[3] = r3;
+        }
+    }
+    // counters: one atomic per warp per counter, after the hot loop
+    c_eval = __reduce_add_sync(full, c_eval);
+    __syncwarp();
+    if (lane == 0) {
+        if (c_eval) atomicAdd(a.counters + 0, (unsigned long long)c_eval);
+        if (w.scnt[0]) atomicAdd(a.counters + 1, (unsigned long long)w.scnt[0]);
+        if (w.scnt[1]) atomicAdd(a.counters + 2, (unsigned long long)w.scnt[1]);
+        if (w.scnt[2]) atomicAdd(a.counters + 3, (unsigned long long)w.scnt[2]);
+    }
+}
+
+// bytes of dynamic shared memory k_pair_fast needs in front of the staged tables
+static inline size_t fast_smem_header() { return 256 + sizeof(unsigned) * 4 * DEM_QCAP + sizeof(float) * 4 * 7 * 32 + sizeof(unsigned) * 16; }
+
+}  // namespace dem

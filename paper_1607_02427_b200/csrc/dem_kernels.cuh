@@ -278,6 +278,7 @@ template <typename real> struct PairArgs {
     BoxDev box;
     double reach2;        // (R_a + R_b + 2^(1/6) sigma)^2 : beyond it no term can be inside the cutoff (exact, R10)
     PairConst<real> pc;
+    real rc2_search;      // FP32 search kernel: squared candidate cutoff (WCA cutoff + slack, dem_fast.cuh)
     unsigned long long* counters;  // [0] pairs evaluated, [1] active, [2] degenerate, [3] parallel
 };
 
@@ -294,9 +295,10 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
     __syncthreads();
     ShapeView<real> A, B;
     A.nv = a.sa.nv; A.ne = a.sa.ne; A.nf = a.sa.nf;
-    A.V = sm; A.E = A.V + A.nv; A.F = A.E + 2 * A.ne; A.FE = A.F + 4 * A.nf;
+    A.V = sm; A.E = A.V + A.nv; A.F = A.E + 2 * A.ne; A.FE = A.F + 4 * A.nf; A.OE = A.FE + 2 * a.sa.nfe;
     B.nv = a.sb.nv; B.ne = a.sb.ne; B.nf = a.sb.nf;
     B.V = same ? sm : sm + a.sa.len; B.E = B.V + B.nv; B.F = B.E + 2 * B.ne; B.FE = B.F + 4 * B.nf;
+    B.OE = B.FE + 2 * a.sb.nfe;
 
     const int np_pad = (a.npairs + 31) & ~31;  // slices are warp-uniform
     const long long n_items = (long long)np_pad * a.slices;

@@ -9,8 +9,11 @@
 #include <vector>
 
 #include "../../include/dem.h"
+#include "dem_fast.cuh"
 #include "dem_kernels.cuh"
 #include "dem_shape.h"
+
+#include <type_traits>
 
 using namespace dem;
 
@@ -60,6 +63,7 @@ struct dem_ctx {
     int class_sa[DEM_MAX_CLASSES], class_sb[DEM_MAX_CLASSES], class_np[DEM_MAX_CLASSES];
     long long npairs_total = 0, nrec_total = 0;
     int force_slices = 0;  // 0 = heuristic
+    bool generic_kernel = false;  // DEM_F32 contexts: use the generic k_pair instead of the packed search kernel
     size_t l2_flush_bytes = 0;  // bench hygiene: overwrite this many bytes of scratch before every time step
     DevBuf l2_scratch;
     // dem_step state (double) for DEM_F32 contexts, plus forces and the positions of the last build
@@ -363,11 +367,30 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
         a.pc.eps_par = (real)ctx->eps_par;
         a.pc.degen2 = (real)((1e-6 * sigma) * (1e-6 * sigma));
         a.counters = ctx->counters.as<unsigned long long>();
-        const size_t smem = sizeof(real4) * (size_t)(a.sa.len + (a.sa.off == a.sb.off ? 0 : a.sb.len));
+        // candidate cutoff of the FP32 search kernel: FP32 rounding of the packed formulation (1e-3 relative) plus
+        // its error on near-parallel edges, at most sin(angle) x edge length with the angle below ~1e-3 where the
+        // line-line solve loses its digits; 4e-3 x longest edge leaves a factor 4
+        const double rc = std::pow(2.0, 1.0 / 6.0) * sigma;
+        const double rcs = rc * (1.0 + 1e-3) + (ctx->dim == 3 ? 4e-3 * std::max(HA.max_edge, HB.max_edge) : 0.0);
+        a.rc2_search = (real)(rcs * rcs);
+        size_t smem = sizeof(real4) * (size_t)(a.sa.len + (a.sa.off == a.sb.off ? 0 : a.sb.len));
         const long long items = (long long)((np + 31) & ~31) * a.slices;
         const int threads = 128;
         const int grid = (int)std::min<long long>(nblk(items, threads), (long long)ctx->sm_count * 64);
-        auto kern = ctx->dim == 3 ? k_pair<real, PosT, 3> : k_pair<real, PosT, 2>;
+        void (*kern)(const PairArgs<real>) = ctx->dim == 3 ? k_pair<real, PosT, 3> : k_pair<real, PosT, 2>;
+        if constexpr (std::is_same<real, float>::value) {
+            if (!ctx->generic_kernel) {
+                smem += fast_smem_header();
+                // packed outer pairs per sweep: 3 when the vertex counts fill tiles of 6 at least as well as tiles of 4
+                auto waste = [](int n, int tile) { return ((n + tile - 1) / tile) * tile - n; };
+                const int nva = HA.nv, nvb = HB.nv;
+                const bool tv3 = waste(nva, 6) + waste(nvb, 6) <= waste(nva, 4) + waste(nvb, 4);
+                if (ctx->dim == 3)
+                    kern = tv3 ? k_pair_fast<PosT, 3, 2, 3> : k_pair_fast<PosT, 3, 2, 2>;
+                else
+                    kern = tv3 ? k_pair_fast<PosT, 2, 2, 3> : k_pair_fast<PosT, 2, 2, 2>;
+            }
+        }
         if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         cudaEvent_t e0 = nullptr, e1 = nullptr;
         if (ctx->timing) {
@@ -535,6 +558,12 @@ int dem_set_slices(dem_ctx* ctx, int slices) {
     if (!ctx || slices < 0) return fail(ctx, DEM_EINVAL, "slices must be >= 0");
     ctx->force_slices = slices;
     ctx->have_list = false;
+    return DEM_OK;
+}
+
+int dem_set_pair_kernel(dem_ctx* ctx, int which) {
+    if (!ctx || (which != DEM_KERNEL_SEARCH && which != DEM_KERNEL_GENERIC)) return fail(ctx, DEM_EINVAL, "unknown pair kernel");
+    ctx->generic_kernel = which == DEM_KERNEL_GENERIC;
     return DEM_OK;
 }
 

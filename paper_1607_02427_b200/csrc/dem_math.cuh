@@ -64,9 +64,11 @@ DEM_HD double rcp(double x) { return 1.0 / x; }
 // two shapes of its class into shared memory and builds these views over them.
 //   V [nv]      (x, y, z, 0)                                   body-frame vertex
 //   E [2 ne]    3D: [2k] = (a.xyz, |e|^2)  [2k+1] = (e.xyz, 1/|e|^2 or 0 if |e| = 0)      edge k = a + s e, s in [0,1]
-//               2D: [2k] = (a.x, a.y, u.x, u.y)  [2k+1] = (|e|, 0, 0, 0)                    u = e/|e| (0 if |e| = 0)
+//               2D: [2k] = (a.x, a.y, u.x, u.y)  [2k+1] = (|e|, cs, cu, 0)                  u = e/|e| (0 if |e| = 0)
+//                   cs = -(u x a), cu = -(u . a): for a point q, side = u x q + cs and along = u . q + cu
 //   F [4 nf]    [4f] = (uhat, -uhat.o) [4f+1] = (vhat, -vhat.o) [4f+2] = (nhat, -nhat.o) [4f+3] = (first FE, count, 0, 0)
 //   FE[2 nfe]   face boundary edges in the face's (uhat, vhat) coordinates, CCW about nhat: same layout as 2D edges
+//   OE[2 ne]    3D only: [2k] = (a.xyz, |e|)  [2k+1] = (e/|e|, 0): the edges as the search kernel's outer features
 template <typename real> struct ShapeView {
     typedef typename vec4<real>::type real4;
     int nv, ne, nf;
@@ -74,6 +76,7 @@ template <typename real> struct ShapeView {
     const real4* E;
     const real4* F;
     const real4* FE;
+    const real4* OE;
 };
 
 template <typename real> struct PairAcc {
@@ -230,6 +233,122 @@ DEM_HD_NOINLINE bool segseg_special(real rx, real ry, real rz, real d1x, real d1
     return false;
 }
 
+// ---- single Eq. 1 / Eq. 2 terms -------------------------------------------------------------------------------------
+// One term each, with the outer feature already brought into the frame of the inner feature's owner.  The pair loops
+// below call them for every term; the FP32 search kernel (dem_fast.cuh) calls them only for the terms its packed
+// search flags as candidates, so both paths share the arithmetic of every contributing term.
+
+// edge (p2, d2, e = |d2|^2, inv_e) of j in i's frame against edge k of i (first sum of Eq. 1)
+template <typename real>
+DEM_HD void term_ee(const ShapeView<real>& A, int k, real p2x, real p2y, real p2z, real d2x, real d2y, real d2z, real e,
+                    real inv_e, const PairConst<real>& pc, PairAcc<real>& acc) {
+    typedef typename vec4<real>::type real4;
+    const real4 a0 = A.E[2 * k], a1 = A.E[2 * k + 1];
+    const real rx = a0.x - p2x, ry = a0.y - p2y, rz = a0.z - p2z;  // r = p1 - p2
+    const real nx = a1.y * d2z - a1.z * d2y, ny = a1.z * d2x - a1.x * d2z, nz = a1.x * d2y - a1.y * d2x;
+    const real nn = nx * nx + ny * ny + nz * nz;
+    real s, tt;
+    bool par = false;
+    if (nn <= pc.eps_par * e * a0.w) {
+        par = segseg_special<real>(rx, ry, rz, a1.x, a1.y, a1.z, a0.w, d2x, d2y, d2z, e, nn, pc.eps_par, s, tt);
+    } else {
+        // skew lines: s = -(d1 x d2).(r x d2) / |d1 x d2|^2 (no cancellation near parallel), then the textbook
+        // clamp cascade written branch-free
+        const real qx = ry * d2z - rz * d2y, qy = rz * d2x - rx * d2z, qz = rx * d2y - ry * d2x;
+        s = sat01(-(nx * qx + ny * qy + nz * qz) * rcp(nn));
+        const real b = a1.x * d2x + a1.y * d2y + a1.z * d2z;
+        const real f = d2x * rx + d2y * ry + d2z * rz;
+        const real c = a1.x * rx + a1.y * ry + a1.z * rz;
+        const real tu = (b * s + f) * inv_e;
+        tt = sat01(tu);
+        const real s2 = sat01((b * tt - c) * a1.w);
+        s = (tu != tt) ? s2 : s;
+    }
+    const real dx = rx + s * a1.x - tt * d2x, dy = ry + s * a1.y - tt * d2y, dz = rz + s * a1.z - tt * d2z;
+    const real r2 = dx * dx + dy * dy + dz * dz;
+    if (r2 < pc.rc2)
+        wca_accumulate<real>(pc, acc, a0.x + s * a1.x, a0.y + s * a1.y, a0.z + s * a1.z, dx, dy, dz, r2, par);
+}
+
+// vertex p of j (in i's frame) against face f of i (third sum of Eq. 1)
+template <typename real>
+DEM_HD void term_vf_own(const ShapeView<real>& A, int f, real px, real py, real pz, const PairConst<real>& pc,
+                        PairAcc<real>& acc) {
+    const real r2 = point_face_r2<real>(A, f, px, py, pz);
+    if (r2 < pc.rc2) {
+        real dx, dy, dz;  // p - c with c on i's face: c_i = c, c_j = p, del = c_i - c_j = -(p - c)
+        point_face_del<real>(A, f, px, py, pz, dx, dy, dz);
+        wca_accumulate<real>(pc, acc, px - dx, py - dy, pz - dz, -dx, -dy, -dz, r2, false);
+    }
+}
+
+// vertex v of i (body frame; p = R^T (v - t) is the same vertex in j's frame) against face f of j (second sum of Eq. 1)
+template <typename real>
+DEM_HD void term_vf_other(const ShapeView<real>& B, int f, real vx, real vy, real vz, real px, real py, real pz,
+                          const real* R, const PairConst<real>& pc, PairAcc<real>& acc) {
+    const real r2 = point_face_r2<real>(B, f, px, py, pz);
+    if (r2 < pc.rc2) {
+        real dx, dy, dz;  // p' - c' in j's frame; c_i = the vertex, del = c_i - c_j = R (p' - c')
+        point_face_del<real>(B, f, px, py, pz, dx, dy, dz);
+        wca_accumulate<real>(pc, acc, vx, vy, vz, R[0] * dx + R[1] * dy + R[2] * dz, R[3] * dx + R[4] * dy + R[5] * dz,
+                             R[6] * dx + R[7] * dy + R[8] * dz, r2, false);
+    }
+}
+
+// 2D: vertex p of j (i's frame) against edge k of i
+template <typename real>
+DEM_HD void term_ve_own(const ShapeView<real>& A, int k, real px, real py, const PairConst<real>& pc,
+                        PairAcc<real>& acc) {
+    typedef typename vec4<real>::type real4;
+    const real4 e0 = A.E[2 * k];
+    const real len = A.E[2 * k + 1].x;
+    real ddx, ddy;
+    const real r2 = point_edge2<real>(px, py, e0.x, e0.y, e0.z, e0.w, len, ddx, ddy);
+    if (r2 < pc.rc2)  // c_i = p - dd on i's edge, c_j = p, del = -dd
+        wca_accumulate<real>(pc, acc, px - ddx, py - ddy, real(0), -ddx, -ddy, real(0), r2, false);
+}
+
+// 2D: vertex v of i (p = the same vertex in j's frame) against edge l of j
+template <typename real>
+DEM_HD void term_ve_other(const ShapeView<real>& B, int l, real vx, real vy, real px, real py, const real* R,
+                          const PairConst<real>& pc, PairAcc<real>& acc) {
+    typedef typename vec4<real>::type real4;
+    const real4 e0 = B.E[2 * l];
+    const real len = B.E[2 * l + 1].x;
+    real ddx, ddy;
+    const real r2 = point_edge2<real>(px, py, e0.x, e0.y, e0.z, e0.w, len, ddx, ddy);
+    if (r2 < pc.rc2)  // c_i = the vertex, del = c_i - c_j = R dd
+        wca_accumulate<real>(pc, acc, vx, vy, real(0), R[0] * ddx + R[1] * ddy, R[3] * ddx + R[4] * ddy, real(0), r2,
+                             false);
+}
+
+// outer features of a pair brought into the frame of the inner feature's owner
+template <typename real>
+DEM_HD void edge_to_i(const ShapeView<real>& B, int l, const real* R, const real* t, real* p2, real* d2, real& e,
+                      real& inv_e) {
+    typedef typename vec4<real>::type real4;
+    const real4 b0 = B.E[2 * l], b1 = B.E[2 * l + 1];
+    p2[0] = R[0] * b0.x + R[1] * b0.y + R[2] * b0.z + t[0];
+    p2[1] = R[3] * b0.x + R[4] * b0.y + R[5] * b0.z + t[1];
+    p2[2] = R[6] * b0.x + R[7] * b0.y + R[8] * b0.z + t[2];
+    d2[0] = R[0] * b1.x + R[1] * b1.y + R[2] * b1.z;
+    d2[1] = R[3] * b1.x + R[4] * b1.y + R[5] * b1.z;
+    d2[2] = R[6] * b1.x + R[7] * b1.y + R[8] * b1.z;
+    e = b0.w;
+    inv_e = b1.w;
+}
+template <typename real> DEM_HD void vertex_to_i(real vx, real vy, real vz, const real* R, const real* t, real* p) {
+    p[0] = R[0] * vx + R[1] * vy + R[2] * vz + t[0];
+    p[1] = R[3] * vx + R[4] * vy + R[5] * vz + t[1];
+    p[2] = R[6] * vx + R[7] * vy + R[8] * vz + t[2];
+}
+template <typename real> DEM_HD void vertex_to_j(real vx, real vy, real vz, const real* R, const real* t, real* p) {
+    const real wx = vx - t[0], wy = vy - t[1], wz = vz - t[2];  // p' = R^T (v - t)
+    p[0] = R[0] * wx + R[3] * wy + R[6] * wz;
+    p[1] = R[1] * wx + R[4] * wy + R[7] * wz;
+    p[2] = R[2] * wx + R[5] * wy + R[8] * wz;
+}
+
 // ---- the pair: 3D --------------------------------------------------------------------------------------------------
 // A = shape of i (its body frame is the working frame), B = shape of j.  R (row-major 3x3) and t bring j's body
 // coordinates into i's frame: p_i = R v_j + t.  [o_begin, o_end) selects a slice of the flattened outer loop
@@ -241,74 +360,23 @@ DEM_HD void pair_eval_3d(const ShapeView<real>& A, const ShapeView<real>& B, con
     const int oE = B.ne, oV = B.ne + B.nv;
     // (1) first sum of Eq. 1: every edge of i against every edge of j
     for (int l = o_begin; l < o_end && l < oE; ++l) {
-        const real4 b0 = B.E[2 * l], b1 = B.E[2 * l + 1];
-        const real p2x = R[0] * b0.x + R[1] * b0.y + R[2] * b0.z + t[0];
-        const real p2y = R[3] * b0.x + R[4] * b0.y + R[5] * b0.z + t[1];
-        const real p2z = R[6] * b0.x + R[7] * b0.y + R[8] * b0.z + t[2];
-        const real d2x = R[0] * b1.x + R[1] * b1.y + R[2] * b1.z;
-        const real d2y = R[3] * b1.x + R[4] * b1.y + R[5] * b1.z;
-        const real d2z = R[6] * b1.x + R[7] * b1.y + R[8] * b1.z;
-        const real e = b0.w, inv_e = b1.w;
-        const real thr_e = pc.eps_par * e;
-        for (int k = 0; k < A.ne; ++k) {
-            const real4 a0 = A.E[2 * k], a1 = A.E[2 * k + 1];
-            const real rx = a0.x - p2x, ry = a0.y - p2y, rz = a0.z - p2z;  // r = p1 - p2
-            const real nx = a1.y * d2z - a1.z * d2y, ny = a1.z * d2x - a1.x * d2z, nz = a1.x * d2y - a1.y * d2x;
-            const real nn = nx * nx + ny * ny + nz * nz;
-            real s, tt;
-            bool par = false;
-            if (nn <= thr_e * a0.w) {
-                par = segseg_special<real>(rx, ry, rz, a1.x, a1.y, a1.z, a0.w, d2x, d2y, d2z, e, nn, pc.eps_par, s, tt);
-            } else {
-                // skew lines: s = -(d1 x d2).(r x d2) / |d1 x d2|^2 (no cancellation near parallel), then the
-                // textbook clamp cascade written branch-free
-                const real qx = ry * d2z - rz * d2y, qy = rz * d2x - rx * d2z, qz = rx * d2y - ry * d2x;
-                s = sat01(-(nx * qx + ny * qy + nz * qz) * rcp(nn));
-                const real b = a1.x * d2x + a1.y * d2y + a1.z * d2z;
-                const real f = d2x * rx + d2y * ry + d2z * rz;
-                const real c = a1.x * rx + a1.y * ry + a1.z * rz;
-                const real tu = (b * s + f) * inv_e;
-                tt = sat01(tu);
-                const real s2 = sat01((b * tt - c) * a1.w);
-                s = (tu != tt) ? s2 : s;
-            }
-            const real dx = rx + s * a1.x - tt * d2x, dy = ry + s * a1.y - tt * d2y, dz = rz + s * a1.z - tt * d2z;
-            const real r2 = dx * dx + dy * dy + dz * dz;
-            if (r2 < pc.rc2)
-                wca_accumulate<real>(pc, acc, a0.x + s * a1.x, a0.y + s * a1.y, a0.z + s * a1.z, dx, dy, dz, r2, par);
-        }
+        real p2[3], d2[3], e, inv_e;
+        edge_to_i<real>(B, l, R, t, p2, d2, e, inv_e);
+        for (int k = 0; k < A.ne; ++k) term_ee<real>(A, k, p2[0], p2[1], p2[2], d2[0], d2[1], d2[2], e, inv_e, pc, acc);
     }
     // (2) third sum of Eq. 1: every vertex of j against every face of i (i's frame)
     for (int o = (o_begin > oE ? o_begin : oE); o < o_end && o < oV; ++o) {
         const real4 v = B.V[o - oE];
-        const real px = R[0] * v.x + R[1] * v.y + R[2] * v.z + t[0];
-        const real py = R[3] * v.x + R[4] * v.y + R[5] * v.z + t[1];
-        const real pz = R[6] * v.x + R[7] * v.y + R[8] * v.z + t[2];
-        for (int f = 0; f < A.nf; ++f) {
-            const real r2 = point_face_r2<real>(A, f, px, py, pz);
-            if (r2 < pc.rc2) {
-                real dx, dy, dz;  // p - c with c on i's face: c_i = c, c_j = p, del = c_i - c_j = -(p - c)
-                point_face_del<real>(A, f, px, py, pz, dx, dy, dz);
-                wca_accumulate<real>(pc, acc, px - dx, py - dy, pz - dz, -dx, -dy, -dz, r2, false);
-            }
-        }
+        real p[3];
+        vertex_to_i<real>(v.x, v.y, v.z, R, t, p);
+        for (int f = 0; f < A.nf; ++f) term_vf_own<real>(A, f, p[0], p[1], p[2], pc, acc);
     }
-    // (3) second sum of Eq. 1: every vertex of i against every face of j, in j's frame: p' = R^T (v - t)
+    // (3) second sum of Eq. 1: every vertex of i against every face of j, in j's frame
     for (int o = (o_begin > oV ? o_begin : oV); o < o_end && o < oV + A.nv; ++o) {
         const real4 v = A.V[o - oV];
-        const real wx = v.x - t[0], wy = v.y - t[1], wz = v.z - t[2];
-        const real px = R[0] * wx + R[3] * wy + R[6] * wz;
-        const real py = R[1] * wx + R[4] * wy + R[7] * wz;
-        const real pz = R[2] * wx + R[5] * wy + R[8] * wz;
-        for (int f = 0; f < B.nf; ++f) {
-            const real r2 = point_face_r2<real>(B, f, px, py, pz);
-            if (r2 < pc.rc2) {
-                real dx, dy, dz;  // p' - c' in j's frame; c_i = the vertex, del = c_i - c_j = R (p' - c')
-                point_face_del<real>(B, f, px, py, pz, dx, dy, dz);
-                wca_accumulate<real>(pc, acc, v.x, v.y, v.z, R[0] * dx + R[1] * dy + R[2] * dz,
-                                     R[3] * dx + R[4] * dy + R[5] * dz, R[6] * dx + R[7] * dy + R[8] * dz, r2, false);
-            }
-        }
+        real p[3];
+        vertex_to_j<real>(v.x, v.y, v.z, R, t, p);
+        for (int f = 0; f < B.nf; ++f) term_vf_other<real>(B, f, v.x, v.y, v.z, p[0], p[1], p[2], R, pc, acc);
     }
 }
 
@@ -321,31 +389,15 @@ DEM_HD void pair_eval_2d(const ShapeView<real>& A, const ShapeView<real>& B, con
     const int oV = B.nv;
     for (int l = o_begin; l < o_end && l < oV; ++l) {
         const real4 v = B.V[l];
-        const real px = R[0] * v.x + R[1] * v.y + t[0];
-        const real py = R[3] * v.x + R[4] * v.y + t[1];
-        for (int k = 0; k < A.ne; ++k) {
-            const real4 e0 = A.E[2 * k];
-            const real len = A.E[2 * k + 1].x;
-            real ddx, ddy;
-            const real r2 = point_edge2<real>(px, py, e0.x, e0.y, e0.z, e0.w, len, ddx, ddy);
-            if (r2 < pc.rc2)  // c_i = p - dd on i's edge, c_j = p, del = -dd
-                wca_accumulate<real>(pc, acc, px - ddx, py - ddy, real(0), -ddx, -ddy, real(0), r2, false);
-        }
+        real p[3];
+        vertex_to_i<real>(v.x, v.y, real(0), R, t, p);
+        for (int k = 0; k < A.ne; ++k) term_ve_own<real>(A, k, p[0], p[1], pc, acc);
     }
     for (int o = (o_begin > oV ? o_begin : oV); o < o_end && o < oV + A.nv; ++o) {
         const real4 v = A.V[o - oV];
-        const real wx = v.x - t[0], wy = v.y - t[1];
-        const real px = R[0] * wx + R[3] * wy;
-        const real py = R[1] * wx + R[4] * wy;
-        for (int l = 0; l < B.ne; ++l) {
-            const real4 e0 = B.E[2 * l];
-            const real len = B.E[2 * l + 1].x;
-            real ddx, ddy;
-            const real r2 = point_edge2<real>(px, py, e0.x, e0.y, e0.z, e0.w, len, ddx, ddy);
-            if (r2 < pc.rc2)  // c_i = the vertex, del = c_i - c_j = R dd
-                wca_accumulate<real>(pc, acc, v.x, v.y, real(0), R[0] * ddx + R[1] * ddy, R[3] * ddx + R[4] * ddy,
-                                     real(0), r2, false);
-        }
+        real p[3];
+        vertex_to_j<real>(v.x, v.y, real(0), R, t, p);
+        for (int l = 0; l < B.ne; ++l) term_ve_other<real>(B, l, v.x, v.y, p[0], p[1], R, pc, acc);
     }
 }
 
@@ -368,24 +420,45 @@ template <typename real> DEM_HD void quat_to_mat(real w, real x, real y, real z,
 // operations per pair against >= 600 FP32 instructions of feature work).
 // out[0..2] = force on i, out[3..5] = torque on i, out[6..8] = torque on j (all lab frame), out[9] = U_ij.
 // The force on j is -out[0..2].  tau_j = -sum c_j x F + d x sum F, and c_j x F = c_i x F because F is along c_i - c_j.
+// relative pose of a pair: Mi = R_i, R = R_i^T R_j, t = R_i^T d, formed in FP64 and rounded ONCE to `real`
+template <typename real>
+DEM_HD void pair_pose(const double* qi, const double* qj, const double* d, real* Mi, real* R, real* t) {
+    double Di[9], Dj[9];
+    quat_to_mat<double>(qi[0], qi[1], qi[2], qi[3], Di);
+    quat_to_mat<double>(qj[0], qj[1], qj[2], qj[3], Dj);
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+            R[3 * r + c] = (real)(Di[r] * Dj[c] + Di[3 + r] * Dj[3 + c] + Di[6 + r] * Dj[6 + c]);
+        t[r] = (real)(Di[r] * d[0] + Di[3 + r] * d[1] + Di[6 + r] * d[2]);
+    }
+#pragma unroll
+    for (int k = 0; k < 9; ++k) Mi[k] = (real)Di[k];
+}
+
+// (F, T, u) of a pair in i's frame -> out[0..2] = force on i, out[3..5] = torque on i, out[6..8] = torque on j (all lab
+// frame), out[9] = U_ij.  The force on j is -out[0..2].  tau_j = -sum c_j x F + d x sum F, and c_j x F = c_i x F
+// because F is along c_i - c_j.
+template <typename real>
+DEM_HD void pair_finish(const real* Mi, const real* t, const real* F, const real* T, real u, real* out) {
+    const real tjx = -T[0] + (t[1] * F[2] - t[2] * F[1]);
+    const real tjy = -T[1] + (t[2] * F[0] - t[0] * F[2]);
+    const real tjz = -T[2] + (t[0] * F[1] - t[1] * F[0]);
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+        out[r] = Mi[3 * r] * F[0] + Mi[3 * r + 1] * F[1] + Mi[3 * r + 2] * F[2];
+        out[3 + r] = Mi[3 * r] * T[0] + Mi[3 * r + 1] * T[1] + Mi[3 * r + 2] * T[2];
+        out[6 + r] = Mi[3 * r] * tjx + Mi[3 * r + 1] * tjy + Mi[3 * r + 2] * tjz;
+    }
+    out[9] = u;
+}
+
 template <typename real, int DIM>
 DEM_HD void pair_lab(const ShapeView<real>& A, const ShapeView<real>& B, const double* qi, const double* qj,
                      const double* d, const PairConst<real>& pc, int o_begin, int o_end, real* out, unsigned* cnt) {
     real Mi[9], R[9], t[3];
-    {
-        double Di[9], Dj[9];
-        quat_to_mat<double>(qi[0], qi[1], qi[2], qi[3], Di);
-        quat_to_mat<double>(qj[0], qj[1], qj[2], qj[3], Dj);
-#pragma unroll
-        for (int r = 0; r < 3; ++r) {
-#pragma unroll
-            for (int c = 0; c < 3; ++c)
-                R[3 * r + c] = (real)(Di[r] * Dj[c] + Di[3 + r] * Dj[3 + c] + Di[6 + r] * Dj[6 + c]);
-            t[r] = (real)(Di[r] * d[0] + Di[3 + r] * d[1] + Di[6 + r] * d[2]);
-        }
-#pragma unroll
-        for (int k = 0; k < 9; ++k) Mi[k] = (real)Di[k];
-    }
+    pair_pose<real>(qi, qj, d, Mi, R, t);
     PairAcc<real> acc;
     acc.F[0] = acc.F[1] = acc.F[2] = acc.T[0] = acc.T[1] = acc.T[2] = acc.u = real(0);
     acc.nactive = acc.ndegen = acc.npar = 0u;
@@ -393,17 +466,7 @@ DEM_HD void pair_lab(const ShapeView<real>& A, const ShapeView<real>& B, const d
         pair_eval_3d<real>(A, B, R, t, pc, o_begin, o_end, acc);
     else
         pair_eval_2d<real>(A, B, R, t, pc, o_begin, o_end, acc);
-    // torque on j about x_j, still in i's frame: -T + t x F
-    const real tjx = -acc.T[0] + (t[1] * acc.F[2] - t[2] * acc.F[1]);
-    const real tjy = -acc.T[1] + (t[2] * acc.F[0] - t[0] * acc.F[2]);
-    const real tjz = -acc.T[2] + (t[0] * acc.F[1] - t[1] * acc.F[0]);
-#pragma unroll
-    for (int r = 0; r < 3; ++r) {
-        out[r] = Mi[3 * r] * acc.F[0] + Mi[3 * r + 1] * acc.F[1] + Mi[3 * r + 2] * acc.F[2];
-        out[3 + r] = Mi[3 * r] * acc.T[0] + Mi[3 * r + 1] * acc.T[1] + Mi[3 * r + 2] * acc.T[2];
-        out[6 + r] = Mi[3 * r] * tjx + Mi[3 * r + 1] * tjy + Mi[3 * r + 2] * tjz;
-    }
-    out[9] = acc.u;
+    pair_finish<real>(Mi, t, acc.F, acc.T, acc.u, out);
     cnt[0] = acc.nactive;
     cnt[1] = acc.ndegen;
     cnt[2] = acc.npar;

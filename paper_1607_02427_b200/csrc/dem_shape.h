@@ -23,9 +23,10 @@ struct HostShape {
     std::vector<int> face_off;   // nf + 1
     std::vector<int> face_verts;
     double rounding = 0, mass = 1, inertia[3] = {1, 1, 1}, circumradius = 0;
-    // flattened table in double, in units of 4 doubles: V (nv) | E (2 ne) | F (4 nf) | FE (2 nfe)
+    // flattened table in double, in units of 4 doubles: V (nv) | E (2 ne) | F (4 nf) | FE (2 nfe) | OE (2 ne, 3D only)
     std::vector<double> table;
-    int table_len4() const { return nv + 2 * ne + 4 * nf + 2 * nfe; }
+    double max_edge = 0;  // longest edge (bounds the search kernel's near-parallel slack)
+    int table_len4() const { return nv + 2 * ne + 4 * nf + 2 * nfe + (dim == 3 ? 2 * ne : 0); }
 };
 
 inline void push4(std::vector<double>& t, double a, double b, double c, double d) {
@@ -119,8 +120,12 @@ inline std::string build_host_shape(HostShape& S, int dim, const double* verts, 
             push4(T, e[0], e[1], e[2], ee > 0 ? 1.0 / ee : 0.0);
         } else {
             const double len = std::sqrt(ee);
-            push4(T, a[0], a[1], len > 0 ? e[0] / len : 0.0, len > 0 ? e[1] / len : 0.0);
-            push4(T, len, 0, 0, 0);
+            // a zero-length edge (disk, R14) gets an arbitrary unit direction: with len = 0 the nearest point is a
+            // whatever u is, and the search kernel's side^2 + excess^2 form needs |u| = 1
+            const double ux = len > 0 ? e[0] / len : 1.0, uy = len > 0 ? e[1] / len : 0.0;
+            push4(T, a[0], a[1], ux, uy);
+            // for a point (x, y): side = ux y - uy x + cs, along = ux x + uy y + cu (used by the search kernel)
+            push4(T, len, -(ux * a[1] - uy * a[0]), -(ux * a[0] + uy * a[1]), 0);
         }
     }
     std::vector<double> FE;
@@ -177,13 +182,28 @@ inline std::string build_host_shape(HostShape& S, int dim, const double* verts, 
             const double ex = p1[0] - p0[0], ey = p1[1] - p0[1];
             const double len = std::sqrt(ex * ex + ey * ey);
             if (!(len > 0)) return "face has a repeated vertex";
-            push4(FE, p0[0], p0[1], ex / len, ey / len);
-            push4(FE, len, 0, 0, 0);
+            // with (x, y) the point in the face frame: side = ux y - uy x + cs (>= 0 inside), along = ux x + uy y + cu
+            const double ux = ex / len, uy = ey / len;
+            push4(FE, p0[0], p0[1], ux, uy);
+            push4(FE, len, -(ux * p0[1] - uy * p0[0]), -(ux * p0[0] + uy * p0[1]), 0);
             nfe++;
         }
     }
     S.nfe = nfe;
     T.insert(T.end(), FE.begin(), FE.end());
+    // OE: the edges again in the form the search kernel wants for its OUTER edge (unit direction, length)
+    S.max_edge = 0;
+    for (int k = 0; k < S.ne; ++k) {
+        const double* a = &S.verts[3 * S.edges[2 * k]];
+        const double* b = &S.verts[3 * S.edges[2 * k + 1]];
+        const double e[3] = {b[0] - a[0], b[1] - a[1], b[2] - a[2]};
+        const double len = std::sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2]);
+        S.max_edge = std::max(S.max_edge, len);
+        if (dim == 3) {
+            push4(T, a[0], a[1], a[2], len);
+            push4(T, len > 0 ? e[0] / len : 0.0, len > 0 ? e[1] / len : 0.0, len > 0 ? e[2] / len : 0.0, 0.0);
+        }
+    }
     return "";
 }
 
