@@ -208,11 +208,13 @@ __device__ __forceinline__ void push_and_drain(WarpCtx& w, int phase, const unsi
 // r^2 - rc_search^2.  Near-parallel edges (|d1 x d2|^2 -> 0) make s inaccurate but never out of [0,1], and t, s2 are
 // then exact for that s, so r is off by at most sin(angle) x edge length: covered by rc_search's slack.
 __device__ __forceinline__ float ee_eval(const f4 e0, const f4 e1, u64 np2x, u64 np2y, u64 np2z, u64 d2x, u64 d2y,
-                                         u64 d2z, float Llo, float Lhi, float nrc2) {
+                                         u64 d2z, u64 g, float Llo, float Lhi, float nrc2) {
     const u64 rx = add2(bc(e0.x), np2x), ry = add2(bc(e0.y), np2y), rz = add2(bc(e0.z), np2z);  // r = p1 - p2
     const u64 b = fma2(bc(e1.z), d2z, fma2(bc(e1.y), d2y, mul2(bc(e1.x), d2x)));              // d1 . d2
     const u64 c = fma2(bc(e1.z), rz, fma2(bc(e1.y), ry, mul2(bc(e1.x), rx)));                 // d1 . r
-    const u64 f = fma2(d2z, rz, fma2(d2y, ry, mul2(d2x, rx)));                                // d2 . r
+    // d2 . r = d2 . p1 + g with g = -d2 . p2 per outer edge: keeps one operand of every FFMA2 a broadcast scalar
+    // (three 64-bit register operands cost the register file a third cycle)
+    const u64 f = fma2(d2z, bc(e0.z), fma2(d2y, bc(e0.y), fma2(d2x, bc(e0.x), g)));
     const u64 nn = fma2(neg2(b), b, bc(e0.w));                                                // |d1|^2 - b^2
     const u64 num = fma2(b, f, neg2(c));
     float nl, nh, ul, uh;
@@ -233,23 +235,66 @@ __device__ __forceinline__ float ee_eval(const f4 e0, const f4 e1, u64 np2x, u64
     return fminf(lo, hi);
 }
 
-// One boundary edge (or 2D edge) e0 = (., ., ux, uy), e1 = (len, cs, cu, .) against two packed points (x, y):
-// side = u x q + cs (>= 0 on the inner side), along = u . q + cu, excess = max(-along, along - len, 0).
+// One boundary edge (or 2D edge) e0 = (., ., ux, uy), e1 = (len, cs, cm, len/2) against two packed points (x, y):
+// side = u x q + cs (>= 0 on the inner side), centred along-edge coordinate am = u . q + cm (0 at the edge's midpoint),
+// excess = max(|am| - len/2, 0): the point's distance^2 from the segment is side^2 + excess^2.
 __device__ __forceinline__ void edge2_eval(const f4 e0, const f4 e1, u64 x, u64 y, u64& side, u64& exc) {
     side = fma2(bc(e0.z), y, fma2(bc(-e0.w), x, bc(e1.y)));
-    const u64 al = fma2(bc(e0.z), x, fma2(bc(e0.w), y, bc(e1.z)));
-    const u64 over = add2(al, bc(-e1.x));
-    float al_l, al_h, ov_l, ov_h;
-    upk(al, al_l, al_h);
-    upk(over, ov_l, ov_h);
-    exc = pk(fmaxf(fmaxf(-al_l, ov_l), 0.f), fmaxf(fmaxf(-al_h, ov_h), 0.f));
+    float am_l, am_h;
+    upk(fma2(bc(e0.z), x, fma2(bc(e0.w), y, bc(e1.z))), am_l, am_h);
+    exc = pk(fmaxf(fabsf(am_l) - e1.w, 0.f), fmaxf(fabsf(am_h) - e1.w, 0.f));
+}
+
+// minimum of n values with 3-input minima (FMNMX3)
+template <int N> __device__ __forceinline__ float min_tree(const float (&v)[N]) {
+    float r = v[0];
+#pragma unroll
+    for (int k = 1; k + 1 < N; k += 2) r = fminf(fminf(r, v[k]), v[k + 1]);
+    if ((N & 1) == 0) r = fminf(r, v[N - 1]);
+    return r;
 }
 
 // Point against closed convex polygon face (R1/R2): two packed points against face header F[0..2] and its M boundary
 // edges.  r^2 = h^2 + (inside ? 0 : min over edges of side^2 + excess^2).  Updates mask[tau] for T packed point pairs.
 template <int T, int M>
-__device__ __forceinline__ void face_eval(const f4* __restrict__ F, const f4* __restrict__ FE, int m_rt, const u64 (&px)[T],
+__device__ __forceinline__ void face_eval(const f4* __restrict__ F, const f4* __restrict__ FE, const u64 (&px)[T],
                                           const u64 (&py)[T], const u64 (&pz)[T], float nrc2, unsigned (&mask)[T]) {
+    const f4 f0 = F[0], f1 = F[1], f2 = F[2];
+    u64 x[T], y[T], hh[T];
+    float sl[T][M], sh[T][M], dl[T][M], dh[T][M];
+#pragma unroll
+    for (int tau = 0; tau < T; ++tau) {
+        x[tau] = fma2(bc(f0.z), pz[tau], fma2(bc(f0.y), py[tau], fma2(bc(f0.x), px[tau], bc(f0.w))));
+        y[tau] = fma2(bc(f1.z), pz[tau], fma2(bc(f1.y), py[tau], fma2(bc(f1.x), px[tau], bc(f1.w))));
+        const u64 h = fma2(bc(f2.z), pz[tau], fma2(bc(f2.y), py[tau], fma2(bc(f2.x), px[tau], bc(f2.w))));
+        hh[tau] = fma2(h, h, bc(nrc2));
+    }
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+        const f4 e0 = FE[2 * m], e1 = FE[2 * m + 1];
+#pragma unroll
+        for (int tau = 0; tau < T; ++tau) {
+            u64 side, exc;
+            edge2_eval(e0, e1, x[tau], y[tau], side, exc);
+            upk(side, sl[tau][m], sh[tau][m]);
+            upk(fma2(exc, exc, mul2(side, side)), dl[tau][m], dh[tau][m]);
+        }
+    }
+#pragma unroll
+    for (int tau = 0; tau < T; ++tau) {
+        const u64 sel = pk(min_tree<M>(sl[tau]) >= 0.f ? 0.f : min_tree<M>(dl[tau]),
+                           min_tree<M>(sh[tau]) >= 0.f ? 0.f : min_tree<M>(dh[tau]));
+        float lo, hi;
+        upk(add2(hh[tau], sel), lo, hi);
+        mask[tau] = push_sign(mask[tau], fminf(lo, hi));
+    }
+}
+
+// the same for any number of boundary edges (run-time loop)
+template <int T>
+__device__ __forceinline__ void face_eval_any(const f4* __restrict__ F, const f4* __restrict__ FE, int mcount,
+                                              const u64 (&px)[T], const u64 (&py)[T], const u64 (&pz)[T], float nrc2,
+                                              unsigned (&mask)[T]) {
     const f4 f0 = F[0], f1 = F[1], f2 = F[2];
     u64 x[T], y[T], hh[T];
     float smin_l[T], smin_h[T], dmin_l[T], dmin_h[T];
@@ -261,8 +306,6 @@ __device__ __forceinline__ void face_eval(const f4* __restrict__ F, const f4* __
         hh[tau] = fma2(h, h, bc(nrc2));
         smin_l[tau] = smin_h[tau] = dmin_l[tau] = dmin_h[tau] = 1e30f;
     }
-    const int mcount = M > 0 ? M : m_rt;
-#pragma unroll
     for (int m = 0; m < mcount; ++m) {
         const f4 e0 = FE[2 * m], e1 = FE[2 * m + 1];
 #pragma unroll
@@ -287,36 +330,141 @@ __device__ __forceinline__ void face_eval(const f4* __restrict__ F, const f4* __
     }
 }
 
-// sweep T packed pairs of points over faces [f0, f1) of shape S (at most 32 faces: one mask bit each)
+// sweep T packed pairs of points over faces [f0, f1) of shape S (at most 32 faces: one mask bit each).  Faces are
+// stored sorted by boundary-edge count; sd lists the runs, so the common sizes run unrolled without a per-face branch.
 template <int T>
-__device__ __forceinline__ void sweep_faces(const ShapeView<float>& S, int f0, int f1, const u64 (&px)[T], const u64 (&py)[T],
-                                            const u64 (&pz)[T], float nrc2, unsigned (&mask)[T]) {
-    for (int f = f0; f < f1; ++f) {
-        const f4* F = S.F + 4 * f;
-        const f4 f3 = F[3];
-        const int m0 = (int)f3.x, mc = (int)f3.y;
-        const f4* FE = S.FE + 2 * m0;
-        switch (mc) {
-            case 3: face_eval<T, 3>(F, FE, 3, px, py, pz, nrc2, mask); break;
-            case 4: face_eval<T, 4>(F, FE, 4, px, py, pz, nrc2, mask); break;
-            case 5: face_eval<T, 5>(F, FE, 5, px, py, pz, nrc2, mask); break;
-            case 6: face_eval<T, 6>(F, FE, 6, px, py, pz, nrc2, mask); break;
-            default: face_eval<T, 0>(F, FE, mc, px, py, pz, nrc2, mask); break;
+__device__ __forceinline__ void sweep_faces(const ShapeView<float>& S, const ShapeDev& sd, int f0, int f1,
+                                            const u64 (&px)[T], const u64 (&py)[T], const u64 (&pz)[T], float nrc2,
+                                            unsigned (&mask)[T]) {
+    if (sd.grp_m[0] == 0) {  // too many different face sizes: read every face's header
+        for (int f = f0; f < f1; ++f) {
+            const f4 f3 = S.F[4 * f + 3];
+            face_eval_any<T>(S.F + 4 * f, S.FE + 2 * (int)f3.x, (int)f3.y, px, py, pz, nrc2, mask);
         }
+        return;
+    }
+    int fbase = 0, febase = 0;
+#pragma unroll 1
+    for (int g = 0; g < DEM_MAX_FACE_GROUPS && sd.grp_n[g] > 0; ++g) {
+        const int m = sd.grp_m[g], fend = fbase + sd.grp_n[g];
+        const int lo = max(f0, fbase), hi = min(f1, fend);
+        if (lo < hi) {
+            const f4* F = S.F + 4 * lo;
+            const f4* FE = S.FE + 2 * (febase + (lo - fbase) * m);
+            const int n = hi - lo;
+            switch (m) {
+                case 3:
+                    for (int f = 0; f < n; ++f, F += 4, FE += 6) face_eval<T, 3>(F, FE, px, py, pz, nrc2, mask);
+                    break;
+                case 4:
+                    for (int f = 0; f < n; ++f, F += 4, FE += 8) face_eval<T, 4>(F, FE, px, py, pz, nrc2, mask);
+                    break;
+                case 5:
+                    for (int f = 0; f < n; ++f, F += 4, FE += 10) face_eval<T, 5>(F, FE, px, py, pz, nrc2, mask);
+                    break;
+                case 6:
+                    for (int f = 0; f < n; ++f, F += 4, FE += 12) face_eval<T, 6>(F, FE, px, py, pz, nrc2, mask);
+                    break;
+                default:
+                    for (int f = 0; f < n; ++f, F += 4, FE += 2 * m) face_eval_any<T>(F, FE, m, px, py, pz, nrc2, mask);
+                    break;
+            }
+        }
+        febase += sd.grp_n[g] * m;
+        fbase = fend;
     }
 }
+
+// ---- a3: relative pose of every pair of a class, compacted -----------------------------------------------------------
+// One thread per unique pair: minimum-image separation d, exact reach test (R10), relative pose R = R_i^T R_j,
+// t = R_i^T d and R_i in FP64, rounded once to float.  Pairs inside the reach are appended to a
+// compact work list (warp-aggregated atomic: their order varies from run to run, the result of a pair does not depend
+// on it); pairs beyond it get their zero result records here and never reach the search kernel, so its warps carry 32
+// live pairs each.  Pose record, plane-major for coalesced loads: [6][npairs] float4 =
+// (R0 R1 R2 R3) (R4 R5 R6 R7) (R8 t0 t1 t2) (M0 M1 M2 M3) (M4 M5 M6 M7) (M8 dx dy dz); pidx[c] = the pair's index.
+struct PoseArgs {
+    const int2* pairs;
+    int npairs, slices;
+    const void* pos;
+    const void* quat;
+    BoxDev box;
+    double reach2;
+    f4* pose;
+    int* pidx;
+    int* count;  // valid pairs of this class (zeroed before the launch)
+    f4* rec;
+    unsigned long long* counters;
+};
+
+template <typename PosT, int DIM> __global__ void __launch_bounds__(128) k_pose(const PoseArgs a) {
+    const unsigned full = 0xffffffffu;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    bool valid = false;
+    float Mi[9], R[9], t[3];
+    double d[3] = {0.0, 0.0, 0.0};
+    if (p < a.npairs) {
+        const int2 ij = a.pairs[p];
+        const d4 xi = load4d(static_cast<const PosT*>(a.pos), ij.x), xj = load4d(static_cast<const PosT*>(a.pos), ij.y);
+        const d4 qi = load4d(static_cast<const PosT*>(a.quat), ij.x), qj = load4d(static_cast<const PosT*>(a.quat), ij.y);
+        // minimum image (any nearest image serves here: the bit-exact predicate R13 belongs to the neighbour list)
+        d[0] = xj.x - xi.x; d[1] = xj.y - xi.y; d[2] = DIM == 3 ? xj.z - xi.z : 0.0;
+        d[0] -= a.box.L[0] * rint(d[0] * a.box.invL[0]);
+        d[1] -= a.box.L[1] * rint(d[1] * a.box.invL[1]);
+        if (DIM == 3) d[2] -= a.box.L[2] * rint(d[2] * a.box.invL[2]);
+        valid = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] < a.reach2;
+        if (valid) {
+            const double qa[4] = {qi.x, qi.y, qi.z, qi.w}, qb[4] = {qj.x, qj.y, qj.z, qj.w};
+            pair_pose<float>(qa, qb, d, Mi, R, t);
+        } else {
+            f4 r0, r1, r2;
+            r0.x = r0.y = r0.z = r0.w = 0.f;
+            r1.x = r1.y = r1.z = 0.f; r1.w = (float)d[0];
+            r2.x = (float)d[1]; r2.y = (float)d[2]; r2.z = r2.w = 0.f;
+            for (int sl = 0; sl < a.slices; ++sl) {
+                f4* rec = a.rec + DEM_REC * ((size_t)p * a.slices + sl);
+                rec[0] = r0; rec[1] = r1; rec[2] = r2;
+            }
+        }
+    }
+    const unsigned m = __ballot_sync(full, valid);
+    int base = 0;
+    if (lane == 0 && m) base = atomicAdd(a.count, __popc(m));
+    base = __shfl_sync(full, base, 0);
+    if (valid) {
+        const int c = base + __popc(m & ((1u << lane) - 1u));
+        const size_t n = (size_t)a.npairs;
+        f4 v;
+        v.x = R[0]; v.y = R[1]; v.z = R[2]; v.w = R[3]; a.pose[c] = v;
+        v.x = R[4]; v.y = R[5]; v.z = R[6]; v.w = R[7]; a.pose[n + c] = v;
+        v.x = R[8]; v.y = t[0]; v.z = t[1]; v.w = t[2]; a.pose[2 * n + c] = v;
+        v.x = Mi[0]; v.y = Mi[1]; v.z = Mi[2]; v.w = Mi[3]; a.pose[3 * n + c] = v;
+        v.x = Mi[4]; v.y = Mi[5]; v.z = Mi[6]; v.w = Mi[7]; a.pose[4 * n + c] = v;
+        v.x = Mi[8]; v.y = (float)d[0]; v.z = (float)d[1]; v.w = (float)d[2]; a.pose[5 * n + c] = v;
+        a.pidx[c] = p;
+    }
+    if (lane == 0 && m) atomicAdd(a.counters, (unsigned long long)__popc(m));
+}
+
+#ifdef DEM_TUNE
+__device__ int g_dbg_phases = 7;  // tuning builds only: bit 0 = edge-edge, bit 1 = vertex-face (own), bit 2 = vertex-face (other)
+#define DEM_DBG_PHASE(bit) (g_dbg_phases & (bit))
+#else
+#define DEM_DBG_PHASE(bit) true
+#endif
 
 // ---- the kernel ---------------------------------------------------------------------------------------------------------
 // One warp = 32 consecutive (pair, slice) items of one pair class (same shapes, same loop bounds).  TE / TV = packed
 // outer pairs per sweep for edges / vertices (2 TE outer edges, 2 TV outer vertices share every inner-feature load).
-template <typename PosT, int DIM, int TE, int TV>
-__global__ void __launch_bounds__(128, 3) k_pair_fast(const PairArgs<float> a) {
+template <typename PosT, int DIM, int TE, int TV, int MINB>
+__global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     FastShared* fs = reinterpret_cast<FastShared*>(smem_raw);
     unsigned* queue = reinterpret_cast<unsigned*>(smem_raw + 256);  // 4 warps x DEM_QCAP
     float* sacc_all = reinterpret_cast<float*>(queue + 4 * DEM_QCAP);  // 4 warps x 7 x 32
     unsigned* scnt_all = reinterpret_cast<unsigned*>(sacc_all + 4 * 7 * 32);  // 4 warps x 4
-    f4* sm = reinterpret_cast<f4*>(scnt_all + 16);
+    f4* stage_pose = reinterpret_cast<f4*>(scnt_all + 16);                 // 4 warps x [2][6][32] float4
+    int* stage_pidx = reinterpret_cast<int*>(stage_pose + 4 * 2 * 6 * 32);  // 4 warps x [2][32]
+    f4* sm = reinterpret_cast<f4*>(stage_pidx + 4 * 2 * 32);
     static_assert(sizeof(FastShared) <= 256, "FastShared header");
     // stage the shape-feature tables of the class (a1) into shared memory
     const bool same = a.sa.off == a.sb.off;
@@ -347,40 +495,52 @@ __global__ void __launch_bounds__(128, 3) k_pair_fast(const PairArgs<float> a) {
     w.qn = 0;
     w.lane = lane;
     const float nrc2 = -a.rc2_search;
-    const int np_pad = (a.npairs + 31) & ~31;  // slices are warp-uniform
+    const int count = *a.count;                // pairs inside the reach, compacted by k_pose
+    const int np_pad = (count + 31) & ~31;     // slices are warp-uniform
     const long long n_wtiles = (long long)(np_pad >> 5) * a.slices;
-    unsigned c_eval = 0;
-    for (long long wt = (long long)blockIdx.x * 4 + warp; wt < n_wtiles; wt += (long long)gridDim.x * 4) {
-        const long long item = wt * 32 + lane;
-        const int slice = (int)(item / np_pad), p = (int)(item - (long long)slice * np_pad);
-        const bool in_list = p < a.npairs;
-        bool valid = false;
-        double d[3] = {0.0, 0.0, 0.0};
-        float Mi[9], R[9], t[3];
-        if (in_list) {
-            const int2 ij = a.pairs[p];
-            const d4 xi = load4d(static_cast<const PosT*>(a.pos), ij.x), xj = load4d(static_cast<const PosT*>(a.pos), ij.y);
-            d[0] = min_image_1(xi.x, xj.x, a.box.L[0]);
-            d[1] = min_image_1(xi.y, xj.y, a.box.L[1]);
-            d[2] = DIM == 3 ? min_image_1(xi.z, xj.z, a.box.L[2]) : 0.0;
-            valid = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] < a.reach2;
-            if (valid) {
-                const d4 qi = load4d(static_cast<const PosT*>(a.quat), ij.x), qj = load4d(static_cast<const PosT*>(a.quat), ij.y);
-                const double qa[4] = {qi.x, qi.y, qi.z, qi.w}, qb[4] = {qj.x, qj.y, qj.z, qj.w};
-                pair_pose<float>(qa, qb, d, Mi, R, t);
+    const size_t plane = (size_t)a.npairs;
+    // Each warp takes every (gridDim.x * 4)-th tile (one tile per warp unless the class has more tiles than the grid
+    // cap).  The pose records of a warp's next tile are copied global -> shared with cp.async while the current tile is
+    // being swept; each lane copies and later reads only its own records.
+    const long long wt_stride = (long long)gridDim.x * 4;
+    f4* spose = stage_pose + warp * (2 * 6 * 32);   // [2][6][32]
+    int* spidx = stage_pidx + warp * (2 * 32);      // [2][32]
+    auto stage = [&](int buf, long long wt_) {
+        if (wt_ < n_wtiles) {
+            const int c_ = (int)((wt_ * 32 + lane) % np_pad);
+            if (c_ < count) {
+#pragma unroll
+                for (int k = 0; k < 6; ++k)
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
+                                     spose + (buf * 6 + k) * 32 + lane)), "l"(a.pose + k * plane + c_));
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(
+                                 spidx + buf * 32 + lane)), "l"(a.pidx + c_));
             }
         }
-        if (!valid) {  // lanes without work sweep a far-away dummy so that the warp stays converged
+        asm volatile("cp.async.commit_group;");
+    };
+    int buf = 0;
+    stage(0, (long long)blockIdx.x * 4 + warp);
+    for (long long wt = (long long)blockIdx.x * 4 + warp; wt < n_wtiles; wt += wt_stride, buf ^= 1) {
+        const long long item = wt * 32 + lane;
+        const int slice = (int)(item / np_pad), c = (int)(item - (long long)slice * np_pad);
+        const bool valid = c < count;
+        stage(buf ^ 1, wt + wt_stride);
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+        float R[9], t[3];
+        if (valid) {
+            const f4 p0 = spose[(buf * 6 + 0) * 32 + lane], p1 = spose[(buf * 6 + 1) * 32 + lane],
+                     p2 = spose[(buf * 6 + 2) * 32 + lane];
+            R[0] = p0.x; R[1] = p0.y; R[2] = p0.z; R[3] = p0.w; R[4] = p1.x; R[5] = p1.y; R[6] = p1.z; R[7] = p1.w;
+            R[8] = p2.x; t[0] = p2.y; t[1] = p2.z; t[2] = p2.w;
+        } else {  // lanes without work sweep a far-away dummy so that the warp stays converged
 #pragma unroll
-            for (int k = 0; k < 9; ++k) Mi[k] = R[k] = (k % 4 == 0) ? 1.f : 0.f;
+            for (int k = 0; k < 9; ++k) R[k] = (k % 4 == 0) ? 1.f : 0.f;
             t[0] = t[1] = 1.0e4f;
             t[2] = DIM == 3 ? 1.0e4f : 0.f;
         }
-        float out[10];
-#pragma unroll
-        for (int k = 0; k < 10; ++k) out[k] = 0.f;
-        if (__any_sync(full, valid)) {
-            c_eval += (valid && slice == 0) ? 1u : 0u;
+        {
+
 #pragma unroll
             for (int k = 0; k < 7; ++k) w.sacc[k * 32 + lane] = 0.f;
             const int ob = (int)((long long)slice * a.n_outer / a.slices);
@@ -388,9 +548,9 @@ __global__ void __launch_bounds__(128, 3) k_pair_fast(const PairArgs<float> a) {
             if (DIM == 3) {
                 const int oE = B.ne, oV = B.ne + B.nv;
                 // (1) first sum of Eq. 1: edges of j (outer, packed) against edges of i (inner)
-                for (int l0 = ob, le = min(oe, oE); l0 < le; l0 += 2 * TE) {
+                for (int l0 = ob, le = DEM_DBG_PHASE(1) ? min(oe, oE) : 0; l0 < le; l0 += 2 * TE) {
                     for (int k0 = 0; k0 < A.ne; k0 += 32) {
-                        u64 np2x[TE], np2y[TE], np2z[TE], d2x[TE], d2y[TE], d2z[TE];
+                        u64 np2x[TE], np2y[TE], np2z[TE], d2x[TE], d2y[TE], d2z[TE], g[TE];
                         float Llo[TE], Lhi[TE];
 #pragma unroll
                         for (int tau = 0; tau < TE; ++tau) {
@@ -405,6 +565,7 @@ __global__ void __launch_bounds__(128, 3) k_pair_fast(const PairArgs<float> a) {
                             d2x[tau] = pk(R[0] * a1.x + R[1] * a1.y + R[2] * a1.z, R[0] * b1.x + R[1] * b1.y + R[2] * b1.z);
                             d2y[tau] = pk(R[3] * a1.x + R[4] * a1.y + R[5] * a1.z, R[3] * b1.x + R[4] * b1.y + R[5] * b1.z);
                             d2z[tau] = pk(R[6] * a1.x + R[7] * a1.y + R[8] * a1.z, R[6] * b1.x + R[7] * b1.y + R[8] * b1.z);
+                            g[tau] = fma2(d2z[tau], np2z[tau], fma2(d2y[tau], np2y[tau], mul2(d2x[tau], np2x[tau])));
                             Llo[tau] = a0.w;
                             Lhi[tau] = b0.w;
                         }
@@ -417,7 +578,7 @@ __global__ void __launch_bounds__(128, 3) k_pair_fast(const PairArgs<float> a) {
 #pragma unroll
                             for (int tau = 0; tau < TE; ++tau)
                                 mask[tau] = push_sign(mask[tau], ee_eval(e0, e1, np2x[tau], np2y[tau], np2z[tau], d2x[tau],
-                                                                         d2y[tau], d2z[tau], Llo[tau], Lhi[tau], nrc2));
+                                                                         d2y[tau], d2z[tau], g[tau], Llo[tau], Lhi[tau], nrc2));
                         }
                         unsigned any = 0u;
 #pragma unroll
@@ -426,7 +587,7 @@ __global__ void __launch_bounds__(128, 3) k_pair_fast(const PairArgs<float> a) {
                     }
                 }
                 // (2) third sum of Eq. 1: vertices of j (outer, packed, i's frame) against faces of i
-                for (int o0 = max(ob, oE) - oE, on = min(oe, oV) - oE; o0 < on; o0 += 2 * TV) {
+                for (int o0 = max(ob, oE) - oE, on = DEM_DBG_PHASE(2) ? min(oe, oV) - oE : 0; o0 < on; o0 += 2 * TV) {
                     for (int f0 = 0; f0 < A.nf; f0 += 32) {
                         u64 px[TV], py[TV], pz[TV];
 #pragma unroll
@@ -443,7 +604,7 @@ __global__ void __launch_bounds__(128, 3) k_pair_fast(const PairArgs<float> a) {
                         unsigned mask[TV];
 #pragma unroll
                         for (int tau = 0; tau < TV; ++tau) mask[tau] = 0u;
-                        sweep_faces<TV>(A, f0, f1, px, py, pz, nrc2, mask);
+                        sweep_faces<TV>(A, a.sa, f0, f1, px, py, pz, nrc2, mask);
                         unsigned any = 0u;
 #pragma unroll
                         for (int tau = 0; tau < TV; ++tau) any |= mask[tau];
@@ -451,7 +612,7 @@ __global__ void __launch_bounds__(128, 3) k_pair_fast(const PairArgs<float> a) {
                     }
                 }
                 // (3) second sum of Eq. 1: vertices of i (outer, packed, j's frame) against faces of j
-                for (int o0 = max(ob, oV) - oV, on = min(oe, oV + A.nv) - oV; o0 < on; o0 += 2 * TV) {
+                for (int o0 = max(ob, oV) - oV, on = DEM_DBG_PHASE(4) ? min(oe, oV + A.nv) - oV : 0; o0 < on; o0 += 2 * TV) {
                     for (int f0 = 0; f0 < B.nf; f0 += 32) {
                         u64 px[TV], py[TV], pz[TV];
 #pragma unroll
@@ -468,7 +629,7 @@ __global__ void __launch_bounds__(128, 3) k_pair_fast(const PairArgs<float> a) {
                         unsigned mask[TV];
 #pragma unroll
                         for (int tau = 0; tau < TV; ++tau) mask[tau] = 0u;
-                        sweep_faces<TV>(B, f0, f1, px, py, pz, nrc2, mask);
+                        sweep_faces<TV>(B, a.sb, f0, f1, px, py, pz, nrc2, mask);
                         unsigned any = 0u;
 #pragma unroll
                         for (int tau = 0; tau < TV; ++tau) any |= mask[tau];
@@ -534,23 +695,24 @@ __global__ void __launch_bounds__(128, 3) k_pair_fast(const PairArgs<float> a) {
                 F[k] = w.sacc[k * 32 + lane];
                 T[k] = w.sacc[(3 + k) * 32 + lane];
             }
-            if (valid) pair_finish<float>(Mi, t, F, T, w.sacc[6 * 32 + lane], out);
-        }
-        if (in_list) {
-            f4* rec = a.rec + 4 * ((size_t)p * a.slices + slice);
-            f4 r0, r1, r2, r3;
-            r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
-            r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = (float)d[0];
-            r2.x = out[6]; r2.y = out[7]; r2.z = out[8]; r2.w = (float)d[1];
-            r3.x = (float)d[2]; r3.y = r3.z = r3.w = 0.f;
-            rec[0] = r0; rec[1] = r1; rec[2] = r2; rec[3] = r3;
+            if (valid) {
+                const f4 p3 = spose[(buf * 6 + 3) * 32 + lane], p4 = spose[(buf * 6 + 4) * 32 + lane],
+                         p5 = spose[(buf * 6 + 5) * 32 + lane];
+                const float Mi[9] = {p3.x, p3.y, p3.z, p3.w, p4.x, p4.y, p4.z, p4.w, p5.x};
+                float out[10];
+                pair_finish<float>(Mi, t, F, T, w.sacc[6 * 32 + lane], out);
+                f4* rec = a.rec + DEM_REC * ((size_t)spidx[buf * 32 + lane] * a.slices + slice);
+                f4 r0, r1, r2;
+                r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
+                r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = p5.y;
+                r2.x = p5.z; r2.y = p5.w; r2.z = r2.w = 0.f;
+                rec[0] = r0; rec[1] = r1; rec[2] = r2;
+            }
         }
     }
     // counters: one atomic per warp per counter, after the hot loop
-    c_eval = __reduce_add_sync(full, c_eval);
     __syncwarp();
     if (lane == 0) {
-        if (c_eval) atomicAdd(a.counters + 0, (unsigned long long)c_eval);
         if (w.scnt[0]) atomicAdd(a.counters + 1, (unsigned long long)w.scnt[0]);
         if (w.scnt[1]) atomicAdd(a.counters + 2, (unsigned long long)w.scnt[1]);
         if (w.scnt[2]) atomicAdd(a.counters + 3, (unsigned long long)w.scnt[2]);
@@ -558,6 +720,9 @@ __global__ void __launch_bounds__(128, 3) k_pair_fast(const PairArgs<float> a) {
 }
 
 // bytes of dynamic shared memory k_pair_fast needs in front of the staged tables
-static inline size_t fast_smem_header() { return 256 + sizeof(unsigned) * 4 * DEM_QCAP + sizeof(float) * 4 * 7 * 32 + sizeof(unsigned) * 16; }
+static inline size_t fast_smem_header() {
+    return 256 + sizeof(unsigned) * 4 * DEM_QCAP + sizeof(float) * 4 * 7 * 32 + sizeof(unsigned) * 16 +
+           sizeof(f4) * 4 * 2 * 6 * 32 + sizeof(int) * 4 * 2 * 32;
+}
 
 }  // namespace dem

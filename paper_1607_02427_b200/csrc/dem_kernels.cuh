@@ -13,11 +13,16 @@
 namespace dem {
 
 #define DEM_MAX_SHAPES_K 8
+#define DEM_REC 3  // real4 per pair result record
 #define DEM_MAX_CLASSES (DEM_MAX_SHAPES_K * (DEM_MAX_SHAPES_K + 1) / 2)
 
+#define DEM_MAX_FACE_GROUPS 4
 struct ShapeDev {
     int nv, ne, nf, nfe;
-    int off, len;  // block [off, off+len) of the device table, in real4 units: V | E | F | FE
+    int off, len;  // block [off, off+len) of the device table, in real4 units: V | E | F | FE | OE
+    // runs of faces with equal boundary-edge counts (faces are stored sorted by that count): grp_n[g] faces with
+    // grp_m[g] edges each; grp_n = 0 ends the list; grp_m[0] = 0 means "more runs than fit: read each face's header"
+    int grp_m[DEM_MAX_FACE_GROUPS], grp_n[DEM_MAX_FACE_GROUPS];
 };
 
 struct ClassTable {  // indexed by pair class c = lut[s_a][s_b]
@@ -29,6 +34,7 @@ struct ClassTable {  // indexed by pair class c = lut[s_a][s_b]
 
 struct BoxDev {
     double L[3];
+    double invL[3];  // 1 / L (the bit-exact neighbour predicate R13 divides by L; everything else multiplies)
     int dim;
 };
 
@@ -279,6 +285,9 @@ template <typename real> struct PairArgs {
     double reach2;        // (R_a + R_b + 2^(1/6) sigma)^2 : beyond it no term can be inside the cutoff (exact, R10)
     PairConst<real> pc;
     real rc2_search;      // FP32 search kernel: squared candidate cutoff (WCA cutoff + slack, dem_fast.cuh)
+    const f4* pose;       // FP32 search kernel: this class's compacted pose records, pair indices and their number
+    const int* pidx;      //   (written by k_pose)
+    const int* count;
     unsigned long long* counters;  // [0] pairs evaluated, [1] active, [2] degenerate, [3] parallel
 };
 
@@ -328,13 +337,14 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
             c_deg += cnt[1];
             c_par += cnt[2];
         }
-        real4* rec = a.rec + 4 * ((size_t)p * a.slices + slice);
-        real4 r0, r1, r2, r3;
+        // result record (DEM_REC real4 each): (F_i, U_ij) (tau_i, d.x) (d.y, d.z, 0, 0); the reduction derives the other
+        // side: F_j = -F_i, tau_j = -tau_i + d x F_i
+        real4* rec = a.rec + DEM_REC * ((size_t)p * a.slices + slice);
+        real4 r0, r1, r2;
         r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
         r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = (real)d[0];
-        r2.x = out[6]; r2.y = out[7]; r2.z = out[8]; r2.w = (real)d[1];
-        r3.x = (real)d[2]; r3.y = r3.z = r3.w = real(0);
-        rec[0] = r0; rec[1] = r1; rec[2] = r2; rec[3] = r3;
+        r2.x = (real)d[1]; r2.y = (real)d[2]; r2.z = r2.w = real(0);
+        rec[0] = r0; rec[1] = r1; rec[2] = r2;
     }
     // counters: one atomic per warp per counter, after the hot loop
 #pragma unroll
@@ -354,45 +364,57 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
 
 // ---- a8: per-particle reduction -------------------------------------------------------------------------------------
 // a particle's total is the sum over its neighbours.  4 lanes per particle walk its neighbour row, each
-// reads the 64-byte result records of its pairs (sign / side from `slot`), and the 4 partial sums are combined with
-// warp shuffles.  The summation order is fixed, so results are bit-reproducible from run to run.
-template <typename real>
-__global__ void k_reduce(int N, const int* __restrict__ counts, const int* __restrict__ list,
-                         const int* __restrict__ slot, int stride, const int* __restrict__ sid, ClassTable ct,
+// reads the result records of its pairs (which side of the pair it is comes from `slot`, the pair's class from the
+// class-major pair index), and the 4 partial sums are combined with warp shuffles.  The summation order is fixed, so
+// results are bit-reproducible from run to run.  With KICK the lane that stores the result also applies the second
+// half kick of velocity Verlet (v += dt/2 F/m, L += dt/2 tau), which saves a pass over the state.
+// `skip`: when non-null and *skip != 0 the kernel does nothing (dem_step launches the force evaluation before the
+// host knows whether the neighbour list is still valid; see step_t).
+struct KickArgs {
+    double half_dt;
+    int dim;
+    d4* vel;
+    d4* ang;
+    double inv_mass[DEM_MAX_SHAPES_K];
+};
+
+template <typename real, bool KICK>
+__global__ void k_reduce(int N, const int* __restrict__ counts, const int* __restrict__ slot, int stride,
+                         const int* __restrict__ sid, ClassTable ct, int nclass,
                          const typename vec4<real>::type* __restrict__ rec, typename vec4<real>::type* __restrict__ force,
-                         typename vec4<real>::type* __restrict__ torque, real* __restrict__ virial) {
+                         typename vec4<real>::type* __restrict__ torque, real* __restrict__ virial,
+                         const int* __restrict__ skip, KickArgs ka) {
     typedef typename vec4<real>::type real4;
+    if (skip && *skip) return;
     const int gid = blockIdx.x * blockDim.x + threadIdx.x;
     const int i = gid >> 2, sub = gid & 3;
     real F[3] = {0, 0, 0}, T[3] = {0, 0, 0}, U = 0, W[6] = {0, 0, 0, 0, 0, 0};
     if (i < N) {
         const int n = min(counts[i], stride);
-        const int si = sid[i];
         for (int k = sub; k < n; k += 4) {
             const int sl = slot[(size_t)i * stride + k];
-            const int j = list[(size_t)i * stride + k];
             const int p = sl >> 1, side = sl & 1;
-            const int sj = sid[j];
-            const int c = side ? ct.lut[sj][si] : ct.lut[si][sj];
+            int c = 0;
+            while (c + 1 < nclass && p >= ct.pair_base[c + 1]) ++c;
             const int S = ct.slices[c];
-            const real4* r = rec + 4 * ((size_t)ct.rec_base[c] + (size_t)(p - ct.pair_base[c]) * S);
-            const real sgn = side ? real(-1) : real(1);
-            for (int s = 0; s < S; ++s, r += 4) {
-                const real4 r0 = r[0], r1 = r[1], r2 = r[2], r3 = r[3];
-                F[0] += sgn * r0.x;
-                F[1] += sgn * r0.y;
-                F[2] += sgn * r0.z;
+            const real4* r = rec + DEM_REC * ((size_t)ct.rec_base[c] + (size_t)(p - ct.pair_base[c]) * S);
+            for (int s = 0; s < S; ++s, r += DEM_REC) {
+                const real4 r0 = r[0], r1 = r[1], r2 = r[2];
+                const real dx = r1.w, dy = r2.x, dz = r2.y;
+                if (side) {  // this particle is the pair's second one: F_j = -F_i, tau_j = -tau_i + d x F_i
+                    F[0] -= r0.x; F[1] -= r0.y; F[2] -= r0.z;
+                    T[0] += (dy * r0.z - dz * r0.y) - r1.x;
+                    T[1] += (dz * r0.x - dx * r0.z) - r1.y;
+                    T[2] += (dx * r0.y - dy * r0.x) - r1.z;
+                } else {
+                    F[0] += r0.x; F[1] += r0.y; F[2] += r0.z;
+                    T[0] += r1.x; T[1] += r1.y; T[2] += r1.z;
+                }
                 U += real(0.5) * r0.w;
-                T[0] += side ? r2.x : r1.x;
-                T[1] += side ? r2.y : r1.y;
-                T[2] += side ? r2.z : r1.z;
                 // W^{ab} = r_ij^a F_ij^b with r_ij = -d: the same tensor seen from either side; half to each (R12)
-                const real hx = real(-0.5) * r1.w, hy = real(-0.5) * r2.w, hz = real(-0.5) * r3.x;
-                W[0] += hx * r0.x;
-                W[1] += hx * r0.y;
-                W[2] += hx * r0.z;
-                W[3] += hy * r0.y;
-                W[4] += hy * r0.z;
+                const real hx = real(-0.5) * dx, hy = real(-0.5) * dy, hz = real(-0.5) * dz;
+                W[0] += hx * r0.x; W[1] += hx * r0.y; W[2] += hx * r0.z;
+                W[3] += hy * r0.y; W[4] += hy * r0.z;
                 W[5] += hz * r0.z;
             }
         }
@@ -420,6 +442,20 @@ __global__ void k_reduce(int N, const int* __restrict__ counts, const int* __res
 #pragma unroll
             for (int a = 0; a < 6; ++a) virial[(size_t)i * 6 + a] = W[a];
         }
+        if (KICK) {
+            const double hm = ka.half_dt * ka.inv_mass[sid[i]];
+            d4 v = ka.vel[i], L = ka.ang[i];
+            v.x += hm * (double)F[0];
+            v.y += hm * (double)F[1];
+            if (ka.dim == 3) {
+                v.z += hm * (double)F[2];
+                L.x += ka.half_dt * (double)T[0];
+                L.y += ka.half_dt * (double)T[1];
+            }
+            L.z += ka.half_dt * (double)T[2];
+            ka.vel[i] = v;
+            ka.ang[i] = L;
+        }
     }
 }
 
@@ -444,17 +480,29 @@ __device__ inline void free_rotate(int dim, const double* I, const double* L, do
     if (spherical) {
         const double I0 = I[2];
         if (!(I0 > 0.0)) return;
-        const double w[3] = {L[0] / I0, L[1] / I0, L[2] / I0};
-        const double wn = sqrt(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
-        if (wn == 0.0) return;
-        double sh, ch;
-        sincos(0.5 * wn * dt, &sh, &ch);
-        const double sn = sh / wn;
-        const double rq[4] = {ch, sn * w[0], sn * w[1], sn * w[2]};
+        // rotation by phi = |a| about a/|a| with a = (dt / 2 I0) L: rq = (cos phi, (sin phi / phi) a)
+        const double h = 0.5 * dt / I0;
+        const double a[3] = {h * L[0], h * L[1], h * L[2]};
+        const double p2 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2];
+        double ch, sc;  // cos phi, sin phi / phi
+        if (p2 < 0.0625) {  // Taylor series: next terms phi^12 / 12! and phi^12 / 13! are below 1.2e-16 here
+            ch = 1.0 + p2 * (-1.0 / 2 + p2 * (1.0 / 24 + p2 * (-1.0 / 720 + p2 * (1.0 / 40320 + p2 * (-1.0 / 3628800)))));
+            sc = 1.0 + p2 * (-1.0 / 6 + p2 * (1.0 / 120 + p2 * (-1.0 / 5040 + p2 * (1.0 / 362880 + p2 * (-1.0 / 39916800)))));
+        } else {
+            const double ph = sqrt(p2);
+            double sh;
+            sincos(ph, &sh, &ch);
+            sc = sh / ph;
+        }
+        const double rq[4] = {ch, sc * a[0], sc * a[1], sc * a[2]};
         double o[4];
         quat_mul_d(rq, q, o);
-        const double n = sqrt(o[0] * o[0] + o[1] * o[1] + o[2] * o[2] + o[3] * o[3]);
-        for (int k = 0; k < 4; ++k) q[k] = o[k] / n;
+        // |o| = |q| (1 + O(1e-16)): two Newton steps of 1/sqrt from 1 renormalise a q that is unit to float precision
+        const double n2 = o[0] * o[0] + o[1] * o[1] + o[2] * o[2] + o[3] * o[3];
+        double inv = 1.5 - 0.5 * n2;
+        inv = inv * (1.5 - 0.5 * n2 * inv * inv);
+        inv = inv * (1.5 - 0.5 * n2 * inv * inv);
+        for (int k = 0; k < 4; ++k) q[k] = o[k] * inv;
         return;
     }
     double M[9], Lb[3];
@@ -494,15 +542,15 @@ __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const int s = sid[i];
-    const double m = mt.mass[s];
+    const double hm = 0.5 * dt / mt.mass[s];
     d4 x = pos[i], v = vel[i], L = ang[i], q = quat[i];
     const typename vec4<real>::type F = force[i], T = torque[i];
     double xs[3] = {x.x, x.y, x.z}, vs[3] = {v.x, v.y, v.z}, Ls[3] = {L.x, L.y, L.z};
     const double Fs[3] = {(double)F.x, (double)F.y, (double)F.z}, Ts[3] = {(double)T.x, (double)T.y, (double)T.z};
     for (int a = 0; a < box.dim; ++a) {
-        vs[a] += 0.5 * dt * Fs[a] / m;
+        vs[a] += hm * Fs[a];
         xs[a] += dt * vs[a];
-        xs[a] -= box.L[a] * rint(xs[a] / box.L[a]);
+        xs[a] -= box.L[a] * rint(xs[a] * box.invL[a]);
     }
     for (int a = (box.dim == 2 ? 2 : 0); a < 3; ++a) Ls[a] += 0.5 * dt * Ts[a];
     double qs[4] = {q.x, q.y, q.z, q.w};
@@ -513,30 +561,11 @@ __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict
     q.x = qs[0]; q.y = qs[1]; q.z = qs[2]; q.w = qs[3];
     pos[i] = x; vel[i] = v; ang[i] = L; quat[i] = q;
     const d4 xb = pos_build[i];
-    const double dx = min_image_1(xb.x, xs[0], box.L[0]), dy = min_image_1(xb.y, xs[1], box.L[1]);
-    const double dz = box.dim == 3 ? min_image_1(xb.z, xs[2], box.L[2]) : 0.0;
+    double dx = xs[0] - xb.x, dy = xs[1] - xb.y, dz = box.dim == 3 ? xs[2] - xb.z : 0.0;
+    dx -= box.L[0] * rint(dx * box.invL[0]);
+    dy -= box.L[1] * rint(dy * box.invL[1]);
+    dz -= box.L[2] * rint(dz * box.invL[2]);
     if (dx * dx + dy * dy + dz * dz > half_skin2) *moved = 1;
-}
-
-template <typename real>
-__global__ void k_kick(int N, int dim, double dt, const int* __restrict__ sid, MassTable mt, d4* __restrict__ vel,
-                       d4* __restrict__ ang, const typename vec4<real>::type* __restrict__ force,
-                       const typename vec4<real>::type* __restrict__ torque) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    const double m = mt.mass[sid[i]];
-    d4 v = vel[i], L = ang[i];
-    const typename vec4<real>::type F = force[i], T = torque[i];
-    v.x += 0.5 * dt * (double)F.x / m;
-    v.y += 0.5 * dt * (double)F.y / m;
-    if (dim == 3) {
-        v.z += 0.5 * dt * (double)F.z / m;
-        L.x += 0.5 * dt * (double)T.x;
-        L.y += 0.5 * dt * (double)T.y;
-    }
-    L.z += 0.5 * dt * (double)T.z;
-    vel[i] = v;
-    ang[i] = L;
 }
 
 // U, K_trans, K_rot: per-block partial sums in double (fixed order), summed on the host.

@@ -58,6 +58,7 @@ struct dem_ctx {
     double box[3] = {0, 0, 0}, r_cut = 0;
     GridDev grid;
     DevBuf cell_of, rank, cell_start, order, xs, counts, list, slot, scratch_scan, pcnt, pairs, rec, flags, counters;
+    DevBuf pose, pidx, ccount;  // FP32 search kernel: compacted pose records per class (k_pose)
     ClassTable ct;
     int nclass = 0;
     int class_sa[DEM_MAX_CLASSES], class_sb[DEM_MAX_CLASSES], class_np[DEM_MAX_CLASSES];
@@ -77,6 +78,8 @@ struct dem_ctx {
     size_t ev_used = 0;
     int64_t last_terms = 0;
     int sm_count = 148;
+    int* h_moved = nullptr;        // pinned host copy of dem_step's "list is stale" flag
+    cudaEvent_t ev_flag = nullptr;
 };
 
 namespace {
@@ -133,6 +136,12 @@ template <typename real> int upload_table(dem_ctx* ctx) {
         d.nv = S.nv; d.ne = S.ne; d.nf = S.nf; d.nfe = S.nfe;
         d.off = (int)host.size();
         d.len = S.table_len4();
+        for (int g = 0; g < DEM_MAX_FACE_GROUPS; ++g) d.grp_m[g] = d.grp_n[g] = 0;
+        if ((int)S.face_groups.size() <= DEM_MAX_FACE_GROUPS)
+            for (size_t g = 0; g < S.face_groups.size(); ++g) {
+                d.grp_m[g] = S.face_groups[g].first;
+                d.grp_n[g] = S.face_groups[g].second;
+            }
         for (int k = 0; k < d.len; ++k) {
             real4 v;
             v.x = (real)S.table[4 * k]; v.y = (real)S.table[4 * k + 1];
@@ -216,6 +225,7 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
     bx.dim = ctx->dim;
     for (int a = 0; a < 3; ++a) bx.L[a] = box[a];
     if (ctx->dim == 2) bx.L[2] = 1.0;
+    for (int a = 0; a < 3; ++a) bx.invL[a] = 1.0 / bx.L[a];
     // cells at least r_cut wide (with a relative margin far above double rounding), at most ~2 N + 64 cells in all
     GridDev g;
     g.nc[0] = g.nc[1] = g.nc[2] = 1;
@@ -315,9 +325,9 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
     ctx->ct.rec_base[nc] = (int)nrec;
     ctx->nrec_total = nrec;
     ctx->last_terms = terms;
-    if (nrec * 4 > 0x7fffffffLL) return fail(ctx, DEM_EOVERFLOW, "too many pair records");
+    if (nrec * DEM_REC > 0x7fffffffLL) return fail(ctx, DEM_EOVERFLOW, "too many pair records");
     CU(ctx->pairs.reserve(sizeof(int2) * (size_t)std::max<long long>(ctx->npairs_total, 1)));
-    CU(ctx->rec.reserve((ctx->prec == DEM_F64 ? sizeof(d4) : sizeof(f4)) * 4 * (size_t)std::max<long long>(nrec, 1)));
+    CU(ctx->rec.reserve((ctx->prec == DEM_F64 ? sizeof(d4) : sizeof(f4)) * DEM_REC * (size_t)std::max<long long>(nrec, 1)));
     k_pair_fill<<<nblk(N, B), B, 0, st>>>(N, ctx->counts.as<int>(), ctx->list.as<int>(), ctx->stride, sid, ctx->ct, nc,
                                           pcnt, ctx->pairs.as<int2>(), ctx->slot.as<int>());
     LAUNCHED(ctx);
@@ -332,17 +342,25 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
 // ---- force evaluation ---------------------------------------------------------------------------------------------
 template <typename real, typename PosT>
 int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* sid, int N, void* force, void* torque,
-              void* virial) {
+              void* virial, const int* skip = nullptr, const KickArgs* kick = nullptr) {
     typedef typename vec4<real>::type real4;
     if (!ctx->have_list) return fail(ctx, DEM_ESTALE, "no neighbour list: call dem_build_neighbors first");
     if (N != ctx->N) return fail(ctx, DEM_ESTALE, "N = %d differs from the last build (%d)", N, ctx->N);
     if (!pos || !quat || !sid || !force || !torque) return fail(ctx, DEM_EINVAL, "null particle array");
     cudaStream_t st = ctx->stream;
     CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8, st));
+    const bool search = std::is_same<real, float>::value && !ctx->generic_kernel;
+    if (search) {
+        CU(ctx->pose.reserve(sizeof(f4) * 6 * (size_t)std::max<long long>(ctx->npairs_total, 1)));
+        CU(ctx->pidx.reserve(sizeof(int) * (size_t)std::max<long long>(ctx->npairs_total, 1)));
+        CU(ctx->ccount.reserve(sizeof(int) * DEM_MAX_CLASSES));
+        CU(cudaMemsetAsync(ctx->ccount.p, 0, sizeof(int) * DEM_MAX_CLASSES, st));
+    }
     BoxDev bx;
     bx.dim = ctx->dim;
     for (int a = 0; a < 3; ++a) bx.L[a] = ctx->box[a];
     if (ctx->dim == 2) bx.L[2] = 1.0;
+    for (int a = 0; a < 3; ++a) bx.invL[a] = 1.0 / bx.L[a];
     for (int c = 0; c < ctx->nclass; ++c) {
         const int np = ctx->class_np[c];
         if (np == 0) continue;
@@ -355,7 +373,7 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
         a.npairs = np;
         a.slices = ctx->ct.slices[c];
         a.n_outer = class_outer(ctx, c);
-        a.rec = ctx->rec.as<real4>() + 4 * (size_t)ctx->ct.rec_base[c];
+        a.rec = ctx->rec.as<real4>() + DEM_REC * (size_t)ctx->ct.rec_base[c];
         a.pos = pos;
         a.quat = quat;
         a.box = bx;
@@ -376,19 +394,50 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
         size_t smem = sizeof(real4) * (size_t)(a.sa.len + (a.sa.off == a.sb.off ? 0 : a.sb.len));
         const long long items = (long long)((np + 31) & ~31) * a.slices;
         const int threads = 128;
-        const int grid = (int)std::min<long long>(nblk(items, threads), (long long)ctx->sm_count * 64);
+        int grid = (int)std::min<long long>(nblk(items, threads), (long long)ctx->sm_count * 64);
         void (*kern)(const PairArgs<real>) = ctx->dim == 3 ? k_pair<real, PosT, 3> : k_pair<real, PosT, 2>;
+        PoseArgs pa;
         if constexpr (std::is_same<real, float>::value) {
-            if (!ctx->generic_kernel) {
+            if (search) {
+                a.pose = ctx->pose.as<f4>() + 6 * (size_t)ctx->ct.pair_base[c];
+                a.pidx = ctx->pidx.as<int>() + ctx->ct.pair_base[c];
+                a.count = ctx->ccount.as<int>() + c;
+                pa.pairs = a.pairs; pa.npairs = np; pa.slices = a.slices; pa.pos = pos; pa.quat = quat; pa.box = bx;
+                pa.reach2 = a.reach2;
+                pa.pose = ctx->pose.as<f4>() + 6 * (size_t)ctx->ct.pair_base[c];
+                pa.pidx = ctx->pidx.as<int>() + ctx->ct.pair_base[c];
+                pa.count = ctx->ccount.as<int>() + c;
+                pa.rec = reinterpret_cast<f4*>(a.rec);
+                pa.counters = a.counters;
                 smem += fast_smem_header();
                 // packed outer pairs per sweep: 3 when the vertex counts fill tiles of 6 at least as well as tiles of 4
                 auto waste = [](int n, int tile) { return ((n + tile - 1) / tile) * tile - n; };
                 const int nva = HA.nv, nvb = HB.nv;
                 const bool tv3 = waste(nva, 6) + waste(nvb, 6) <= waste(nva, 4) + waste(nvb, 4);
                 if (ctx->dim == 3)
-                    kern = tv3 ? k_pair_fast<PosT, 3, 2, 3> : k_pair_fast<PosT, 3, 2, 2>;
+                    kern = tv3 ? k_pair_fast<PosT, 3, 2, 3, 4> : k_pair_fast<PosT, 3, 2, 2, 4>;
                 else
-                    kern = tv3 ? k_pair_fast<PosT, 2, 2, 3> : k_pair_fast<PosT, 2, 2, 2>;
+                    kern = tv3 ? k_pair_fast<PosT, 2, 2, 3, 4> : k_pair_fast<PosT, 2, 2, 2, 4>;
+                int resident = 64;  // grid cap in blocks per SM (measured on cfg4: one tile per warp beats one persistent wave)
+#ifdef DEM_TUNE
+                if (const char* v = getenv("DEM_VARIANT")) {
+                    if (ctx->dim == 3 && sizeof(PosT) == 8) {
+                        switch (atoi(v)) {
+                            case 0: kern = k_pair_fast<PosT, 3, 2, 3, 3>; break;
+                            case 1: kern = k_pair_fast<PosT, 3, 2, 3, 4>; break;
+                            case 2: kern = k_pair_fast<PosT, 3, 1, 3, 4>; break;
+                            case 5: kern = k_pair_fast<PosT, 3, 2, 2, 4>; break;
+                            case 7: kern = k_pair_fast<PosT, 3, 3, 3, 3>; break;
+                        }
+                    }
+                }
+                if (const char* v = getenv("DEM_RESIDENT")) resident = atoi(v);
+                if (const char* v = getenv("DEM_PHASES")) {
+                    const int ph = atoi(v);
+                    cudaMemcpyToSymbolAsync(g_dbg_phases, &ph, sizeof ph, 0, cudaMemcpyHostToDevice, st);
+                }
+#endif
+                grid = (int)std::min<long long>(nblk(items, threads), (long long)ctx->sm_count * resident);
             }
         }
         if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -405,14 +454,25 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
             ctx->ev_used++;
             CU(cudaEventRecord(e0, st));
         }
+        if (search) {  // a3 (relative poses, compaction) runs as its own kernel in front of the search kernel
+            if (ctx->dim == 3)
+                k_pose<PosT, 3><<<nblk(np, 128), 128, 0, st>>>(pa);
+            else
+                k_pose<PosT, 2><<<nblk(np, 128), 128, 0, st>>>(pa);
+            LAUNCHED(ctx);
+        }
         kern<<<grid, threads, smem, st>>>(a);
         LAUNCHED(ctx);
         if (ctx->timing) CU(cudaEventRecord(e1, st));
     }
-    k_reduce<real><<<nblk(4LL * N, 128), 128, 0, st>>>(N, ctx->counts.as<int>(), ctx->list.as<int>(), ctx->slot.as<int>(),
-                                                      ctx->stride, sid, ctx->ct, ctx->rec.as<real4>(),
-                                                      static_cast<real4*>(force), static_cast<real4*>(torque),
-                                                      static_cast<real*>(virial));
+    if (kick)
+        k_reduce<real, true><<<nblk(4LL * N, 128), 128, 0, st>>>(
+            N, ctx->counts.as<int>(), ctx->slot.as<int>(), ctx->stride, sid, ctx->ct, ctx->nclass, ctx->rec.as<real4>(),
+            static_cast<real4*>(force), static_cast<real4*>(torque), static_cast<real*>(virial), skip, *kick);
+    else
+        k_reduce<real, false><<<nblk(4LL * N, 128), 128, 0, st>>>(
+            N, ctx->counts.as<int>(), ctx->slot.as<int>(), ctx->stride, sid, ctx->ct, ctx->nclass, ctx->rec.as<real4>(),
+            static_cast<real4*>(force), static_cast<real4*>(torque), static_cast<real*>(virial), skip, KickArgs());
     LAUNCHED(ctx);
     CU(cudaGetLastError());
     return DEM_OK;
@@ -453,24 +513,37 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     bx.dim = ctx->dim;
     for (int a = 0; a < 3; ++a) bx.L[a] = box[a];
     if (ctx->dim == 2) bx.L[2] = 1.0;
+    for (int a = 0; a < 3; ++a) bx.invL[a] = 1.0 / bx.L[a];
     CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
     CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr)));
     int* moved = ctx->flags.as<int>() + 8;
     const double half_skin2 = 0.25 * skin * skin;
     if (ctx->l2_flush_bytes) CU(ctx->l2_scratch.reserve(ctx->l2_flush_bytes));
+    if (!ctx->h_moved) CU(cudaHostAlloc(&ctx->h_moved, sizeof(int), cudaHostAllocDefault));
+    if (!ctx->ev_flag) CU(cudaEventCreateWithFlags(&ctx->ev_flag, cudaEventDisableTiming));
+    KickArgs ka;
+    ka.half_dt = 0.5 * dt;
+    ka.dim = ctx->dim;
+    ka.vel = v;
+    ka.ang = L;
+    for (int k = 0; k < DEM_MAX_SHAPES_K; ++k) ka.inv_mass[k] = ctx->mt.mass[k] > 0 ? 1.0 / ctx->mt.mass[k] : 0.0;
     for (int s = 0; s < nsteps; ++s) {
         if (ctx->l2_flush_bytes) CU(cudaMemsetAsync(ctx->l2_scratch.p, s & 0xff, ctx->l2_flush_bytes, st));
         CU(cudaMemsetAsync(moved, 0, sizeof(int), st));
         k_kick_drift<real><<<nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T, ctx->pos_build.as<d4>(),
                                                      half_skin2, moved);
         LAUNCHED(ctx);
-        int m = 0;
-        CU(cudaMemcpyAsync(&m, moved, sizeof(int), cudaMemcpyDeviceToHost, st));
-        CU(cudaStreamSynchronize(st));
-        if (m) CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
-        CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr)));
-        k_kick<real><<<nblk(N, B), B, 0, st>>>(N, ctx->dim, dt, sid, ctx->mt, v, L, F, T);
-        LAUNCHED(ctx);
+        CU(cudaMemcpyAsync(ctx->h_moved, moved, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CU(cudaEventRecord(ctx->ev_flag, st));
+        // The force evaluation and the second half kick are queued before the host knows whether some particle has
+        // left its skin: the reduction (which alone changes state) does nothing if `moved` is set, so the GPU never
+        // idles on the host's answer.  In the rare step that needs a new list the host rebuilds it and evaluates again.
+        CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr, moved, &ka)));
+        CU(cudaEventSynchronize(ctx->ev_flag));
+        if (*ctx->h_moved) {
+            CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
+            CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr, nullptr, &ka)));
+        }
     }
     if (conv) {
         void* out[4] = {pos, quat, vel, ang};
@@ -533,10 +606,12 @@ int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda
 int dem_destroy(dem_ctx* c) {
     if (!c) return DEM_EINVAL;
     DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
-                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->st_pos, &c->st_quat,
+                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->pose, &c->pidx, &c->ccount, &c->st_pos, &c->st_quat,
                       &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->pos_build, &c->epart, &c->h_pos,
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();
+    if (c->h_moved) cudaFreeHost(c->h_moved);
+    if (c->ev_flag) cudaEventDestroy(c->ev_flag);
     for (auto& e : c->ev_pool) {
         cudaEventDestroy(e.first);
         cudaEventDestroy(e.second);

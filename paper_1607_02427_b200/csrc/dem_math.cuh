@@ -64,8 +64,9 @@ DEM_HD double rcp(double x) { return 1.0 / x; }
 // two shapes of its class into shared memory and builds these views over them.
 //   V [nv]      (x, y, z, 0)                                   body-frame vertex
 //   E [2 ne]    3D: [2k] = (a.xyz, |e|^2)  [2k+1] = (e.xyz, 1/|e|^2 or 0 if |e| = 0)      edge k = a + s e, s in [0,1]
-//               2D: [2k] = (a.x, a.y, u.x, u.y)  [2k+1] = (|e|, cs, cu, 0)                  u = e/|e| (0 if |e| = 0)
-//                   cs = -(u x a), cu = -(u . a): for a point q, side = u x q + cs and along = u . q + cu
+//               2D: [2k] = (a.x, a.y, u.x, u.y)  [2k+1] = (|e|, cs, cm, |e|/2)              u = e/|e| ((1,0) if |e| = 0)
+//                   cs = -(u x a), cm = -(u . a) - |e|/2: for a point q, side = u x q + cs and u . q + cm is the
+//                   along-edge coordinate measured from the edge's midpoint
 //   F [4 nf]    [4f] = (uhat, -uhat.o) [4f+1] = (vhat, -vhat.o) [4f+2] = (nhat, -nhat.o) [4f+3] = (first FE, count, 0, 0)
 //   FE[2 nfe]   face boundary edges in the face's (uhat, vhat) coordinates, CCW about nhat: same layout as 2D edges
 //   OE[2 ne]    3D only: [2k] = (a.xyz, |e|)  [2k+1] = (e/|e|, 0): the edges as the search kernel's outer features

@@ -25,6 +25,7 @@ struct HostShape {
     double rounding = 0, mass = 1, inertia[3] = {1, 1, 1}, circumradius = 0;
     // flattened table in double, in units of 4 doubles: V (nv) | E (2 ne) | F (4 nf) | FE (2 nfe) | OE (2 ne, 3D only)
     std::vector<double> table;
+    std::vector<std::pair<int, int>> face_groups;  // runs of faces with the same number of boundary edges
     double max_edge = 0;  // longest edge (bounds the search kernel's near-parallel slack)
     int table_len4() const { return nv + 2 * ne + 4 * nf + 2 * nfe + (dim == 3 ? 2 * ne : 0); }
 };
@@ -70,6 +71,28 @@ inline std::string build_host_shape(HostShape& S, int dim, const double* verts, 
             S.face_verts.push_back(face_verts[m]);
         }
         S.face_off.push_back((int)S.face_verts.size());
+    }
+    // faces are kept sorted by vertex count (stable), so that the search kernel sweeps runs of equal-sized faces with
+    // unrolled code; the order of faces has no meaning in the method (Eq. 1 sums over all of them)
+    {
+        std::vector<int> idx(nf);
+        for (int f = 0; f < nf; ++f) idx[f] = f;
+        std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) {
+            return S.face_off[a + 1] - S.face_off[a] < S.face_off[b + 1] - S.face_off[b];
+        });
+        std::vector<int> off(1, 0), fv;
+        for (int f : idx) {
+            for (int m = S.face_off[f]; m < S.face_off[f + 1]; ++m) fv.push_back(S.face_verts[m]);
+            off.push_back((int)fv.size());
+        }
+        S.face_off.swap(off);
+        S.face_verts.swap(fv);
+        S.face_groups.clear();  // (vertex count, number of faces) runs
+        for (int f = 0; f < nf; ++f) {
+            const int n = S.face_off[f + 1] - S.face_off[f];
+            if (S.face_groups.empty() || S.face_groups.back().first != n) S.face_groups.push_back({n, 0});
+            S.face_groups.back().second++;
+        }
     }
     // edges: explicit, or derived (2D: closed CCW polygon; 3D: unique boundary edges of the faces)
     S.edges.clear();
@@ -124,8 +147,9 @@ inline std::string build_host_shape(HostShape& S, int dim, const double* verts, 
             // whatever u is, and the search kernel's side^2 + excess^2 form needs |u| = 1
             const double ux = len > 0 ? e[0] / len : 1.0, uy = len > 0 ? e[1] / len : 0.0;
             push4(T, a[0], a[1], ux, uy);
-            // for a point (x, y): side = ux y - uy x + cs, along = ux x + uy y + cu (used by the search kernel)
-            push4(T, len, -(ux * a[1] - uy * a[0]), -(ux * a[0] + uy * a[1]), 0);
+            // for a point (x, y): side = ux y - uy x + cs, centred along-edge coordinate = ux x + uy y + cm (0 at the
+            // edge's midpoint); used by the search kernel
+            push4(T, len, -(ux * a[1] - uy * a[0]), -(ux * a[0] + uy * a[1]) - 0.5 * len, 0.5 * len);
         }
     }
     std::vector<double> FE;
@@ -182,10 +206,11 @@ inline std::string build_host_shape(HostShape& S, int dim, const double* verts, 
             const double ex = p1[0] - p0[0], ey = p1[1] - p0[1];
             const double len = std::sqrt(ex * ex + ey * ey);
             if (!(len > 0)) return "face has a repeated vertex";
-            // with (x, y) the point in the face frame: side = ux y - uy x + cs (>= 0 inside), along = ux x + uy y + cu
+            // with (x, y) the point in the face frame: side = ux y - uy x + cs (>= 0 inside), centred along-edge
+            // coordinate = ux x + uy y + cm (0 at the edge's midpoint)
             const double ux = ex / len, uy = ey / len;
             push4(FE, p0[0], p0[1], ux, uy);
-            push4(FE, len, -(ux * p0[1] - uy * p0[0]), -(ux * p0[0] + uy * p0[1]), 0);
+            push4(FE, len, -(ux * p0[1] - uy * p0[0]), -(ux * p0[0] + uy * p0[1]) - 0.5 * len, 0.5 * len);
             nfe++;
         }
     }
