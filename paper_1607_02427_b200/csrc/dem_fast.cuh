@@ -393,12 +393,13 @@ struct PoseArgs {
     int* pidx;
     int* count;  // valid pairs of this class (zeroed before the launch)
     f4* rec;
-    unsigned long long* counters;
 };
 
-template <typename PosT, int DIM> __global__ void __launch_bounds__(128) k_pose(const PoseArgs a) {
+#define DEM_POSE_THREADS 256
+template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THREADS) k_pose(const PoseArgs a) {
+    __shared__ int wcount[DEM_POSE_THREADS / 32], wbase[DEM_POSE_THREADS / 32];
     const unsigned full = 0xffffffffu;
-    const int p = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     bool valid = false;
     float Mi[9], R[9], t[3];
     double d[3] = {0.0, 0.0, 0.0};
@@ -426,12 +427,22 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(128) k_pose(
             }
         }
     }
+    // compaction: one atomic per block (same-address atomics serialise in L2: one per warp costs as much as the poses)
     const unsigned m = __ballot_sync(full, valid);
-    int base = 0;
-    if (lane == 0 && m) base = atomicAdd(a.count, __popc(m));
-    base = __shfl_sync(full, base, 0);
+    if (lane == 0) wcount[warp] = __popc(m);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int tot = 0;
+        for (int k = 0; k < DEM_POSE_THREADS / 32; ++k) {
+            wbase[k] = tot;
+            tot += wcount[k];
+        }
+        const int b = tot ? atomicAdd(a.count, tot) : 0;
+        for (int k = 0; k < DEM_POSE_THREADS / 32; ++k) wbase[k] += b;
+    }
+    __syncthreads();
     if (valid) {
-        const int c = base + __popc(m & ((1u << lane) - 1u));
+        const int c = wbase[warp] + __popc(m & ((1u << lane) - 1u));
         const size_t n = (size_t)a.npairs;
         f4 v;
         v.x = R[0]; v.y = R[1]; v.z = R[2]; v.w = R[3]; a.pose[c] = v;
@@ -442,7 +453,6 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(128) k_pose(
         v.x = Mi[8]; v.y = (float)d[0]; v.z = (float)d[1]; v.w = (float)d[2]; a.pose[5 * n + c] = v;
         a.pidx[c] = p;
     }
-    if (lane == 0 && m) atomicAdd(a.counters, (unsigned long long)__popc(m));
 }
 
 #ifdef DEM_TUNE

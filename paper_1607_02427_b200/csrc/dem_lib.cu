@@ -58,7 +58,7 @@ struct dem_ctx {
     double box[3] = {0, 0, 0}, r_cut = 0;
     GridDev grid;
     DevBuf cell_of, rank, cell_start, order, xs, counts, list, slot, scratch_scan, pcnt, pairs, rec, flags, counters;
-    DevBuf pose, pidx, ccount;  // FP32 search kernel: compacted pose records per class (k_pose)
+    DevBuf pose, pidx;  // FP32 search kernel: compacted pose records per class (k_pose)
     ClassTable ct;
     int nclass = 0;
     int class_sa[DEM_MAX_CLASSES], class_sb[DEM_MAX_CLASSES], class_np[DEM_MAX_CLASSES];
@@ -248,7 +248,7 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
     CU(ctx->counts.reserve(sizeof(int) * (size_t)N));
     CU(ctx->scratch_scan.reserve(sizeof(int) * scan_ints));
     CU(ctx->flags.reserve(sizeof(int) * 16));
-    CU(ctx->counters.reserve(sizeof(unsigned long long) * 8));
+    CU(ctx->counters.reserve(sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES));
     CU(ctx->pos_build.reserve(sizeof(d4) * (size_t)N));
     int* cell_start = ctx->cell_start.as<int>();
     CU(cudaMemsetAsync(cell_start, 0, sizeof(int) * ((size_t)g.ncell + 1), st));
@@ -348,13 +348,13 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
     if (N != ctx->N) return fail(ctx, DEM_ESTALE, "N = %d differs from the last build (%d)", N, ctx->N);
     if (!pos || !quat || !sid || !force || !torque) return fail(ctx, DEM_EINVAL, "null particle array");
     cudaStream_t st = ctx->stream;
-    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8, st));
+    // counters[0..7] (unsigned long long) followed by the per-class numbers of in-reach pairs (int): one memset
+    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES, st));
+    int* ccount = reinterpret_cast<int*>(ctx->counters.as<unsigned long long>() + 8);
     const bool search = std::is_same<real, float>::value && !ctx->generic_kernel;
     if (search) {
         CU(ctx->pose.reserve(sizeof(f4) * 6 * (size_t)std::max<long long>(ctx->npairs_total, 1)));
         CU(ctx->pidx.reserve(sizeof(int) * (size_t)std::max<long long>(ctx->npairs_total, 1)));
-        CU(ctx->ccount.reserve(sizeof(int) * DEM_MAX_CLASSES));
-        CU(cudaMemsetAsync(ctx->ccount.p, 0, sizeof(int) * DEM_MAX_CLASSES, st));
     }
     BoxDev bx;
     bx.dim = ctx->dim;
@@ -401,14 +401,13 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
             if (search) {
                 a.pose = ctx->pose.as<f4>() + 6 * (size_t)ctx->ct.pair_base[c];
                 a.pidx = ctx->pidx.as<int>() + ctx->ct.pair_base[c];
-                a.count = ctx->ccount.as<int>() + c;
+                a.count = ccount + c;
                 pa.pairs = a.pairs; pa.npairs = np; pa.slices = a.slices; pa.pos = pos; pa.quat = quat; pa.box = bx;
                 pa.reach2 = a.reach2;
                 pa.pose = ctx->pose.as<f4>() + 6 * (size_t)ctx->ct.pair_base[c];
                 pa.pidx = ctx->pidx.as<int>() + ctx->ct.pair_base[c];
-                pa.count = ctx->ccount.as<int>() + c;
+                pa.count = ccount + c;
                 pa.rec = reinterpret_cast<f4*>(a.rec);
-                pa.counters = a.counters;
                 smem += fast_smem_header();
                 // packed outer pairs per sweep: 3 when the vertex counts fill tiles of 6 at least as well as tiles of 4
                 auto waste = [](int n, int tile) { return ((n + tile - 1) / tile) * tile - n; };
@@ -456,9 +455,9 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
         }
         if (search) {  // a3 (relative poses, compaction) runs as its own kernel in front of the search kernel
             if (ctx->dim == 3)
-                k_pose<PosT, 3><<<nblk(np, 128), 128, 0, st>>>(pa);
+                k_pose<PosT, 3><<<nblk(np, DEM_POSE_THREADS), DEM_POSE_THREADS, 0, st>>>(pa);
             else
-                k_pose<PosT, 2><<<nblk(np, 128), 128, 0, st>>>(pa);
+                k_pose<PosT, 2><<<nblk(np, DEM_POSE_THREADS), DEM_POSE_THREADS, 0, st>>>(pa);
             LAUNCHED(ctx);
         }
         kern<<<grid, threads, smem, st>>>(a);
@@ -606,7 +605,7 @@ int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda
 int dem_destroy(dem_ctx* c) {
     if (!c) return DEM_EINVAL;
     DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
-                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->pose, &c->pidx, &c->ccount, &c->st_pos, &c->st_quat,
+                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->pose, &c->pidx, &c->st_pos, &c->st_quat,
                       &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->pos_build, &c->epart, &c->h_pos,
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();
@@ -703,9 +702,14 @@ int dem_compute(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* 
 int dem_get_counters(dem_ctx* ctx, int64_t out[6]) {
     if (!ctx || !out) return DEM_EINVAL;
     if (!ctx->counters.p) return fail(ctx, DEM_ESTALE, "no evaluation yet");
-    unsigned long long h[4];
+    unsigned long long h[8 + DEM_MAX_CLASSES / 2];
     CU(cudaMemcpyAsync(h, ctx->counters.p, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
+    if (ctx->prec == DEM_F32 && !ctx->generic_kernel) {  // the search path counts its evaluated pairs per class (k_pose)
+        const int* cc = reinterpret_cast<const int*>(h + 8);
+        h[0] = 0;
+        for (int c = 0; c < ctx->nclass; ++c) h[0] += (unsigned long long)cc[c];
+    }
     // terms evaluated = nominal terms of the evaluated pairs; with a single class this is exact, with several classes
     // pairs rejected by the reach test are attributed proportionally (the list is normally built at r_cut = reach)
     out[0] = (int64_t)h[0];
