@@ -202,6 +202,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
     ap.add_argument("--no-l2-flush", action="store_true")
+    ap.add_argument("--slices", type=int, default=0, help="lanes per pair in the pair kernel (0 = library heuristic)")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
@@ -234,6 +235,8 @@ def main():
     st = di.make_config(k, seed=rank)  # independent replica per rank
     n, dt_step, skin = st["N"], st["dt"], SKIN[k]
     dem, t = pkg.from_state(st, "f32")
+    if args.slices:
+        dem.set_slices(args.slices)
     if not args.no_l2_flush:
         dem.set_l2_flush(L2_FLUSH_BYTES)
     force = torch.empty((n, 4), dtype=torch.float32, device="cuda")

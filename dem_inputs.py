@@ -152,6 +152,14 @@ def box_shape(lx, ly, lz, rounding, mass=1.0):
                               for z in (-lz / 2, lz / 2)], rounding, mass)
 
 
+def prism(n, circumradius=0.5, height=0.6, rounding=0.05, mass=1.0):
+    """Right prism over a regular n-gon (two n-gon faces, n rectangles): faces with many boundary edges."""
+    ang = 2 * math.pi * np.arange(n) / n
+    ring = np.stack([circumradius * np.cos(ang), circumradius * np.sin(ang)], 1)
+    v = np.concatenate([np.c_[ring, np.full(n, -height / 2)], np.c_[ring, np.full(n, height / 2)]])
+    return convex_polyhedron(v, rounding, mass)
+
+
 def octahedron(circumradius=0.5, rounding=0.075, mass=1.0):
     r = circumradius
     return convex_polyhedron([[r, 0, 0], [-r, 0, 0], [0, r, 0], [0, -r, 0], [0, 0, r], [0, 0, -r]], rounding, mass)

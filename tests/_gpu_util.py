@@ -19,12 +19,14 @@ def scales(st, of, ot):
     return max(np.abs(of[:, :3]).max(), eps / sig), max(np.abs(ot[:, :3]).max(), eps), max(np.abs(of[:, 3]).max(), eps)
 
 
-def gpu_compute(st, precision, slices=0, r_cut=None, virial=True):
+def gpu_compute(st, precision, slices=0, r_cut=None, virial=True, kernel=None):
     import paper_1607_02427_b200 as pkg
 
     dem, t = pkg.from_state(st, precision)
     if slices:
         dem.set_slices(slices)
+    if kernel is not None:
+        dem.set_pair_kernel(kernel)
     dem.build_neighbors(t["pos"], t["shape_id"], st["box"], st["r_cut"] if r_cut is None else r_cut)
     f, tq, w = dem.compute(t["pos"], t["quat"], t["shape_id"], virial=virial)
     out = (f.cpu().numpy().astype(np.float64), tq.cpu().numpy().astype(np.float64),
@@ -33,10 +35,10 @@ def gpu_compute(st, precision, slices=0, r_cut=None, virial=True):
     return out
 
 
-def assert_parity(st, precision, oracle, slices=0, subset=None, r_cut=None, tol=None):
+def assert_parity(st, precision, oracle, slices=0, subset=None, r_cut=None, tol=None, kernel=None):
     """Element-by-element comparison of force, torque, energy, virial and of the term counters."""
     st = round_state(st, precision)
-    f, tq, w, cnt = gpu_compute(st, precision, slices, r_cut)
+    f, tq, w, cnt = gpu_compute(st, precision, slices, r_cut, kernel=kernel)
     of, ot, ow, ocnt = oracle.compute(st, subset=subset)
     if subset is not None:
         f, tq, w = f[subset], tq[subset], w[subset]

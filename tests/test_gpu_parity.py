@@ -97,6 +97,41 @@ def test_sliced_pairs_match(pkg, oracle, kind, cells, slices):
     assert_parity(di.dense_state(kind, cells), "f32", oracle, slices=slices)
 
 
+@pytest.mark.parametrize("kind,cells", [("pentagons", 12), ("cubes", 6), ("mixed", 5)])
+def test_generic_kernel_fp32(pkg, oracle, kind, cells):
+    """A DEM_F32 context runs the packed search kernel by default; the generic fused kernel (the one DEM_F64 contexts
+    use) must find the same contributing terms and the same sums up to rounding."""
+    st = di.dense_state(kind, cells)
+    a = assert_parity(st, "f32", oracle, kernel=1)
+    b = assert_parity(st, "f32", oracle, kernel=0)
+    for key in ("active", "degenerate", "parallel", "pairs_evaluated", "terms"):
+        assert a["counters"][key] == b["counters"][key], key
+
+
+@pytest.mark.parametrize("kind,cells,extra", [("cubes", 6, 0.45), ("pentagons", 12, 0.5), ("mixed", 5, 0.5)])
+def test_list_with_skin_compacts_out_of_reach_pairs(pkg, oracle, kind, cells, extra):
+    """A neighbour list built with a skin holds pairs beyond the interaction reach: the pose kernel drops them from
+    the search kernel's work list and writes their zero records; sums and counters must not change."""
+    st = di.dense_state(kind, cells)
+    r0 = assert_parity(st, "f32", oracle)
+    r1 = assert_parity(st, "f32", oracle, r_cut=st["r_cut"] + extra)
+    assert r1["counters"]["pairs_listed"] > r0["counters"]["pairs_listed"]
+    assert r1["counters"]["pairs_evaluated"] == r0["counters"]["pairs_evaluated"] and r1["counters"]["active"] == r0["counters"]["active"]
+    assert_parity(st, "f64", oracle, r_cut=st["r_cut"] + extra)
+
+
+@pytest.mark.parametrize("n", [7, 9])
+def test_faces_with_many_edges(pkg, oracle, n):
+    """Prisms over a heptagon / nonagon: faces whose boundary-edge count has no unrolled sweep (run-time edge loop),
+    mixed with quadrilaterals in one shape, against cubes."""
+    shapes = [di.prism(n, 0.5, 0.9, 0.06), di.cube(0.8, 0.06)]
+    st = di.lattice_state(3, shapes, (5, 5, 5), 1.145, seed=4, jitter=0.01, orient="small", max_angle=0.1,
+                          shape_fractions=(0.6, 0.4))
+    for precision in ("f32", "f64"):
+        r = assert_parity(st, precision, oracle)
+        assert r["counters"]["active"] > 30
+
+
 def test_exactly_aligned_cube_lattice_closed_form(pkg):
     """Aligned unit cubes at spacing 1 + sigma: every face-neighbour pair has 56 terms at r = sigma (PAPER.md:61 as
     corrected by Eq. 1), so U_i = 1/2 * 6 * 56 eps = 168 eps, F_i = tau_i = 0.  Of the 32 edge-edge terms of a pair, the
