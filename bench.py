@@ -284,6 +284,13 @@ def main():
     peak_tf = sm_count * 128 * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
     achieved_tf = flops / (kern_ms_per_eval * 1e-3) / 1e12
     fma_measured = dem.fp32_peak(1 << 15)
+    # DRAM traffic of the dominant kernel per launch: from the committed `ncu --set full` summary of this workload
+    traffic = None
+    prof = os.path.join(ROOT, "profiles", "r01_step_%s_ncu.md" % args.workload)
+    if os.path.exists(prof):
+        for ln in open(prof):
+            if ln.startswith("traffic_bytes_per_launch"):
+                traffic = int(ln.split(":")[1])
 
     # ---- end to end through the host-buffer entry point -------------------------------------------------------------
     h = {kk: t[kk].cpu().pin_memory() for kk in ("pos", "quat", "vel", "angmom")}
@@ -322,8 +329,8 @@ def main():
                               if not args.no_l2_flush else "not flushed (working set < L2)")},
             "feature_pair_evals_per_s": terms * world * (args.steps + 1) / (elapsed_ms * 1e-3),
             "feature_pairs_per_step": terms, "unique_pairs": int(cls.sum()), "active_terms_last_step": cnt["active"],
-            "roofline": {"bound": "alu", "kernel": "k_pair", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                         "frac": achieved_tf / peak_tf, "traffic": None,
+            "roofline": {"bound": "alu", "kernel": "k_pose + k_pair_fast", "achieved": achieved_tf, "peak": peak_tf,
+                         "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": traffic,
                          "peak_source": "%d SM x 128 FP32 lanes x 2 x %.0f MHz (clocks.max.sm, %s)" % (
                              sm_count, float(peaks.get("sm_max_mhz", 1965.0)), peak_kind),
                          "flops_per_launch": flops, "kernel_ms": kern_ms_per_eval, "launches_timed": n_pair_launches,
