@@ -203,6 +203,8 @@ def main():
     ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
     ap.add_argument("--no-l2-flush", action="store_true")
     ap.add_argument("--slices", type=int, default=0, help="lanes per pair in the pair kernel (0 = library heuristic)")
+    ap.add_argument("--pair-kernel", default="auto", choices=["auto", "search", "generic"],
+                    help="search = packed FP32 contact search; generic = fused scalar kernel; auto = library default")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
@@ -237,6 +239,8 @@ def main():
     dem, t = pkg.from_state(st, "f32")
     if args.slices:
         dem.set_slices(args.slices)
+    if args.pair_kernel != "auto":
+        dem.set_pair_kernel({"search": 0, "generic": 1}[args.pair_kernel])
     if not args.no_l2_flush:
         dem.set_l2_flush(L2_FLUSH_BYTES)
     force = torch.empty((n, 4), dtype=torch.float32, device="cuda")
@@ -329,7 +333,7 @@ def main():
                               if not args.no_l2_flush else "not flushed (working set < L2)")},
             "feature_pair_evals_per_s": terms * world * (args.steps + 1) / (elapsed_ms * 1e-3),
             "feature_pairs_per_step": terms, "unique_pairs": int(cls.sum()), "active_terms_last_step": cnt["active"],
-            "roofline": {"bound": "alu", "kernel": "k_pose + k_pair_fast", "achieved": achieved_tf, "peak": peak_tf,
+            "roofline": {"bound": "alu", "kernel": "k_pose + k_pair_fast" if st["dim"] == 3 and args.pair_kernel != "generic" else "k_pair", "achieved": achieved_tf, "peak": peak_tf,
                          "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": traffic,
                          "peak_source": "%d SM x 128 FP32 lanes x 2 x %.0f MHz (clocks.max.sm, %s)" % (
                              sm_count, float(peaks.get("sm_max_mhz", 1965.0)), peak_kind),

@@ -160,12 +160,15 @@ int dem_step_host(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, 
  * lanes to fill the GPU when there are few pairs).  Takes effect at the next neighbour build. */
 int dem_set_slices(dem_ctx* ctx, int slices);
 
-/* Which pair-feature kernel a DEM_F32 context runs.  DEM_KERNEL_SEARCH (default): the packed-FP32 contact search with
+/* Which pair-feature kernel a DEM_F32 context runs.  DEM_KERNEL_SEARCH: the packed-FP32 contact search with
  * cooperative evaluation of the candidate terms.  DEM_KERNEL_GENERIC: the fused scalar kernel
- * that DEM_F64 contexts always use (every Eq. 1 / Eq. 2 term evaluated in place).  Both produce the same contributing
- * terms; sums may differ in rounding order.  Takes effect at the next dem_compute / dem_step. */
+ * that DEM_F64 contexts always use (every Eq. 1 / Eq. 2 term evaluated in place).  DEM_KERNEL_AUTO (default): SEARCH in
+ * 3D, GENERIC in 2D, where a pair has so few terms (2 V E) that the pose records and the candidate queue cost more than
+ * they save (measured on config 3: 64 us against 91 us per evaluation).  Both produce the same contributing terms;
+ * sums may differ in rounding order.  Takes effect at the next dem_compute / dem_step. */
 #define DEM_KERNEL_SEARCH 0
 #define DEM_KERNEL_GENERIC 1
+#define DEM_KERNEL_AUTO 2
 int dem_set_pair_kernel(dem_ctx* ctx, int which);
 
 /* Benchmark hygiene: when bytes > 0, dem_step overwrites a scratch buffer of that size (larger than the 126 MB L2)

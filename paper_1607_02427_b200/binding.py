@@ -118,7 +118,7 @@ class Dem:
         _check(self._ctx, lib().dem_set_slices(self._ctx, C.c_int(slices)))
 
     def set_pair_kernel(self, which):
-        """0 = packed search kernel (default for f32), 1 = generic fused kernel."""
+        """0 = packed search kernel, 1 = generic fused kernel, 2 = auto (default: search in 3D, generic in 2D)."""
         _check(self._ctx, lib().dem_set_pair_kernel(self._ctx, C.c_int(which)))
 
     def set_l2_flush(self, nbytes):

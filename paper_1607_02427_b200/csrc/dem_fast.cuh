@@ -82,11 +82,11 @@ __device__ __forceinline__ unsigned q_entry(int lane, int phase, int outer, int 
 // ---- evaluate: up to 32 queued candidates, one per lane -----------------------------------------------------------------
 // q: this warp's queue (qn entries, the first cnt <= 32 are consumed and the rest moved to the front); sacc: this warp's
 // per-lane accumulators [7][32] = (F.xyz, T.xyz, u) in the owner's body frame; scnt: this warp's counters (active,
-// degenerate, parallel).  R*, t*: the CALLING lane's pose; the evaluating lane fetches its owner's with shuffles.
+// degenerate, parallel).  sp: the warp's staged pose records [6][32] (plane-major, indexed by owner lane); the
+// evaluating lane reads its owner's pose from there.
 // Contributions are added to the owner in queue order, so the result does not depend on scheduling.
 __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* q, float* sacc, unsigned* scnt, int cnt, int qn,
-                                         float R0, float R1, float R2, float R3, float R4, float R5, float R6, float R7,
-                                         float R8, float t0, float t1, float t2) {
+                                         const f4* sp) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const unsigned e = lane < cnt ? q[lane] : DEM_Q_INVALID;
@@ -98,10 +98,11 @@ __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* q, floa
     __syncwarp();
     const int owner = e == DEM_Q_INVALID ? lane : (int)(e >> 27);
     float R[9], t[3];
-    R[0] = __shfl_sync(full, R0, owner); R[1] = __shfl_sync(full, R1, owner); R[2] = __shfl_sync(full, R2, owner);
-    R[3] = __shfl_sync(full, R3, owner); R[4] = __shfl_sync(full, R4, owner); R[5] = __shfl_sync(full, R5, owner);
-    R[6] = __shfl_sync(full, R6, owner); R[7] = __shfl_sync(full, R7, owner); R[8] = __shfl_sync(full, R8, owner);
-    t[0] = __shfl_sync(full, t0, owner); t[1] = __shfl_sync(full, t1, owner); t[2] = __shfl_sync(full, t2, owner);
+    {
+        const f4 p0 = sp[owner], p1 = sp[32 + owner], p2 = sp[64 + owner];
+        R[0] = p0.x; R[1] = p0.y; R[2] = p0.z; R[3] = p0.w; R[4] = p1.x; R[5] = p1.y; R[6] = p1.z; R[7] = p1.w;
+        R[8] = p2.x; t[0] = p2.y; t[1] = p2.z; t[2] = p2.w;
+    }
     PairAcc<float> loc;
     loc.F[0] = loc.F[1] = loc.F[2] = loc.T[0] = loc.T[1] = loc.T[2] = loc.u = 0.f;
     loc.nactive = loc.ndegen = loc.npar = 0u;
@@ -165,39 +166,44 @@ struct WarpCtx {
     unsigned* scnt;
     int qn;    // queued candidates (warp-uniform)
     int lane;
+    const f4* sp;  // staged pose records of the current tile, [6][32]
 };
 
 // ---- queue: append the candidates flagged in mask[] and evaluate while a full warp of them is waiting ------------------
-// mask[tau] bit (n - 1 - i) <=> the packed evaluation of inner feature k0 + i against outer features o0 + 2 tau and
-// o0 + 2 tau + 1 flagged a candidate (either half: both terms are queued, the scalar routine sorts them out).
-template <int T>
-__device__ __forceinline__ void push_and_drain(WarpCtx& w, int phase, const unsigned (&mask)[T], int n, int k0, int o0,
-                                               int o_end, const float* R, const float* t) {
+// mask bit (n - 1 - i) <=> the packed evaluation of inner feature k0 + i flagged a candidate in either half: both
+// terms are queued (the scalar routine sorts them out).  The halves belong to (owner lane, outer feature) = (wa, oa)
+// and (wb, ob); ok_a / ok_b say whether the half holds a real feature (tiles and item lists are padded).
+__device__ __forceinline__ void push_one(WarpCtx& w, int phase, unsigned m, int n, int k0, int wa, int oa, bool ok_a,
+                                         int wb, int ob, bool ok_b) {
     const unsigned full = 0xffffffffu;
     const unsigned lt = (1u << w.lane) - 1u;
-#pragma unroll
-    for (int tau = 0; tau < T; ++tau) {
-        unsigned m = mask[tau];
-        const int oa = o0 + 2 * tau, ob = oa + 1;
-        while (__any_sync(full, m != 0u)) {
-            const bool have = m != 0u;
-            const int bit = 31 - __clz((int)m);
-            const int k = k0 + (n - 1 - bit);
-            if (have) m &= ~(1u << bit);
-            const bool ha = have && oa < o_end, hb = have && ob < o_end;
-            const unsigned ba = __ballot_sync(full, ha), bb = __ballot_sync(full, hb);
-            const int na = __popc(ba);
-            if (ha) w.q[w.qn + __popc(ba & lt)] = q_entry(w.lane, phase, oa, k);
-            if (hb) w.q[w.qn + na + __popc(bb & lt)] = q_entry(w.lane, phase, ob, k);
-            w.qn += na + __popc(bb);
-            __syncwarp();
-            while (w.qn >= 32) {
-                drain_terms(w.fs, w.q, w.sacc, w.scnt, 32, w.qn, R[0], R[1], R[2], R[3], R[4], R[5], R[6], R[7], R[8],
-                            t[0], t[1], t[2]);
-                w.qn -= 32;
-            }
+    while (__any_sync(full, m != 0u)) {
+        const bool have = m != 0u;
+        const int bit = 31 - __clz((int)m);
+        const int k = k0 + (n - 1 - bit);
+        if (have) m &= ~(1u << bit);
+        const bool ha = have && ok_a, hb = have && ok_b;
+        const unsigned ba = __ballot_sync(full, ha), bb = __ballot_sync(full, hb);
+        const int na = __popc(ba);
+        if (ha) w.q[w.qn + __popc(ba & lt)] = q_entry(wa, phase, oa, k);
+        if (hb) w.q[w.qn + na + __popc(bb & lt)] = q_entry(wb, phase, ob, k);
+        w.qn += na + __popc(bb);
+        __syncwarp();
+        while (w.qn >= 32) {
+            drain_terms(w.fs, w.q, w.sacc, w.scnt, 32, w.qn, w.sp);
+            w.qn -= 32;
         }
     }
+}
+
+// tile form: lane-owned outer features o0 + 2 tau and o0 + 2 tau + 1
+template <int T>
+__device__ __forceinline__ void push_and_drain(WarpCtx& w, int phase, const unsigned (&mask)[T], int n, int k0, int o0,
+                                               int o_end) {
+#pragma unroll
+    for (int tau = 0; tau < T; ++tau)
+        push_one(w, phase, mask[tau], n, k0, w.lane, o0 + 2 * tau, o0 + 2 * tau < o_end, w.lane, o0 + 2 * tau + 1,
+                 o0 + 2 * tau + 1 < o_end);
 }
 
 // ---- search: packed nearest-point distances ---------------------------------------------------------------------------
@@ -537,6 +543,8 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
         const bool valid = c < count;
         stage(buf ^ 1, wt + wt_stride);
         asm volatile("cp.async.wait_group 1;" ::: "memory");
+        __syncwarp();  // the cooperative evaluation reads other lanes' staged poses
+        w.sp = spose + buf * 6 * 32;
         float R[9], t[3];
         if (valid) {
             const f4 p0 = spose[(buf * 6 + 0) * 32 + lane], p1 = spose[(buf * 6 + 1) * 32 + lane],
@@ -593,7 +601,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
                         unsigned any = 0u;
 #pragma unroll
                         for (int tau = 0; tau < TE; ++tau) any |= mask[tau];
-                        if (__any_sync(full, any != 0u)) push_and_drain<TE>(w, PH_EE, mask, k1 - k0, k0, l0, le, R, t);
+                        if (__any_sync(full, any != 0u)) push_and_drain<TE>(w, PH_EE, mask, k1 - k0, k0, l0, le);
                     }
                 }
                 // (2) third sum of Eq. 1: vertices of j (outer, packed, i's frame) against faces of i
@@ -618,7 +626,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
                         unsigned any = 0u;
 #pragma unroll
                         for (int tau = 0; tau < TV; ++tau) any |= mask[tau];
-                        if (__any_sync(full, any != 0u)) push_and_drain<TV>(w, PH_VF_OWN, mask, f1 - f0, f0, o0, on, R, t);
+                        if (__any_sync(full, any != 0u)) push_and_drain<TV>(w, PH_VF_OWN, mask, f1 - f0, f0, o0, on);
                     }
                 }
                 // (3) second sum of Eq. 1: vertices of i (outer, packed, j's frame) against faces of j
@@ -643,7 +651,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
                         unsigned any = 0u;
 #pragma unroll
                         for (int tau = 0; tau < TV; ++tau) any |= mask[tau];
-                        if (__any_sync(full, any != 0u)) push_and_drain<TV>(w, PH_VF_OTHER, mask, f1 - f0, f0, o0, on, R, t);
+                        if (__any_sync(full, any != 0u)) push_and_drain<TV>(w, PH_VF_OTHER, mask, f1 - f0, f0, o0, on);
                     }
                 }
             } else {
@@ -689,14 +697,13 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
 #pragma unroll
                             for (int tau = 0; tau < TV; ++tau) any |= mask[tau];
                             if (__any_sync(full, any != 0u))
-                                push_and_drain<TV>(w, side == 0 ? PH_VE_OWN : PH_VE_OTHER, mask, k1 - k0, k0, o0, on, R, t);
+                                push_and_drain<TV>(w, side == 0 ? PH_VE_OWN : PH_VE_OTHER, mask, k1 - k0, k0, o0, on);
                         }
                     }
                 }
             }
             if (w.qn > 0) {
-                drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, R[0], R[1], R[2], R[3], R[4], R[5], R[6], R[7], R[8], t[0],
-                            t[1], t[2]);
+                drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp);
                 w.qn = 0;
             }
             float F[3], T[3];

@@ -596,6 +596,7 @@ int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda
     c->eps = epsilon;
     c->prec = precision;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
+    c->generic_kernel = dim == 2;  // DEM_KERNEL_AUTO
     memset(&c->ct, 0, sizeof c->ct);
     memset(&c->mt, 0, sizeof c->mt);
     *out = c;
@@ -636,8 +637,9 @@ int dem_set_slices(dem_ctx* ctx, int slices) {
 }
 
 int dem_set_pair_kernel(dem_ctx* ctx, int which) {
-    if (!ctx || (which != DEM_KERNEL_SEARCH && which != DEM_KERNEL_GENERIC)) return fail(ctx, DEM_EINVAL, "unknown pair kernel");
-    ctx->generic_kernel = which == DEM_KERNEL_GENERIC;
+    if (!ctx || (which != DEM_KERNEL_SEARCH && which != DEM_KERNEL_GENERIC && which != DEM_KERNEL_AUTO))
+        return fail(ctx, DEM_EINVAL, "unknown pair kernel");
+    ctx->generic_kernel = which == DEM_KERNEL_GENERIC || (which == DEM_KERNEL_AUTO && ctx->dim == 2);
     return DEM_OK;
 }
 

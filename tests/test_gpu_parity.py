@@ -97,10 +97,10 @@ def test_sliced_pairs_match(pkg, oracle, kind, cells, slices):
     assert_parity(di.dense_state(kind, cells), "f32", oracle, slices=slices)
 
 
-@pytest.mark.parametrize("kind,cells", [("pentagons", 12), ("cubes", 6), ("mixed", 5)])
+@pytest.mark.parametrize("kind,cells", [("squares", 12), ("pentagons", 12), ("cubes", 6), ("mixed", 5)])
 def test_generic_kernel_fp32(pkg, oracle, kind, cells):
-    """A DEM_F32 context runs the packed search kernel by default; the generic fused kernel (the one DEM_F64 contexts
-    use) must find the same contributing terms and the same sums up to rounding."""
+    """A DEM_F32 context runs the packed search kernel (default in 3D) or the generic fused kernel (default in 2D,
+    always in DEM_F64 contexts); both must find the same contributing terms and the same sums up to rounding."""
     st = di.dense_state(kind, cells)
     a = assert_parity(st, "f32", oracle, kernel=1)
     b = assert_parity(st, "f32", oracle, kernel=0)
@@ -113,8 +113,8 @@ def test_list_with_skin_compacts_out_of_reach_pairs(pkg, oracle, kind, cells, ex
     """A neighbour list built with a skin holds pairs beyond the interaction reach: the pose kernel drops them from
     the search kernel's work list and writes their zero records; sums and counters must not change."""
     st = di.dense_state(kind, cells)
-    r0 = assert_parity(st, "f32", oracle)
-    r1 = assert_parity(st, "f32", oracle, r_cut=st["r_cut"] + extra)
+    r0 = assert_parity(st, "f32", oracle, kernel=0)
+    r1 = assert_parity(st, "f32", oracle, r_cut=st["r_cut"] + extra, kernel=0)
     assert r1["counters"]["pairs_listed"] > r0["counters"]["pairs_listed"]
     assert r1["counters"]["pairs_evaluated"] == r0["counters"]["pairs_evaluated"] and r1["counters"]["active"] == r0["counters"]["active"]
     assert_parity(st, "f64", oracle, r_cut=st["r_cut"] + extra)
