@@ -203,6 +203,7 @@ def main():
     ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
     ap.add_argument("--no-l2-flush", action="store_true")
     ap.add_argument("--slices", type=int, default=0, help="lanes per pair in the pair kernel (0 = library heuristic)")
+    ap.add_argument("--no-cull", action="store_true", help="sweep every Eq. 1 term (no exact per-feature culling)")
     ap.add_argument("--pair-kernel", default="auto", choices=["auto", "search", "generic"],
                     help="search = packed FP32 contact search; generic = fused scalar kernel; auto = library default")
     ap.add_argument("--e2e-steps", type=int, default=10)
@@ -239,6 +240,8 @@ def main():
     dem, t = pkg.from_state(st, "f32")
     if args.slices:
         dem.set_slices(args.slices)
+    if args.no_cull:
+        dem.set_culling(False)
     if args.pair_kernel != "auto":
         dem.set_pair_kernel({"search": 0, "generic": 1}[args.pair_kernel])
     if not args.no_l2_flush:

@@ -124,9 +124,11 @@ int dem_compute(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* 
                 void* torque, void* virial6);
 
 /* Counters of the last dem_compute (synchronises): out[0] unique particle pairs evaluated, out[1] Eq. 1/2 terms
- * evaluated (polygon faces, each unique pair once), out[2] terms inside the WCA cutoff, out[3] degenerate terms
- * skipped, out[4] terms that took the parallel-edge branch, out[5] unique pairs in the work list. HOST int64[6]. */
-int dem_get_counters(dem_ctx* ctx, int64_t out[6]);
+ * of those pairs (polygon faces, each unique pair once), out[2] terms inside the WCA cutoff, out[3] degenerate terms
+ * skipped, out[4] terms that took the parallel-edge branch, out[5] unique pairs in the work list, out[6] terms whose
+ * nearest-point search was actually executed (= out[1] unless exact culling proved features out of reach: see
+ * dem_set_culling). HOST int64[7]. */
+int dem_get_counters(dem_ctx* ctx, int64_t out[7]);
 
 /*
  * nsteps of velocity-Verlet NVE with quaternion rotation (reading R15): half-kick v and L; drift x
@@ -170,6 +172,14 @@ int dem_set_slices(dem_ctx* ctx, int slices);
 #define DEM_KERNEL_GENERIC 1
 #define DEM_KERNEL_AUTO 2
 int dem_set_pair_kernel(dem_ctx* ctx, int which);
+
+/* Exact per-feature culling in the packed search kernel (3D, DEM_F32; default ON).  Every feature of a particle lies
+ * within its circumradius R of its centre, so a feature of the other particle whose distance from that centre is at
+ * least R + (search cutoff) cannot be within the WCA cutoff of ANY of its features: the search skips it, with
+ * identical results (same contributing terms, same arithmetic; PAPER.md:129 names such shape-local culling as the next
+ * step).  0 = sweep every Eq. 1 term (the paper's method as stated).  Takes effect at the next
+ * dem_compute / dem_step. */
+int dem_set_culling(dem_ctx* ctx, int enabled);
 
 /* Benchmark hygiene: when bytes > 0, dem_step overwrites a scratch buffer of that size (larger than the 126 MB L2)
  * before every time step, so that no step finds its inputs cached by the previous one.  0 (default) = off. */

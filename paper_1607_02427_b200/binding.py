@@ -21,7 +21,7 @@ STATUS_NAMES = {0: "DEM_OK", -1: "DEM_EINVAL", -2: "DEM_ENOMEM", -3: "DEM_ECUDA"
 # every symbol include/dem.h declares (tests check that the built library exports all of them)
 EXPORTS = ["dem_create", "dem_destroy", "dem_last_error", "dem_set_eps_par", "dem_create_shape", "dem_build_neighbors",
            "dem_get_neighbors", "dem_copy_neighbors", "dem_compute", "dem_get_counters", "dem_step", "dem_energy",
-           "dem_compute_host", "dem_step_host", "dem_set_slices", "dem_set_pair_kernel", "dem_set_l2_flush", "dem_set_timing", "dem_kernel_time",
+           "dem_compute_host", "dem_step_host", "dem_set_slices", "dem_set_pair_kernel", "dem_set_culling", "dem_set_l2_flush", "dem_set_timing", "dem_kernel_time",
            "dem_launch_count", "dem_fp32_peak", "dem_version"]
 
 _lib = None
@@ -121,6 +121,9 @@ class Dem:
         """0 = packed search kernel, 1 = generic fused kernel, 2 = auto (default: search in 3D, generic in 2D)."""
         _check(self._ctx, lib().dem_set_pair_kernel(self._ctx, C.c_int(which)))
 
+    def set_culling(self, enabled):
+        _check(self._ctx, lib().dem_set_culling(self._ctx, C.c_int(1 if enabled else 0)))
+
     def set_l2_flush(self, nbytes):
         _check(self._ctx, lib().dem_set_l2_flush(self._ctx, C.c_int64(nbytes)))
 
@@ -191,10 +194,10 @@ class Dem:
         return f, t, w
 
     def get_counters(self):
-        out = (C.c_int64 * 6)()
+        out = (C.c_int64 * 7)()
         _check(self._ctx, lib().dem_get_counters(self._ctx, out))
         return dict(pairs_evaluated=out[0], terms=out[1], active=out[2], degenerate=out[3], parallel=out[4],
-                    pairs_listed=out[5])
+                    pairs_listed=out[5], terms_swept=out[6])
 
     # ---- dem_step / dem_energy -----------------------------------------------------------------------------------------
     def step(self, pos, quat, vel, angmom, shape_id, box, dt, nsteps, skin, force=None, torque=None):

@@ -383,9 +383,9 @@ __device__ __forceinline__ void sweep_faces(const ShapeView<float>& S, const Sha
 
 // ---- a3: relative pose of every pair of a class, compacted -----------------------------------------------------------
 // One thread per unique pair: minimum-image separation d, exact reach test (R10), relative pose R = R_i^T R_j,
-// t = R_i^T d and R_i in FP64, rounded once to float.  Pairs inside the reach are appended to a
-// compact work list (warp-aggregated atomic: their order varies from run to run, the result of a pair does not depend
-// on it); pairs beyond it get their zero result records here and never reach the search kernel, so its warps carry 32
+// t = R_i^T d and R_i in FP64, rounded once to float.  Pairs inside the reach are compacted, in
+// pair order (single-pass look-back scan: the list is the same from run to run), into the class's work list; pairs
+// beyond it get their zero result records here and never reach the search kernel, so its warps carry 32
 // live pairs each.  Pose record, plane-major for coalesced loads: [6][npairs] float4 =
 // (R0 R1 R2 R3) (R4 R5 R6 R7) (R8 t0 t1 t2) (M0 M1 M2 M3) (M4 M5 M6 M7) (M8 dx dy dz); pidx[c] = the pair's index.
 struct PoseArgs {
@@ -397,58 +397,97 @@ struct PoseArgs {
     double reach2;
     f4* pose;
     int* pidx;
-    int* count;  // valid pairs of this class (zeroed before the launch)
+    int* count;  // valid pairs of this class (written by the last block)
+    int* ticket;  // block numbering (zeroed before the launch)
+    unsigned long long* scan_state;  // one word per block (look-back scan), never reset
+    unsigned epoch;                  // launch number, 1 .. 2^30 - 1
     f4* rec;
 };
 
 #define DEM_POSE_THREADS 256
 template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THREADS) k_pose(const PoseArgs a) {
-    __shared__ int wcount[DEM_POSE_THREADS / 32], wbase[DEM_POSE_THREADS / 32];
+    __shared__ int wcount[DEM_POSE_THREADS / 32], wbase[DEM_POSE_THREADS / 32], s_bid, s_prefix;
     const unsigned full = 0xffffffffu;
-    const int p = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // blocks take their number from a ticket, so that every block's predecessors in the scan have already started
+    if (threadIdx.x == 0) s_bid = atomicAdd(a.ticket, 1);
+    __syncthreads();
+    const int bid = s_bid;
+    const int p = bid * blockDim.x + threadIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     bool valid = false;
-    float Mi[9], R[9], t[3];
     double d[3] = {0.0, 0.0, 0.0};
+    d4 qi, qj;
+    qi.x = qj.x = 1.0; qi.y = qi.z = qi.w = qj.y = qj.z = qj.w = 0.0;
     if (p < a.npairs) {
         const int2 ij = a.pairs[p];
         const d4 xi = load4d(static_cast<const PosT*>(a.pos), ij.x), xj = load4d(static_cast<const PosT*>(a.pos), ij.y);
-        const d4 qi = load4d(static_cast<const PosT*>(a.quat), ij.x), qj = load4d(static_cast<const PosT*>(a.quat), ij.y);
+        qi = load4d(static_cast<const PosT*>(a.quat), ij.x);
+        qj = load4d(static_cast<const PosT*>(a.quat), ij.y);
         // minimum image (any nearest image serves here: the bit-exact predicate R13 belongs to the neighbour list)
         d[0] = xj.x - xi.x; d[1] = xj.y - xi.y; d[2] = DIM == 3 ? xj.z - xi.z : 0.0;
         d[0] -= a.box.L[0] * rint(d[0] * a.box.invL[0]);
         d[1] -= a.box.L[1] * rint(d[1] * a.box.invL[1]);
         if (DIM == 3) d[2] -= a.box.L[2] * rint(d[2] * a.box.invL[2]);
         valid = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] < a.reach2;
-        if (valid) {
-            const double qa[4] = {qi.x, qi.y, qi.z, qi.w}, qb[4] = {qj.x, qj.y, qj.z, qj.w};
-            pair_pose<float>(qa, qb, d, Mi, R, t);
-        } else {
-            f4 r0, r1, r2;
-            r0.x = r0.y = r0.z = r0.w = 0.f;
-            r1.x = r1.y = r1.z = 0.f; r1.w = (float)d[0];
-            r2.x = (float)d[1]; r2.y = (float)d[2]; r2.z = r2.w = 0.f;
-            for (int sl = 0; sl < a.slices; ++sl) {
-                f4* rec = a.rec + DEM_REC * ((size_t)p * a.slices + sl);
-                rec[0] = r0; rec[1] = r1; rec[2] = r2;
-            }
-        }
     }
-    // compaction: one atomic per block (same-address atomics serialise in L2: one per warp costs as much as the poses)
+    // Ordered compaction (pair order is kept, so the work list and every sum downstream are the same from run to run):
+    // single-pass scan over the blocks with decoupled look-back.  Each block publishes (epoch, kind, value) in one
+    // 64-bit word: kind 1 = its own count (as early as possible), kind 2 = its inclusive prefix; warp 0 adds up the
+    // predecessors' words, 32 at a time, back to the nearest inclusive one.  The epoch makes the words of earlier
+    // launches invisible (no reset).
     const unsigned m = __ballot_sync(full, valid);
     if (lane == 0) wcount[warp] = __popc(m);
     __syncthreads();
-    if (threadIdx.x == 0) {
-        int tot = 0;
-        for (int k = 0; k < DEM_POSE_THREADS / 32; ++k) {
-            wbase[k] = tot;
-            tot += wcount[k];
+    int tot = 0;
+#pragma unroll
+    for (int k = 0; k < DEM_POSE_THREADS / 32; ++k) tot += wcount[k];
+    const unsigned long long tag = (unsigned long long)a.epoch << 34;
+    volatile unsigned long long* st = a.scan_state;
+    if (threadIdx.x == 0 && bid > 0) {
+        st[bid] = tag | (1ull << 32) | (unsigned)tot;
+        __threadfence();
+    }
+    // the pose itself (FP64), while the predecessors publish
+    float Mi[9], R[9], t[3];
+    if (valid) {
+        const double qa[4] = {qi.x, qi.y, qi.z, qi.w}, qb[4] = {qj.x, qj.y, qj.z, qj.w};
+        pair_pose<float>(qa, qb, d, Mi, R, t);
+    } else if (p < a.npairs) {
+        f4 r0, r1, r2;
+        r0.x = r0.y = r0.z = r0.w = 0.f;
+        r1.x = r1.y = r1.z = 0.f; r1.w = (float)d[0];
+        r2.x = (float)d[1]; r2.y = (float)d[2]; r2.z = r2.w = 0.f;
+        for (int sl = 0; sl < a.slices; ++sl) {
+            f4* rec = a.rec + DEM_REC * ((size_t)p * a.slices + sl);
+            rec[0] = r0; rec[1] = r1; rec[2] = r2;
         }
-        const int b = tot ? atomicAdd(a.count, tot) : 0;
-        for (int k = 0; k < DEM_POSE_THREADS / 32; ++k) wbase[k] += b;
+    }
+    if (warp == 0) {
+        int prefix = 0;
+        for (int j0 = bid - 1; j0 >= 0; j0 -= 32) {
+            const int j = j0 - lane;
+            unsigned long long v = 0ull;
+            if (j >= 0) {
+                do {
+                    v = st[j];
+                } while ((v >> 34) != a.epoch || ((v >> 32) & 3ull) == 0ull);
+            }
+            const unsigned incl = __ballot_sync(full, j >= 0 && ((v >> 32) & 3ull) == 2ull);
+            const int stop = incl ? __ffs(incl) - 1 : 31;  // nearest inclusive prefix among these 32 (lane order = backwards)
+            prefix += __reduce_add_sync(full, (j >= 0 && lane <= stop) ? (int)(unsigned)v : 0);
+            if (incl) break;
+        }
+        if (lane == 0) {
+            st[bid] = tag | (2ull << 32) | (unsigned)(prefix + tot);
+            __threadfence();
+            if (bid == (int)gridDim.x - 1) *a.count = prefix + tot;
+            s_prefix = prefix;
+        }
     }
     __syncthreads();
     if (valid) {
-        const int c = wbase[warp] + __popc(m & ((1u << lane) - 1u));
+        int wb = s_prefix;
+        for (int k = 0; k < warp; ++k) wb += wcount[k];
+        const int c = wb + __popc(m & ((1u << lane) - 1u));
         const size_t n = (size_t)a.npairs;
         f4 v;
         v.x = R[0]; v.y = R[1]; v.z = R[2]; v.w = R[3]; a.pose[c] = v;
@@ -741,5 +780,244 @@ static inline size_t fast_smem_header() {
     return 256 + sizeof(unsigned) * 4 * DEM_QCAP + sizeof(float) * 4 * 7 * 32 + sizeof(unsigned) * 16 +
            sizeof(f4) * 4 * 2 * 6 * 32 + sizeof(int) * 4 * 2 * 32;
 }
+
+// ---- the kernel with exact per-feature culling (3D) ----------------------------------------------------------------------
+// Every feature of particle i lies inside the ball of radius R_i (its circumradius) around its centre, so an outer
+// feature of j whose distance from that centre is at least R_i + rc_search cannot be a candidate against ANY feature
+// of i: the whole inner sweep for it can be skipped, exactly (PAPER.md:129 names such shape-local culling as the next
+// step).  The test costs ~15 instructions per outer feature and needs no rotation (|R v + t| = |v + R^T t|).
+// Because lanes disagree on which of their outer features survive, the survivors of the 32 pairs of a tile are
+// compacted into a warp-private list of (owner lane, outer feature) items, and the sweeps run over ITEMS, two per lane
+// in the halves of the packed registers (the halves may belong to different pairs: inner features are shared by the
+// whole class, poses come from the staged records).  Candidates and their evaluation are as in k_pair_fast.
+#define DEM_IQCAP 512
+
+struct CullCtx {
+    unsigned* iq;    // item list of the warp
+    int iqn;         // items queued (warp-uniform)
+    unsigned swept;  // terms this lane swept (for the flop count)
+};
+
+__device__ __forceinline__ void load_pose(const f4* sp, int owner, float* R, float* t) {
+    const f4 p0 = sp[owner], p1 = sp[32 + owner], p2 = sp[64 + owner];
+    R[0] = p0.x; R[1] = p0.y; R[2] = p0.z; R[3] = p0.w; R[4] = p1.x; R[5] = p1.y; R[6] = p1.z; R[7] = p1.w;
+    R[8] = p2.x; t[0] = p2.y; t[1] = p2.z; t[2] = p2.w;
+}
+
+// sweep the queued items of one phase, 64 per pass (two per lane)
+template <int PHASE>
+__device__ __forceinline__ void sweep_items(WarpCtx& w, CullCtx& cc, const ShapeView<float>& A, const ShapeView<float>& B,
+                                            const ShapeDev& sda, const ShapeDev& sdb, float nrc2) {
+    const unsigned full = 0xffffffffu;
+    __syncwarp();
+    for (int base = 0; base < cc.iqn; base += 64) {
+        const int ia = base + w.lane, ib = ia + 32;
+        const bool ok_a = ia < cc.iqn, ok_b = ib < cc.iqn;
+        const unsigned ea = ok_a ? cc.iq[ia] : 0u, eb = ok_b ? cc.iq[ib] : ea;
+        const int wa = (int)(ea >> 16), oa = (int)(ea & 0xffffu), wb = (int)(eb >> 16), ob = (int)(eb & 0xffffu);
+        float Ra[9], ta[3], Rb[9], tb[3];
+        load_pose(w.sp, wa, Ra, ta);
+        load_pose(w.sp, wb, Rb, tb);
+        if (!ok_a) ta[0] = tb[0] = 1.0e4f;  // idle lane: a far-away dummy keeps the warp converged
+        if (PHASE == PH_EE) {
+            const f4 a0 = B.OE[2 * oa], a1 = B.OE[2 * oa + 1], b0 = B.OE[2 * ob], b1 = B.OE[2 * ob + 1];
+            float pa[3], pb[3];
+            vertex_to_i<float>(a0.x, a0.y, a0.z, Ra, ta, pa);
+            vertex_to_i<float>(b0.x, b0.y, b0.z, Rb, tb, pb);
+            const u64 np2x = pk(-pa[0], -pb[0]), np2y = pk(-pa[1], -pb[1]), np2z = pk(-pa[2], -pb[2]);
+            const u64 d2x = pk(Ra[0] * a1.x + Ra[1] * a1.y + Ra[2] * a1.z, Rb[0] * b1.x + Rb[1] * b1.y + Rb[2] * b1.z);
+            const u64 d2y = pk(Ra[3] * a1.x + Ra[4] * a1.y + Ra[5] * a1.z, Rb[3] * b1.x + Rb[4] * b1.y + Rb[5] * b1.z);
+            const u64 d2z = pk(Ra[6] * a1.x + Ra[7] * a1.y + Ra[8] * a1.z, Rb[6] * b1.x + Rb[7] * b1.y + Rb[8] * b1.z);
+            const u64 g = fma2(d2z, np2z, fma2(d2y, np2y, mul2(d2x, np2x)));
+            for (int k0 = 0; k0 < A.ne; k0 += 32) {
+                const int k1 = min(k0 + 32, A.ne);
+                unsigned mask = 0u;
+                for (int k = k0; k < k1; ++k)
+                    mask = push_sign(mask, ee_eval(A.E[2 * k], A.E[2 * k + 1], np2x, np2y, np2z, d2x, d2y, d2z, g, a0.w,
+                                                   b0.w, nrc2));
+                if (__any_sync(full, mask != 0u)) push_one(w, PHASE, mask, k1 - k0, k0, wa, oa, ok_a, wb, ob, ok_b);
+            }
+            cc.swept += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)A.ne;
+        } else {
+            const ShapeView<float>& In = PHASE == PH_VF_OWN ? A : B;
+            const ShapeView<float>& Out = PHASE == PH_VF_OWN ? B : A;
+            const ShapeDev& sd = PHASE == PH_VF_OWN ? sda : sdb;
+            const f4 va = Out.V[oa], vb = Out.V[ob];
+            float pa[3], pb[3];
+            if (PHASE == PH_VF_OWN) {
+                vertex_to_i<float>(va.x, va.y, va.z, Ra, ta, pa);
+                vertex_to_i<float>(vb.x, vb.y, vb.z, Rb, tb, pb);
+            } else {
+                vertex_to_j<float>(va.x, va.y, va.z, Ra, ta, pa);
+                vertex_to_j<float>(vb.x, vb.y, vb.z, Rb, tb, pb);
+            }
+            u64 px[1] = {pk(pa[0], pb[0])}, py[1] = {pk(pa[1], pb[1])}, pz[1] = {pk(pa[2], pb[2])};
+            for (int f0 = 0; f0 < In.nf; f0 += 32) {
+                const int f1 = min(f0 + 32, In.nf);
+                unsigned mask[1] = {0u};
+                sweep_faces<1>(In, sd, f0, f1, px, py, pz, nrc2, mask);
+                if (__any_sync(full, mask[0] != 0u)) push_one(w, PHASE, mask[0], f1 - f0, f0, wa, oa, ok_a, wb, ob, ok_b);
+            }
+            cc.swept += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)In.nf;
+        }
+    }
+    cc.iqn = 0;
+}
+
+// append the lanes' surviving outer feature o to the item list (ballot-ranked: order fixed by the data)
+__device__ __forceinline__ void push_item(const WarpCtx& w, CullCtx& cc, bool survive, int o) {
+    const unsigned m = __ballot_sync(0xffffffffu, survive);
+    if (survive) cc.iq[cc.iqn + __popc(m & ((1u << w.lane) - 1u))] = ((unsigned)w.lane << 16) | (unsigned)o;
+    cc.iqn += __popc(m);
+}
+
+template <typename PosT, int MINB>
+__global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    FastShared* fs = reinterpret_cast<FastShared*>(smem_raw);
+    unsigned* queue = reinterpret_cast<unsigned*>(smem_raw + 256);  // 4 warps x DEM_QCAP
+    float* sacc_all = reinterpret_cast<float*>(queue + 4 * DEM_QCAP);  // 4 warps x 7 x 32
+    unsigned* scnt_all = reinterpret_cast<unsigned*>(sacc_all + 4 * 7 * 32);  // 4 warps x 4
+    f4* stage_pose = reinterpret_cast<f4*>(scnt_all + 16);                 // 4 warps x [2][6][32] float4
+    int* stage_pidx = reinterpret_cast<int*>(stage_pose + 4 * 2 * 6 * 32);  // 4 warps x [2][32]
+    unsigned* items = reinterpret_cast<unsigned*>(stage_pidx + 4 * 2 * 32);  // 4 warps x DEM_IQCAP
+    f4* sm = reinterpret_cast<f4*>(items + 4 * DEM_IQCAP);
+    const bool same = a.sa.off == a.sb.off;
+    for (int k = threadIdx.x; k < a.sa.len; k += blockDim.x) sm[k] = a.table[a.sa.off + k];
+    if (!same)
+        for (int k = threadIdx.x; k < a.sb.len; k += blockDim.x) sm[a.sa.len + k] = a.table[a.sb.off + k];
+    ShapeView<float> A, B;
+    A.nv = a.sa.nv; A.ne = a.sa.ne; A.nf = a.sa.nf;
+    A.V = sm; A.E = A.V + A.nv; A.F = A.E + 2 * A.ne; A.FE = A.F + 4 * A.nf; A.OE = A.FE + 2 * a.sa.nfe;
+    B.nv = a.sb.nv; B.ne = a.sb.ne; B.nf = a.sb.nf;
+    B.V = same ? sm : sm + a.sa.len; B.E = B.V + B.nv; B.F = B.E + 2 * B.ne; B.FE = B.F + 4 * B.nf;
+    B.OE = B.FE + 2 * a.sb.nfe;
+    if (threadIdx.x == 0) {
+        fs->A = A;
+        fs->B = B;
+        fs->pc = a.pc;
+    }
+    if (threadIdx.x < 16) scnt_all[threadIdx.x] = 0u;
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpCtx w;
+    w.fs = fs;
+    w.q = queue + warp * DEM_QCAP;
+    w.sacc = sacc_all + warp * 7 * 32;
+    w.scnt = scnt_all + warp * 4;
+    w.qn = 0;
+    w.lane = lane;
+    CullCtx cc;
+    cc.iq = items + warp * DEM_IQCAP;
+    cc.iqn = 0;
+    cc.swept = 0u;
+    const float nrc2 = -a.rc2_search;
+    const int count = *a.count;
+    const int np_pad = (count + 31) & ~31;
+    const long long n_wtiles = (long long)(np_pad >> 5) * a.slices;
+    const size_t plane = (size_t)a.npairs;
+    const long long wt_stride = (long long)gridDim.x * 4;
+    f4* spose = stage_pose + warp * (2 * 6 * 32);
+    int* spidx = stage_pidx + warp * (2 * 32);
+    auto stage = [&](int buf, long long wt_) {
+        if (wt_ < n_wtiles) {
+            const int c_ = (int)((wt_ * 32 + lane) % np_pad);
+            if (c_ < count) {
+#pragma unroll
+                for (int k = 0; k < 6; ++k)
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
+                                     spose + (buf * 6 + k) * 32 + lane)), "l"(a.pose + k * plane + c_));
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(
+                                 spidx + buf * 32 + lane)), "l"(a.pidx + c_));
+            }
+        }
+        asm volatile("cp.async.commit_group;");
+    };
+    int buf = 0;
+    stage(0, (long long)blockIdx.x * 4 + warp);
+    for (long long wt = (long long)blockIdx.x * 4 + warp; wt < n_wtiles; wt += wt_stride, buf ^= 1) {
+        const long long item = wt * 32 + lane;
+        const int slice = (int)(item / np_pad), c = (int)(item - (long long)slice * np_pad);
+        const bool valid = c < count;
+        stage(buf ^ 1, wt + wt_stride);
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+        __syncwarp();
+        w.sp = spose + buf * 6 * 32;
+        float R[9], t[3], tp[3] = {1.0e4f, 1.0e4f, 1.0e4f};
+        if (valid) {
+            load_pose(w.sp, lane, R, t);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) tp[k] = R[k] * t[0] + R[3 + k] * t[1] + R[6 + k] * t[2];  // R^T t
+        } else {
+            t[0] = t[1] = t[2] = 1.0e4f;
+        }
+#pragma unroll
+        for (int k = 0; k < 7; ++k) w.sacc[k * 32 + lane] = 0.f;
+        const int ob = (int)((long long)slice * a.n_outer / a.slices);
+        const int oe = (int)((long long)(slice + 1) * a.n_outer / a.slices);
+        const int oE = B.ne, oV = B.ne + B.nv;
+        // (1) edges of j whose distance from i's centre is below R_i + rc_search: in j's frame the centre of i is -R^T t
+        for (int l = ob, le = min(oe, oE); l < le; ++l) {
+            if (cc.iqn + 32 > DEM_IQCAP) sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
+            const f4 a0 = B.OE[2 * l], a1 = B.OE[2 * l + 1];
+            const float qx = a0.x + tp[0], qy = a0.y + tp[1], qz = a0.z + tp[2];
+            const float s = fminf(fmaxf(-(qx * a1.x + qy * a1.y + qz * a1.z), 0.f), a0.w);
+            const float cx = qx + s * a1.x, cy = qy + s * a1.y, cz = qz + s * a1.z;
+            push_item(w, cc, valid && cx * cx + cy * cy + cz * cz < a.cull_a2, l);
+        }
+        sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
+        // (2) vertices of j near i
+        for (int o = max(ob, oE) - oE, on = min(oe, oV) - oE; o < on; ++o) {
+            if (cc.iqn + 32 > DEM_IQCAP) sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
+            const f4 v = B.V[o];
+            const float qx = v.x + tp[0], qy = v.y + tp[1], qz = v.z + tp[2];
+            push_item(w, cc, valid && qx * qx + qy * qy + qz * qz < a.cull_a2, o);
+        }
+        sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
+        // (3) vertices of i near j: |R^T (v - t)| = |v - t|
+        for (int o = max(ob, oV) - oV, on = min(oe, oV + A.nv) - oV; o < on; ++o) {
+            if (cc.iqn + 32 > DEM_IQCAP) sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
+            const f4 v = A.V[o];
+            const float qx = v.x - t[0], qy = v.y - t[1], qz = v.z - t[2];
+            push_item(w, cc, valid && qx * qx + qy * qy + qz * qz < a.cull_b2, o);
+        }
+        sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
+        if (w.qn > 0) {
+            drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp);
+            w.qn = 0;
+        }
+        if (valid) {
+            float F[3], T[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                F[k] = w.sacc[k * 32 + lane];
+                T[k] = w.sacc[(3 + k) * 32 + lane];
+            }
+            const f4 p3 = spose[(buf * 6 + 3) * 32 + lane], p4 = spose[(buf * 6 + 4) * 32 + lane],
+                     p5 = spose[(buf * 6 + 5) * 32 + lane];
+            const float Mi[9] = {p3.x, p3.y, p3.z, p3.w, p4.x, p4.y, p4.z, p4.w, p5.x};
+            float out[10];
+            pair_finish<float>(Mi, t, F, T, w.sacc[6 * 32 + lane], out);
+            f4* rec = a.rec + DEM_REC * ((size_t)spidx[buf * 32 + lane] * a.slices + slice);
+            f4 r0, r1, r2;
+            r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
+            r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = p5.y;
+            r2.x = p5.z; r2.y = p5.w; r2.z = r2.w = 0.f;
+            rec[0] = r0; rec[1] = r1; rec[2] = r2;
+        }
+        __syncwarp();  // the next tile's stage() overwrites the other buffer only; sacc is re-zeroed by its own lane
+    }
+    const unsigned swept = __reduce_add_sync(0xffffffffu, cc.swept);
+    if (lane == 0) {
+        if (w.scnt[0]) atomicAdd(a.counters + 1, (unsigned long long)w.scnt[0]);
+        if (w.scnt[1]) atomicAdd(a.counters + 2, (unsigned long long)w.scnt[1]);
+        if (w.scnt[2]) atomicAdd(a.counters + 3, (unsigned long long)w.scnt[2]);
+        if (swept) atomicAdd(a.counters + 4, (unsigned long long)swept);
+    }
+}
+
+// bytes of dynamic shared memory k_pair_cull needs in front of the staged tables
+static inline size_t cull_smem_header() { return fast_smem_header() + sizeof(unsigned) * 4 * DEM_IQCAP; }
 
 }  // namespace dem

@@ -285,6 +285,7 @@ template <typename real> struct PairArgs {
     double reach2;        // (R_a + R_b + 2^(1/6) sigma)^2 : beyond it no term can be inside the cutoff (exact, R10)
     PairConst<real> pc;
     real rc2_search;      // FP32 search kernel: squared candidate cutoff (WCA cutoff + slack, dem_fast.cuh)
+    real cull_a2, cull_b2;  // culling kernel: (R_first + rc_search)^2, (R_second + rc_search)^2 (circumradii)
     const f4* pose;       // FP32 search kernel: this class's compacted pose records, pair indices and their number
     const int* pidx;      //   (written by k_pose)
     const int* count;

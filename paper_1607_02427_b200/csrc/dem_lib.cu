@@ -58,12 +58,14 @@ struct dem_ctx {
     double box[3] = {0, 0, 0}, r_cut = 0;
     GridDev grid;
     DevBuf cell_of, rank, cell_start, order, xs, counts, list, slot, scratch_scan, pcnt, pairs, rec, flags, counters;
-    DevBuf pose, pidx;  // FP32 search kernel: compacted pose records per class (k_pose)
+    DevBuf pose, pidx, scan_state;  // FP32 search kernel: compacted pose records per class (k_pose)
+    unsigned epoch = 0;
     ClassTable ct;
     int nclass = 0;
     int class_sa[DEM_MAX_CLASSES], class_sb[DEM_MAX_CLASSES], class_np[DEM_MAX_CLASSES];
     long long npairs_total = 0, nrec_total = 0;
     int force_slices = 0;  // 0 = heuristic
+    bool cull = true;             // packed search kernel in 3D: exact per-feature culling (dem_set_culling)
     bool generic_kernel = false;  // DEM_F32 contexts: use the generic k_pair instead of the packed search kernel
     size_t l2_flush_bytes = 0;  // bench hygiene: overwrite this many bytes of scratch before every time step
     DevBuf l2_scratch;
@@ -248,7 +250,7 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
     CU(ctx->counts.reserve(sizeof(int) * (size_t)N));
     CU(ctx->scratch_scan.reserve(sizeof(int) * scan_ints));
     CU(ctx->flags.reserve(sizeof(int) * 16));
-    CU(ctx->counters.reserve(sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES));
+    CU(ctx->counters.reserve(sizeof(unsigned long long) * 8 + sizeof(int) * 2 * DEM_MAX_CLASSES));
     CU(ctx->pos_build.reserve(sizeof(d4) * (size_t)N));
     int* cell_start = ctx->cell_start.as<int>();
     CU(cudaMemsetAsync(cell_start, 0, sizeof(int) * ((size_t)g.ncell + 1), st));
@@ -348,13 +350,22 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
     if (N != ctx->N) return fail(ctx, DEM_ESTALE, "N = %d differs from the last build (%d)", N, ctx->N);
     if (!pos || !quat || !sid || !force || !torque) return fail(ctx, DEM_EINVAL, "null particle array");
     cudaStream_t st = ctx->stream;
-    // counters[0..7] (unsigned long long) followed by the per-class numbers of in-reach pairs (int): one memset
-    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES, st));
+    // counters[0..7] (unsigned long long) followed by the per-class numbers of in-reach pairs and block tickets of
+    // k_pose (int): one memset
+    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8 + sizeof(int) * 2 * DEM_MAX_CLASSES, st));
     int* ccount = reinterpret_cast<int*>(ctx->counters.as<unsigned long long>() + 8);
+    int* tickets = ccount + DEM_MAX_CLASSES;
+    ctx->epoch = ctx->epoch % 0x3fffffffu + 1u;
     const bool search = std::is_same<real, float>::value && !ctx->generic_kernel;
     if (search) {
         CU(ctx->pose.reserve(sizeof(f4) * 6 * (size_t)std::max<long long>(ctx->npairs_total, 1)));
         CU(ctx->pidx.reserve(sizeof(int) * (size_t)std::max<long long>(ctx->npairs_total, 1)));
+        // look-back scan words of k_pose: one per block, classes back to back (never reset: words carry the epoch)
+        const size_t words = (size_t)ctx->npairs_total / DEM_POSE_THREADS + DEM_MAX_CLASSES + 1;
+        if (ctx->scan_state.cap < words * 8) {
+            CU(ctx->scan_state.reserve(words * 8));
+            CU(cudaMemsetAsync(ctx->scan_state.p, 0, ctx->scan_state.cap, st));
+        }
     }
     BoxDev bx;
     bx.dim = ctx->dim;
@@ -407,6 +418,9 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
                 pa.pose = ctx->pose.as<f4>() + 6 * (size_t)ctx->ct.pair_base[c];
                 pa.pidx = ctx->pidx.as<int>() + ctx->ct.pair_base[c];
                 pa.count = ccount + c;
+                pa.ticket = tickets + c;
+                pa.scan_state = ctx->scan_state.as<unsigned long long>() + ctx->ct.pair_base[c] / DEM_POSE_THREADS + c;
+                pa.epoch = ctx->epoch;
                 pa.rec = reinterpret_cast<f4*>(a.rec);
                 smem += fast_smem_header();
                 // packed outer pairs per sweep: 3 when the vertex counts fill tiles of 6 at least as well as tiles of 4
@@ -436,6 +450,13 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
                     cudaMemcpyToSymbolAsync(g_dbg_phases, &ph, sizeof ph, 0, cudaMemcpyHostToDevice, st);
                 }
 #endif
+                if (ctx->dim == 3 && ctx->cull) {
+                    kern = k_pair_cull<PosT, 4>;
+                    smem += cull_smem_header() - fast_smem_header();
+                    const double ra = HA.circumradius + rcs, rb = HB.circumradius + rcs;
+                    a.cull_a2 = (real)(ra * ra);
+                    a.cull_b2 = (real)(rb * rb);
+                }
                 grid = (int)std::min<long long>(nblk(items, threads), (long long)ctx->sm_count * resident);
             }
         }
@@ -606,7 +627,7 @@ int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda
 int dem_destroy(dem_ctx* c) {
     if (!c) return DEM_EINVAL;
     DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
-                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->pose, &c->pidx, &c->st_pos, &c->st_quat,
+                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->pose, &c->pidx, &c->scan_state, &c->st_pos, &c->st_quat,
                       &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->pos_build, &c->epart, &c->h_pos,
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();
@@ -640,6 +661,12 @@ int dem_set_pair_kernel(dem_ctx* ctx, int which) {
     if (!ctx || (which != DEM_KERNEL_SEARCH && which != DEM_KERNEL_GENERIC && which != DEM_KERNEL_AUTO))
         return fail(ctx, DEM_EINVAL, "unknown pair kernel");
     ctx->generic_kernel = which == DEM_KERNEL_GENERIC || (which == DEM_KERNEL_AUTO && ctx->dim == 2);
+    return DEM_OK;
+}
+
+int dem_set_culling(dem_ctx* ctx, int enabled) {
+    if (!ctx) return DEM_EINVAL;
+    ctx->cull = enabled != 0;
     return DEM_OK;
 }
 
@@ -701,10 +728,10 @@ int dem_compute(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* 
                                    force_energy, torque, virial6);
 }
 
-int dem_get_counters(dem_ctx* ctx, int64_t out[6]) {
+int dem_get_counters(dem_ctx* ctx, int64_t out[7]) {
     if (!ctx || !out) return DEM_EINVAL;
     if (!ctx->counters.p) return fail(ctx, DEM_ESTALE, "no evaluation yet");
-    unsigned long long h[8 + DEM_MAX_CLASSES / 2];
+    unsigned long long h[8 + DEM_MAX_CLASSES];
     CU(cudaMemcpyAsync(h, ctx->counters.p, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     if (ctx->prec == DEM_F32 && !ctx->generic_kernel) {  // the search path counts its evaluated pairs per class (k_pose)
@@ -720,6 +747,10 @@ int dem_get_counters(dem_ctx* ctx, int64_t out[6]) {
     out[3] = (int64_t)h[2];
     out[4] = (int64_t)h[3];
     out[5] = ctx->npairs_total;
+    // terms whose nearest-point search was executed: all of them unless the culling kernel proved some features out of
+    // reach (it counts what it sweeps)
+    const bool culled = ctx->prec == DEM_F32 && !ctx->generic_kernel && ctx->dim == 3 && ctx->cull;
+    out[6] = culled ? (int64_t)h[4] : out[1];
     return DEM_OK;
 }
 
