@@ -383,9 +383,8 @@ __device__ __forceinline__ void sweep_faces(const ShapeView<float>& S, const Sha
 
 // ---- a3: relative pose of every pair of a class, compacted -----------------------------------------------------------
 // One thread per unique pair: minimum-image separation d, exact reach test (R10), relative pose R = R_i^T R_j,
-// t = R_i^T d and R_i in FP64, rounded once to float.  Pairs inside the reach are compacted, in
-// pair order (single-pass look-back scan: the list is the same from run to run), into the class's work list; pairs
-// beyond it get their zero result records here and never reach the search kernel, so its warps carry 32
+// t = R_i^T d and R_i in FP64, rounded once to float.  Pairs inside the reach are compacted into the
+// class's work list (block slices padded to whole warps: see below); pairs beyond it get their zero result records here and never reach the search kernel, so its warps carry 32
 // live pairs each.  Pose record, plane-major for coalesced loads: [6][npairs] float4 =
 // (R0 R1 R2 R3) (R4 R5 R6 R7) (R8 t0 t1 t2) (M0 M1 M2 M3) (M4 M5 M6 M7) (M8 dx dy dz); pidx[c] = the pair's index.
 struct PoseArgs {
@@ -397,22 +396,17 @@ struct PoseArgs {
     double reach2;
     f4* pose;
     int* pidx;
-    int* count;  // valid pairs of this class (written by the last block)
-    int* ticket;  // block numbering (zeroed before the launch)
-    unsigned long long* scan_state;  // one word per block (look-back scan), never reset
-    unsigned epoch;                  // launch number, 1 .. 2^30 - 1
+    int* count;  // entries of this class's work list, padding included (zeroed before the launch)
+    size_t plane;  // stride of the pose planes = capacity of the work list (pairs + 32 per k_pose block)
+    unsigned long long* counters;  // [0] += pairs inside the reach
     f4* rec;
 };
 
-#define DEM_POSE_THREADS 256
+#define DEM_POSE_THREADS 512
 template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THREADS) k_pose(const PoseArgs a) {
-    __shared__ int wcount[DEM_POSE_THREADS / 32], wbase[DEM_POSE_THREADS / 32], s_bid, s_prefix;
+    __shared__ int wcount[DEM_POSE_THREADS / 32], s_prefix;
     const unsigned full = 0xffffffffu;
-    // blocks take their number from a ticket, so that every block's predecessors in the scan have already started
-    if (threadIdx.x == 0) s_bid = atomicAdd(a.ticket, 1);
-    __syncthreads();
-    const int bid = s_bid;
-    const int p = bid * blockDim.x + threadIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     bool valid = false;
     double d[3] = {0.0, 0.0, 0.0};
     d4 qi, qj;
@@ -429,24 +423,21 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THR
         if (DIM == 3) d[2] -= a.box.L[2] * rint(d[2] * a.box.invL[2]);
         valid = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] < a.reach2;
     }
-    // Ordered compaction (pair order is kept, so the work list and every sum downstream are the same from run to run):
-    // single-pass scan over the blocks with decoupled look-back.  Each block publishes (epoch, kind, value) in one
-    // 64-bit word: kind 1 = its own count (as early as possible), kind 2 = its inclusive prefix; warp 0 adds up the
-    // predecessors' words, 32 at a time, back to the nearest inclusive one.  The epoch makes the words of earlier
-    // launches invisible (no reset).
+    // Compaction.  Inside a block the pairs keep their order; a block's slice of the work list is padded to a multiple of
+    // 32 entries (pidx = -1) and placed with one atomicAdd, so every warp of the search kernel gets 32 consecutive
+    // entries of ONE block: which pairs share a warp, and with it every sum downstream, is the same from run to run
+    // although the order of the blocks' slices is not.
     const unsigned m = __ballot_sync(full, valid);
     if (lane == 0) wcount[warp] = __popc(m);
     __syncthreads();
     int tot = 0;
 #pragma unroll
     for (int k = 0; k < DEM_POSE_THREADS / 32; ++k) tot += wcount[k];
-    const unsigned long long tag = (unsigned long long)a.epoch << 34;
-    volatile unsigned long long* st = a.scan_state;
-    if (threadIdx.x == 0 && bid > 0) {
-        st[bid] = tag | (1ull << 32) | (unsigned)tot;
-        __threadfence();
+    const int tot_pad = (tot + 31) & ~31;
+    if (threadIdx.x == 0) {
+        s_prefix = tot_pad ? atomicAdd(a.count, tot_pad) : 0;
+        if (tot) atomicAdd(a.counters, (unsigned long long)tot);
     }
-    // the pose itself (FP64), while the predecessors publish
     float Mi[9], R[9], t[3];
     if (valid) {
         const double qa[4] = {qi.x, qi.y, qi.z, qi.w}, qb[4] = {qj.x, qj.y, qj.z, qj.w};
@@ -461,34 +452,13 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THR
             rec[0] = r0; rec[1] = r1; rec[2] = r2;
         }
     }
-    if (warp == 0) {
-        int prefix = 0;
-        for (int j0 = bid - 1; j0 >= 0; j0 -= 32) {
-            const int j = j0 - lane;
-            unsigned long long v = 0ull;
-            if (j >= 0) {
-                do {
-                    v = st[j];
-                } while ((v >> 34) != a.epoch || ((v >> 32) & 3ull) == 0ull);
-            }
-            const unsigned incl = __ballot_sync(full, j >= 0 && ((v >> 32) & 3ull) == 2ull);
-            const int stop = incl ? __ffs(incl) - 1 : 31;  // nearest inclusive prefix among these 32 (lane order = backwards)
-            prefix += __reduce_add_sync(full, (j >= 0 && lane <= stop) ? (int)(unsigned)v : 0);
-            if (incl) break;
-        }
-        if (lane == 0) {
-            st[bid] = tag | (2ull << 32) | (unsigned)(prefix + tot);
-            __threadfence();
-            if (bid == (int)gridDim.x - 1) *a.count = prefix + tot;
-            s_prefix = prefix;
-        }
-    }
     __syncthreads();
+    if ((int)threadIdx.x < tot_pad - tot) a.pidx[s_prefix + tot + threadIdx.x] = -1;
     if (valid) {
         int wb = s_prefix;
         for (int k = 0; k < warp; ++k) wb += wcount[k];
         const int c = wb + __popc(m & ((1u << lane) - 1u));
-        const size_t n = (size_t)a.npairs;
+        const size_t n = a.plane;
         f4 v;
         v.x = R[0]; v.y = R[1]; v.z = R[2]; v.w = R[3]; a.pose[c] = v;
         v.x = R[4]; v.y = R[5]; v.z = R[6]; v.w = R[7]; a.pose[n + c] = v;
@@ -553,7 +523,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
     const int count = *a.count;                // pairs inside the reach, compacted by k_pose
     const int np_pad = (count + 31) & ~31;     // slices are warp-uniform
     const long long n_wtiles = (long long)(np_pad >> 5) * a.slices;
-    const size_t plane = (size_t)a.npairs;
+    const size_t plane = a.plane;
     // Each warp takes every (gridDim.x * 4)-th tile (one tile per warp unless the class has more tiles than the grid
     // cap).  The pose records of a warp's next tile are copied global -> shared with cp.async while the current tile is
     // being swept; each lane copies and later reads only its own records.
@@ -579,11 +549,12 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
     for (long long wt = (long long)blockIdx.x * 4 + warp; wt < n_wtiles; wt += wt_stride, buf ^= 1) {
         const long long item = wt * 32 + lane;
         const int slice = (int)(item / np_pad), c = (int)(item - (long long)slice * np_pad);
-        const bool valid = c < count;
+        const bool in_list = c < count;
         stage(buf ^ 1, wt + wt_stride);
         asm volatile("cp.async.wait_group 1;" ::: "memory");
         __syncwarp();  // the cooperative evaluation reads other lanes' staged poses
         w.sp = spose + buf * 6 * 32;
+        const bool valid = in_list && spidx[buf * 32 + lane] >= 0;  // the work list is padded to whole warps per k_pose block
         float R[9], t[3];
         if (valid) {
             const f4 p0 = spose[(buf * 6 + 0) * 32 + lane], p1 = spose[(buf * 6 + 1) * 32 + lane],
@@ -916,7 +887,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     const int count = *a.count;
     const int np_pad = (count + 31) & ~31;
     const long long n_wtiles = (long long)(np_pad >> 5) * a.slices;
-    const size_t plane = (size_t)a.npairs;
+    const size_t plane = a.plane;
     const long long wt_stride = (long long)gridDim.x * 4;
     f4* spose = stage_pose + warp * (2 * 6 * 32);
     int* spidx = stage_pidx + warp * (2 * 32);
@@ -939,11 +910,12 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     for (long long wt = (long long)blockIdx.x * 4 + warp; wt < n_wtiles; wt += wt_stride, buf ^= 1) {
         const long long item = wt * 32 + lane;
         const int slice = (int)(item / np_pad), c = (int)(item - (long long)slice * np_pad);
-        const bool valid = c < count;
+        const bool in_list = c < count;
         stage(buf ^ 1, wt + wt_stride);
         asm volatile("cp.async.wait_group 1;" ::: "memory");
         __syncwarp();
         w.sp = spose + buf * 6 * 32;
+        const bool valid = in_list && spidx[buf * 32 + lane] >= 0;  // the work list is padded to whole warps per k_pose block
         float R[9], t[3], tp[3] = {1.0e4f, 1.0e4f, 1.0e4f};
         if (valid) {
             load_pose(w.sp, lane, R, t);

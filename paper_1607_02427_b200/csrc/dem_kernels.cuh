@@ -289,6 +289,7 @@ template <typename real> struct PairArgs {
     const f4* pose;       // FP32 search kernel: this class's compacted pose records, pair indices and their number
     const int* pidx;      //   (written by k_pose)
     const int* count;
+    size_t plane;         //   stride of the pose planes
     unsigned long long* counters;  // [0] pairs evaluated, [1] active, [2] degenerate, [3] parallel
 };
 

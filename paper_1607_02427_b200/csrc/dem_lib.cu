@@ -58,8 +58,7 @@ struct dem_ctx {
     double box[3] = {0, 0, 0}, r_cut = 0;
     GridDev grid;
     DevBuf cell_of, rank, cell_start, order, xs, counts, list, slot, scratch_scan, pcnt, pairs, rec, flags, counters;
-    DevBuf pose, pidx, scan_state;  // FP32 search kernel: compacted pose records per class (k_pose)
-    unsigned epoch = 0;
+    DevBuf pose, pidx;  // FP32 search kernel: compacted pose records per class (k_pose)
     ClassTable ct;
     int nclass = 0;
     int class_sa[DEM_MAX_CLASSES], class_sb[DEM_MAX_CLASSES], class_np[DEM_MAX_CLASSES];
@@ -250,7 +249,7 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
     CU(ctx->counts.reserve(sizeof(int) * (size_t)N));
     CU(ctx->scratch_scan.reserve(sizeof(int) * scan_ints));
     CU(ctx->flags.reserve(sizeof(int) * 16));
-    CU(ctx->counters.reserve(sizeof(unsigned long long) * 8 + sizeof(int) * 2 * DEM_MAX_CLASSES));
+    CU(ctx->counters.reserve(sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES));
     CU(ctx->pos_build.reserve(sizeof(d4) * (size_t)N));
     int* cell_start = ctx->cell_start.as<int>();
     CU(cudaMemsetAsync(cell_start, 0, sizeof(int) * ((size_t)g.ncell + 1), st));
@@ -350,22 +349,18 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
     if (N != ctx->N) return fail(ctx, DEM_ESTALE, "N = %d differs from the last build (%d)", N, ctx->N);
     if (!pos || !quat || !sid || !force || !torque) return fail(ctx, DEM_EINVAL, "null particle array");
     cudaStream_t st = ctx->stream;
-    // counters[0..7] (unsigned long long) followed by the per-class numbers of in-reach pairs and block tickets of
-    // k_pose (int): one memset
-    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8 + sizeof(int) * 2 * DEM_MAX_CLASSES, st));
+    // counters[0..7] (unsigned long long) followed by the per-class lengths of the k_pose work lists (int): one memset
+    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES, st));
     int* ccount = reinterpret_cast<int*>(ctx->counters.as<unsigned long long>() + 8);
-    int* tickets = ccount + DEM_MAX_CLASSES;
-    ctx->epoch = ctx->epoch % 0x3fffffffu + 1u;
+    // capacity of a class's work list: its pairs plus the padding of every k_pose block to a whole warp
+    auto list_cap = [&](int c) { return (size_t)ctx->class_np[c] + 32u * (size_t)nblk(ctx->class_np[c], DEM_POSE_THREADS); };
+    size_t list_base[DEM_MAX_CLASSES + 1];
+    list_base[0] = 0;
+    for (int c = 0; c < ctx->nclass; ++c) list_base[c + 1] = list_base[c] + list_cap(c);
     const bool search = std::is_same<real, float>::value && !ctx->generic_kernel;
     if (search) {
-        CU(ctx->pose.reserve(sizeof(f4) * 6 * (size_t)std::max<long long>(ctx->npairs_total, 1)));
-        CU(ctx->pidx.reserve(sizeof(int) * (size_t)std::max<long long>(ctx->npairs_total, 1)));
-        // look-back scan words of k_pose: one per block, classes back to back (never reset: words carry the epoch)
-        const size_t words = (size_t)ctx->npairs_total / DEM_POSE_THREADS + DEM_MAX_CLASSES + 1;
-        if (ctx->scan_state.cap < words * 8) {
-            CU(ctx->scan_state.reserve(words * 8));
-            CU(cudaMemsetAsync(ctx->scan_state.p, 0, ctx->scan_state.cap, st));
-        }
+        CU(ctx->pose.reserve(sizeof(f4) * 6 * std::max<size_t>(list_base[ctx->nclass], 1)));
+        CU(ctx->pidx.reserve(sizeof(int) * std::max<size_t>(list_base[ctx->nclass], 1)));
     }
     BoxDev bx;
     bx.dim = ctx->dim;
@@ -410,17 +405,17 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
         PoseArgs pa;
         if constexpr (std::is_same<real, float>::value) {
             if (search) {
-                a.pose = ctx->pose.as<f4>() + 6 * (size_t)ctx->ct.pair_base[c];
-                a.pidx = ctx->pidx.as<int>() + ctx->ct.pair_base[c];
+                a.pose = ctx->pose.as<f4>() + 6 * list_base[c];
+                a.pidx = ctx->pidx.as<int>() + list_base[c];
+                a.plane = list_cap(c);
                 a.count = ccount + c;
                 pa.pairs = a.pairs; pa.npairs = np; pa.slices = a.slices; pa.pos = pos; pa.quat = quat; pa.box = bx;
                 pa.reach2 = a.reach2;
-                pa.pose = ctx->pose.as<f4>() + 6 * (size_t)ctx->ct.pair_base[c];
-                pa.pidx = ctx->pidx.as<int>() + ctx->ct.pair_base[c];
+                pa.pose = ctx->pose.as<f4>() + 6 * list_base[c];
+                pa.pidx = ctx->pidx.as<int>() + list_base[c];
                 pa.count = ccount + c;
-                pa.ticket = tickets + c;
-                pa.scan_state = ctx->scan_state.as<unsigned long long>() + ctx->ct.pair_base[c] / DEM_POSE_THREADS + c;
-                pa.epoch = ctx->epoch;
+                pa.plane = list_cap(c);
+                pa.counters = a.counters;
                 pa.rec = reinterpret_cast<f4*>(a.rec);
                 smem += fast_smem_header();
                 // packed outer pairs per sweep: 3 when the vertex counts fill tiles of 6 at least as well as tiles of 4
@@ -457,7 +452,8 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
                     a.cull_a2 = (real)(ra * ra);
                     a.cull_b2 = (real)(rb * rb);
                 }
-                grid = (int)std::min<long long>(nblk(items, threads), (long long)ctx->sm_count * resident);
+                const long long list_items = (long long)list_cap(c) * a.slices;  // the padded work list bounds the tiles
+                grid = (int)std::min<long long>(nblk(list_items, threads), (long long)ctx->sm_count * resident);
             }
         }
         if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -627,7 +623,7 @@ int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda
 int dem_destroy(dem_ctx* c) {
     if (!c) return DEM_EINVAL;
     DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
-                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->pose, &c->pidx, &c->scan_state, &c->st_pos, &c->st_quat,
+                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->pose, &c->pidx, &c->st_pos, &c->st_quat,
                       &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->pos_build, &c->epart, &c->h_pos,
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();
@@ -731,14 +727,9 @@ int dem_compute(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* 
 int dem_get_counters(dem_ctx* ctx, int64_t out[7]) {
     if (!ctx || !out) return DEM_EINVAL;
     if (!ctx->counters.p) return fail(ctx, DEM_ESTALE, "no evaluation yet");
-    unsigned long long h[8 + DEM_MAX_CLASSES];
+    unsigned long long h[8];
     CU(cudaMemcpyAsync(h, ctx->counters.p, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
-    if (ctx->prec == DEM_F32 && !ctx->generic_kernel) {  // the search path counts its evaluated pairs per class (k_pose)
-        const int* cc = reinterpret_cast<const int*>(h + 8);
-        h[0] = 0;
-        for (int c = 0; c < ctx->nclass; ++c) h[0] += (unsigned long long)cc[c];
-    }
     // terms evaluated = nominal terms of the evaluated pairs; with a single class this is exact, with several classes
     // pairs rejected by the reach test are attributed proportionally (the list is normally built at r_cut = reach)
     out[0] = (int64_t)h[0];
