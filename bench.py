@@ -203,7 +203,8 @@ def main():
     ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
     ap.add_argument("--no-l2-flush", action="store_true")
     ap.add_argument("--slices", type=int, default=0, help="lanes per pair in the pair kernel (0 = library heuristic)")
-    ap.add_argument("--no-cull", action="store_true", help="sweep every Eq. 1 term (no exact per-feature culling)")
+    ap.add_argument("--cull", action="store_true",
+                    help="headline arm with exact per-feature culling (default: every Eq. 1 term swept; culling is the second arm)")
     ap.add_argument("--pair-kernel", default="auto", choices=["auto", "search", "generic"],
                     help="search = packed FP32 contact search; generic = fused scalar kernel; auto = library default")
     ap.add_argument("--e2e-steps", type=int, default=10)
@@ -240,8 +241,10 @@ def main():
     dem, t = pkg.from_state(st, "f32")
     if args.slices:
         dem.set_slices(args.slices)
-    if args.no_cull:
-        dem.set_culling(False)
+    # headline arm: every Eq. 1 / Eq. 2 term is swept (the paper's method as stated); the
+    # library's default, exact per-feature culling, is measured as a second arm ("culled") on the same state
+    search3d = st["dim"] == 3 and args.pair_kernel != "generic"
+    dem.set_culling(bool(args.cull))
     if args.pair_kernel != "auto":
         dem.set_pair_kernel({"search": 0, "generic": 1}[args.pair_kernel])
     if not args.no_l2_flush:
@@ -253,27 +256,36 @@ def main():
         dem.step(t["pos"], t["quat"], t["vel"], t["angmom"], t["shape_id"], st["box"], dt_step, nsteps, skin, force, torque)
 
     # ---- device-resident throughput ---------------------------------------------------------------------------
-    step(args.warmup)
-    dem.set_timing(True)
-    dem.kernel_time()
-    launches0 = dem.launch_count()
-    sampler = ClockSampler(local) if rank == 0 else None
-    barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    step(args.steps)
-    e1.record()
-    barrier()
-    elapsed_ms = e0.elapsed_time(e1)
-    clocks = sampler.stop() if sampler else None
-    gpu_launches = dem.launch_count() - launches0
-    n_pair_launches, pair_ms = dem.kernel_time()
-    dem.set_timing(False)
-    cnt = dem.get_counters()
-    tm = torch.tensor([elapsed_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-    elapsed_ms = float(tm.item())
+    def timed(nwarm, nsteps, sample_clocks):
+        """nwarm untimed + nsteps timed steps; (ms, clocks, launches, pair-kernel launches, their ms, counters)."""
+        step(nwarm)
+        dem.set_timing(True)
+        dem.kernel_time()
+        l0 = dem.launch_count()
+        sampler = ClockSampler(local) if (rank == 0 and sample_clocks) else None
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        step(nsteps)
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        clk = sampler.stop() if sampler else None
+        nl = dem.launch_count() - l0
+        npl, pms = dem.kernel_time()
+        dem.set_timing(False)
+        tm = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+        return float(tm.item()), clk, nl, npl, pms, dem.get_counters()
+
+    def swept_flops(c):
+        """Algorithmic flop of the terms whose search was executed in the last evaluation (library counters)."""
+        if st["dim"] == 2:
+            return FLOP_VE_2D * c["ee_swept"]
+        return FLOP_EE * c["ee_swept"] + FLOP_VF_FACE * (c["terms_swept"] - c["ee_swept"]) + FLOP_VF_EDGE * c["face_edges_swept"]
+
+    elapsed_ms, clocks, gpu_launches, n_pair_launches, pair_ms, cnt = timed(args.warmup, args.steps, True)
     value = n * world * args.steps / (elapsed_ms * 1e-3)
 
     # ---- roofline of the pair-feature kernel ---------------------------------------------------------------------
@@ -289,8 +301,22 @@ def main():
     peaks, peak_kind = measured_peaks()
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     peak_tf = sm_count * 128 * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
-    achieved_tf = flops / (kern_ms_per_eval * 1e-3) / 1e12
+    flops_swept = swept_flops(cnt)
+    achieved_tf = flops_swept / (kern_ms_per_eval * 1e-3) / 1e12
     fma_measured = dem.fp32_peak(1 << 15)
+    # second arm: the same steps with the library's default, exact per-feature culling
+    culled = None
+    if search3d and not args.cull:
+        dem.set_culling(True)
+        cms, _, _, cnpl, cpms, ccnt = timed(3, args.steps, False)
+        dem.set_culling(False)
+        ckern = cpms / max(cnpl // max(n_classes, 1), 1)
+        ctf = swept_flops(ccnt) / (ckern * 1e-3) / 1e12
+        culled = {"value": n * world * args.steps / (cms * 1e-3), "unit": "particle-timesteps/s",
+                  "ms_per_step": cms / args.steps, "kernel": "k_pose + k_pair_cull", "kernel_ms": ckern,
+                  "terms_swept_last_step": ccnt["terms_swept"], "terms_last_step": ccnt["terms"],
+                  "flops_per_launch": swept_flops(ccnt), "achieved": ctf, "frac": ctf / peak_tf,
+                  "note": "same results; the kernel is no longer ALU-bound (cull tests, queues, pose traffic)"}
     # DRAM traffic of the dominant kernel per launch: from the committed `ncu --set full` summary of this workload
     traffic = None
     prof = os.path.join(ROOT, "profiles", "r01_step_%s_ncu.md" % args.workload)
@@ -333,16 +359,21 @@ def main():
             "config": {"workload": di.CONFIG_NAMES[k], "N": n, "dt": dt_step, "skin": skin,
                        "parallelism": "replicas x%d" % world if world > 1 else "1 GPU",
                        "l2": ("flushed before every step (160 MiB memset inside the timed region)"
-                              if not args.no_l2_flush else "not flushed (working set < L2)")},
+                              if not args.no_l2_flush else "not flushed (working set < L2)"),
+                       "culling": ("on" if args.cull else "off: every Eq. 1/2 term of every in-reach pair is swept; 'culled' = "
+                                   "the same steps with the library default (exact per-feature culling)")},
             "feature_pair_evals_per_s": terms * world * (args.steps + 1) / (elapsed_ms * 1e-3),
             "feature_pairs_per_step": terms, "unique_pairs": int(cls.sum()), "active_terms_last_step": cnt["active"],
-            "roofline": {"bound": "alu", "kernel": "k_pose + k_pair_fast" if st["dim"] == 3 and args.pair_kernel != "generic" else "k_pair", "achieved": achieved_tf, "peak": peak_tf,
+            "roofline": {"bound": "alu", "kernel": ("k_pose + k_pair_cull" if (args.cull and search3d) else "k_pose + k_pair_fast")
+                         if (st["dim"] == 3 or args.pair_kernel == "search") and args.pair_kernel != "generic" else "k_pair", "achieved": achieved_tf, "peak": peak_tf,
                          "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": traffic,
                          "peak_source": "%d SM x 128 FP32 lanes x 2 x %.0f MHz (clocks.max.sm, %s)" % (
                              sm_count, float(peaks.get("sm_max_mhz", 1965.0)), peak_kind),
-                         "flops_per_launch": flops, "kernel_ms": kern_ms_per_eval, "launches_timed": n_pair_launches,
+                         "flops_per_launch": flops_swept, "flops_all_terms": flops,
+                         "terms_swept_last_step": cnt["terms_swept"], "kernel_ms": kern_ms_per_eval, "launches_timed": n_pair_launches,
                          "kernel_share_of_step": pair_ms / elapsed_ms,
                          "fma_chain_measured_tflops": fma_measured},
+            "culled": culled,
             "cpu_baseline": cpu_baseline,
             "e2e": {"value": e2e_value, "unit": "particle-timesteps/s", "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "steps": args.e2e_steps},

@@ -127,8 +127,10 @@ int dem_compute(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* 
  * of those pairs (polygon faces, each unique pair once), out[2] terms inside the WCA cutoff, out[3] degenerate terms
  * skipped, out[4] terms that took the parallel-edge branch, out[5] unique pairs in the work list, out[6] terms whose
  * nearest-point search was actually executed (= out[1] unless exact culling proved features out of reach: see
- * dem_set_culling). HOST int64[7]. */
-int dem_get_counters(dem_ctx* ctx, int64_t out[7]);
+ * dem_set_culling), out[7] of which edge-edge terms (3D; in 2D all terms are vertex-edge and are counted here),
+ * out[8] face boundary-edge tests inside the executed vertex-face terms (out[7] and out[8] feed the flop count of
+ * bench.py). HOST int64[9]. */
+int dem_get_counters(dem_ctx* ctx, int64_t out[9]);
 
 /*
  * nsteps of velocity-Verlet NVE with quaternion rotation (reading R15): half-kick v and L; drift x

@@ -194,10 +194,10 @@ class Dem:
         return f, t, w
 
     def get_counters(self):
-        out = (C.c_int64 * 7)()
+        out = (C.c_int64 * 9)()
         _check(self._ctx, lib().dem_get_counters(self._ctx, out))
         return dict(pairs_evaluated=out[0], terms=out[1], active=out[2], degenerate=out[3], parallel=out[4],
-                    pairs_listed=out[5], terms_swept=out[6])
+                    pairs_listed=out[5], terms_swept=out[6], ee_swept=out[7], face_edges_swept=out[8])
 
     # ---- dem_step / dem_energy -----------------------------------------------------------------------------------------
     def step(self, pos, quat, vel, angmom, shape_id, box, dt, nsteps, skin, force=None, torque=None):

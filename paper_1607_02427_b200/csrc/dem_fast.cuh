@@ -524,6 +524,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
     const int np_pad = (count + 31) & ~31;     // slices are warp-uniform
     const long long n_wtiles = (long long)(np_pad >> 5) * a.slices;
     const size_t plane = a.plane;
+    unsigned n_ee = 0u, n_vf = 0u, n_vfe = 0u;
     // Each warp takes every (gridDim.x * 4)-th tile (one tile per warp unless the class has more tiles than the grid
     // cap).  The pose records of a warp's next tile are copied global -> shared with cp.async while the current tile is
     // being swept; each lane copies and later reads only its own records.
@@ -573,6 +574,19 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
             for (int k = 0; k < 7; ++k) w.sacc[k * 32 + lane] = 0.f;
             const int ob = (int)((long long)slice * a.n_outer / a.slices);
             const int oe = (int)((long long)(slice + 1) * a.n_outer / a.slices);
+            if (valid) {  // terms this lane sweeps (for the flop count; the kernel sweeps every term of its pairs)
+                if (DIM == 3) {
+                    const int oE_ = B.ne, oV_ = B.ne + B.nv;
+                    const int r1 = max(min(oe, oE_) - ob, 0), r2 = max(min(oe, oV_) - max(ob, oE_), 0),
+                              r3 = max(min(oe, oV_ + A.nv) - max(ob, oV_), 0);
+                    n_ee += (unsigned)(r1 * A.ne);
+                    n_vf += (unsigned)(r2 * A.nf + r3 * B.nf);
+                    n_vfe += (unsigned)(r2 * a.sa.nfe + r3 * a.sb.nfe);
+                } else {
+                    const int r1 = max(min(oe, B.nv) - ob, 0), r2 = max(min(oe, B.nv + A.nv) - max(ob, B.nv), 0);
+                    n_ee += (unsigned)(r1 * A.ne + r2 * B.ne);  // 2D: vertex-edge terms
+                }
+            }
             if (DIM == 3) {
                 const int oE = B.ne, oV = B.ne + B.nv;
                 // (1) first sum of Eq. 1: edges of j (outer, packed) against edges of i (inner)
@@ -739,7 +753,12 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
     }
     // counters: one atomic per warp per counter, after the hot loop
     __syncwarp();
+    const unsigned long long s_ee = __reduce_add_sync(full, n_ee), s_vf = __reduce_add_sync(full, n_vf),
+                             s_vfe = __reduce_add_sync(full, n_vfe);
     if (lane == 0) {
+        if (s_ee) atomicAdd(a.counters + 4, s_ee);
+        if (s_vf) atomicAdd(a.counters + 5, s_vf);
+        if (s_vfe) atomicAdd(a.counters + 6, s_vfe);
         if (w.scnt[0]) atomicAdd(a.counters + 1, (unsigned long long)w.scnt[0]);
         if (w.scnt[1]) atomicAdd(a.counters + 2, (unsigned long long)w.scnt[1]);
         if (w.scnt[2]) atomicAdd(a.counters + 3, (unsigned long long)w.scnt[2]);
@@ -761,12 +780,12 @@ static inline size_t fast_smem_header() {
 // compacted into a warp-private list of (owner lane, outer feature) items, and the sweeps run over ITEMS, two per lane
 // in the halves of the packed registers (the halves may belong to different pairs: inner features are shared by the
 // whole class, poses come from the staged records).  Candidates and their evaluation are as in k_pair_fast.
-#define DEM_IQCAP 512
+#define DEM_IQCAP 1024  // 32 lanes x 32 outer features per round
 
 struct CullCtx {
     unsigned* iq;    // item list of the warp
     int iqn;         // items queued (warp-uniform)
-    unsigned swept;  // terms this lane swept (for the flop count)
+    unsigned swept_ee, swept_vf, swept_vfe;  // this lane's swept edge-edge terms, vertex-face terms, face-edge tests
 };
 
 __device__ __forceinline__ void load_pose(const f4* sp, int owner, float* R, float* t) {
@@ -808,7 +827,7 @@ __device__ __forceinline__ void sweep_items(WarpCtx& w, CullCtx& cc, const Shape
                                                    b0.w, nrc2));
                 if (__any_sync(full, mask != 0u)) push_one(w, PHASE, mask, k1 - k0, k0, wa, oa, ok_a, wb, ob, ok_b);
             }
-            cc.swept += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)A.ne;
+            cc.swept_ee += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)A.ne;
         } else {
             const ShapeView<float>& In = PHASE == PH_VF_OWN ? A : B;
             const ShapeView<float>& Out = PHASE == PH_VF_OWN ? B : A;
@@ -829,17 +848,31 @@ __device__ __forceinline__ void sweep_items(WarpCtx& w, CullCtx& cc, const Shape
                 sweep_faces<1>(In, sd, f0, f1, px, py, pz, nrc2, mask);
                 if (__any_sync(full, mask[0] != 0u)) push_one(w, PHASE, mask[0], f1 - f0, f0, wa, oa, ok_a, wb, ob, ok_b);
             }
-            cc.swept += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)In.nf;
+            cc.swept_vf += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)In.nf;
+            cc.swept_vfe += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)sd.nfe;
         }
     }
     cc.iqn = 0;
 }
 
-// append the lanes' surviving outer feature o to the item list (ballot-ranked: order fixed by the data)
-__device__ __forceinline__ void push_item(const WarpCtx& w, CullCtx& cc, bool survive, int o) {
-    const unsigned m = __ballot_sync(0xffffffffu, survive);
-    if (survive) cc.iq[cc.iqn + __popc(m & ((1u << w.lane) - 1u))] = ((unsigned)w.lane << 16) | (unsigned)o;
-    cc.iqn += __popc(m);
+// append the lanes' surviving outer features (bit k of mask <=> feature o0 + k survives) to the item list, lane by
+// lane (exclusive prefix of the lanes' counts: the order is fixed by the data)
+__device__ __forceinline__ void emit_items(const WarpCtx& w, CullCtx& cc, unsigned mask, int o0) {
+    const unsigned full = 0xffffffffu;
+    const int cnt = __popc(mask);
+    int incl = cnt;
+#pragma unroll
+    for (int dlt = 1; dlt < 32; dlt <<= 1) {
+        const int y = __shfl_up_sync(full, incl, dlt);
+        if (w.lane >= dlt) incl += y;
+    }
+    int pos = cc.iqn + incl - cnt;
+    while (mask) {
+        const int b = __ffs(mask) - 1;
+        mask &= mask - 1u;
+        cc.iq[pos++] = ((unsigned)w.lane << 16) | (unsigned)(o0 + b);
+    }
+    cc.iqn += __shfl_sync(full, incl, 31);
 }
 
 template <typename PosT, int MINB>
@@ -882,7 +915,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     CullCtx cc;
     cc.iq = items + warp * DEM_IQCAP;
     cc.iqn = 0;
-    cc.swept = 0u;
+    cc.swept_ee = cc.swept_vf = cc.swept_vfe = 0u;
     const float nrc2 = -a.rc2_search;
     const int count = *a.count;
     const int np_pad = (count + 31) & ~31;
@@ -930,31 +963,43 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
         const int oe = (int)((long long)(slice + 1) * a.n_outer / a.slices);
         const int oE = B.ne, oV = B.ne + B.nv;
         // (1) edges of j whose distance from i's centre is below R_i + rc_search: in j's frame the centre of i is -R^T t
-        for (int l = ob, le = min(oe, oE); l < le; ++l) {
-            if (cc.iqn + 32 > DEM_IQCAP) sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
-            const f4 a0 = B.OE[2 * l], a1 = B.OE[2 * l + 1];
-            const float qx = a0.x + tp[0], qy = a0.y + tp[1], qz = a0.z + tp[2];
-            const float s = fminf(fmaxf(-(qx * a1.x + qy * a1.y + qz * a1.z), 0.f), a0.w);
-            const float cx = qx + s * a1.x, cy = qy + s * a1.y, cz = qz + s * a1.z;
-            push_item(w, cc, valid && cx * cx + cy * cy + cz * cz < a.cull_a2, l);
+        for (int l0 = ob, le = min(oe, oE); l0 < le; l0 += 32) {
+            const int n = min(32, le - l0);
+            unsigned mask = 0u;
+            for (int k = 0; k < n; ++k) {
+                const f4 a0 = B.OE[2 * (l0 + k)], a1 = B.OE[2 * (l0 + k) + 1];
+                const float qx = a0.x + tp[0], qy = a0.y + tp[1], qz = a0.z + tp[2];
+                const float s = fminf(fmaxf(-(qx * a1.x + qy * a1.y + qz * a1.z), 0.f), a0.w);
+                const float cx = qx + s * a1.x, cy = qy + s * a1.y, cz = qz + s * a1.z;
+                mask |= (cx * cx + cy * cy + cz * cz < a.cull_a2 ? 1u : 0u) << k;
+            }
+            emit_items(w, cc, valid ? mask : 0u, l0);
+            sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
         }
-        sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
         // (2) vertices of j near i
-        for (int o = max(ob, oE) - oE, on = min(oe, oV) - oE; o < on; ++o) {
-            if (cc.iqn + 32 > DEM_IQCAP) sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
-            const f4 v = B.V[o];
-            const float qx = v.x + tp[0], qy = v.y + tp[1], qz = v.z + tp[2];
-            push_item(w, cc, valid && qx * qx + qy * qy + qz * qz < a.cull_a2, o);
+        for (int o0 = max(ob, oE) - oE, on = min(oe, oV) - oE; o0 < on; o0 += 32) {
+            const int n = min(32, on - o0);
+            unsigned mask = 0u;
+            for (int k = 0; k < n; ++k) {
+                const f4 v = B.V[o0 + k];
+                const float qx = v.x + tp[0], qy = v.y + tp[1], qz = v.z + tp[2];
+                mask |= (qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
+            }
+            emit_items(w, cc, valid ? mask : 0u, o0);
+            sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
         }
-        sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
         // (3) vertices of i near j: |R^T (v - t)| = |v - t|
-        for (int o = max(ob, oV) - oV, on = min(oe, oV + A.nv) - oV; o < on; ++o) {
-            if (cc.iqn + 32 > DEM_IQCAP) sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
-            const f4 v = A.V[o];
-            const float qx = v.x - t[0], qy = v.y - t[1], qz = v.z - t[2];
-            push_item(w, cc, valid && qx * qx + qy * qy + qz * qz < a.cull_b2, o);
+        for (int o0 = max(ob, oV) - oV, on = min(oe, oV + A.nv) - oV; o0 < on; o0 += 32) {
+            const int n = min(32, on - o0);
+            unsigned mask = 0u;
+            for (int k = 0; k < n; ++k) {
+                const f4 v = A.V[o0 + k];
+                const float qx = v.x - t[0], qy = v.y - t[1], qz = v.z - t[2];
+                mask |= (qx * qx + qy * qy + qz * qz < a.cull_b2 ? 1u : 0u) << k;
+            }
+            emit_items(w, cc, valid ? mask : 0u, o0);
+            sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
         }
-        sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
         if (w.qn > 0) {
             drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp);
             w.qn = 0;
@@ -980,12 +1025,15 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
         }
         __syncwarp();  // the next tile's stage() overwrites the other buffer only; sacc is re-zeroed by its own lane
     }
-    const unsigned swept = __reduce_add_sync(0xffffffffu, cc.swept);
+    const unsigned s_ee = __reduce_add_sync(0xffffffffu, cc.swept_ee), s_vf = __reduce_add_sync(0xffffffffu, cc.swept_vf),
+                   s_vfe = __reduce_add_sync(0xffffffffu, cc.swept_vfe);
     if (lane == 0) {
         if (w.scnt[0]) atomicAdd(a.counters + 1, (unsigned long long)w.scnt[0]);
         if (w.scnt[1]) atomicAdd(a.counters + 2, (unsigned long long)w.scnt[1]);
         if (w.scnt[2]) atomicAdd(a.counters + 3, (unsigned long long)w.scnt[2]);
-        if (swept) atomicAdd(a.counters + 4, (unsigned long long)swept);
+        if (s_ee) atomicAdd(a.counters + 4, (unsigned long long)s_ee);
+        if (s_vf) atomicAdd(a.counters + 5, (unsigned long long)s_vf);
+        if (s_vfe) atomicAdd(a.counters + 6, (unsigned long long)s_vfe);
     }
 }
 

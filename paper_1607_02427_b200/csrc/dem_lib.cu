@@ -724,7 +724,7 @@ int dem_compute(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* 
                                    force_energy, torque, virial6);
 }
 
-int dem_get_counters(dem_ctx* ctx, int64_t out[7]) {
+int dem_get_counters(dem_ctx* ctx, int64_t out[9]) {
     if (!ctx || !out) return DEM_EINVAL;
     if (!ctx->counters.p) return fail(ctx, DEM_ESTALE, "no evaluation yet");
     unsigned long long h[8];
@@ -738,10 +738,29 @@ int dem_get_counters(dem_ctx* ctx, int64_t out[7]) {
     out[3] = (int64_t)h[2];
     out[4] = (int64_t)h[3];
     out[5] = ctx->npairs_total;
-    // terms whose nearest-point search was executed: all of them unless the culling kernel proved some features out of
-    // reach (it counts what it sweeps)
-    const bool culled = ctx->prec == DEM_F32 && !ctx->generic_kernel && ctx->dim == 3 && ctx->cull;
-    out[6] = culled ? (int64_t)h[4] : out[1];
+    // terms whose nearest-point search was executed (the search kernels count what they sweep; the generic kernel
+    // sweeps every term of the pairs it evaluates)
+    if (ctx->prec == DEM_F32 && !ctx->generic_kernel) {
+        out[6] = (int64_t)(h[4] + h[5]);
+        out[7] = (int64_t)h[4];
+        out[8] = (int64_t)h[6];
+    } else {
+        const double f = ctx->npairs_total > 0 ? (double)h[0] / (double)ctx->npairs_total : 0.0;
+        double ee = 0, vfe = 0;
+        for (int c = 0; c < ctx->nclass; ++c) {
+            const HostShape &A = ctx->shapes[ctx->class_sa[c]], &B = ctx->shapes[ctx->class_sb[c]];
+            const double np = ctx->class_np[c];
+            if (ctx->dim == 3) {
+                ee += np * A.ne * B.ne;
+                vfe += np * ((double)B.nv * A.nfe + (double)A.nv * B.nfe);
+            } else {
+                ee += np * ((double)B.nv * A.ne + (double)A.nv * B.ne);
+            }
+        }
+        out[6] = out[1];
+        out[7] = (int64_t)(ee * f + 0.5);
+        out[8] = (int64_t)(vfe * f + 0.5);
+    }
     return DEM_OK;
 }
 

@@ -19,7 +19,7 @@ def scales(st, of, ot):
     return max(np.abs(of[:, :3]).max(), eps / sig), max(np.abs(ot[:, :3]).max(), eps), max(np.abs(of[:, 3]).max(), eps)
 
 
-def gpu_compute(st, precision, slices=0, r_cut=None, virial=True, kernel=None):
+def gpu_compute(st, precision, slices=0, r_cut=None, virial=True, kernel=None, cull=None):
     import paper_1607_02427_b200 as pkg
 
     dem, t = pkg.from_state(st, precision)
@@ -27,6 +27,8 @@ def gpu_compute(st, precision, slices=0, r_cut=None, virial=True, kernel=None):
         dem.set_slices(slices)
     if kernel is not None:
         dem.set_pair_kernel(kernel)
+    if cull is not None:
+        dem.set_culling(cull)
     dem.build_neighbors(t["pos"], t["shape_id"], st["box"], st["r_cut"] if r_cut is None else r_cut)
     f, tq, w = dem.compute(t["pos"], t["quat"], t["shape_id"], virial=virial)
     out = (f.cpu().numpy().astype(np.float64), tq.cpu().numpy().astype(np.float64),
@@ -35,10 +37,10 @@ def gpu_compute(st, precision, slices=0, r_cut=None, virial=True, kernel=None):
     return out
 
 
-def assert_parity(st, precision, oracle, slices=0, subset=None, r_cut=None, tol=None, kernel=None):
+def assert_parity(st, precision, oracle, slices=0, subset=None, r_cut=None, tol=None, kernel=None, cull=None):
     """Element-by-element comparison of force, torque, energy, virial and of the term counters."""
     st = round_state(st, precision)
-    f, tq, w, cnt = gpu_compute(st, precision, slices, r_cut, kernel=kernel)
+    f, tq, w, cnt = gpu_compute(st, precision, slices, r_cut, kernel=kernel, cull=cull)
     of, ot, ow, ocnt = oracle.compute(st, subset=subset)
     if subset is not None:
         f, tq, w = f[subset], tq[subset], w[subset]

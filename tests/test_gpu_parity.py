@@ -120,6 +120,20 @@ def test_list_with_skin_compacts_out_of_reach_pairs(pkg, oracle, kind, cells, ex
     assert_parity(st, "f64", oracle, r_cut=st["r_cut"] + extra)
 
 
+@pytest.mark.parametrize("kind,cells,slices", [("cubes", 6, 0), ("octahedra", 6, 0), ("mixed", 5, 0), ("mixed", 4, 5)])
+def test_search_kernel_with_and_without_culling(pkg, oracle, kind, cells, slices):
+    """Exact per-feature culling (default) must not change which terms contribute: same counters as the kernel that
+    sweeps every Eq. 1 term, same sums up to rounding; it must sweep fewer terms, and without it all of them."""
+    st = di.dense_state(kind, cells)
+    a = assert_parity(st, "f32", oracle, cull=False, slices=slices)
+    b = assert_parity(st, "f32", oracle, cull=True, slices=slices)
+    for key in ("active", "degenerate", "parallel", "pairs_evaluated", "terms"):
+        assert a["counters"][key] == b["counters"][key], key
+    assert a["counters"]["terms_swept"] == a["counters"]["terms"]
+    assert 0 < b["counters"]["terms_swept"] < a["counters"]["terms_swept"]
+    assert b["counters"]["terms_swept"] >= b["counters"]["active"]
+
+
 @pytest.mark.parametrize("n", [7, 9])
 def test_faces_with_many_edges(pkg, oracle, n):
     """Prisms over a heptagon / nonagon: faces whose boundary-edge count has no unrolled sweep (run-time edge loop),
