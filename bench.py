@@ -273,19 +273,20 @@ def main():
         clk = sampler.stop() if sampler else None
         nl = dem.launch_count() - l0
         npl, pms = dem.kernel_time()
+        tot = dem.swept_totals()
         dem.set_timing(False)
         tm = torch.tensor([ms], dtype=torch.float64, device="cuda")
         if world > 1:
             dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-        return float(tm.item()), clk, nl, npl, pms, dem.get_counters()
+        return float(tm.item()), clk, nl, npl, pms, dem.get_counters(), tot
 
-    def swept_flops(c):
-        """Algorithmic flop of the terms whose search was executed in the last evaluation (library counters)."""
+    def swept_flops(tot):
+        """Algorithmic flop of the terms whose search was executed, summed over the timed evaluations (library counters)."""
         if st["dim"] == 2:
-            return FLOP_VE_2D * c["ee_swept"]
-        return FLOP_EE * c["ee_swept"] + FLOP_VF_FACE * (c["terms_swept"] - c["ee_swept"]) + FLOP_VF_EDGE * c["face_edges_swept"]
+            return FLOP_VE_2D * tot["ee_swept"]
+        return FLOP_EE * tot["ee_swept"] + FLOP_VF_FACE * tot["vf_swept"] + FLOP_VF_EDGE * tot["face_edges_swept"]
 
-    elapsed_ms, clocks, gpu_launches, n_pair_launches, pair_ms, cnt = timed(args.warmup, args.steps, True)
+    elapsed_ms, clocks, gpu_launches, n_pair_launches, pair_ms, cnt, tot = timed(args.warmup, args.steps, True)
     value = n * world * args.steps / (elapsed_ms * 1e-3)
 
     # ---- roofline of the pair-feature kernel ---------------------------------------------------------------------
@@ -301,21 +302,25 @@ def main():
     peaks, peak_kind = measured_peaks()
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     peak_tf = sm_count * 128 * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
-    flops_swept = swept_flops(cnt)
+    searched = st["dim"] == 3 and args.pair_kernel != "generic" or args.pair_kernel == "search"
+    # per evaluation: summed over the timed evaluations by the search kernels themselves; the generic kernel sweeps
+    # every term of every listed pair in reach (nominal count)
+    flops_swept = swept_flops(tot) / evals if searched else flops
     achieved_tf = flops_swept / (kern_ms_per_eval * 1e-3) / 1e12
     fma_measured = dem.fp32_peak(1 << 15)
     # second arm: the same steps with the library's default, exact per-feature culling
     culled = None
     if search3d and not args.cull:
         dem.set_culling(True)
-        cms, _, _, cnpl, cpms, ccnt = timed(3, args.steps, False)
+        cms, _, _, cnpl, cpms, ccnt, ctot = timed(3, args.steps, False)
         dem.set_culling(False)
-        ckern = cpms / max(cnpl // max(n_classes, 1), 1)
-        ctf = swept_flops(ccnt) / (ckern * 1e-3) / 1e12
+        cev = max(cnpl // max(n_classes, 1), 1)
+        ckern = cpms / cev
+        ctf = swept_flops(ctot) / cev / (ckern * 1e-3) / 1e12
         culled = {"value": n * world * args.steps / (cms * 1e-3), "unit": "particle-timesteps/s",
                   "ms_per_step": cms / args.steps, "kernel": "k_pose + k_pair_cull", "kernel_ms": ckern,
                   "terms_swept_last_step": ccnt["terms_swept"], "terms_last_step": ccnt["terms"],
-                  "flops_per_launch": swept_flops(ccnt), "achieved": ctf, "frac": ctf / peak_tf,
+                  "flops_per_launch": swept_flops(ctot) / cev, "achieved": ctf, "frac": ctf / peak_tf,
                   "note": "same results; the kernel is no longer ALU-bound (cull tests, queues, pose traffic)"}
     # DRAM traffic of the dominant kernel per launch: from the committed `ncu --set full` summary of this workload
     traffic = None

@@ -192,6 +192,10 @@ int dem_set_l2_flush(dem_ctx* ctx, int64_t bytes);
  * summed duration in milliseconds (synchronises). */
 int dem_set_timing(dem_ctx* ctx, int enabled);
 int dem_kernel_time(dem_ctx* ctx, int64_t* launches, double* total_ms);
+/* While timing is enabled the packed search kernels' swept-term counters (dem_get_counters out[7], out[6] - out[7],
+ * out[8]) are also summed over all evaluations since dem_set_timing(ctx, 1): out[0] edge-edge terms (2D: vertex-edge
+ * terms), out[1] vertex-face terms, out[2] face boundary-edge tests.  HOST int64[3]; synchronises. */
+int dem_swept_totals(dem_ctx* ctx, int64_t out[3]);
 /* Number of kernels the library has launched on this context since creation (all kernels). */
 int64_t dem_launch_count(const dem_ctx* ctx);
 

@@ -21,7 +21,7 @@ STATUS_NAMES = {0: "DEM_OK", -1: "DEM_EINVAL", -2: "DEM_ENOMEM", -3: "DEM_ECUDA"
 # every symbol include/dem.h declares (tests check that the built library exports all of them)
 EXPORTS = ["dem_create", "dem_destroy", "dem_last_error", "dem_set_eps_par", "dem_create_shape", "dem_build_neighbors",
            "dem_get_neighbors", "dem_copy_neighbors", "dem_compute", "dem_get_counters", "dem_step", "dem_energy",
-           "dem_compute_host", "dem_step_host", "dem_set_slices", "dem_set_pair_kernel", "dem_set_culling", "dem_set_l2_flush", "dem_set_timing", "dem_kernel_time",
+           "dem_compute_host", "dem_step_host", "dem_set_slices", "dem_set_pair_kernel", "dem_set_culling", "dem_set_l2_flush", "dem_set_timing", "dem_kernel_time", "dem_swept_totals",
            "dem_launch_count", "dem_fp32_peak", "dem_version"]
 
 _lib = None
@@ -120,6 +120,11 @@ class Dem:
     def set_pair_kernel(self, which):
         """0 = packed search kernel, 1 = generic fused kernel, 2 = auto (default: search in 3D, generic in 2D)."""
         _check(self._ctx, lib().dem_set_pair_kernel(self._ctx, C.c_int(which)))
+
+    def swept_totals(self):
+        out = (C.c_int64 * 3)()
+        _check(self._ctx, lib().dem_swept_totals(self._ctx, out))
+        return dict(ee_swept=out[0], vf_swept=out[1], face_edges_swept=out[2])
 
     def set_culling(self, enabled):
         _check(self._ctx, lib().dem_set_culling(self._ctx, C.c_int(1 if enabled else 0)))

@@ -620,6 +620,11 @@ __global__ void k_d4_to_f4(int n, const d4* __restrict__ in, f4* __restrict__ ou
     out[i] = r;
 }
 
+// running totals of the swept-term counters (bench accounting: dem_set_timing / dem_swept_totals)
+__global__ void k_accum_counters(const unsigned long long* __restrict__ counters, unsigned long long* __restrict__ cum) {
+    if (threadIdx.x < 3) cum[threadIdx.x] += counters[4 + threadIdx.x];
+}
+
 // ---- FP32 FMA-chain microbenchmark (roofline denominator) --------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_fma_peak(int iters, float seed, float* __restrict__ out) {
     float a0 = seed + threadIdx.x, a1 = a0 + 1.f, a2 = a0 + 2.f, a3 = a0 + 3.f, a4 = a0 + 4.f, a5 = a0 + 5.f,

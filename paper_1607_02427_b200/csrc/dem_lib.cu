@@ -58,6 +58,7 @@ struct dem_ctx {
     double box[3] = {0, 0, 0}, r_cut = 0;
     GridDev grid;
     DevBuf cell_of, rank, cell_start, order, xs, counts, list, slot, scratch_scan, pcnt, pairs, rec, flags, counters;
+    DevBuf cum;         // running totals of the swept-term counters while timing is on
     DevBuf pose, pidx;  // FP32 search kernel: compacted pose records per class (k_pose)
     ClassTable ct;
     int nclass = 0;
@@ -490,6 +491,10 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
             N, ctx->counts.as<int>(), ctx->slot.as<int>(), ctx->stride, sid, ctx->ct, ctx->nclass, ctx->rec.as<real4>(),
             static_cast<real4*>(force), static_cast<real4*>(torque), static_cast<real*>(virial), skip, KickArgs());
     LAUNCHED(ctx);
+    if (ctx->timing && search && ctx->cum.p) {
+        k_accum_counters<<<1, 32, 0, st>>>(ctx->counters.as<unsigned long long>(), ctx->cum.as<unsigned long long>());
+        LAUNCHED(ctx);
+    }
     CU(cudaGetLastError());
     return DEM_OK;
 }
@@ -623,7 +628,7 @@ int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda
 int dem_destroy(dem_ctx* c) {
     if (!c) return DEM_EINVAL;
     DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
-                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->pose, &c->pidx, &c->st_pos, &c->st_quat,
+                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->pose, &c->pidx, &c->cum, &c->st_pos, &c->st_quat,
                       &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->pos_build, &c->epart, &c->h_pos,
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();
@@ -843,6 +848,21 @@ int dem_set_l2_flush(dem_ctx* ctx, int64_t bytes) {
 int dem_set_timing(dem_ctx* ctx, int enabled) {
     if (!ctx) return DEM_EINVAL;
     ctx->timing = enabled != 0;
+    if (ctx->timing) {
+        CU(ctx->cum.reserve(sizeof(unsigned long long) * 4));
+        CU(cudaMemsetAsync(ctx->cum.p, 0, sizeof(unsigned long long) * 4, ctx->stream));
+    }
+    return DEM_OK;
+}
+
+int dem_swept_totals(dem_ctx* ctx, int64_t out[3]) {
+    if (!ctx || !out) return DEM_EINVAL;
+    out[0] = out[1] = out[2] = 0;
+    if (!ctx->cum.p) return DEM_OK;
+    unsigned long long h[3];
+    CU(cudaMemcpyAsync(h, ctx->cum.p, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (int k = 0; k < 3; ++k) out[k] = (int64_t)h[k];
     return DEM_OK;
 }
 
