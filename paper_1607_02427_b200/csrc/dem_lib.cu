@@ -447,7 +447,14 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
                 }
 #endif
                 if (ctx->dim == 3 && ctx->cull) {
-                    kern = k_pair_cull<PosT, 4>;
+                    kern = k_pair_cull<PosT, 3>;  // measured on cfg4: 167 registers without spills beat 128 / 96 / 80 with
+#ifdef DEM_TUNE
+                    if (const char* v = getenv("DEM_CULL_MINB")) {
+                        if (atoi(v) == 4) kern = k_pair_cull<PosT, 4>;
+                        if (atoi(v) == 5) kern = k_pair_cull<PosT, 5>;
+                        if (atoi(v) == 6) kern = k_pair_cull<PosT, 6>;
+                    }
+#endif
                     smem += cull_smem_header() - fast_smem_header();
                     const double ra = HA.circumradius + rcs, rb = HB.circumradius + rcs;
                     a.cull_a2 = (real)(ra * ra);
