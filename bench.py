@@ -194,6 +194,23 @@ def run_reference(args, rank, world):
     print(json.dumps(line))
 
 
+def max_over_ranks(x, world, device):
+    """The slowest rank's figure (replicas only: the one collective of a multi-GPU run)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(n_particles, world, steps, elapsed_ms):
+    """Whole-job particle-timesteps/s of `world` replicas that each advanced n_particles by `steps` steps."""
+    return n_particles * world * steps / (elapsed_ms * 1e-3)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -275,10 +292,7 @@ def main():
         npl, pms = dem.kernel_time()
         tot = dem.swept_totals()
         dem.set_timing(False)
-        tm = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-        return float(tm.item()), clk, nl, npl, pms, dem.get_counters(), tot
+        return max_over_ranks(ms, world, "cuda"), clk, nl, npl, pms, dem.get_counters(), tot
 
     def swept_flops(tot):
         """Algorithmic flop of the terms whose search was executed, summed over the timed evaluations (library counters)."""
@@ -287,7 +301,7 @@ def main():
         return FLOP_EE * tot["ee_swept"] + FLOP_VF_FACE * tot["vf_swept"] + FLOP_VF_EDGE * tot["face_edges_swept"]
 
     elapsed_ms, clocks, gpu_launches, n_pair_launches, pair_ms, cnt, tot = timed(args.warmup, args.steps, True)
-    value = n * world * args.steps / (elapsed_ms * 1e-3)
+    value = aggregate_value(n, world, args.steps, elapsed_ms)
 
     # ---- roofline of the pair-feature kernel ---------------------------------------------------------------------
     counts, rows = dem.get_neighbors()
@@ -343,10 +357,7 @@ def main():
         dem.step_host(h["pos"], h["quat"], h["vel"], h["angmom"], hsid, st["box"], dt_step, 1, skin, hf, None)
     barrier()
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = n * world * args.e2e_steps / float(te.item())
+    e2e_value = aggregate_value(n, world, args.e2e_steps, max_over_ranks(e2e_s, world, "cuda") * 1e3)
     h2d = 4 * n * 16 + n * 4
     d2h = 5 * n * 16
 
