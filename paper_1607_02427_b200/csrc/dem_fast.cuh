@@ -67,7 +67,7 @@ __device__ __forceinline__ unsigned push_sign(unsigned mask, float v) { return _
 
 #define DEM_QCAP 96        // 31 left over + at most 64 appended per round
 #define DEM_Q_INVALID 0xffffffffu
-enum { PH_EE = 0, PH_VF_OWN = 1, PH_VF_OTHER = 2, PH_VE_OWN = 3, PH_VE_OTHER = 4 };
+enum { PH_EE = 0, PH_VF_OWN = 1, PH_VF_OTHER = 2, PH_VE_OWN = 3, PH_VE_OTHER = 4, PH_VF_BOTH = 5 /* sweeps only */ };
 
 // what the cooperative evaluation needs, kept in shared memory (the hot loops hold their own copies in registers)
 struct FastShared {
@@ -173,8 +173,8 @@ struct WarpCtx {
 // mask bit (n - 1 - i) <=> the packed evaluation of inner feature k0 + i flagged a candidate in either half: both
 // terms are queued (the scalar routine sorts them out).  The halves belong to (owner lane, outer feature) = (wa, oa)
 // and (wb, ob); ok_a / ok_b say whether the half holds a real feature (tiles and item lists are padded).
-__device__ __forceinline__ void push_one(WarpCtx& w, int phase, unsigned m, int n, int k0, int wa, int oa, bool ok_a,
-                                         int wb, int ob, bool ok_b) {
+__device__ __forceinline__ void push_one(WarpCtx& w, int phase_a, int phase_b, unsigned m, int n, int k0, int wa, int oa,
+                                         bool ok_a, int wb, int ob, bool ok_b) {
     const unsigned full = 0xffffffffu;
     const unsigned lt = (1u << w.lane) - 1u;
     while (__any_sync(full, m != 0u)) {
@@ -185,8 +185,8 @@ __device__ __forceinline__ void push_one(WarpCtx& w, int phase, unsigned m, int 
         const bool ha = have && ok_a, hb = have && ok_b;
         const unsigned ba = __ballot_sync(full, ha), bb = __ballot_sync(full, hb);
         const int na = __popc(ba);
-        if (ha) w.q[w.qn + __popc(ba & lt)] = q_entry(wa, phase, oa, k);
-        if (hb) w.q[w.qn + na + __popc(bb & lt)] = q_entry(wb, phase, ob, k);
+        if (ha) w.q[w.qn + __popc(ba & lt)] = q_entry(wa, phase_a, oa, k);
+        if (hb) w.q[w.qn + na + __popc(bb & lt)] = q_entry(wb, phase_b, ob, k);
         w.qn += na + __popc(bb);
         __syncwarp();
         while (w.qn >= 32) {
@@ -202,7 +202,7 @@ __device__ __forceinline__ void push_and_drain(WarpCtx& w, int phase, const unsi
                                                int o_end) {
 #pragma unroll
     for (int tau = 0; tau < T; ++tau)
-        push_one(w, phase, mask[tau], n, k0, w.lane, o0 + 2 * tau, o0 + 2 * tau < o_end, w.lane, o0 + 2 * tau + 1,
+        push_one(w, phase, phase, mask[tau], n, k0, w.lane, o0 + 2 * tau, o0 + 2 * tau < o_end, w.lane, o0 + 2 * tau + 1,
                  o0 + 2 * tau + 1 < o_end);
 }
 
@@ -825,28 +825,36 @@ __device__ __forceinline__ void sweep_items(WarpCtx& w, CullCtx& cc, const Shape
                 for (int k = k0; k < k1; ++k)
                     mask = push_sign(mask, ee_eval(A.E[2 * k], A.E[2 * k + 1], np2x, np2y, np2z, d2x, d2y, d2z, g, a0.w,
                                                    b0.w, nrc2));
-                if (__any_sync(full, mask != 0u)) push_one(w, PHASE, mask, k1 - k0, k0, wa, oa, ok_a, wb, ob, ok_b);
+                if (__any_sync(full, mask != 0u)) push_one(w, PHASE, PHASE, mask, k1 - k0, k0, wa, oa, ok_a, wb, ob, ok_b);
             }
             cc.swept_ee += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)A.ne;
         } else {
-            const ShapeView<float>& In = PHASE == PH_VF_OWN ? A : B;
-            const ShapeView<float>& Out = PHASE == PH_VF_OWN ? B : A;
-            const ShapeDev& sd = PHASE == PH_VF_OWN ? sda : sdb;
-            const f4 va = Out.V[oa], vb = Out.V[ob];
+            // vertex-face items.  PH_VF_BOTH (one-shape classes: the faces of i and of j are the same table): bit 15 of
+            // an item says which sum it belongs to, so both sums share one pass
+            const ShapeView<float>& In = PHASE == PH_VF_OTHER ? B : A;
+            const ShapeView<float>& Out = PHASE == PH_VF_OTHER ? A : B;
+            const ShapeDev& sd = PHASE == PH_VF_OTHER ? sdb : sda;
+            const bool oth_a = PHASE == PH_VF_OTHER || (PHASE == PH_VF_BOTH && (oa & 0x8000)),
+                       oth_b = PHASE == PH_VF_OTHER || (PHASE == PH_VF_BOTH && (ob & 0x8000));
+            const int va_i = oa & 0x7fff, vb_i = ob & 0x7fff;
+            const f4 va = Out.V[va_i], vb = Out.V[vb_i];
             float pa[3], pb[3];
-            if (PHASE == PH_VF_OWN) {
-                vertex_to_i<float>(va.x, va.y, va.z, Ra, ta, pa);
-                vertex_to_i<float>(vb.x, vb.y, vb.z, Rb, tb, pb);
-            } else {
+            if (oth_a)
                 vertex_to_j<float>(va.x, va.y, va.z, Ra, ta, pa);
+            else
+                vertex_to_i<float>(va.x, va.y, va.z, Ra, ta, pa);
+            if (oth_b)
                 vertex_to_j<float>(vb.x, vb.y, vb.z, Rb, tb, pb);
-            }
+            else
+                vertex_to_i<float>(vb.x, vb.y, vb.z, Rb, tb, pb);
             u64 px[1] = {pk(pa[0], pb[0])}, py[1] = {pk(pa[1], pb[1])}, pz[1] = {pk(pa[2], pb[2])};
             for (int f0 = 0; f0 < In.nf; f0 += 32) {
                 const int f1 = min(f0 + 32, In.nf);
                 unsigned mask[1] = {0u};
                 sweep_faces<1>(In, sd, f0, f1, px, py, pz, nrc2, mask);
-                if (__any_sync(full, mask[0] != 0u)) push_one(w, PHASE, mask[0], f1 - f0, f0, wa, oa, ok_a, wb, ob, ok_b);
+                if (__any_sync(full, mask[0] != 0u))
+                    push_one(w, oth_a ? PH_VF_OTHER : PH_VF_OWN, oth_b ? PH_VF_OTHER : PH_VF_OWN, mask[0], f1 - f0, f0, wa,
+                             va_i, ok_a, wb, vb_i, ok_b);
             }
             cc.swept_vf += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)In.nf;
             cc.swept_vfe += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)sd.nfe;
@@ -855,9 +863,11 @@ __device__ __forceinline__ void sweep_items(WarpCtx& w, CullCtx& cc, const Shape
     cc.iqn = 0;
 }
 
-// append the lanes' surviving outer features (bit k of mask <=> feature o0 + k survives) to the item list, lane by
-// lane (exclusive prefix of the lanes' counts: the order is fixed by the data)
-__device__ __forceinline__ void emit_items(const WarpCtx& w, CullCtx& cc, unsigned mask, int o0) {
+// Appending the lanes' surviving outer features (bit k of mask <=> feature o0 + k survives) to the item list, lane by
+// lane (exclusive prefix of the lanes' counts: the order is fixed by the data), takes two steps so that the caller can
+// sweep the list first when the new items would not fit: count_items returns the warp's total and the lane's offset,
+// write_items stores the lane's items.
+__device__ __forceinline__ int count_items(const WarpCtx& w, unsigned mask, int& offset) {
     const unsigned full = 0xffffffffu;
     const int cnt = __popc(mask);
     int incl = cnt;
@@ -866,14 +876,28 @@ __device__ __forceinline__ void emit_items(const WarpCtx& w, CullCtx& cc, unsign
         const int y = __shfl_up_sync(full, incl, dlt);
         if (w.lane >= dlt) incl += y;
     }
-    int pos = cc.iqn + incl - cnt;
+    offset = incl - cnt;
+    return __shfl_sync(full, incl, 31);
+}
+__device__ __forceinline__ void write_items(const WarpCtx& w, CullCtx& cc, unsigned mask, int o0, unsigned flag, int offset,
+                                            int total) {
+    int pos = cc.iqn + offset;
     while (mask) {
         const int b = __ffs(mask) - 1;
         mask &= mask - 1u;
-        cc.iq[pos++] = ((unsigned)w.lane << 16) | (unsigned)(o0 + b);
+        cc.iq[pos++] = ((unsigned)w.lane << 16) | flag | (unsigned)(o0 + b);
     }
-    cc.iqn += __shfl_sync(full, incl, 31);
+    cc.iqn += total;
 }
+// the list is swept when the next batch would overflow it and at the end of a phase: passes run as full as possible
+#define DEM_EMIT(PH, MASK, O0, FLAG)                                                      \
+    do {                                                                                  \
+        int off_;                                                                         \
+        const unsigned m_ = (MASK);                                                       \
+        const int tot_ = count_items(w, m_, off_);                                        \
+        if (cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH>(w, cc, A, B, a.sa, a.sb, nrc2);    \
+        write_items(w, cc, m_, (O0), (FLAG), off_, tot_);                                 \
+    } while (0)
 
 template <typename PosT, int MINB>
 __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a) {
@@ -973,31 +997,49 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
                 const float cx = qx + s * a1.x, cy = qy + s * a1.y, cz = qz + s * a1.z;
                 mask |= (cx * cx + cy * cy + cz * cz < a.cull_a2 ? 1u : 0u) << k;
             }
-            emit_items(w, cc, valid ? mask : 0u, l0);
-            sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
+            DEM_EMIT(PH_EE, valid ? mask : 0u, l0, 0u);
         }
-        // (2) vertices of j near i
-        for (int o0 = max(ob, oE) - oE, on = min(oe, oV) - oE; o0 < on; o0 += 32) {
-            const int n = min(32, on - o0);
-            unsigned mask = 0u;
-            for (int k = 0; k < n; ++k) {
-                const f4 v = B.V[o0 + k];
-                const float qx = v.x + tp[0], qy = v.y + tp[1], qz = v.z + tp[2];
-                mask |= (qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
+        sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
+        // (2) vertices of j near i: |R v + t| = |v + R^T t|;  (3) vertices of i near j: |R^T (v - t)| = |v - t|
+        const int o2 = max(ob, oE) - oE, n2 = min(oe, oV) - oE, o3 = max(ob, oV) - oV, n3 = min(oe, oV + A.nv) - oV;
+        if (same) {  // one shape: both sums sweep the same face table, so their survivors share the passes
+            for (int c0 = 0; c0 < A.nv; c0 += 32) {
+                unsigned m2 = 0u, m3 = 0u;
+                for (int k = 0; k < 32; ++k) {
+                    const int o = c0 + k;
+                    if (o >= A.nv) break;
+                    const f4 v = A.V[o];
+                    const float qx = v.x + tp[0], qy = v.y + tp[1], qz = v.z + tp[2];
+                    const float rx = v.x - t[0], ry = v.y - t[1], rz = v.z - t[2];
+                    m2 |= (o >= o2 && o < n2 && qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
+                    m3 |= (o >= o3 && o < n3 && rx * rx + ry * ry + rz * rz < a.cull_b2 ? 1u : 0u) << k;
+                }
+                DEM_EMIT(PH_VF_BOTH, valid ? m2 : 0u, c0, 0u);
+                DEM_EMIT(PH_VF_BOTH, valid ? m3 : 0u, c0, 0x8000u);
             }
-            emit_items(w, cc, valid ? mask : 0u, o0);
+            sweep_items<PH_VF_BOTH>(w, cc, A, B, a.sa, a.sb, nrc2);
+        } else {
+            for (int o0 = o2; o0 < n2; o0 += 32) {
+                const int n = min(32, n2 - o0);
+                unsigned mask = 0u;
+                for (int k = 0; k < n; ++k) {
+                    const f4 v = B.V[o0 + k];
+                    const float qx = v.x + tp[0], qy = v.y + tp[1], qz = v.z + tp[2];
+                    mask |= (qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
+                }
+                DEM_EMIT(PH_VF_OWN, valid ? mask : 0u, o0, 0u);
+            }
             sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
-        }
-        // (3) vertices of i near j: |R^T (v - t)| = |v - t|
-        for (int o0 = max(ob, oV) - oV, on = min(oe, oV + A.nv) - oV; o0 < on; o0 += 32) {
-            const int n = min(32, on - o0);
-            unsigned mask = 0u;
-            for (int k = 0; k < n; ++k) {
-                const f4 v = A.V[o0 + k];
-                const float qx = v.x - t[0], qy = v.y - t[1], qz = v.z - t[2];
-                mask |= (qx * qx + qy * qy + qz * qz < a.cull_b2 ? 1u : 0u) << k;
+            for (int o0 = o3; o0 < n3; o0 += 32) {
+                const int n = min(32, n3 - o0);
+                unsigned mask = 0u;
+                for (int k = 0; k < n; ++k) {
+                    const f4 v = A.V[o0 + k];
+                    const float qx = v.x - t[0], qy = v.y - t[1], qz = v.z - t[2];
+                    mask |= (qx * qx + qy * qy + qz * qz < a.cull_b2 ? 1u : 0u) << k;
+                }
+                DEM_EMIT(PH_VF_OTHER, valid ? mask : 0u, o0, 0u);
             }
-            emit_items(w, cc, valid ? mask : 0u, o0);
             sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
         }
         if (w.qn > 0) {
