@@ -759,6 +759,11 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
         if (s_ee) atomicAdd(a.counters + 4, s_ee);
         if (s_vf) atomicAdd(a.counters + 5, s_vf);
         if (s_vfe) atomicAdd(a.counters + 6, s_vfe);
+        if (a.cum) {
+            if (s_ee) atomicAdd(a.cum + 0, s_ee);
+            if (s_vf) atomicAdd(a.cum + 1, s_vf);
+            if (s_vfe) atomicAdd(a.cum + 2, s_vfe);
+        }
         if (w.scnt[0]) atomicAdd(a.counters + 1, (unsigned long long)w.scnt[0]);
         if (w.scnt[1]) atomicAdd(a.counters + 2, (unsigned long long)w.scnt[1]);
         if (w.scnt[2]) atomicAdd(a.counters + 3, (unsigned long long)w.scnt[2]);
@@ -1076,6 +1081,11 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
         if (s_ee) atomicAdd(a.counters + 4, (unsigned long long)s_ee);
         if (s_vf) atomicAdd(a.counters + 5, (unsigned long long)s_vf);
         if (s_vfe) atomicAdd(a.counters + 6, (unsigned long long)s_vfe);
+        if (a.cum) {
+            if (s_ee) atomicAdd(a.cum + 0, (unsigned long long)s_ee);
+            if (s_vf) atomicAdd(a.cum + 1, (unsigned long long)s_vf);
+            if (s_vfe) atomicAdd(a.cum + 2, (unsigned long long)s_vfe);
+        }
     }
 }
 

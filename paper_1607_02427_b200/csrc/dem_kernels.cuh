@@ -290,7 +290,8 @@ template <typename real> struct PairArgs {
     const int* pidx;      //   (written by k_pose)
     const int* count;
     size_t plane;         //   stride of the pose planes
-    unsigned long long* counters;  // [0] pairs evaluated, [1] active, [2] degenerate, [3] parallel
+    unsigned long long* counters;  // [0] pairs evaluated, [1] active, [2] degenerate, [3] parallel, [4..6] swept terms
+    unsigned long long* cum;       // running totals of [4..6] while bench's timing is on (else null)
 };
 
 template <typename real, typename PosT, int DIM>
@@ -541,33 +542,47 @@ __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict
                              const typename vec4<real>::type* __restrict__ force,
                              const typename vec4<real>::type* __restrict__ torque, const d4* __restrict__ pos_build,
                              double half_skin2, int* __restrict__ moved) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    // The translational and the rotational half of a particle's update are independent: the first half of the grid
+    // does x, v (and the skin test), the second q, L -- twice the memory-level parallelism, half the dependent chain.
+    const int half = gridDim.x >> 1;
+    const bool rot = (int)blockIdx.x >= half;
+    const int i = (blockIdx.x - (rot ? half : 0)) * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const int s = sid[i];
-    const double hm = 0.5 * dt / mt.mass[s];
-    d4 x = pos[i], v = vel[i], L = ang[i], q = quat[i];
-    const typename vec4<real>::type F = force[i], T = torque[i];
-    double xs[3] = {x.x, x.y, x.z}, vs[3] = {v.x, v.y, v.z}, Ls[3] = {L.x, L.y, L.z};
-    const double Fs[3] = {(double)F.x, (double)F.y, (double)F.z}, Ts[3] = {(double)T.x, (double)T.y, (double)T.z};
-    for (int a = 0; a < box.dim; ++a) {
-        vs[a] += hm * Fs[a];
-        xs[a] += dt * vs[a];
-        xs[a] -= box.L[a] * rint(xs[a] * box.invL[a]);
+    if (!rot) {
+        const double hm = 0.5 * dt / mt.mass[s];
+        d4 x = pos[i], v = vel[i];
+        const typename vec4<real>::type F = force[i];
+        const d4 xb = pos_build[i];
+        double xs[3] = {x.x, x.y, x.z}, vs[3] = {v.x, v.y, v.z};
+        const double Fs[3] = {(double)F.x, (double)F.y, (double)F.z};
+        for (int a = 0; a < box.dim; ++a) {
+            vs[a] += hm * Fs[a];
+            xs[a] += dt * vs[a];
+            xs[a] -= box.L[a] * rint(xs[a] * box.invL[a]);
+        }
+        x.x = xs[0]; x.y = xs[1]; x.z = xs[2];
+        v.x = vs[0]; v.y = vs[1]; v.z = vs[2];
+        pos[i] = x;
+        vel[i] = v;
+        double dx = xs[0] - xb.x, dy = xs[1] - xb.y, dz = box.dim == 3 ? xs[2] - xb.z : 0.0;
+        dx -= box.L[0] * rint(dx * box.invL[0]);
+        dy -= box.L[1] * rint(dy * box.invL[1]);
+        dz -= box.L[2] * rint(dz * box.invL[2]);
+        if (dx * dx + dy * dy + dz * dz > half_skin2) *moved = 1;
+    } else {
+        d4 L = ang[i], q = quat[i];
+        const typename vec4<real>::type T = torque[i];
+        double Ls[3] = {L.x, L.y, L.z};
+        const double Ts[3] = {(double)T.x, (double)T.y, (double)T.z};
+        for (int a = (box.dim == 2 ? 2 : 0); a < 3; ++a) Ls[a] += 0.5 * dt * Ts[a];
+        double qs[4] = {q.x, q.y, q.z, q.w};
+        free_rotate(box.dim, mt.inertia[s], Ls, dt, qs);
+        L.x = Ls[0]; L.y = Ls[1]; L.z = Ls[2];
+        q.x = qs[0]; q.y = qs[1]; q.z = qs[2]; q.w = qs[3];
+        ang[i] = L;
+        quat[i] = q;
     }
-    for (int a = (box.dim == 2 ? 2 : 0); a < 3; ++a) Ls[a] += 0.5 * dt * Ts[a];
-    double qs[4] = {q.x, q.y, q.z, q.w};
-    free_rotate(box.dim, mt.inertia[s], Ls, dt, qs);
-    x.x = xs[0]; x.y = xs[1]; x.z = xs[2];
-    v.x = vs[0]; v.y = vs[1]; v.z = vs[2];
-    L.x = Ls[0]; L.y = Ls[1]; L.z = Ls[2];
-    q.x = qs[0]; q.y = qs[1]; q.z = qs[2]; q.w = qs[3];
-    pos[i] = x; vel[i] = v; ang[i] = L; quat[i] = q;
-    const d4 xb = pos_build[i];
-    double dx = xs[0] - xb.x, dy = xs[1] - xb.y, dz = box.dim == 3 ? xs[2] - xb.z : 0.0;
-    dx -= box.L[0] * rint(dx * box.invL[0]);
-    dy -= box.L[1] * rint(dy * box.invL[1]);
-    dz -= box.L[2] * rint(dz * box.invL[2]);
-    if (dx * dx + dy * dy + dz * dz > half_skin2) *moved = 1;
 }
 
 // U, K_trans, K_rot: per-block partial sums in double (fixed order), summed on the host.
@@ -618,11 +633,6 @@ __global__ void k_d4_to_f4(int n, const d4* __restrict__ in, f4* __restrict__ ou
     f4 r;
     r.x = (float)v.x; r.y = (float)v.y; r.z = (float)v.z; r.w = (float)v.w;
     out[i] = r;
-}
-
-// running totals of the swept-term counters (bench accounting: dem_set_timing / dem_swept_totals)
-__global__ void k_accum_counters(const unsigned long long* __restrict__ counters, unsigned long long* __restrict__ cum) {
-    if (threadIdx.x < 3) cum[threadIdx.x] += counters[4 + threadIdx.x];
 }
 
 // ---- FP32 FMA-chain microbenchmark (roofline denominator) --------------------------------------------------------------

@@ -392,6 +392,7 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
         a.pc.eps_par = (real)ctx->eps_par;
         a.pc.degen2 = (real)((1e-6 * sigma) * (1e-6 * sigma));
         a.counters = ctx->counters.as<unsigned long long>();
+        a.cum = (ctx->timing && ctx->cum.p) ? ctx->cum.as<unsigned long long>() : nullptr;
         // candidate cutoff of the FP32 search kernel: FP32 rounding of the packed formulation (1e-3 relative) plus
         // its error on near-parallel edges, at most sin(angle) x edge length with the angle below ~1e-3 where the
         // line-line solve loses its digits; 4e-3 x longest edge leaves a factor 4
@@ -498,10 +499,6 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
             N, ctx->counts.as<int>(), ctx->slot.as<int>(), ctx->stride, sid, ctx->ct, ctx->nclass, ctx->rec.as<real4>(),
             static_cast<real4*>(force), static_cast<real4*>(torque), static_cast<real*>(virial), skip, KickArgs());
     LAUNCHED(ctx);
-    if (ctx->timing && search && ctx->cum.p) {
-        k_accum_counters<<<1, 32, 0, st>>>(ctx->counters.as<unsigned long long>(), ctx->cum.as<unsigned long long>());
-        LAUNCHED(ctx);
-    }
     CU(cudaGetLastError());
     return DEM_OK;
 }
@@ -558,7 +555,7 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     for (int s = 0; s < nsteps; ++s) {
         if (ctx->l2_flush_bytes) CU(cudaMemsetAsync(ctx->l2_scratch.p, s & 0xff, ctx->l2_flush_bytes, st));
         CU(cudaMemsetAsync(moved, 0, sizeof(int), st));
-        k_kick_drift<real><<<nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T, ctx->pos_build.as<d4>(),
+        k_kick_drift<real><<<2 * nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T, ctx->pos_build.as<d4>(),
                                                      half_skin2, moved);
         LAUNCHED(ctx);
         CU(cudaMemcpyAsync(ctx->h_moved, moved, sizeof(int), cudaMemcpyDeviceToHost, st));
