@@ -904,7 +904,7 @@ __device__ __forceinline__ void write_items(const WarpCtx& w, CullCtx& cc, unsig
         write_items(w, cc, m_, (O0), (FLAG), off_, tot_);                                 \
     } while (0)
 
-template <typename PosT, int MINB>
+template <typename PosT, int MINB, bool SAME>  // SAME: both particles of the class have the same shape
 __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     FastShared* fs = reinterpret_cast<FastShared*>(smem_raw);
@@ -915,7 +915,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     int* stage_pidx = reinterpret_cast<int*>(stage_pose + 4 * 2 * 6 * 32);  // 4 warps x [2][32]
     unsigned* items = reinterpret_cast<unsigned*>(stage_pidx + 4 * 2 * 32);  // 4 warps x DEM_IQCAP
     f4* sm = reinterpret_cast<f4*>(items + 4 * DEM_IQCAP);
-    const bool same = a.sa.off == a.sb.off;
+    const bool same = SAME;
     for (int k = threadIdx.x; k < a.sa.len; k += blockDim.x) sm[k] = a.table[a.sa.off + k];
     if (!same)
         for (int k = threadIdx.x; k < a.sb.len; k += blockDim.x) sm[a.sa.len + k] = a.table[a.sb.off + k];
@@ -1007,7 +1007,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
         sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
         // (2) vertices of j near i: |R v + t| = |v + R^T t|;  (3) vertices of i near j: |R^T (v - t)| = |v - t|
         const int o2 = max(ob, oE) - oE, n2 = min(oe, oV) - oE, o3 = max(ob, oV) - oV, n3 = min(oe, oV + A.nv) - oV;
-        if (same) {  // one shape: both sums sweep the same face table, so their survivors share the passes
+        if constexpr (SAME) {  // one shape: both sums sweep the same face table, so their survivors share the passes
             for (int c0 = 0; c0 < A.nv; c0 += 32) {
                 unsigned m2 = 0u, m3 = 0u;
                 for (int k = 0; k < 32; ++k) {

@@ -448,12 +448,11 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
                 }
 #endif
                 if (ctx->dim == 3 && ctx->cull) {
-                    kern = k_pair_cull<PosT, 3>;  // measured on cfg4: 167 registers without spills beat 128 / 96 / 80 with
+                    // measured on cfg4: 167 registers without spills beat 128 / 96 / 80 with
+                    kern = a.sa.off == a.sb.off ? k_pair_cull<PosT, 3, true> : k_pair_cull<PosT, 3, false>;
 #ifdef DEM_TUNE
                     if (const char* v = getenv("DEM_CULL_MINB")) {
-                        if (atoi(v) == 4) kern = k_pair_cull<PosT, 4>;
-                        if (atoi(v) == 5) kern = k_pair_cull<PosT, 5>;
-                        if (atoi(v) == 6) kern = k_pair_cull<PosT, 6>;
+                        if (atoi(v) == 4) kern = k_pair_cull<PosT, 4, false>;
                     }
 #endif
                     smem += cull_smem_header() - fast_smem_header();
