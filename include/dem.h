@@ -192,6 +192,10 @@ int dem_set_l2_flush(dem_ctx* ctx, int64_t bytes);
  * summed duration in milliseconds (synchronises). */
 int dem_set_timing(dem_ctx* ctx, int enabled);
 int dem_kernel_time(dem_ctx* ctx, int64_t* launches, double* total_ms);
+/* The same, split: *pair_ms = the pair-feature kernels alone (k_pair_fast / k_pair_cull / k_pair), *pose_ms = the pose
+ * kernel in front of them (k_pose; 0 for the generic kernel, which forms the pose itself).  dem_kernel_time returns
+ * their sum.  Either call resets the bracket list. */
+int dem_kernel_time_split(dem_ctx* ctx, int64_t* launches, double* pair_ms, double* pose_ms);
 /* While timing is enabled the packed search kernels' swept-term counters (dem_get_counters out[7], out[6] - out[7],
  * out[8]) are also summed over all evaluations since dem_set_timing(ctx, 1): out[0] edge-edge terms (2D: vertex-edge
  * terms), out[1] vertex-face terms, out[2] face boundary-edge tests.  HOST int64[3]; synchronises. */

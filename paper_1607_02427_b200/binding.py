@@ -21,7 +21,7 @@ STATUS_NAMES = {0: "DEM_OK", -1: "DEM_EINVAL", -2: "DEM_ENOMEM", -3: "DEM_ECUDA"
 # every symbol include/dem.h declares (tests check that the built library exports all of them)
 EXPORTS = ["dem_create", "dem_destroy", "dem_last_error", "dem_set_eps_par", "dem_create_shape", "dem_build_neighbors",
            "dem_get_neighbors", "dem_copy_neighbors", "dem_compute", "dem_get_counters", "dem_step", "dem_energy",
-           "dem_compute_host", "dem_step_host", "dem_set_slices", "dem_set_pair_kernel", "dem_set_culling", "dem_set_l2_flush", "dem_set_timing", "dem_kernel_time", "dem_swept_totals",
+           "dem_compute_host", "dem_step_host", "dem_set_slices", "dem_set_pair_kernel", "dem_set_culling", "dem_set_l2_flush", "dem_set_timing", "dem_kernel_time", "dem_kernel_time_split", "dem_swept_totals",
            "dem_launch_count", "dem_fp32_peak", "dem_version"]
 
 _lib = None
@@ -255,6 +255,11 @@ class Dem:
         n, ms = C.c_int64(), C.c_double()
         _check(self._ctx, lib().dem_kernel_time(self._ctx, C.byref(n), C.byref(ms)))
         return n.value, ms.value
+
+    def kernel_time_split(self):
+        n, pair, pose = C.c_int64(), C.c_double(), C.c_double()
+        _check(self._ctx, lib().dem_kernel_time_split(self._ctx, C.byref(n), C.byref(pair), C.byref(pose)))
+        return n.value, pair.value, pose.value
 
     def launch_count(self):
         return int(lib().dem_launch_count(self._ctx))

@@ -76,7 +76,8 @@ struct dem_ctx {
     // accounting
     int64_t launches = 0;
     bool timing = false;
-    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pool;
+    struct EvTriple { cudaEvent_t first, mid, second; };  // before k_pose, between k_pose and the pair kernel, after
+    std::vector<EvTriple> ev_pool;
     size_t ev_used = 0;
     int64_t last_terms = 0;
     int sm_count = 148;
@@ -465,15 +466,17 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
             }
         }
         if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        cudaEvent_t e0 = nullptr, em = nullptr, e1 = nullptr;
         if (ctx->timing) {
             if (ctx->ev_used == ctx->ev_pool.size()) {
-                cudaEvent_t x, y;
+                cudaEvent_t x, y, z;
                 CU(cudaEventCreate(&x));
                 CU(cudaEventCreate(&y));
-                ctx->ev_pool.push_back({x, y});
+                CU(cudaEventCreate(&z));
+                ctx->ev_pool.push_back({x, y, z});
             }
             e0 = ctx->ev_pool[ctx->ev_used].first;
+            em = ctx->ev_pool[ctx->ev_used].mid;
             e1 = ctx->ev_pool[ctx->ev_used].second;
             ctx->ev_used++;
             CU(cudaEventRecord(e0, st));
@@ -485,6 +488,7 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
                 k_pose<PosT, 2><<<nblk(np, DEM_POSE_THREADS), DEM_POSE_THREADS, 0, st>>>(pa);
             LAUNCHED(ctx);
         }
+        if (ctx->timing) CU(cudaEventRecord(em, st));
         kern<<<grid, threads, smem, st>>>(a);
         LAUNCHED(ctx);
         if (ctx->timing) CU(cudaEventRecord(e1, st));
@@ -638,6 +642,7 @@ int dem_destroy(dem_ctx* c) {
     if (c->h_moved) cudaFreeHost(c->h_moved);
     if (c->ev_flag) cudaEventDestroy(c->ev_flag);
     for (auto& e : c->ev_pool) {
+        cudaEventDestroy(e.mid);
         cudaEventDestroy(e.first);
         cudaEventDestroy(e.second);
     }
@@ -869,18 +874,29 @@ int dem_swept_totals(dem_ctx* ctx, int64_t out[3]) {
     return DEM_OK;
 }
 
-int dem_kernel_time(dem_ctx* ctx, int64_t* launches, double* total_ms) {
-    if (!ctx || !launches || !total_ms) return DEM_EINVAL;
+int dem_kernel_time_split(dem_ctx* ctx, int64_t* launches, double* pair_ms, double* pose_ms) {
+    if (!ctx || !launches || !pair_ms || !pose_ms) return DEM_EINVAL;
     CU(cudaStreamSynchronize(ctx->stream));
-    double tot = 0;
+    double tp = 0, tq = 0;
     for (size_t k = 0; k < ctx->ev_used; ++k) {
-        float ms = 0;
-        CU(cudaEventElapsedTime(&ms, ctx->ev_pool[k].first, ctx->ev_pool[k].second));
-        tot += ms;
+        float a = 0, b = 0;
+        CU(cudaEventElapsedTime(&a, ctx->ev_pool[k].first, ctx->ev_pool[k].mid));
+        CU(cudaEventElapsedTime(&b, ctx->ev_pool[k].mid, ctx->ev_pool[k].second));
+        tq += a;
+        tp += b;
     }
     *launches = (int64_t)ctx->ev_used;
-    *total_ms = tot;
+    *pair_ms = tp;
+    *pose_ms = tq;
     ctx->ev_used = 0;
+    return DEM_OK;
+}
+
+int dem_kernel_time(dem_ctx* ctx, int64_t* launches, double* total_ms) {
+    if (!total_ms) return DEM_EINVAL;
+    double pose = 0;
+    CHECK(dem_kernel_time_split(ctx, launches, total_ms, &pose));
+    *total_ms += pose;
     return DEM_OK;
 }
 
