@@ -75,8 +75,9 @@ struct FastShared {
     PairConst<float> pc;
 };
 
-__device__ __forceinline__ unsigned q_entry(int lane, int phase, int outer, int inner) {
-    return ((unsigned)lane << 27) | ((unsigned)phase << 24) | ((unsigned)outer << 12) | (unsigned)inner;
+// candidate entry: owner slot (6 bits: up to 64 pairs per warp tile) | phase (3) | outer feature (11) | inner feature (12)
+__device__ __forceinline__ unsigned q_entry(int owner, int phase, int outer, int inner) {
+    return ((unsigned)owner << 26) | ((unsigned)phase << 23) | ((unsigned)outer << 12) | (unsigned)inner;
 }
 
 // ---- evaluate: up to 32 queued candidates, one per lane -----------------------------------------------------------------
@@ -86,7 +87,7 @@ __device__ __forceinline__ unsigned q_entry(int lane, int phase, int outer, int 
 // evaluating lane reads its owner's pose from there.
 // Contributions are added to the owner in queue order, so the result does not depend on scheduling.
 __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* q, float* sacc, unsigned* scnt, int cnt, int qn,
-                                         const f4* sp) {
+                                         const f4* sp, int nown) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const unsigned e = lane < cnt ? q[lane] : DEM_Q_INVALID;
@@ -96,10 +97,10 @@ __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* q, floa
     if (lane < rem) q[lane] = v0;
     if (lane + 32 < rem) q[32 + lane] = v1;
     __syncwarp();
-    const int owner = e == DEM_Q_INVALID ? lane : (int)(e >> 27);
+    const int owner = e == DEM_Q_INVALID ? lane : (int)(e >> 26);
     float R[9], t[3];
     {
-        const f4 p0 = sp[owner], p1 = sp[32 + owner], p2 = sp[64 + owner];
+        const f4 p0 = sp[owner], p1 = sp[nown + owner], p2 = sp[2 * nown + owner];
         R[0] = p0.x; R[1] = p0.y; R[2] = p0.z; R[3] = p0.w; R[4] = p1.x; R[5] = p1.y; R[6] = p1.z; R[7] = p1.w;
         R[8] = p2.x; t[0] = p2.y; t[1] = p2.z; t[2] = p2.w;
     }
@@ -107,7 +108,7 @@ __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* q, floa
     loc.F[0] = loc.F[1] = loc.F[2] = loc.T[0] = loc.T[1] = loc.T[2] = loc.u = 0.f;
     loc.nactive = loc.ndegen = loc.npar = 0u;
     if (e != DEM_Q_INVALID) {
-        const int phase = (int)((e >> 24) & 7u), o = (int)((e >> 12) & 0xfffu), k = (int)(e & 0xfffu);
+        const int phase = (int)((e >> 23) & 7u), o = (int)((e >> 12) & 0x7ffu), k = (int)(e & 0xfffu);
         const ShapeView<float> A = fs->A, B = fs->B;
         const PairConst<float> pc = fs->pc;
         float p[3];
@@ -149,10 +150,10 @@ __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* q, floa
                     fz = __shfl_sync(full, loc.F[2], s), tx = __shfl_sync(full, loc.T[0], s),
                     ty = __shfl_sync(full, loc.T[1], s), tz = __shfl_sync(full, loc.T[2], s),
                     uu = __shfl_sync(full, loc.u, s);
-        if (lane == ow) {
-            sacc[0 * 32 + lane] += fx; sacc[1 * 32 + lane] += fy; sacc[2 * 32 + lane] += fz;
-            sacc[3 * 32 + lane] += tx; sacc[4 * 32 + lane] += ty; sacc[5 * 32 + lane] += tz;
-            sacc[6 * 32 + lane] += uu;
+        if (lane == (ow & 31)) {  // owner slots ow and ow + 32 (64-pair tiles) belong to the same lane
+            sacc[0 * nown + ow] += fx; sacc[1 * nown + ow] += fy; sacc[2 * nown + ow] += fz;
+            sacc[3 * nown + ow] += tx; sacc[4 * nown + ow] += ty; sacc[5 * nown + ow] += tz;
+            sacc[6 * nown + ow] += uu;
         }
     }
     __syncwarp();
@@ -166,7 +167,8 @@ struct WarpCtx {
     unsigned* scnt;
     int qn;    // queued candidates (warp-uniform)
     int lane;
-    const f4* sp;  // staged pose records of the current tile, [6][32]
+    const f4* sp;  // staged pose records of the current tile, [6][nown]
+    int nown;      // pairs per warp tile: 32 (k_pair_fast) or 64 (k_pair_cull)
 };
 
 // ---- queue: append the candidates flagged in mask[] and evaluate while a full warp of them is waiting ------------------
@@ -190,7 +192,7 @@ __device__ __forceinline__ void push_one(WarpCtx& w, int phase_a, int phase_b, u
         w.qn += na + __popc(bb);
         __syncwarp();
         while (w.qn >= 32) {
-            drain_terms(w.fs, w.q, w.sacc, w.scnt, 32, w.qn, w.sp);
+            drain_terms(w.fs, w.q, w.sacc, w.scnt, 32, w.qn, w.sp, w.nown);
             w.qn -= 32;
         }
     }
@@ -433,7 +435,7 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THR
     int tot = 0;
 #pragma unroll
     for (int k = 0; k < DEM_POSE_THREADS / 32; ++k) tot += wcount[k];
-    const int tot_pad = (tot + 31) & ~31;
+    const int tot_pad = (tot + 63) & ~63;
     if (threadIdx.x == 0) {
         s_prefix = tot_pad ? atomicAdd(a.count, tot_pad) : 0;
         if (tot) atomicAdd(a.counters, (unsigned long long)tot);
@@ -519,6 +521,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
     w.scnt = scnt_all + warp * 4;
     w.qn = 0;
     w.lane = lane;
+    w.nown = 32;
     const float nrc2 = -a.rc2_search;
     const int count = *a.count;                // pairs inside the reach, compacted by k_pose
     const int np_pad = (count + 31) & ~31;     // slices are warp-uniform
@@ -556,6 +559,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
         __syncwarp();  // the cooperative evaluation reads other lanes' staged poses
         w.sp = spose + buf * 6 * 32;
         const bool valid = in_list && spidx[buf * 32 + lane] >= 0;  // the work list is padded to whole warps per k_pose block
+        if (!__any_sync(full, valid)) continue;                    // a tile of padding only
         float R[9], t[3];
         if (valid) {
             const f4 p0 = spose[(buf * 6 + 0) * 32 + lane], p1 = spose[(buf * 6 + 1) * 32 + lane],
@@ -727,7 +731,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
                 }
             }
             if (w.qn > 0) {
-                drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp);
+                drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp, w.nown);
                 w.qn = 0;
             }
             float F[3], T[3];
@@ -793,8 +797,8 @@ struct CullCtx {
     unsigned swept_ee, swept_vf, swept_vfe;  // this lane's swept edge-edge terms, vertex-face terms, face-edge tests
 };
 
-__device__ __forceinline__ void load_pose(const f4* sp, int owner, float* R, float* t) {
-    const f4 p0 = sp[owner], p1 = sp[32 + owner], p2 = sp[64 + owner];
+__device__ __forceinline__ void load_pose(const f4* sp, int nown, int owner, float* R, float* t) {
+    const f4 p0 = sp[owner], p1 = sp[nown + owner], p2 = sp[2 * nown + owner];
     R[0] = p0.x; R[1] = p0.y; R[2] = p0.z; R[3] = p0.w; R[4] = p1.x; R[5] = p1.y; R[6] = p1.z; R[7] = p1.w;
     R[8] = p2.x; t[0] = p2.y; t[1] = p2.z; t[2] = p2.w;
 }
@@ -811,8 +815,8 @@ __device__ __forceinline__ void sweep_items(WarpCtx& w, CullCtx& cc, const Shape
         const unsigned ea = ok_a ? cc.iq[ia] : 0u, eb = ok_b ? cc.iq[ib] : ea;
         const int wa = (int)(ea >> 16), oa = (int)(ea & 0xffffu), wb = (int)(eb >> 16), ob = (int)(eb & 0xffffu);
         float Ra[9], ta[3], Rb[9], tb[3];
-        load_pose(w.sp, wa, Ra, ta);
-        load_pose(w.sp, wb, Rb, tb);
+        load_pose(w.sp, w.nown, wa, Ra, ta);
+        load_pose(w.sp, w.nown, wb, Rb, tb);
         if (!ok_a) ta[0] = tb[0] = 1.0e4f;  // idle lane: a far-away dummy keeps the warp converged
         if (PHASE == PH_EE) {
             const f4 a0 = B.OE[2 * oa], a1 = B.OE[2 * oa + 1], b0 = B.OE[2 * ob], b1 = B.OE[2 * ob + 1];
@@ -941,6 +945,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     w.scnt = scnt_all + warp * 4;
     w.qn = 0;
     w.lane = lane;
+    w.nown = 32;
     CullCtx cc;
     cc.iq = items + warp * DEM_IQCAP;
     cc.iqn = 0;
@@ -980,7 +985,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
         const bool valid = in_list && spidx[buf * 32 + lane] >= 0;  // the work list is padded to whole warps per k_pose block
         float R[9], t[3], tp[3] = {1.0e4f, 1.0e4f, 1.0e4f};
         if (valid) {
-            load_pose(w.sp, lane, R, t);
+            load_pose(w.sp, w.nown, lane, R, t);
 #pragma unroll
             for (int k = 0; k < 3; ++k) tp[k] = R[k] * t[0] + R[3 + k] * t[1] + R[6 + k] * t[2];  // R^T t
         } else {
@@ -1048,7 +1053,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
             sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
         }
         if (w.qn > 0) {
-            drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp);
+            drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp, w.nown);
             w.qn = 0;
         }
         if (valid) {

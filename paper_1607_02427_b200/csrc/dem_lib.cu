@@ -355,7 +355,7 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
     CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES, st));
     int* ccount = reinterpret_cast<int*>(ctx->counters.as<unsigned long long>() + 8);
     // capacity of a class's work list: its pairs plus the padding of every k_pose block to a whole warp
-    auto list_cap = [&](int c) { return (size_t)ctx->class_np[c] + 32u * (size_t)nblk(ctx->class_np[c], DEM_POSE_THREADS); };
+    auto list_cap = [&](int c) { return (size_t)ctx->class_np[c] + 64u * (size_t)nblk(ctx->class_np[c], DEM_POSE_THREADS); };
     size_t list_base[DEM_MAX_CLASSES + 1];
     list_base[0] = 0;
     for (int c = 0; c < ctx->nclass; ++c) list_base[c + 1] = list_base[c] + list_cap(c);
