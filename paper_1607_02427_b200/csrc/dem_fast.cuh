@@ -399,7 +399,8 @@ struct PoseArgs {
     f4* pose;
     int* pidx;
     int* count;  // entries of this class's work list, padding included (zeroed before the launch)
-    size_t plane;  // stride of the pose planes = capacity of the work list (pairs + 32 per k_pose block)
+    size_t plane;  // stride of the pose planes = capacity of the work list (pairs + 64 per k_pose block)
+    int pad;       // entries per warp tile of the kernel that follows: 32 (k_pair_fast) or 64 (k_pair_cull)
     unsigned long long* counters;  // [0] += pairs inside the reach
     f4* rec;
 };
@@ -435,7 +436,7 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THR
     int tot = 0;
 #pragma unroll
     for (int k = 0; k < DEM_POSE_THREADS / 32; ++k) tot += wcount[k];
-    const int tot_pad = (tot + 63) & ~63;
+    const int tot_pad = (tot + a.pad - 1) & ~(a.pad - 1);
     if (threadIdx.x == 0) {
         s_prefix = tot_pad ? atomicAdd(a.count, tot_pad) : 0;
         if (tot) atomicAdd(a.counters, (unsigned long long)tot);
@@ -888,36 +889,37 @@ __device__ __forceinline__ int count_items(const WarpCtx& w, unsigned mask, int&
     offset = incl - cnt;
     return __shfl_sync(full, incl, 31);
 }
-__device__ __forceinline__ void write_items(const WarpCtx& w, CullCtx& cc, unsigned mask, int o0, unsigned flag, int offset,
+__device__ __forceinline__ void write_items(CullCtx& cc, unsigned mask, int owner, int o0, unsigned flag, int offset,
                                             int total) {
     int pos = cc.iqn + offset;
     while (mask) {
         const int b = __ffs(mask) - 1;
         mask &= mask - 1u;
-        cc.iq[pos++] = ((unsigned)w.lane << 16) | flag | (unsigned)(o0 + b);
+        cc.iq[pos++] = ((unsigned)owner << 16) | flag | (unsigned)(o0 + b);
     }
     cc.iqn += total;
 }
 // the list is swept when the next batch would overflow it and at the end of a phase: passes run as full as possible
-#define DEM_EMIT(PH, MASK, O0, FLAG)                                                      \
+#define DEM_EMIT(PH, MASK, OWNER, O0, FLAG)                                               \
     do {                                                                                  \
         int off_;                                                                         \
         const unsigned m_ = (MASK);                                                       \
         const int tot_ = count_items(w, m_, off_);                                        \
         if (cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH>(w, cc, A, B, a.sa, a.sb, nrc2);    \
-        write_items(w, cc, m_, (O0), (FLAG), off_, tot_);                                 \
+        write_items(cc, m_, (OWNER), (O0), (FLAG), off_, tot_);                           \
     } while (0)
 
 template <typename PosT, int MINB, bool SAME>  // SAME: both particles of the class have the same shape
 __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a) {
+    // a warp tile is 64 pairs (two per lane: owner slots lane and lane + 32), so that the item passes run fuller
     extern __shared__ __align__(16) unsigned char smem_raw[];
     FastShared* fs = reinterpret_cast<FastShared*>(smem_raw);
-    unsigned* queue = reinterpret_cast<unsigned*>(smem_raw + 256);  // 4 warps x DEM_QCAP
-    float* sacc_all = reinterpret_cast<float*>(queue + 4 * DEM_QCAP);  // 4 warps x 7 x 32
-    unsigned* scnt_all = reinterpret_cast<unsigned*>(sacc_all + 4 * 7 * 32);  // 4 warps x 4
-    f4* stage_pose = reinterpret_cast<f4*>(scnt_all + 16);                 // 4 warps x [2][6][32] float4
-    int* stage_pidx = reinterpret_cast<int*>(stage_pose + 4 * 2 * 6 * 32);  // 4 warps x [2][32]
-    unsigned* items = reinterpret_cast<unsigned*>(stage_pidx + 4 * 2 * 32);  // 4 warps x DEM_IQCAP
+    unsigned* queue = reinterpret_cast<unsigned*>(smem_raw + 256);        // 4 warps x DEM_QCAP
+    float* sacc_all = reinterpret_cast<float*>(queue + 4 * DEM_QCAP);      // 4 warps x 7 x 64
+    unsigned* scnt_all = reinterpret_cast<unsigned*>(sacc_all + 4 * 7 * 64);  // 4 warps x 4
+    f4* stage_pose = reinterpret_cast<f4*>(scnt_all + 16);                 // 4 warps x [6][64] float4
+    int* stage_pidx = reinterpret_cast<int*>(stage_pose + 4 * 6 * 64);      // 4 warps x [64]
+    unsigned* items = reinterpret_cast<unsigned*>(stage_pidx + 4 * 64);     // 4 warps x DEM_IQCAP
     f4* sm = reinterpret_cast<f4*>(items + 4 * DEM_IQCAP);
     const bool same = SAME;
     for (int k = threadIdx.x; k < a.sa.len; k += blockDim.x) sm[k] = a.table[a.sa.off + k];
@@ -937,118 +939,126 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     if (threadIdx.x < 16) scnt_all[threadIdx.x] = 0u;
     __syncthreads();
 
+    const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpCtx w;
     w.fs = fs;
     w.q = queue + warp * DEM_QCAP;
-    w.sacc = sacc_all + warp * 7 * 32;
+    w.sacc = sacc_all + warp * 7 * 64;
     w.scnt = scnt_all + warp * 4;
     w.qn = 0;
     w.lane = lane;
-    w.nown = 32;
+    w.nown = 64;
     CullCtx cc;
     cc.iq = items + warp * DEM_IQCAP;
     cc.iqn = 0;
     cc.swept_ee = cc.swept_vf = cc.swept_vfe = 0u;
     const float nrc2 = -a.rc2_search;
-    const int count = *a.count;
-    const int np_pad = (count + 31) & ~31;
-    const long long n_wtiles = (long long)(np_pad >> 5) * a.slices;
+    const int count = *a.count;  // a multiple of 64 (k_pose pads its block slices)
+    const long long n_wtiles = (long long)(count >> 6) * a.slices;
     const size_t plane = a.plane;
-    const long long wt_stride = (long long)gridDim.x * 4;
-    f4* spose = stage_pose + warp * (2 * 6 * 32);
-    int* spidx = stage_pidx + warp * (2 * 32);
-    auto stage = [&](int buf, long long wt_) {
-        if (wt_ < n_wtiles) {
-            const int c_ = (int)((wt_ * 32 + lane) % np_pad);
-            if (c_ < count) {
+    f4* spose = stage_pose + warp * (6 * 64);
+    int* spidx = stage_pidx + warp * 64;
+    w.sp = spose;
+    for (long long wt = (long long)blockIdx.x * 4 + warp; wt < n_wtiles; wt += (long long)gridDim.x * 4) {
+        const int slice = (int)(wt / (count >> 6)), cbase = (int)(wt - (long long)slice * (count >> 6)) * 64;
+        __syncwarp();  // the previous tile's readers of the staged poses are done
 #pragma unroll
-                for (int k = 0; k < 6; ++k)
-                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
-                                     spose + (buf * 6 + k) * 32 + lane)), "l"(a.pose + k * plane + c_));
-                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(
-                                 spidx + buf * 32 + lane)), "l"(a.pidx + c_));
-            }
+        for (int h = 0; h < 2; ++h) {
+            const int own = lane + 32 * h, c_ = cbase + own;
+#pragma unroll
+            for (int k = 0; k < 6; ++k)
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
+                                 spose + k * 64 + own)), "l"(a.pose + k * plane + c_));
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(spidx + own)),
+                         "l"(a.pidx + c_));
         }
         asm volatile("cp.async.commit_group;");
-    };
-    int buf = 0;
-    stage(0, (long long)blockIdx.x * 4 + warp);
-    for (long long wt = (long long)blockIdx.x * 4 + warp; wt < n_wtiles; wt += wt_stride, buf ^= 1) {
-        const long long item = wt * 32 + lane;
-        const int slice = (int)(item / np_pad), c = (int)(item - (long long)slice * np_pad);
-        const bool in_list = c < count;
-        stage(buf ^ 1, wt + wt_stride);
-        asm volatile("cp.async.wait_group 1;" ::: "memory");
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncwarp();
-        w.sp = spose + buf * 6 * 32;
-        const bool valid = in_list && spidx[buf * 32 + lane] >= 0;  // the work list is padded to whole warps per k_pose block
-        float R[9], t[3], tp[3] = {1.0e4f, 1.0e4f, 1.0e4f};
-        if (valid) {
-            load_pose(w.sp, w.nown, lane, R, t);
+        bool valid[2];
+        valid[0] = spidx[lane] >= 0;  // the work list is padded to whole tiles per k_pose block (pidx = -1)
+        valid[1] = spidx[lane + 32] >= 0;
+        if (!__any_sync(full, valid[0] || valid[1])) continue;
 #pragma unroll
-            for (int k = 0; k < 3; ++k) tp[k] = R[k] * t[0] + R[3 + k] * t[1] + R[6 + k] * t[2];  // R^T t
-        } else {
-            t[0] = t[1] = t[2] = 1.0e4f;
-        }
-#pragma unroll
-        for (int k = 0; k < 7; ++k) w.sacc[k * 32 + lane] = 0.f;
+        for (int k = 0; k < 7; ++k) w.sacc[k * 64 + lane] = w.sacc[k * 64 + lane + 32] = 0.f;
         const int ob = (int)((long long)slice * a.n_outer / a.slices);
         const int oe = (int)((long long)(slice + 1) * a.n_outer / a.slices);
         const int oE = B.ne, oV = B.ne + B.nv;
-        // (1) edges of j whose distance from i's centre is below R_i + rc_search: in j's frame the centre of i is -R^T t
+        // this lane's two poses: t and R^T t (in j's frame the centre of i is -R^T t)
+        float tq[2][3], tp[2][3];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            float R[9];
+            load_pose(w.sp, 64, lane + 32 * h, R, tq[h]);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) tp[h][k] = R[k] * tq[h][0] + R[3 + k] * tq[h][1] + R[6 + k] * tq[h][2];
+        }
+        // (1) edges of j whose distance from i's centre is below R_i + rc_search
         for (int l0 = ob, le = min(oe, oE); l0 < le; l0 += 32) {
             const int n = min(32, le - l0);
-            unsigned mask = 0u;
-            for (int k = 0; k < n; ++k) {
-                const f4 a0 = B.OE[2 * (l0 + k)], a1 = B.OE[2 * (l0 + k) + 1];
-                const float qx = a0.x + tp[0], qy = a0.y + tp[1], qz = a0.z + tp[2];
-                const float s = fminf(fmaxf(-(qx * a1.x + qy * a1.y + qz * a1.z), 0.f), a0.w);
-                const float cx = qx + s * a1.x, cy = qy + s * a1.y, cz = qz + s * a1.z;
-                mask |= (cx * cx + cy * cy + cz * cz < a.cull_a2 ? 1u : 0u) << k;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                unsigned mask = 0u;
+                for (int k = 0; k < n; ++k) {
+                    const f4 a0 = B.OE[2 * (l0 + k)], a1 = B.OE[2 * (l0 + k) + 1];
+                    const float qx = a0.x + tp[h][0], qy = a0.y + tp[h][1], qz = a0.z + tp[h][2];
+                    const float s = fminf(fmaxf(-(qx * a1.x + qy * a1.y + qz * a1.z), 0.f), a0.w);
+                    const float cx = qx + s * a1.x, cy = qy + s * a1.y, cz = qz + s * a1.z;
+                    mask |= (cx * cx + cy * cy + cz * cz < a.cull_a2 ? 1u : 0u) << k;
+                }
+                DEM_EMIT(PH_EE, valid[h] ? mask : 0u, lane + 32 * h, l0, 0u);
             }
-            DEM_EMIT(PH_EE, valid ? mask : 0u, l0, 0u);
         }
         sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
         // (2) vertices of j near i: |R v + t| = |v + R^T t|;  (3) vertices of i near j: |R^T (v - t)| = |v - t|
         const int o2 = max(ob, oE) - oE, n2 = min(oe, oV) - oE, o3 = max(ob, oV) - oV, n3 = min(oe, oV + A.nv) - oV;
         if constexpr (SAME) {  // one shape: both sums sweep the same face table, so their survivors share the passes
             for (int c0 = 0; c0 < A.nv; c0 += 32) {
-                unsigned m2 = 0u, m3 = 0u;
-                for (int k = 0; k < 32; ++k) {
-                    const int o = c0 + k;
-                    if (o >= A.nv) break;
-                    const f4 v = A.V[o];
-                    const float qx = v.x + tp[0], qy = v.y + tp[1], qz = v.z + tp[2];
-                    const float rx = v.x - t[0], ry = v.y - t[1], rz = v.z - t[2];
-                    m2 |= (o >= o2 && o < n2 && qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
-                    m3 |= (o >= o3 && o < n3 && rx * rx + ry * ry + rz * rz < a.cull_b2 ? 1u : 0u) << k;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    unsigned m2 = 0u, m3 = 0u;
+                    for (int k = 0; k < 32; ++k) {
+                        const int o = c0 + k;
+                        if (o >= A.nv) break;
+                        const f4 v = A.V[o];
+                        const float qx = v.x + tp[h][0], qy = v.y + tp[h][1], qz = v.z + tp[h][2];
+                        const float rx = v.x - tq[h][0], ry = v.y - tq[h][1], rz = v.z - tq[h][2];
+                        m2 |= (o >= o2 && o < n2 && qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
+                        m3 |= (o >= o3 && o < n3 && rx * rx + ry * ry + rz * rz < a.cull_b2 ? 1u : 0u) << k;
+                    }
+                    DEM_EMIT(PH_VF_BOTH, valid[h] ? m2 : 0u, lane + 32 * h, c0, 0u);
+                    DEM_EMIT(PH_VF_BOTH, valid[h] ? m3 : 0u, lane + 32 * h, c0, 0x8000u);
                 }
-                DEM_EMIT(PH_VF_BOTH, valid ? m2 : 0u, c0, 0u);
-                DEM_EMIT(PH_VF_BOTH, valid ? m3 : 0u, c0, 0x8000u);
             }
             sweep_items<PH_VF_BOTH>(w, cc, A, B, a.sa, a.sb, nrc2);
         } else {
             for (int o0 = o2; o0 < n2; o0 += 32) {
                 const int n = min(32, n2 - o0);
-                unsigned mask = 0u;
-                for (int k = 0; k < n; ++k) {
-                    const f4 v = B.V[o0 + k];
-                    const float qx = v.x + tp[0], qy = v.y + tp[1], qz = v.z + tp[2];
-                    mask |= (qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    unsigned mask = 0u;
+                    for (int k = 0; k < n; ++k) {
+                        const f4 v = B.V[o0 + k];
+                        const float qx = v.x + tp[h][0], qy = v.y + tp[h][1], qz = v.z + tp[h][2];
+                        mask |= (qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
+                    }
+                    DEM_EMIT(PH_VF_OWN, valid[h] ? mask : 0u, lane + 32 * h, o0, 0u);
                 }
-                DEM_EMIT(PH_VF_OWN, valid ? mask : 0u, o0, 0u);
             }
             sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
             for (int o0 = o3; o0 < n3; o0 += 32) {
                 const int n = min(32, n3 - o0);
-                unsigned mask = 0u;
-                for (int k = 0; k < n; ++k) {
-                    const f4 v = A.V[o0 + k];
-                    const float qx = v.x - t[0], qy = v.y - t[1], qz = v.z - t[2];
-                    mask |= (qx * qx + qy * qy + qz * qz < a.cull_b2 ? 1u : 0u) << k;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    unsigned mask = 0u;
+                    for (int k = 0; k < n; ++k) {
+                        const f4 v = A.V[o0 + k];
+                        const float qx = v.x - tq[h][0], qy = v.y - tq[h][1], qz = v.z - tq[h][2];
+                        mask |= (qx * qx + qy * qy + qz * qz < a.cull_b2 ? 1u : 0u) << k;
+                    }
+                    DEM_EMIT(PH_VF_OTHER, valid[h] ? mask : 0u, lane + 32 * h, o0, 0u);
                 }
-                DEM_EMIT(PH_VF_OTHER, valid ? mask : 0u, o0, 0u);
             }
             sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
         }
@@ -1056,26 +1066,27 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
             drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp, w.nown);
             w.qn = 0;
         }
-        if (valid) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            if (!valid[h]) continue;
+            const int own = lane + 32 * h;
             float F[3], T[3];
 #pragma unroll
             for (int k = 0; k < 3; ++k) {
-                F[k] = w.sacc[k * 32 + lane];
-                T[k] = w.sacc[(3 + k) * 32 + lane];
+                F[k] = w.sacc[k * 64 + own];
+                T[k] = w.sacc[(3 + k) * 64 + own];
             }
-            const f4 p3 = spose[(buf * 6 + 3) * 32 + lane], p4 = spose[(buf * 6 + 4) * 32 + lane],
-                     p5 = spose[(buf * 6 + 5) * 32 + lane];
+            const f4 p3 = spose[3 * 64 + own], p4 = spose[4 * 64 + own], p5 = spose[5 * 64 + own];
             const float Mi[9] = {p3.x, p3.y, p3.z, p3.w, p4.x, p4.y, p4.z, p4.w, p5.x};
             float out[10];
-            pair_finish<float>(Mi, t, F, T, w.sacc[6 * 32 + lane], out);
-            f4* rec = a.rec + DEM_REC * ((size_t)spidx[buf * 32 + lane] * a.slices + slice);
+            pair_finish<float>(Mi, tq[h], F, T, w.sacc[6 * 64 + own], out);
+            f4* rec = a.rec + DEM_REC * ((size_t)spidx[own] * a.slices + slice);
             f4 r0, r1, r2;
             r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
             r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = p5.y;
             r2.x = p5.z; r2.y = p5.w; r2.z = r2.w = 0.f;
             rec[0] = r0; rec[1] = r1; rec[2] = r2;
         }
-        __syncwarp();  // the next tile's stage() overwrites the other buffer only; sacc is re-zeroed by its own lane
     }
     const unsigned s_ee = __reduce_add_sync(0xffffffffu, cc.swept_ee), s_vf = __reduce_add_sync(0xffffffffu, cc.swept_vf),
                    s_vfe = __reduce_add_sync(0xffffffffu, cc.swept_vfe);
@@ -1095,6 +1106,9 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
 }
 
 // bytes of dynamic shared memory k_pair_cull needs in front of the staged tables
-static inline size_t cull_smem_header() { return fast_smem_header() + sizeof(unsigned) * 4 * DEM_IQCAP; }
+static inline size_t cull_smem_header() {
+    return 256 + sizeof(unsigned) * 4 * DEM_QCAP + sizeof(float) * 4 * 7 * 64 + sizeof(unsigned) * 16 +
+           sizeof(f4) * 4 * 6 * 64 + sizeof(int) * 4 * 64 + sizeof(unsigned) * 4 * DEM_IQCAP;
+}
 
 }  // namespace dem

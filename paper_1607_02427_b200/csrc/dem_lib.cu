@@ -418,6 +418,7 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
                 pa.pidx = ctx->pidx.as<int>() + list_base[c];
                 pa.count = ccount + c;
                 pa.plane = list_cap(c);
+                pa.pad = (ctx->dim == 3 && ctx->cull) ? 64 : 32;
                 pa.counters = a.counters;
                 pa.rec = reinterpret_cast<f4*>(a.rec);
                 smem += fast_smem_header();
@@ -461,7 +462,8 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
                     a.cull_a2 = (real)(ra * ra);
                     a.cull_b2 = (real)(rb * rb);
                 }
-                const long long list_items = (long long)list_cap(c) * a.slices;  // the padded work list bounds the tiles
+                // the padded work list bounds the tiles; a warp of k_pair_cull takes 64 entries, of k_pair_fast 32
+                const long long list_items = (long long)list_cap(c) * a.slices / (ctx->dim == 3 && ctx->cull ? 2 : 1);
                 grid = (int)std::min<long long>(nblk(list_items, threads), (long long)ctx->sm_count * resident);
             }
         }
