@@ -454,7 +454,8 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
                     kern = a.sa.off == a.sb.off ? k_pair_cull<PosT, 3, true> : k_pair_cull<PosT, 3, false>;
 #ifdef DEM_TUNE
                     if (const char* v = getenv("DEM_CULL_MINB")) {
-                        if (atoi(v) == 4) kern = k_pair_cull<PosT, 4, false>;
+                        if (atoi(v) == 4) kern = a.sa.off == a.sb.off ? k_pair_cull<PosT, 4, true> : k_pair_cull<PosT, 4, false>;
+                        if (atoi(v) == 5) kern = a.sa.off == a.sb.off ? k_pair_cull<PosT, 5, true> : k_pair_cull<PosT, 5, false>;
                     }
 #endif
                     smem += cull_smem_header() - fast_smem_header();
