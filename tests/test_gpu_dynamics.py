@@ -163,3 +163,39 @@ def test_step_host_matches_device(pkg):
     for k in ("pos", "quat", "vel", "angmom"):
         assert np.array_equal(h[k].numpy().astype(np.float64), dev[k]), k
     dem.close()
+
+
+@pytest.mark.parametrize("k,skin", [(3, 0.2), (4, 0.3)])
+def test_full_size_fp32_runs_of_the_configs(pkg, oracle, k, skin):
+    """BASELINE.json configs 3 and 4 as stated: FP32, force evaluation + 1000 NVE steps at the config's dt (the launch
+    configuration bench.py times).  Reported: max_t |E(t) - E(0)| / N (R18 gates the drift in FP64 only; the
+    FP32 contexts integrate in double with FP32 forces, so a loose bound of 1e-3 eps per particle is asserted).
+    P1: the state REACHED by the run -- particles have moved, pairs have left the reach, contacts have
+    formed -- is evaluated again and sampled rows are compared with the oracle at the north_star tolerance."""
+    import torch
+
+    st = round_state(di.make_config(k), "f32")
+    got = _run(pkg, st, "f32", st["dt"], 1000, skin=skin, chunks=10)
+    e = got["energies"].sum(1)
+    drift = np.abs(e - got["e0"]).max() / st["N"]
+    print("config %d: N = %d, 1000 steps, dt = %g: max |E(t) - E(0)| / N = %.3e" % (k, st["N"], st["dt"], drift))
+    assert np.isfinite(e).all() and drift < 1e-3, drift
+    # P1: parity on the reached state
+    end = dict(st)
+    for key in ("pos", "quat", "vel", "angmom"):
+        end[key] = got[key]
+    dem, t = pkg.from_state(end, "f32")
+    dem.build_neighbors(t["pos"], t["shape_id"], end["box"], end["r_cut"])
+    f, tq, w = dem.compute(t["pos"], t["quat"], t["shape_id"])
+    cnt = dem.get_counters()
+    dem.close()
+    f, tq = f.cpu().numpy().astype(np.float64), tq.cpu().numpy().astype(np.float64)
+    sub = np.sort(np.random.default_rng(40 + k).choice(st["N"], 128, replace=False)).astype(np.int32)
+    of, ot, _, _ = oracle.compute(end, subset=sub)
+    sig = min(2 * s["rounding"] for s in st["shapes"])
+    fs = max(np.abs(f[:, :3]).max(), 1.0 / sig)
+    ts = max(np.abs(tq[:, :3]).max(), 1.0)
+    assert np.abs(f[sub, :3] - of[:, :3]).max() / fs < 1e-4
+    assert np.abs(tq[sub, :3] - ot[:, :3]).max() / ts < 1e-4
+    assert np.abs(f[sub, 3] - of[:, 3]).max() / max(np.abs(of[:, 3]).max(), 1.0) < 1e-4
+    assert cnt["active"] > 0
