@@ -373,6 +373,34 @@ def make_config(k, seed=0, scale=1):
     raise ValueError(k)
 
 
+TABLE1_CELLS = {256: (8, 8, 4), 4096: (16, 16, 16), 65536: (64, 32, 32)}
+TABLE1_SHAPES = ("sphere", "plate", "cube", "icosahedron")
+
+
+def table1_state(shape, n, seed=0):
+    """Stand-ins for the paper's Table I / Figure 4 workloads ("dense fluids" of spheres, triangular
+    plates, cubes and icosahedra at N = 256, 4096, 65536; densities, rounding radii and initial states are not given).
+    Start states here: a simple-cubic lattice at a spacing that leaves no overlap, thermal velocities at kT = 1; the
+    caller equilibrates with NVE steps before timing.  Spheres: one vertex, rho = 0.5 (sigma = 1), number density 0.8.
+    Cubes (edge 1, rho = 0.15): near-aligned at spacing 1.62 (volume fraction of the rounded cube ~0.5).  Icosahedra
+    (R = 0.5, rho = 0.05): near-aligned at spacing 1.0 (~0.45).  Plates (R = 0.5, rho = 0.05): random orientations at
+    spacing 2R + sigma = 1.1.  Returns a state dict with dt set for the shape's sigma."""
+    cells = TABLE1_CELLS[n]
+    kw = dict(seed=seed, nsteps=0, dtype="f32", name="table1_%s_N%d" % (shape, n))
+    if shape == "sphere":
+        return lattice_state(3, [sphere(0.5, inertia=0.1)], cells, 0.8 ** (-1.0 / 3.0), jitter=0.02, orient="none",
+                             dt=1e-3, **kw)
+    if shape == "cube":
+        return lattice_state(3, [cube(1.0, 0.15)], cells, 1.62, jitter=0.02, orient="small", max_angle=0.2,
+                             dt=2e-4, **kw)
+    if shape == "icosahedron":
+        return lattice_state(3, [icosahedron(0.5, 0.05)], cells, 1.0, jitter=0.01, orient="small", max_angle=0.1,
+                             dt=1e-4, **kw)
+    if shape == "plate":
+        return lattice_state(3, [triangular_plate(0.5, 0.05)], cells, 1.1, dt=2e-4, **kw)
+    raise ValueError(shape)
+
+
 def dense_state(kind, cells, seed=1, max_angle=0.05, jitter=0.02, spacing=None):
     """P2: dense near-aligned lattices in which many pairs interact through many terms.  Default
     spacings were chosen (with the oracle, offline) so that U/N is a few epsilon: in contact, nothing overlapping.

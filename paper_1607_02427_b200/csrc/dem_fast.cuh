@@ -403,11 +403,13 @@ struct PoseArgs {
     int pad;       // entries per warp tile of the kernel that follows: 32 (k_pair_fast) or 64 (k_pair_cull)
     unsigned long long* counters;  // [0] += pairs inside the reach
     f4* rec;
+    const int* skip;  // dem_step: non-null and *skip != 0 => the list is stale, the kernel does nothing (see step_t)
 };
 
 #define DEM_POSE_THREADS 512
 template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THREADS) k_pose(const PoseArgs a) {
     __shared__ int wcount[DEM_POSE_THREADS / 32], s_prefix;
+    if (a.skip && *a.skip) return;  // the work-list count stays 0: the search kernel behind finds no tile
     const unsigned full = 0xffffffffu;
     const int p = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     bool valid = false;

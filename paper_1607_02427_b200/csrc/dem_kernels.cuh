@@ -371,8 +371,10 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
 // class-major pair index), and the 4 partial sums are combined with warp shuffles.  The summation order is fixed, so
 // results are bit-reproducible from run to run.  With KICK the lane that stores the result also applies the second
 // half kick of velocity Verlet (v += dt/2 F/m, L += dt/2 tau), which saves a pass over the state.
-// `skip`: when non-null and *skip != 0 the kernel does nothing (dem_step launches the force evaluation before the
-// host knows whether the neighbour list is still valid; see step_t).
+// `flags` (dem_step only, else null): flags[0] = "some particle left its skin in this step's drift" (k_kick_drift),
+// flags[1] = halt, flags[2] = steps completed.  dem_step queues many steps before the host looks at the flags: with
+// flags[0] set the list is stale, so the kernel changes nothing and raises halt, which turns every later
+// k_kick_drift of the chunk into a no-op; otherwise it counts the step as completed (see step_t).
 struct KickArgs {
     double half_dt;
     int dim;
@@ -386,10 +388,16 @@ __global__ void k_reduce(int N, const int* __restrict__ counts, const int* __res
                          const int* __restrict__ sid, ClassTable ct, int nclass,
                          const typename vec4<real>::type* __restrict__ rec, typename vec4<real>::type* __restrict__ force,
                          typename vec4<real>::type* __restrict__ torque, real* __restrict__ virial,
-                         const int* __restrict__ skip, KickArgs ka) {
+                         int* __restrict__ flags, KickArgs ka) {
     typedef typename vec4<real>::type real4;
-    if (skip && *skip) return;
     const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (flags) {
+        if (flags[0]) {
+            if (gid == 0) flags[1] = 1;
+            return;
+        }
+        if (gid == 0) flags[2] += 1;  // nothing in this kernel reads flags[2]
+    }
     const int i = gid >> 2, sub = gid & 3;
     real F[3] = {0, 0, 0}, T[3] = {0, 0, 0}, U = 0, W[6] = {0, 0, 0, 0, 0, 0};
     if (i < N) {
@@ -535,7 +543,8 @@ __device__ inline void free_rotate(int dim, const double* I, const double* L, do
 }
 
 // first half of velocity Verlet: v += dt/2 F/m; x += dt v (wrapped); L += dt/2 tau; free rotation of q.
-// Also raises *moved when a particle is farther than skin/2 from where it was at the last neighbour build.
+// Also raises moved[0] when a particle is farther than skin/2 from where it was at the last neighbour build.
+// Does nothing once moved[1] (halt, raised by k_reduce of an earlier step of the same chunk) is set.
 template <typename real>
 __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict__ sid, MassTable mt,
                              d4* __restrict__ pos, d4* __restrict__ quat, d4* __restrict__ vel, d4* __restrict__ ang,
@@ -544,6 +553,7 @@ __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict
                              double half_skin2, int* __restrict__ moved) {
     // The translational and the rotational half of a particle's update are independent: the first half of the grid
     // does x, v (and the skin test), the second q, L -- twice the memory-level parallelism, half the dependent chain.
+    if (moved[1]) return;
     const int half = gridDim.x >> 1;
     const bool rot = (int)blockIdx.x >= half;
     const int i = (blockIdx.x - (rot ? half : 0)) * blockDim.x + threadIdx.x;
@@ -569,7 +579,7 @@ __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict
         dx -= box.L[0] * rint(dx * box.invL[0]);
         dy -= box.L[1] * rint(dy * box.invL[1]);
         dz -= box.L[2] * rint(dz * box.invL[2]);
-        if (dx * dx + dy * dy + dz * dz > half_skin2) *moved = 1;
+        if (dx * dx + dy * dy + dz * dz > half_skin2) moved[0] = 1;
     } else {
         d4 L = ang[i], q = quat[i];
         const typename vec4<real>::type T = torque[i];

@@ -81,8 +81,8 @@ struct dem_ctx {
     size_t ev_used = 0;
     int64_t last_terms = 0;
     int sm_count = 148;
-    int* h_moved = nullptr;        // pinned host copy of dem_step's "list is stale" flag
-    cudaEvent_t ev_flag = nullptr;
+    int* h_moved = nullptr;        // pinned host copy of dem_step's flags (moved, halt, steps completed)
+    int rebuild_interval = 8;      // steps between the last two neighbour rebuilds of dem_step (sizes its chunks)
 };
 
 namespace {
@@ -345,7 +345,7 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
 // ---- force evaluation ---------------------------------------------------------------------------------------------
 template <typename real, typename PosT>
 int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* sid, int N, void* force, void* torque,
-              void* virial, const int* skip = nullptr, const KickArgs* kick = nullptr) {
+              void* virial, int* skip = nullptr, const KickArgs* kick = nullptr) {
     typedef typename vec4<real>::type real4;
     if (!ctx->have_list) return fail(ctx, DEM_ESTALE, "no neighbour list: call dem_build_neighbors first");
     if (N != ctx->N) return fail(ctx, DEM_ESTALE, "N = %d differs from the last build (%d)", N, ctx->N);
@@ -421,6 +421,7 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
                 pa.pad = (ctx->dim == 3 && ctx->cull) ? 64 : 32;
                 pa.counters = a.counters;
                 pa.rec = reinterpret_cast<f4*>(a.rec);
+                pa.skip = skip;
                 smem += fast_smem_header();
                 // packed outer pairs per sweep: 3 when the vertex counts fill tiles of 6 at least as well as tiles of 4
                 auto waste = [](int n, int tile) { return ((n + tile - 1) / tile) * tile - n; };
@@ -547,34 +548,46 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     for (int a = 0; a < 3; ++a) bx.invL[a] = 1.0 / bx.L[a];
     CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
     CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr)));
-    int* moved = ctx->flags.as<int>() + 8;
+    int* flags = ctx->flags.as<int>() + 8;  // [0] moved, [1] halt, [2] steps completed (k_kick_drift, k_reduce)
     const double half_skin2 = 0.25 * skin * skin;
     if (ctx->l2_flush_bytes) CU(ctx->l2_scratch.reserve(ctx->l2_flush_bytes));
-    if (!ctx->h_moved) CU(cudaHostAlloc(&ctx->h_moved, sizeof(int), cudaHostAllocDefault));
-    if (!ctx->ev_flag) CU(cudaEventCreateWithFlags(&ctx->ev_flag, cudaEventDisableTiming));
+    if (!ctx->h_moved) CU(cudaHostAlloc(&ctx->h_moved, 4 * sizeof(int), cudaHostAllocDefault));
     KickArgs ka;
     ka.half_dt = 0.5 * dt;
     ka.dim = ctx->dim;
     ka.vel = v;
     ka.ang = L;
     for (int k = 0; k < DEM_MAX_SHAPES_K; ++k) ka.inv_mass[k] = ctx->mt.mass[k] > 0 ? 1.0 / ctx->mt.mass[k] : 0.0;
-    for (int s = 0; s < nsteps; ++s) {
-        if (ctx->l2_flush_bytes) CU(cudaMemsetAsync(ctx->l2_scratch.p, s & 0xff, ctx->l2_flush_bytes, st));
-        CU(cudaMemsetAsync(moved, 0, sizeof(int), st));
-        k_kick_drift<real><<<2 * nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T, ctx->pos_build.as<d4>(),
-                                                     half_skin2, moved);
-        LAUNCHED(ctx);
-        CU(cudaMemcpyAsync(ctx->h_moved, moved, sizeof(int), cudaMemcpyDeviceToHost, st));
-        CU(cudaEventRecord(ctx->ev_flag, st));
-        // The force evaluation and the second half kick are queued before the host knows whether some particle has
-        // left its skin: the reduction (which alone changes state) does nothing if `moved` is set, so the GPU never
-        // idles on the host's answer.  In the rare step that needs a new list the host rebuilds it and evaluates again.
-        CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr, moved, &ka)));
-        CU(cudaEventSynchronize(ctx->ev_flag));
-        if (*ctx->h_moved) {
+    // Steps are queued in chunks without the host in between: k_kick_drift raises flags[0] when a particle leaves its
+    // skin; k_reduce (which alone completes a step) then changes nothing and raises halt, and the rest of the chunk
+    // turns into no-ops.  The host reads the flags once per chunk: a halted chunk stopped after the drift of step
+    // `done + 1`, which is completed here with a new list.  The chunk length follows the last observed interval
+    // between rebuilds, so that few launches are wasted behind a halt.
+    int remaining = nsteps, since = 0;
+    while (remaining > 0) {
+        const int hint = std::max(ctx->rebuild_interval, 1);
+        const int chunk = std::min(remaining, std::min(64, std::max(hint - since, std::max(1, hint / 8))));
+        CU(cudaMemsetAsync(flags, 0, 3 * sizeof(int), st));
+        for (int s = 0; s < chunk; ++s) {
+            if (ctx->l2_flush_bytes) CU(cudaMemsetAsync(ctx->l2_scratch.p, s & 0xff, ctx->l2_flush_bytes, st));
+            k_kick_drift<real><<<2 * nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T,
+                                                         ctx->pos_build.as<d4>(), half_skin2, flags);
+            LAUNCHED(ctx);
+            CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr, flags, &ka)));
+        }
+        CU(cudaMemcpyAsync(ctx->h_moved, flags, 3 * sizeof(int), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        int done = ctx->h_moved[2];
+        if (ctx->h_moved[0]) {
             CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
             CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr, nullptr, &ka)));
+            done += 1;
+            ctx->rebuild_interval = since + done;
+            since = 0;
+        } else {
+            since += done;
         }
+        remaining -= done;
     }
     if (conv) {
         void* out[4] = {pos, quat, vel, ang};
@@ -643,7 +656,6 @@ int dem_destroy(dem_ctx* c) {
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();
     if (c->h_moved) cudaFreeHost(c->h_moved);
-    if (c->ev_flag) cudaEventDestroy(c->ev_flag);
     for (auto& e : c->ev_pool) {
         cudaEventDestroy(e.mid);
         cudaEventDestroy(e.first);

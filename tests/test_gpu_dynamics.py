@@ -199,3 +199,26 @@ def test_full_size_fp32_runs_of_the_configs(pkg, oracle, k, skin):
     assert np.abs(tq[sub, :3] - ot[:, :3]).max() / ts < 1e-4
     assert np.abs(f[sub, 3] - of[:, 3]).max() / max(np.abs(of[:, 3]).max(), 1.0) < 1e-4
     assert cnt["active"] > 0
+
+
+@pytest.mark.parametrize("shape", di.TABLE1_SHAPES)
+def test_table1_workloads_parity_before_and_after_a_run(pkg, oracle, shape):
+    """the Table I / Figure 4 shape families (spheres with a central WCA, triangular
+    plates, cubes, icosahedra) as dem_inputs.table1_state builds them, at N = 256: neighbour list bit-exact and
+    force / torque / energy / virial against the all-pairs oracle on the start state and on the state reached after
+    an NVE run of the library (contacts formed), FP32 and FP64; the FP64 run conserves energy."""
+    from _gpu_util import assert_neighbors_exact, assert_parity
+
+    st = di.table1_state(shape, 256)
+    assert_neighbors_exact(st, "f32", oracle)
+    assert_parity(st, "f32", oracle)
+    got = _run(pkg, st, "f64", st["dt"], 600, skin=0.2, chunks=6)
+    e = got["energies"].sum(1)
+    assert np.abs(e - got["e0"]).max() / st["N"] < 1e-4
+    end = dict(st)
+    for key in ("pos", "quat", "vel", "angmom"):
+        end[key] = got[key]
+    for precision in ("f32", "f64"):
+        cnt = assert_parity(end, precision, oracle)
+    if shape != "cube":      # cubes start out of reach of one another (volume fraction 0.5): contacts take longer
+        assert got["energies"][-1][0] > 0
