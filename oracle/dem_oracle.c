@@ -632,6 +632,70 @@ int orc_step(const orc_shapes* S, const double* mass, const double* inertia3, in
     return 0;
 }
 
+/*
+ * NVT ("a standard Nose-Hoover thermostat applied to both translational and
+ * rotational degrees of freedom", ref. 23).  Reading (R19): ONE friction variable xi for all degrees of
+ * freedom, dv/dt = F/m - xi v, dL/dt = tau - xi L, dxi/dt = (2K - g kT)/Q, deta/dt = xi, Q = g kT tau_T^2,
+ * K = K_trans + K_rot, g = dim (N - 1) + number of (particle, rotation axis) with I > 0 (2D: the z axis only).
+ * One step = thermostat half step, the NVE step above, thermostat half step, where a thermostat half step is
+ *     xi += (dt/4)(2K - g kT)/Q;  s = exp(-xi dt/2);  v *= s;  L *= s;  K *= s^2;  eta += (dt/2) xi;
+ *     xi += (dt/4)(2K - g kT)/Q
+ * (symmetric, time-reversible).  Conserved: U + K + Q xi^2/2 + g kT eta.
+ * thermo[2] = (xi, eta), in and out.  energies (may be NULL): [(nsteps+1)][5] = U, K_trans, K_rot, xi, eta.
+ * Returns g.
+ */
+static double nvt_dof(int dim, int N, const double* inertia3, const int* sid) {
+    double g = (double)dim * (N - 1);
+    for (int i = 0; i < N; ++i)
+        for (int a = (dim == 2 ? 2 : 0); a < 3; ++a)
+            if (inertia3[3 * sid[i] + a] > 0.0) g += 1.0;
+    return g;
+}
+
+static void nvt_half(int dim, int N, const double* mass, const double* inertia3, const int* sid, const double* quat4,
+                     double* vel4, double* ang4, const double* force4, double dt, double g, double kT, double Q,
+                     double thermo[2]) {
+    double e[3];
+    orc_energy(dim, N, mass, inertia3, sid, quat4, vel4, ang4, force4, e);
+    double K = e[1] + e[2];
+    thermo[0] += 0.25 * dt * (2.0 * K - g * kT) / Q;
+    const double s = exp(-thermo[0] * 0.5 * dt);
+    for (int i = 0; i < N; ++i)
+        for (int a = 0; a < 3; ++a) {
+            vel4[4 * (size_t)i + a] *= s;
+            ang4[4 * (size_t)i + a] *= s;
+        }
+    K *= s * s;
+    thermo[1] += 0.5 * dt * thermo[0];
+    thermo[0] += 0.25 * dt * (2.0 * K - g * kT) / Q;
+}
+
+double orc_step_nvt(const orc_shapes* S, const double* mass, const double* inertia3, int dim, int N,
+                    const double box[3], double* pos4, double* quat4, double* vel4, double* ang4, const int* sid,
+                    double eps, double eps_par, double dt, int nsteps, double kT, double tau_T, double thermo[2],
+                    double* force4, double* torque4, double* energies) {
+    const double g = nvt_dof(dim, N, inertia3, sid), Q = g * kT * tau_T * tau_T;
+    orc_compute(S, dim, N, box, pos4, quat4, sid, eps, eps_par, 1, NULL, 0, force4, torque4, NULL, NULL);
+    if (energies) {
+        orc_energy(dim, N, mass, inertia3, sid, quat4, vel4, ang4, force4, energies);
+        energies[3] = thermo[0];
+        energies[4] = thermo[1];
+    }
+    for (int step = 1; step <= nsteps; ++step) {
+        nvt_half(dim, N, mass, inertia3, sid, quat4, vel4, ang4, force4, dt, g, kT, Q, thermo);
+        orc_step(S, mass, inertia3, dim, N, box, pos4, quat4, vel4, ang4, sid, eps, eps_par, dt, 1, force4, torque4,
+                 NULL);
+        nvt_half(dim, N, mass, inertia3, sid, quat4, vel4, ang4, force4, dt, g, kT, Q, thermo);
+        if (energies) {
+            double* e = energies + 5 * (size_t)step;
+            orc_energy(dim, N, mass, inertia3, sid, quat4, vel4, ang4, force4, e);
+            e[3] = thermo[0];
+            e[4] = thermo[1];
+        }
+    }
+    return g;
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -194,6 +194,25 @@ def step(state, dt, nsteps, eps_par=DEFAULT_EPS_PAR, record_energy=True):
     return dict(pos=pos, quat=quat, vel=vel, angmom=ang, force=f, torque=t, energies=en)
 
 
+def step_nvt(state, dt, nsteps, kT, tau, thermo=(0.0, 0.0), eps_par=DEFAULT_EPS_PAR):
+    """Nose-Hoover NVT integration of a COPY of the state (orc_step_nvt; R19).  Returns dict(pos, quat, vel,
+    angmom, force, torque, energies [nsteps+1][5] = U, K_trans, K_rot, xi, eta, thermo = final (xi, eta), dof = g)."""
+    tab = state.get("_tab") or ShapeTable(state["shapes"])
+    pos, quat = _f64(state["pos"]).copy(), _f64(state["quat"]).copy()
+    vel, ang = _f64(state["vel"]).copy(), _f64(state["angmom"]).copy()
+    n = len(pos)
+    f, t = np.zeros((n, 4)), np.zeros((n, 4))
+    en = np.zeros((nsteps + 1, 5))
+    th = np.array(thermo, dtype=np.float64)
+    sid = np.ascontiguousarray(state["shape_id"], dtype=np.int32)
+    fn = lib().orc_step_nvt
+    fn.restype = C.c_double
+    g = fn(C.byref(tab.c), _p(tab.mass), _p(tab.inertia), C.c_int(state["dim"]), C.c_int(n), _p(_f64(state["box"])),
+           _p(pos), _p(quat), _p(vel), _p(ang), _p(sid), C.c_double(state["epsilon"]), C.c_double(eps_par),
+           C.c_double(dt), C.c_int(nsteps), C.c_double(kT), C.c_double(tau), _p(th), _p(f), _p(t), _p(en))
+    return dict(pos=pos, quat=quat, vel=vel, angmom=ang, force=f, torque=t, energies=en, thermo=th, dof=g)
+
+
 def energy(state, force):
     tab = state.get("_tab") or ShapeTable(state["shapes"])
     out = np.zeros(3)
