@@ -145,6 +145,24 @@ int dem_get_counters(dem_ctx* ctx, int64_t out[9]);
 int dem_step(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const int32_t* shape_id, int N,
              const double box[3], double dt, int nsteps, double skin, void* force_energy, void* torque);
 
+/*
+ * NVT: dem_step with a Nose-Hoover thermostat "applied to both translational and rotational degrees of freedom"
+ * (R19).  One friction variable xi for all degrees of freedom:
+ *     dv/dt = F/m - xi v,   dL/dt = tau - xi L,   dxi/dt = (2K - g kT)/Q,   deta/dt = xi,   Q = g kT tau^2,
+ * K = K_trans + K_rot, g = dim (N - 1) + number of (particle, rotation axis) with inertia > 0 (2D: the z axis).
+ * One step = thermostat half step, the NVE step of dem_step, thermostat half step; a half step is
+ *     xi += (dt/4)(2K - g kT)/Q;  s = exp(-xi dt/2);  v *= s;  L *= s;  K *= s^2;  eta += (dt/2) xi;
+ *     xi += (dt/4)(2K - g kT)/Q.
+ * U + K + Q xi^2 / 2 + g kT eta is conserved.  The barostat of PAPER.md:115 is not built.
+ *   kT, tau        target temperature and thermostat period (> 0)
+ *   thermostat[2]  HOST, in and out: (xi, eta); start a run from (0, 0) and pass the values back in to continue it
+ *   *dof           HOST, may be NULL: receives g
+ * Everything else as dem_step.  Errors: those of dem_step; DEM_EINVAL for kT <= 0, tau <= 0, N < 2.
+ */
+int dem_step_nvt(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const int32_t* shape_id, int N,
+                 const double box[3], double dt, int nsteps, double skin, double kT, double tau, double thermostat[2],
+                 double* dof, void* force_energy, void* torque);
+
 /* U = sum_i U_i (from force_energy[.][3]), K_trans, K_rot of a state; DEVICE inputs, HOST out[3]; synchronises. */
 int dem_energy(dem_ctx* ctx, const void* quat, const void* vel, const void* angmom, const int32_t* shape_id,
                const void* force_energy, int N, double out[3]);

@@ -20,7 +20,7 @@ STATUS_NAMES = {0: "DEM_OK", -1: "DEM_EINVAL", -2: "DEM_ENOMEM", -3: "DEM_ECUDA"
 
 # every symbol include/dem.h declares (tests check that the built library exports all of them)
 EXPORTS = ["dem_create", "dem_destroy", "dem_last_error", "dem_set_eps_par", "dem_create_shape", "dem_build_neighbors",
-           "dem_get_neighbors", "dem_copy_neighbors", "dem_compute", "dem_get_counters", "dem_step", "dem_energy",
+           "dem_get_neighbors", "dem_copy_neighbors", "dem_compute", "dem_get_counters", "dem_step", "dem_step_nvt", "dem_energy",
            "dem_compute_host", "dem_step_host", "dem_set_slices", "dem_set_pair_kernel", "dem_set_culling", "dem_set_l2_flush", "dem_set_timing", "dem_kernel_time", "dem_kernel_time_split", "dem_swept_totals",
            "dem_launch_count", "dem_fp32_peak", "dem_version"]
 
@@ -214,6 +214,22 @@ class Dem:
                             C.c_int(nsteps), C.c_double(skin), _dev(force, self.dtype), _dev(torque, self.dtype))
         _check(self._ctx, rc)
         self._n_last = n
+
+    def step_nvt(self, pos, quat, vel, angmom, shape_id, box, dt, nsteps, skin, kT, tau, thermostat=(0.0, 0.0),
+                 force=None, torque=None):
+        """dem_step_nvt; returns ((xi, eta), g)."""
+        torch = self.torch
+        n = pos.shape[0]
+        th = (C.c_double * 2)(float(thermostat[0]), float(thermostat[1]))
+        dof = C.c_double(0.0)
+        rc = lib().dem_step_nvt(self._ctx, _dev(pos, self.dtype, "pos"), _dev(quat, self.dtype, "quat"),
+                                _dev(vel, self.dtype, "vel"), _dev(angmom, self.dtype, "angmom"),
+                                _dev(shape_id, torch.int32, "shape_id"), C.c_int(n), _host(_box(box)), C.c_double(dt),
+                                C.c_int(nsteps), C.c_double(skin), C.c_double(kT), C.c_double(tau), th, C.byref(dof),
+                                _dev(force, self.dtype), _dev(torque, self.dtype))
+        _check(self._ctx, rc)
+        self._n_last = n
+        return (th[0], th[1]), dof.value
 
     def energy(self, quat, vel, angmom, shape_id, force):
         torch = self.torch

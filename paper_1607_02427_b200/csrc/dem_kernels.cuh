@@ -542,6 +542,12 @@ __device__ inline void free_rotate(int dim, const double* I, const double* L, do
     for (int k = 0; k < 4; ++k) q[k] /= n;
 }
 
+// Nose-Hoover thermostat (dem_step_nvt; R19): friction xi, its time integral eta, the scaling
+// of v and L that the next k_kick_drift (or k_scale_momenta) still has to apply, and the degrees of freedom g.
+struct ThermoDev {
+    double xi, eta, scale, dof;
+};
+
 // first half of velocity Verlet: v += dt/2 F/m; x += dt v (wrapped); L += dt/2 tau; free rotation of q.
 // Also raises moved[0] when a particle is farther than skin/2 from where it was at the last neighbour build.
 // Does nothing once moved[1] (halt, raised by k_reduce of an earlier step of the same chunk) is set.
@@ -550,7 +556,7 @@ __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict
                              d4* __restrict__ pos, d4* __restrict__ quat, d4* __restrict__ vel, d4* __restrict__ ang,
                              const typename vec4<real>::type* __restrict__ force,
                              const typename vec4<real>::type* __restrict__ torque, const d4* __restrict__ pos_build,
-                             double half_skin2, int* __restrict__ moved) {
+                             double half_skin2, int* __restrict__ moved, const ThermoDev* __restrict__ thermo) {
     // The translational and the rotational half of a particle's update are independent: the first half of the grid
     // does x, v (and the skin test), the second q, L -- twice the memory-level parallelism, half the dependent chain.
     if (moved[1]) return;
@@ -559,12 +565,13 @@ __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict
     const int i = (blockIdx.x - (rot ? half : 0)) * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const int s = sid[i];
+    const double sc = thermo ? thermo->scale : 1.0;  // NVT: pending thermostat scaling of v and L (k_thermostat)
     if (!rot) {
         const double hm = 0.5 * dt / mt.mass[s];
         d4 x = pos[i], v = vel[i];
         const typename vec4<real>::type F = force[i];
         const d4 xb = pos_build[i];
-        double xs[3] = {x.x, x.y, x.z}, vs[3] = {v.x, v.y, v.z};
+        double xs[3] = {x.x, x.y, x.z}, vs[3] = {v.x * sc, v.y * sc, v.z * sc};
         const double Fs[3] = {(double)F.x, (double)F.y, (double)F.z};
         for (int a = 0; a < box.dim; ++a) {
             vs[a] += hm * Fs[a];
@@ -583,7 +590,7 @@ __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict
     } else {
         d4 L = ang[i], q = quat[i];
         const typename vec4<real>::type T = torque[i];
-        double Ls[3] = {L.x, L.y, L.z};
+        double Ls[3] = {L.x * sc, L.y * sc, L.z * sc};
         const double Ts[3] = {(double)T.x, (double)T.y, (double)T.z};
         for (int a = (box.dim == 2 ? 2 : 0); a < 3; ++a) Ls[a] += 0.5 * dt * Ts[a];
         double qs[4] = {q.x, q.y, q.z, q.w};
@@ -593,6 +600,92 @@ __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict
         ang[i] = L;
         quat[i] = q;
     }
+}
+
+// NVT: per-block partial sums of K_trans + K_rot and of the rotational degrees of freedom (axes with I > 0), in double,
+// fixed order.  partial[2 b] = K, partial[2 b + 1] = degrees of freedom.
+__global__ void k_kinetic(int N, int dim, const int* __restrict__ sid, MassTable mt, const d4* __restrict__ quat,
+                          const d4* __restrict__ vel, const d4* __restrict__ ang, double* __restrict__ partial) {
+    __shared__ double sh[2][256];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double K = 0, dof = 0;
+    if (i < N) {
+        const int s = sid[i];
+        const d4 v = vel[i], L = ang[i], q = quat[i];
+        K = 0.5 * mt.mass[s] * (v.x * v.x + v.y * v.y + v.z * v.z);
+        double M[9];
+        quat_to_mat<double>(q.x, q.y, q.z, q.w, M);
+        for (int a = (dim == 2 ? 2 : 0); a < 3; ++a) {
+            const double Lb = M[a] * L.x + M[3 + a] * L.y + M[6 + a] * L.z;
+            const double I = mt.inertia[s][a];
+            if (I > 0.0) {
+                K += 0.5 * Lb * Lb / I;
+                dof += 1.0;
+            }
+        }
+    }
+    sh[0][threadIdx.x] = K; sh[1][threadIdx.x] = dof;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+            sh[0][threadIdx.x] += sh[0][threadIdx.x + o];
+            sh[1][threadIdx.x] += sh[1][threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        partial[2 * blockIdx.x] = sh[0][0];
+        partial[2 * blockIdx.x + 1] = sh[1][0];
+    }
+}
+
+// NVT: one block sums the partials of k_kinetic and advances (xi, eta) by `halves` thermostat half steps (1: the end
+// of the run, or its start; 2: the end of one step and the start of the next, which are adjacent).  The scaling of v
+// and L is left in th->scale for the next k_kick_drift / k_scale_momenta.  Does nothing when the step it follows was
+// not completed (flags[1] = halt, see k_reduce).
+__global__ void k_thermostat(int nb, const double* __restrict__ partial, int dim, int N, double dt, double kT,
+                             double tau, int halves, const int* __restrict__ flags, ThermoDev* __restrict__ th) {
+    __shared__ double sh[2][256];
+    if (flags && flags[1]) return;
+    double K = 0, dof = 0;
+    for (int b = threadIdx.x; b < nb; b += 256) {
+        K += partial[2 * b];
+        dof += partial[2 * b + 1];
+    }
+    sh[0][threadIdx.x] = K; sh[1][threadIdx.x] = dof;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+            sh[0][threadIdx.x] += sh[0][threadIdx.x + o];
+            sh[1][threadIdx.x] += sh[1][threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x != 0) return;
+    K = sh[0][0];
+    const double g = (double)dim * (N - 1) + sh[1][0], Q = g * kT * tau * tau;
+    double xi = th->xi, eta = th->eta, scale = 1.0;
+    for (int h = 0; h < halves; ++h) {
+        xi += 0.25 * dt * (2.0 * K - g * kT) / Q;
+        const double s = exp(-xi * 0.5 * dt);
+        K *= s * s;
+        scale *= s;
+        eta += 0.5 * dt * xi;
+        xi += 0.25 * dt * (2.0 * K - g * kT) / Q;
+    }
+    th->xi = xi; th->eta = eta; th->scale = scale; th->dof = g;
+}
+
+// NVT: the scaling left by the last thermostat half step of a run.
+__global__ void k_scale_momenta(int N, d4* __restrict__ vel, d4* __restrict__ ang, const ThermoDev* __restrict__ th) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double s = th->scale;
+    d4 v = vel[i], L = ang[i];
+    v.x *= s; v.y *= s; v.z *= s;
+    L.x *= s; L.y *= s; L.z *= s;
+    vel[i] = v;
+    ang[i] = L;
 }
 
 // U, K_trans, K_rot: per-block partial sums in double (fixed order), summed on the host.

@@ -57,7 +57,7 @@ struct dem_ctx {
     int N = 0, stride = 16, max_count = 0;
     double box[3] = {0, 0, 0}, r_cut = 0;
     GridDev grid;
-    DevBuf cell_of, rank, cell_start, order, xs, counts, list, slot, scratch_scan, pcnt, pairs, rec, flags, counters;
+    DevBuf cell_of, rank, cell_start, order, xs, counts, list, slot, scratch_scan, pcnt, pairs, rec, flags, counters, thermo;
     DevBuf cum;         // running totals of the swept-term counters while timing is on
     DevBuf pose, pidx;  // FP32 search kernel: compacted pose records per class (k_pose)
     ClassTable ct;
@@ -82,6 +82,7 @@ struct dem_ctx {
     int64_t last_terms = 0;
     int sm_count = 148;
     int* h_moved = nullptr;        // pinned host copy of dem_step's flags (moved, halt, steps completed)
+    double nvt_dof = 0;            // degrees of freedom counted by the last dem_step_nvt
     int rebuild_interval = 8;      // steps between the last two neighbour rebuilds of dem_step (sizes its chunks)
 };
 
@@ -510,9 +511,14 @@ int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* si
     return DEM_OK;
 }
 
+struct NvtArgs {  // dem_step_nvt: target temperature, thermostat period, (xi, eta) in and out (host)
+    double kT, tau;
+    double* thermo;
+};
+
 template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* vel, void* ang, const int32_t* sid,
                                     int N, const double box[3], double dt, int nsteps, double skin, void* force_out,
-                                    void* torque_out) {
+                                    void* torque_out, const NvtArgs* nvt = nullptr) {
     typedef typename vec4<real>::type real4;
     if (N < 1 || !pos || !quat || !vel || !ang || !sid) return fail(ctx, DEM_EINVAL, "bad particle arrays");
     if (nsteps < 0 || !(skin >= 0)) return fail(ctx, DEM_EINVAL, "bad nsteps / skin");
@@ -548,6 +554,26 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     for (int a = 0; a < 3; ++a) bx.invL[a] = 1.0 / bx.L[a];
     CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
     CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr)));
+    // NVT (R19): k_kinetic + k_thermostat after every completed step advance (xi, eta) by the half step that
+    // ends it and the half step that begins the next one; the scaling of v and L is applied by the next k_kick_drift.
+    ThermoDev* th = nullptr;
+    const int nbk = nblk(N, 256);
+    auto thermostat = [&](int halves, const int* fl) -> int {
+        k_kinetic<<<nbk, 256, 0, st>>>(N, ctx->dim, sid, ctx->mt, q, v, L, ctx->epart.as<double>());
+        LAUNCHED(ctx);
+        k_thermostat<<<1, 256, 0, st>>>(nbk, ctx->epart.as<double>(), ctx->dim, N, dt, nvt->kT, nvt->tau, halves, fl, th);
+        LAUNCHED(ctx);
+        return DEM_OK;
+    };
+    if (nvt && nsteps > 0) {
+        CU(ctx->thermo.reserve(sizeof(ThermoDev)));
+        CU(ctx->epart.reserve(sizeof(double) * 3 * (size_t)nbk));
+        th = ctx->thermo.as<ThermoDev>();
+        const ThermoDev h0 = {nvt->thermo[0], nvt->thermo[1], 1.0, 0.0};
+        CU(cudaMemcpyAsync(th, &h0, sizeof h0, cudaMemcpyHostToDevice, st));
+        CU(cudaStreamSynchronize(st));  // h0 is on the stack
+        CHECK(thermostat(1, nullptr));
+    }
     int* flags = ctx->flags.as<int>() + 8;  // [0] moved, [1] halt, [2] steps completed (k_kick_drift, k_reduce)
     const double half_skin2 = 0.25 * skin * skin;
     if (ctx->l2_flush_bytes) CU(ctx->l2_scratch.reserve(ctx->l2_flush_bytes));
@@ -571,9 +597,10 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
         for (int s = 0; s < chunk; ++s) {
             if (ctx->l2_flush_bytes) CU(cudaMemsetAsync(ctx->l2_scratch.p, s & 0xff, ctx->l2_flush_bytes, st));
             k_kick_drift<real><<<2 * nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T,
-                                                         ctx->pos_build.as<d4>(), half_skin2, flags);
+                                                         ctx->pos_build.as<d4>(), half_skin2, flags, th);
             LAUNCHED(ctx);
             CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr, flags, &ka)));
+            if (th) CHECK(thermostat(nsteps - remaining + s == nsteps - 1 ? 1 : 2, flags));
         }
         CU(cudaMemcpyAsync(ctx->h_moved, flags, 3 * sizeof(int), cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
@@ -582,12 +609,17 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
             CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
             CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr, nullptr, &ka)));
             done += 1;
+            if (th) CHECK(thermostat(nsteps - remaining + done == nsteps ? 1 : 2, nullptr));
             ctx->rebuild_interval = since + done;
             since = 0;
         } else {
             since += done;
         }
         remaining -= done;
+    }
+    if (th) {
+        k_scale_momenta<<<nblk(N, B), B, 0, st>>>(N, v, L, th);
+        LAUNCHED(ctx);
     }
     if (conv) {
         void* out[4] = {pos, quat, vel, ang};
@@ -599,8 +631,15 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     }
     if (force_out) CU(cudaMemcpyAsync(force_out, F, sizeof(real4) * (size_t)N, cudaMemcpyDeviceToDevice, st));
     if (torque_out) CU(cudaMemcpyAsync(torque_out, T, sizeof(real4) * (size_t)N, cudaMemcpyDeviceToDevice, st));
+    ThermoDev h1;
+    if (th) CU(cudaMemcpyAsync(&h1, th, sizeof h1, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
     CU(cudaGetLastError());
+    if (th) {
+        nvt->thermo[0] = h1.xi;
+        nvt->thermo[1] = h1.eta;
+        ctx->nvt_dof = h1.dof;
+    }
     // the internal list was built from internal (double) positions; a later dem_compute on caller arrays is still valid
     return DEM_OK;
 }
@@ -651,7 +690,7 @@ int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda
 int dem_destroy(dem_ctx* c) {
     if (!c) return DEM_EINVAL;
     DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
-                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->pose, &c->pidx, &c->cum, &c->st_pos, &c->st_quat,
+                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->thermo, &c->pose, &c->pidx, &c->cum, &c->st_pos, &c->st_quat,
                       &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->pos_build, &c->epart, &c->h_pos,
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();
@@ -799,6 +838,23 @@ int dem_step(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const
     if (ctx->prec == DEM_F64)
         return step_t<double>(ctx, pos, quat, vel, angmom, shape_id, N, box, dt, nsteps, skin, force_energy, torque);
     return step_t<float>(ctx, pos, quat, vel, angmom, shape_id, N, box, dt, nsteps, skin, force_energy, torque);
+}
+
+int dem_step_nvt(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const int32_t* shape_id, int N,
+                 const double box[3], double dt, int nsteps, double skin, double kT, double tau, double thermostat[2],
+                 double* dof, void* force_energy, void* torque) {
+    if (!ctx) return DEM_EINVAL;
+    if (!box || !thermostat) return fail(ctx, DEM_EINVAL, "null box / thermostat");
+    if (!(kT > 0) || !(tau > 0)) return fail(ctx, DEM_EINVAL, "kT and tau must be > 0");
+    if (N < 2) return fail(ctx, DEM_EINVAL, "the thermostat needs N >= 2");
+    const NvtArgs nvt = {kT, tau, thermostat};
+    int rc;
+    if (ctx->prec == DEM_F64)
+        rc = step_t<double>(ctx, pos, quat, vel, angmom, shape_id, N, box, dt, nsteps, skin, force_energy, torque, &nvt);
+    else
+        rc = step_t<float>(ctx, pos, quat, vel, angmom, shape_id, N, box, dt, nsteps, skin, force_energy, torque, &nvt);
+    if (rc == DEM_OK && dof) *dof = ctx->nvt_dof;
+    return rc;
 }
 
 int dem_energy(dem_ctx* ctx, const void* quat, const void* vel, const void* angmom, const int32_t* shape_id,

@@ -222,3 +222,58 @@ def test_table1_workloads_parity_before_and_after_a_run(pkg, oracle, shape):
         cnt = assert_parity(end, precision, oracle)
     if shape != "cube":      # cubes start out of reach of one another (volume fraction 0.5): contacts take longer
         assert got["energies"][-1][0] > 0
+
+
+@pytest.mark.parametrize("kind,cells,spacing,dt", [("cubes", 4, 1.38, 5e-4), ("squares", 8, None, 5e-4),
+                                                   ("mixed", 4, None, 2.5e-4)])
+def test_nvt_matches_oracle_f64(pkg, oracle, kind, cells, spacing, dt):
+    """dem_step_nvt (R19) against orc_step_nvt: trajectory, thermostat variables and degrees of
+    freedom.  The run is split over three calls (the thermostat state is handed back in) and uses a thin skin, so
+    that neighbour rebuilds fall inside the queued chunks of steps."""
+    import torch
+
+    st = di.dense_state(kind, cells, spacing=spacing)
+    kT, tau, n = 0.6, 0.1, 120
+    ref = oracle.step_nvt(st, dt, n, kT, tau)
+    dem, t = pkg.from_state(st, "f64")
+    f = torch.empty((st["N"], 4), dtype=torch.float64, device="cuda")
+    th, l0 = (0.0, 0.0), dem.launch_count()
+    for part in range(3):
+        th, dof = dem.step_nvt(t["pos"], t["quat"], t["vel"], t["angmom"], t["shape_id"], st["box"], dt, n // 3, 0.04,
+                               kT, tau, th, f)
+        row = ref["energies"][(part + 1) * (n // 3)]
+        e = dem.energy(t["quat"], t["vel"], t["angmom"], t["shape_id"], f)
+        assert np.allclose(e, row[:3], rtol=1e-9, atol=1e-9)
+        assert abs(th[0] - row[3]) < 1e-9 and abs(th[1] - row[4]) < 1e-9
+    assert dof == ref["dof"]
+    for k in ("pos", "quat", "vel", "angmom"):
+        assert np.abs(t[k].cpu().numpy() - ref[k]).max() < 1e-8, k
+    assert abs(ref["thermo"][0]) > 1e-2                     # the thermostat acted
+    dem.close()
+
+
+def test_nvt_fp32_reaches_the_target_temperature(pkg):
+    """FP32 context, 4096 cubes of the Table I stand-in.  dxi/dt = (2K - g kT)/Q with xi bounded makes the time average
+    of the kinetic temperature 2K/g equal to the target (a single Nose-Hoover variable oscillates about it), and
+    U + K + Q xi^2/2 + g kT eta stays put while E itself changes by much more."""
+    import torch
+
+    st = di.table1_state("cube", 4096)
+    kT, tau = 1.6, 0.1
+    dem, t = pkg.from_state(st, "f32")
+    f = torch.empty((st["N"], 4), dtype=torch.float32, device="cuda")
+    args = (t["pos"], t["quat"], t["vel"], t["angmom"], t["shape_id"], st["box"], st["dt"])
+    dem.step(*args, 0, 0.3, f)
+    e0 = dem.energy(t["quat"], t["vel"], t["angmom"], t["shape_id"], f)
+    th, temps, cons = (0.0, 0.0), [], []
+    for _ in range(40):
+        th, g = dem.step_nvt(*args, 250, 0.3, kT, tau, th, f)
+        e = dem.energy(t["quat"], t["vel"], t["angmom"], t["shape_id"], f)
+        temps.append(2.0 * (e[1] + e[2]) / g)
+        cons.append(e.sum() + 0.5 * g * kT * tau * tau * th[0] ** 2 + g * kT * th[1])
+    dem.close()
+    n = st["N"]
+    assert g == 3 * (n - 1) + 3 * n
+    assert abs(np.mean(temps) - kT) < 0.06 * kT and min(temps) < kT < max(temps), temps
+    assert np.abs(np.array(cons) - e0.sum()).max() / n < 2e-3, cons
+    assert abs(e.sum() - e0.sum()) / n > 1.0
