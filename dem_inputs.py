@@ -401,6 +401,23 @@ def table1_state(shape, n, seed=0):
     raise ValueError(shape)
 
 
+def fig3_state(kind, seed=0):
+    """Stand-ins for the systems of the paper's short-term energy-conservation test (Fig. 3): "a fluid
+    of squares (with edge length 4.24 sigma) in 2D and tetrahedra (with edge length 8.49 sigma) in 3D ... thermalized at
+    T* = 1"; N, density and state are not given.  Units sigma = epsilon = m = 1, so the rounding radius is 0.5.  Here:
+    32 x 32 squares (circumradius 3) / 8^3 tetrahedra (circumradius 8.49 sqrt(6)/4) on a lattice of spacing
+    2R + 1.2 sigma with random orientations, kT = 1; the caller thermalises with NVE steps."""
+    if kind == "squares":
+        r = 4.24 / math.sqrt(2.0)
+        return lattice_state(2, [regular_polygon(4, r, 0.5)], (32, 32), 2 * r + 1.2, seed=seed, nsteps=0, dt=5e-3,
+                             dtype="f64", name="fig3_squares_N1024")
+    if kind == "tetrahedra":
+        r = 8.49 * math.sqrt(6.0) / 4.0
+        return lattice_state(3, [tetrahedron(r, 0.5)], (8, 8, 8), 2 * r + 1.2, seed=seed, nsteps=0, dt=5e-3,
+                             dtype="f64", name="fig3_tetrahedra_N512")
+    raise ValueError(kind)
+
+
 def dense_state(kind, cells, seed=1, max_angle=0.05, jitter=0.02, spacing=None):
     """P2: dense near-aligned lattices in which many pairs interact through many terms.  Default
     spacings were chosen (with the oracle, offline) so that U/N is a few epsilon: in contact, nothing overlapping.

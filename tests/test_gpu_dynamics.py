@@ -277,3 +277,16 @@ def test_nvt_fp32_reaches_the_target_temperature(pkg):
     assert abs(np.mean(temps) - kT) < 0.06 * kT and min(temps) < kT < max(temps), temps
     assert np.abs(np.array(cons) - e0.sum()).max() / n < 2e-3, cons
     assert abs(e.sum() - e0.sum()) / n > 1.0
+
+
+@pytest.mark.parametrize("kind", ["squares", "tetrahedra"])
+def test_fig3_energy_fluctuations_scale_with_dt_squared(pkg, kind):
+    """PAPER.md:83-85 (Fig. 3): for a second-order integrator sigma(E/N) over a short NVE run grows as dt^2 until rounding
+    saturates it; single precision saturates first.  Stand-in systems of dem_inputs.fig3_state, 4 tau per run."""
+    from paper_1607_02427_b200 import fig3
+
+    st = fig3.thermalise(pkg, di.fig3_state(kind), 5.0)
+    s64 = [fig3.sigma_e(pkg, st, "f64", dt, 4.0)[0] for dt in (1e-3, 2e-3, 4e-3)]
+    assert s64[0] < s64[1] < s64[2] and 6.0 < s64[2] / s64[0] < 45.0, s64     # dt x 4: 16 for dt^2
+    lo32, lo64 = (fig3.sigma_e(pkg, st, p, 1e-4, 0.5, records=50)[0] for p in ("f32", "f64"))
+    assert lo64 < 5e-7 and lo64 < lo32 < 1e-4, (lo32, lo64)
