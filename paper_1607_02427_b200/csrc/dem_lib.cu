@@ -82,6 +82,9 @@ struct dem_ctx {
     int64_t last_terms = 0;
     int sm_count = 148;
     int* h_moved = nullptr;        // pinned host copy of dem_step's flags (moved, halt, steps completed)
+    cudaStream_t copy_stream = nullptr;  // dem_step_host: second H2D stream (velocities, angular momenta)
+    cudaEvent_t ev_copy = nullptr;
+    bool ev_copy_pending = false;
     double nvt_dof = 0;            // degrees of freedom counted by the last dem_step_nvt
     int rebuild_interval = 8;      // steps between the last two neighbour rebuilds of dem_step (sizes its chunks)
 };
@@ -535,7 +538,7 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
         x = ctx->st_pos.as<d4>(); q = ctx->st_quat.as<d4>(); v = ctx->st_vel.as<d4>(); L = ctx->st_ang.as<d4>();
         const void* in[4] = {pos, quat, vel, ang};
         d4* out[4] = {x, q, v, L};
-        for (int k = 0; k < 4; ++k) {
+        for (int k = 0; k < 2; ++k) {  // velocities and angular momenta follow the first evaluation (see below)
             k_f4_to_d4<<<nblk(N, B), B, 0, st>>>(N, static_cast<const f4*>(in[k]), out[k]);
             LAUNCHED(ctx);
         }
@@ -554,6 +557,18 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     for (int a = 0; a < 3; ++a) bx.invL[a] = 1.0 / bx.L[a];
     CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
     CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr)));
+    // The list build and the first evaluation need positions and orientations only: dem_step_host copies velocities
+    // and angular momenta on a second stream meanwhile, and they are waited for (and converted) here.
+    if (ctx->ev_copy_pending) {
+        CU(cudaStreamWaitEvent(st, ctx->ev_copy, 0));
+        ctx->ev_copy_pending = false;
+    }
+    if (conv) {
+        k_f4_to_d4<<<nblk(N, B), B, 0, st>>>(N, static_cast<const f4*>(vel), v);
+        LAUNCHED(ctx);
+        k_f4_to_d4<<<nblk(N, B), B, 0, st>>>(N, static_cast<const f4*>(ang), L);
+        LAUNCHED(ctx);
+    }
     // NVT (R19): k_kinetic + k_thermostat after every completed step advance (xi, eta) by the half step that
     // ends it and the half step that begins the next one; the scaling of v and L is applied by the next k_kick_drift.
     ThermoDev* th = nullptr;
@@ -695,6 +710,8 @@ int dem_destroy(dem_ctx* c) {
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();
     if (c->h_moved) cudaFreeHost(c->h_moved);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->ev_copy) cudaEventDestroy(c->ev_copy);
     for (auto& e : c->ev_pool) {
         cudaEventDestroy(e.mid);
         cudaEventDestroy(e.first);
@@ -901,16 +918,30 @@ int dem_step_host(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, 
     cudaStream_t st = ctx->stream;
     DevBuf* bufs[4] = {&ctx->h_pos, &ctx->h_quat, &ctx->h_vel, &ctx->h_ang};
     void* host[4] = {pos, quat, vel, angmom};
-    for (int k = 0; k < 4; ++k) {
-        CU(bufs[k]->reserve(r4 * N));
-        CU(cudaMemcpyAsync(bufs[k]->p, host[k], r4 * N, cudaMemcpyHostToDevice, st));
+    if (!ctx->copy_stream) {
+        CU(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&ctx->ev_copy, cudaEventDisableTiming));
     }
+    for (int k = 0; k < 4; ++k) CU(bufs[k]->reserve(r4 * N));
     CU(ctx->h_sid.reserve(sizeof(int32_t) * (size_t)N));
+    CU(cudaStreamSynchronize(st));  // the device scratch may still be in use by earlier work of the caller's stream
+    // positions, orientations and shape ids first, on the caller's stream: the list build and the first evaluation
+    // start as soon as they have arrived; velocities and angular momenta travel on a second stream beside them
+    for (int k = 0; k < 2; ++k) CU(cudaMemcpyAsync(bufs[k]->p, host[k], r4 * N, cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(ctx->h_sid.p, shape_id, sizeof(int32_t) * (size_t)N, cudaMemcpyHostToDevice, st));
+    for (int k = 2; k < 4; ++k)
+        CU(cudaMemcpyAsync(bufs[k]->p, host[k], r4 * N, cudaMemcpyHostToDevice, ctx->copy_stream));
+    CU(cudaEventRecord(ctx->ev_copy, ctx->copy_stream));
+    ctx->ev_copy_pending = true;
     CU(ctx->h_force.reserve(r4 * N));
     CU(ctx->h_torque.reserve(r4 * N));
-    CHECK(dem_step(ctx, ctx->h_pos.p, ctx->h_quat.p, ctx->h_vel.p, ctx->h_ang.p, ctx->h_sid.as<int32_t>(), N, box, dt,
-                   nsteps, skin, ctx->h_force.p, ctx->h_torque.p));
+    const int rc = dem_step(ctx, ctx->h_pos.p, ctx->h_quat.p, ctx->h_vel.p, ctx->h_ang.p, ctx->h_sid.as<int32_t>(), N,
+                            box, dt, nsteps, skin, ctx->h_force.p, ctx->h_torque.p);
+    if (rc != DEM_OK) {  // the caller's host arrays must not be in use by a copy when an error is returned
+        cudaStreamSynchronize(ctx->copy_stream);
+        ctx->ev_copy_pending = false;
+        return rc;
+    }
     for (int k = 0; k < 4; ++k) CU(cudaMemcpyAsync(host[k], bufs[k]->p, r4 * N, cudaMemcpyDeviceToHost, st));
     if (force_energy) CU(cudaMemcpyAsync(force_energy, ctx->h_force.p, r4 * N, cudaMemcpyDeviceToHost, st));
     if (torque) CU(cudaMemcpyAsync(torque, ctx->h_torque.p, r4 * N, cudaMemcpyDeviceToHost, st));
