@@ -620,6 +620,8 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
         CU(cudaMemcpyAsync(ctx->h_moved, flags, 3 * sizeof(int), cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
         int done = ctx->h_moved[2];
+        if (done < 0 || done > chunk || (done < chunk && !ctx->h_moved[0]))
+            return fail(ctx, DEM_ECUDA, "dem_step: inconsistent step flags (done %d of %d, moved %d)", done, chunk, ctx->h_moved[0]);
         if (ctx->h_moved[0]) {
             CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
             CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr, nullptr, &ka)));
