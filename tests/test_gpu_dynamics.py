@@ -290,3 +290,15 @@ def test_fig3_energy_fluctuations_scale_with_dt_squared(pkg, kind):
     assert s64[0] < s64[1] < s64[2] and 6.0 < s64[2] / s64[0] < 45.0, s64     # dt x 4: 16 for dt^2
     lo32, lo64 = (fig3.sigma_e(pkg, st, p, 1e-4, 0.5, records=50)[0] for p in ("f32", "f64"))
     assert lo64 < 5e-7 and lo64 < lo32 < 1e-4, (lo32, lo64)
+
+
+def test_config4_fp32_drift_over_ten_thousand_steps(pkg):
+    """north_star's drift bar (< 1e-4 epsilon per particle over 10^4 NVE steps) on the bench workload itself, in the
+    precision and launch configuration bench.py times: config 4, DEM_F32 context, dt = 2e-4, skin 0.3."""
+    st = di.make_config(4)
+    got = _run(pkg, st, "f32", st["dt"], 10000, skin=0.3, chunks=20)
+    e = got["energies"].sum(1)
+    drift = np.abs(e - got["e0"]).max() / st["N"]
+    print("config 4, fp32, 10^4 steps: max |E(t) - E(0)| / N = %.3e" % drift)
+    assert drift < 1e-4, drift
+    assert got["energies"][-1][0] / st["N"] > 0.01          # a fluid in contact by then, not the initial lattice
