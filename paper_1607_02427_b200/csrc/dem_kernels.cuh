@@ -55,9 +55,14 @@ __device__ __forceinline__ d4 load4d(const double* p, int i) {
 
 // Minimum image with the operation order both sides of the bit-exact neighbour test use (R13):
 // d = x_j - x_i; d -= L * rint(d / L), each operation rounded separately (no FMA contraction).
-__device__ __forceinline__ double min_image_1(double xi, double xj, double L) {
+// The quotient is formed as da * (1/L), which lies within 2 ulp of the correctly rounded da / L: unless it is that
+// close to a half-integer (where the division is carried out) both round to the same integer, so the result is the
+// one the definition gives, bit for bit, at the cost of a multiplication instead of an FP64 division.
+__device__ __forceinline__ double min_image_1(double xi, double xj, double L, double invL) {
     const double da = __dsub_rn(xj, xi);
-    const double k = rint(__ddiv_rn(da, L));
+    const double t = __dmul_rn(da, invL);
+    double k = rint(t);
+    if (fabs(fabs(t - k) - 0.5) < 1e-9 * (1.0 + fabs(t))) k = rint(__ddiv_rn(da, L));
     return __dsub_rn(da, __dmul_rn(L, k));
 }
 __device__ __forceinline__ double norm2_fma(double dx, double dy, double dz) {
@@ -179,9 +184,9 @@ __global__ void k_neigh(int N, BoxDev box, GridDev g, double rc2, const int* __r
                 for (int m = b; m < e; ++m) {
                     if (m == s) continue;
                     const d4 xj = xs[m];
-                    const double dx = min_image_1(xi.x, xj.x, box.L[0]);
-                    const double dy = min_image_1(xi.y, xj.y, box.L[1]);
-                    const double dz = box.dim == 3 ? min_image_1(xi.z, xj.z, box.L[2]) : 0.0;
+                    const double dx = min_image_1(xi.x, xj.x, box.L[0], box.invL[0]);
+                    const double dy = min_image_1(xi.y, xj.y, box.L[1], box.invL[1]);
+                    const double dz = box.dim == 3 ? min_image_1(xi.z, xj.z, box.L[2], box.invL[2]) : 0.0;
                     if (norm2_fma(dx, dy, dz) < rc2) {
                         if (cnt < stride) row[cnt] = order[m];
                         ++cnt;
@@ -322,9 +327,9 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
         const int2 ij = a.pairs[p];
         const d4 xi = load4d(static_cast<const PosT*>(a.pos), ij.x), xj = load4d(static_cast<const PosT*>(a.pos), ij.y);
         double d[3];
-        d[0] = min_image_1(xi.x, xj.x, a.box.L[0]);
-        d[1] = min_image_1(xi.y, xj.y, a.box.L[1]);
-        d[2] = DIM == 3 ? min_image_1(xi.z, xj.z, a.box.L[2]) : 0.0;
+        d[0] = min_image_1(xi.x, xj.x, a.box.L[0], a.box.invL[0]);
+        d[1] = min_image_1(xi.y, xj.y, a.box.L[1], a.box.invL[1]);
+        d[2] = DIM == 3 ? min_image_1(xi.z, xj.z, a.box.L[2], a.box.invL[2]) : 0.0;
         real out[10];
 #pragma unroll
         for (int k = 0; k < 10; ++k) out[k] = real(0);
