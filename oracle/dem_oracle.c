@@ -18,9 +18,14 @@
  *   WCA ..................................................... pinned (closed forms of Eq. 3-4, PAPER.md:61 value)
  *   force / torque / virial ................................ pinned (finite differences of U, balances, invariance)
  *   neighbour predicate .................................... pinned (brute force without minimum-image shortcut)
- *   integrator ............................................. pinned (free-rotor invariants, dt^2 order, reversal)
- *   parallel-edge rule ....................... PARITY UNPINNED beyond the exactly-parallel case
- *   per-particle split of U and virial (convention) ........ PARITY UNPINNED (totals are pinned)
+ *   virial tensor, all components and their index order .... pinned (finite-difference shear of an isolated cluster,
+ *                                                            antisymmetric part against the torque balance)
+ *   integrator ............................................. pinned (free-rotor invariants, dt^2 order, reversal;
+ *                                                            asymmetric top against RK4 on Euler's equations)
+ *   parallel-edge rule ....................... PARITY UNPINNED beyond the exactly-parallel case (the
+ *                                                            paper gives no formula); for 0 < angle < 1e-3 only the
+ *                                                            bound r - r_min <= sin(angle) max(L1, L2) is pinned
+ *   per-particle split of U and virial (convention) ........ PARITY UNPINNED (system totals are pinned)
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC dem_oracle.c -o libdem_oracle.so -lm
  */

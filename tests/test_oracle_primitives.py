@@ -115,6 +115,44 @@ def test_parallel_edge_rule(oracle):
     assert br == 0
 
 
+def test_near_parallel_branch_stays_within_its_error_bound(oracle):
+    """PAPER.md:59 gives no formula for 'sufficiently close to parallel' edges; reading R5 takes the midpoints of the
+    overlap intervals.  What mathematics still fixes for 0 < theta < 1e-3: both points lie on their segments, the
+    distance between them is never below the true minimum, and it exceeds it by at most sin(theta) max(L1, L2)
+    (the two lines diverge by at most that much over the overlap)."""
+    rng = np.random.default_rng(21)
+    n = 1601
+    taken = 0
+    for trial in range(200):
+        theta = 10.0 ** rng.uniform(-6, np.log10(0.99e-3))
+        p1 = rng.uniform(-1, 1, 3)
+        u = rng.standard_normal(3)
+        u /= np.linalg.norm(u)
+        w = np.cross(u, rng.standard_normal(3))
+        w /= np.linalg.norm(w)
+        l1, l2 = rng.uniform(0.3, 2.0, 2)
+        q1 = p1 + l1 * u
+        d2 = (np.cos(theta) * u + np.sin(theta) * w) * (1 if trial % 2 else -1)
+        n3 = np.cross(u, w)
+        start = p1 + rng.uniform(-0.5, 0.9) * l1 * u + rng.uniform(0.05, 0.4) * (n3 if trial % 3 else w)
+        p2, q2 = start, start + l2 * d2
+        c1, c2, br = oracle.segment_segment(p1, q1, p2, q2)
+        if br != 1:
+            continue                                       # no overlap: the general routine (pinned above)
+        taken += 1
+        s = np.dot(c1 - p1, q1 - p1) / l1 ** 2
+        t = np.dot(c2 - p2, q2 - p2) / l2 ** 2
+        assert 0 <= s <= 1 and 0 <= t <= 1
+        assert np.allclose(c1, p1 + s * (q1 - p1), atol=1e-13) and np.allclose(c2, p2 + t * (q2 - p2), atol=1e-13)
+        a, b = _seg_points(p1, q1, n), _seg_points(p2, q2, n)
+        brute = np.sqrt(((a[:, None, :] - b[None, :, :]) ** 2).sum(-1).min())
+        r = np.linalg.norm(c1 - c2)
+        h = 0.5 * (l1 + l2) / (n - 1)                      # sampling error of the brute-force minimum
+        assert r >= brute - h - 1e-12
+        assert r - brute <= np.sin(theta) * max(l1, l2) + 1e-12, (trial, theta, r, brute)
+    assert taken > 100
+
+
 def _polygon_samples(poly, n=160):
     """Dense samples of a convex planar polygon: fan triangles sampled on a barycentric grid (incl. boundary)."""
     u = np.linspace(0, 1, n)

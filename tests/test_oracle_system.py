@@ -273,6 +273,48 @@ def test_virial_is_minus_du_dlambda(oracle, kind):
 
 
 @pytest.mark.parametrize("kind", ["cubes", "mixed", "pentagons"])
+def test_virial_off_diagonals_are_minus_du_dshear(oracle, kind):
+    """Pins every component of the virial tensor, off-diagonals and their index order included: for an isolated
+    cluster (huge box: no image involved) sheared as x^a += gamma x^b with orientations fixed,
+    dU/dgamma = sum_i dU/dx_i^a x_i^b = -sum_i F_i^a x_i^b = -sum_pairs r_ij^b F_ij^a = -W^{ba}
+    with W^{ab} = r_ij^a F_ij^b (R12).  Transposing a component (r^b F^a stored as W^{ab}) fails here
+    because F is not central: W is not symmetric.  The lower triangle, which is not stored, is checked against the
+    angular-momentum balance: W^{ab} - W^{ba} = -(sum_i tau_i) . e_c for (a, b, c) cyclic."""
+    st = _dense(kind)
+    st["box"] = st["box"] * 20
+    f, t, w, cnt = oracle.compute(st, use_reject=False)
+    assert cnt[2] > 20 and cnt[4] == 0
+    wsum = w.sum(0)                                        # xx, xy, xz, yy, yz, zz
+    dim = st["dim"]
+    comp = {(0, 0): 0, (0, 1): 1, (0, 2): 2, (1, 1): 3, (1, 2): 4, (2, 2): 5}
+    h = 1e-7
+    scale = np.abs(wsum).max()
+
+    def du_dshear(a, b):                                   # x^a += gamma x^b
+        us = []
+        for g in (+h, -h):
+            p = st["pos"].copy()
+            p[:, a] += g * st["pos"][:, b]
+            us.append(oracle.compute(st, pos=p, use_reject=False)[0][:, 3].sum())
+        return (us[0] - us[1]) / (2 * h)
+
+    asym = 0.0
+    for (a, b), k in comp.items():
+        if a >= dim or b >= dim:
+            continue
+        # stored component W^{ab} (a <= b) is minus the derivative under x^b += gamma x^a
+        assert wsum[k] == pytest.approx(-du_dshear(b, a), abs=3e-6 * scale), (a, b)
+        if a != b:
+            lower = -du_dshear(a, b)                       # W^{ba}
+            c = 3 - a - b
+            sign = 1.0 if (a, b, c) in ((0, 1, 2), (1, 2, 0), (2, 0, 1)) else -1.0
+            # sum_i tau_i = -sum_pairs r_ij x F_ij, and (r x F)_c = sign (r^a F^b - r^b F^a)
+            assert wsum[k] - lower == pytest.approx(-sign * t[:, c].sum(), abs=3e-6 * scale), (a, b)
+            asym = max(asym, abs(wsum[k] - lower))
+    assert asym > 1e-3 * scale                             # the tensor really is asymmetric: a transposition would show
+
+
+@pytest.mark.parametrize("kind", ["cubes", "mixed", "pentagons"])
 def test_momentum_and_angular_momentum_balance(oracle, kind):
     st = _dense(kind)
     # non-periodic cluster: put the same particles in a huge box so that x_i x F_i is meaningful
