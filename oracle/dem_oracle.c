@@ -525,6 +525,133 @@ int orc_compute(const orc_shapes* S, int dim, int N, const double box[3], const 
     return 0;
 }
 
+/*
+ * The same per-particle sums as orc_compute(use_reject = 1), visiting only the particles of the 3^dim adjacent cells of a
+ * plain cell grid (cell width >= the interaction reach R10, so every pair the reject test keeps is found).  The
+ * candidates of a row are sorted by index before they are evaluated, so every sum runs over the same pairs in the same
+ * order as the all-pairs loop and the results are identical bit for bit (tests/test_oracle_system.py).  It exists so
+ * that the full-size configurations (N = 262,144) can be checked row by row in seconds and so that bench.py can time
+ * the oracle's feature work without the O(N) scan per particle; the all-pairs routine above stays the definition.
+ */
+static int cmp_int(const void* a, const void* b) {
+    const int x = *(const int*)a, y = *(const int*)b;
+    return x < y ? -1 : (x > y ? 1 : 0);
+}
+
+int orc_compute_cells(const orc_shapes* S, int dim, int N, const double box[3], const double* pos4, const double* quat4,
+                      const int* sid, double eps, double eps_par, const int* subset, int nsub, double* force4,
+                      double* torque4, double* virial6, int64_t* counters) {
+    const int rows = subset ? nsub : N;
+    double* R = (double*)malloc(sizeof(double) * (size_t)S->nshapes);
+    for (int s = 0; s < S->nshapes; ++s) R[s] = shape_circumradius(S, s);
+    const double rcw = pow(2.0, 1.0 / 6.0);
+    double reach_max = 0.0;
+    for (int a = 0; a < S->nshapes; ++a)
+        for (int b = 0; b < S->nshapes; ++b) {
+            const double r = R[a] + R[b] + rcw * (S->rounding[a] + S->rounding[b]);
+            if (r > reach_max) reach_max = r;
+        }
+    int nc[3] = {1, 1, 1};
+    for (int a = 0; a < dim; ++a) {
+        nc[a] = (int)floor(box[a] / (reach_max * (1.0 + 1e-9)));
+        if (nc[a] < 1) nc[a] = 1;
+        if (nc[a] > 1024) nc[a] = 1024;
+    }
+    const int ncell = nc[0] * nc[1] * nc[2];
+    int* cell_of = (int*)malloc(sizeof(int) * (size_t)N);
+    int* start = (int*)calloc((size_t)ncell + 1, sizeof(int));
+    int* members = (int*)malloc(sizeof(int) * (size_t)N);
+    for (int i = 0; i < N; ++i) {
+        int c[3] = {0, 0, 0};
+        for (int a = 0; a < dim; ++a) {
+            double f = pos4[4 * (size_t)i + a] / box[a] + 0.5;
+            f -= floor(f);
+            int ca = (int)(f * nc[a]);
+            c[a] = ca < 0 ? 0 : (ca >= nc[a] ? nc[a] - 1 : ca);
+        }
+        cell_of[i] = (c[2] * nc[1] + c[1]) * nc[0] + c[0];
+        start[cell_of[i] + 1]++;
+    }
+    for (int c = 0; c < ncell; ++c) start[c + 1] += start[c];
+    {
+        int* fill = (int*)malloc(sizeof(int) * (size_t)ncell);
+        memcpy(fill, start, sizeof(int) * (size_t)ncell);
+        for (int i = 0; i < N; ++i) members[fill[cell_of[i]]++] = i;
+        free(fill);
+    }
+    int64_t c0 = 0, c1 = 0, c2 = 0, c3 = 0, c4 = 0;
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : c0, c1, c2, c3, c4)
+    for (int k = 0; k < rows; ++k) {
+        const int i = subset ? subset[k] : k;
+        int cap = 64, ncand = 0;
+        int* cand = (int*)malloc(sizeof(int) * (size_t)cap);
+        int ci = cell_of[i];
+        const int cx = ci % nc[0];
+        ci /= nc[0];
+        const int cy = ci % nc[1], cz = ci / nc[1];
+        const int nx = nc[0] < 3 ? nc[0] : 3, ny = nc[1] < 3 ? nc[1] : 3, nz = nc[2] < 3 ? nc[2] : 3;
+        for (int iz = 0; iz < nz; ++iz) {
+            const int z = nc[2] < 3 ? iz : (cz + iz - 1 + nc[2]) % nc[2];
+            for (int iy = 0; iy < ny; ++iy) {
+                const int y = nc[1] < 3 ? iy : (cy + iy - 1 + nc[1]) % nc[1];
+                for (int ix = 0; ix < nx; ++ix) {
+                    const int x = nc[0] < 3 ? ix : (cx + ix - 1 + nc[0]) % nc[0];
+                    const int c = (z * nc[1] + y) * nc[0] + x;
+                    for (int m = start[c]; m < start[c + 1]; ++m) {
+                        if (members[m] == i) continue;
+                        if (ncand == cap) {
+                            cap *= 2;
+                            cand = (int*)realloc(cand, sizeof(int) * (size_t)cap);
+                        }
+                        cand[ncand++] = members[m];
+                    }
+                }
+            }
+        }
+        qsort(cand, (size_t)ncand, sizeof(int), cmp_int);
+        double F[3] = {0, 0, 0}, T[3] = {0, 0, 0}, U = 0.0, W[6] = {0, 0, 0, 0, 0, 0};
+        for (int m = 0; m < ncand; ++m) {
+            const int j = cand[m];
+            double d[3];
+            min_image(dim, box, pos4 + 4 * (size_t)i, pos4 + 4 * (size_t)j, d);
+            const double reach = R[sid[i]] + R[sid[j]] + rcw * (S->rounding[sid[i]] + S->rounding[sid[j]]);
+            if (dot3(d, d) >= reach * reach) continue;
+            orc_pair_out o;
+            pair_eval(S, dim, sid[i], sid[j], quat4 + 4 * (size_t)i, quat4 + 4 * (size_t)j, d, eps, eps_par, &o, NULL, 0);
+            for (int a = 0; a < 3; ++a) {
+                F[a] += o.Fi[a];
+                T[a] += o.Ti[a];
+            }
+            U += 0.5 * o.u;
+            for (int a = 0; a < 6; ++a) W[a] += 0.5 * o.W[a];
+            c0 += 1;
+            c1 += o.nterms;
+            c2 += o.nactive;
+            c3 += o.ndegenerate;
+            c4 += o.nparallel;
+        }
+        free(cand);
+        force4[4 * (size_t)k + 0] = F[0];
+        force4[4 * (size_t)k + 1] = F[1];
+        force4[4 * (size_t)k + 2] = F[2];
+        force4[4 * (size_t)k + 3] = U;
+        torque4[4 * (size_t)k + 0] = T[0];
+        torque4[4 * (size_t)k + 1] = T[1];
+        torque4[4 * (size_t)k + 2] = T[2];
+        torque4[4 * (size_t)k + 3] = 0.0;
+        if (virial6)
+            for (int a = 0; a < 6; ++a) virial6[6 * (size_t)k + a] = W[a];
+    }
+    if (counters) {
+        counters[0] = c0; counters[1] = c1; counters[2] = c2; counters[3] = c3; counters[4] = c4;
+    }
+    free(R);
+    free(cell_of);
+    free(start);
+    free(members);
+    return 0;
+}
+
 /* ------------------------------------------------------------------------------------------------------------ */
 /* NVE integrator ("second-order integrator", ref. 23; reading R15)                                  */
 /* ------------------------------------------------------------------------------------------------------------ */
@@ -698,6 +825,109 @@ double orc_step_nvt(const orc_shapes* S, const double* mass, const double* inert
             e[4] = thermo[1];
         }
     }
+    return g;
+}
+
+/*
+ * NPT ("We simulate ... in the NPT ensemble ... a standard Nose-Hoover thermostat
+ * applied to both translational and rotational degrees of freedom, and the barostat computes the pressure from the
+ * virial tensor, just as in MD" (ref. 25)).  The paper gives no equations; reading DESIGN.md R22: the isotropic
+ * Martyna-Tobias-Klein barostat on the box strain rate nu = d ln L / dt, coupled to the CENTRE-OF-MASS motion of the
+ * rigid bodies only (orientations and angular momenta do not feel the box), with the one-variable thermostat of R19:
+ *     dx/dt  = v + nu x                      dL_box/dt = nu L_box     (V = prod_a L_a, dV/dt = d nu V)
+ *     dv/dt  = F/m - (alpha nu + xi) v       alpha = 1 + d / N_f,  N_f = d (N - 1)
+ *     dL/dt  = tau - xi L                    (free rotation as in the NVE step)
+ *     dnu/dt = [alpha 2 K_trans + tr W - d V P_ext] / W_b,   W_b = d N kT tau_P^2,   tr W = sum_i tr W_i = sum_pairs r_ij . F_ij
+ *              (= d V (P_int - P_ext) + (d / N_f) 2 K_trans with P_int = (2 K_trans + tr W) / (d V): "pressure from the virial")
+ *     dxi/dt = (2 K - g kT) / Q,  deta/dt = xi      (R19)
+ * Conserved: U + K + P_ext V + W_b nu^2 / 2 + Q xi^2 / 2 + g kT eta.
+ * One step (palindromic, hence time-reversible and second order), h = dt / 2:
+ *     T(h)  thermostat half step (nvt_half above)
+ *     B(h)  nu += h [alpha 2 K_trans + tr W - d V P_ext] / W_b
+ *     K(h)  s = exp(-alpha nu h / 2);  v = (v s + h F / m) s;  L += h tau
+ *     D(dt) x = x e^{nu dt} + v dt e^{nu dt / 2} sinh(nu dt / 2) / (nu dt / 2);  L_box *= e^{nu dt};  wrap;  free rotation
+ *     force evaluation (with the virial)
+ *     K(h)  B(h)  T(h)
+ * state[3] = (xi, eta, nu), in and out; box[3] in and out.  energies (may be NULL): [(nsteps+1)][8] = U, K_trans,
+ * K_rot, xi, eta, nu, V, tr W.  Returns g.  tau_T = inf gives NPH, tau_P = inf with nu = 0 gives orc_step_nvt.
+ */
+static double sum_trace_virial(int dim, int N, const double* virial6) {
+    double t = 0.0;
+    for (int i = 0; i < N; ++i) {
+        const double* w = virial6 + 6 * (size_t)i;
+        t += w[0] + w[3] + (dim == 3 ? w[5] : 0.0);
+    }
+    return t;
+}
+
+static double box_volume(int dim, const double box[3]) { return dim == 3 ? box[0] * box[1] * box[2] : box[0] * box[1]; }
+
+static void npt_baro_half(int dim, int N, const double* mass, const double* inertia3, const int* sid, const double* quat4,
+                          const double* vel4, const double* ang4, const double* force4, double trW, double V, double h,
+                          double alpha, double P_ext, double Wb, double state[3]) {
+    double e[3];
+    orc_energy(dim, N, mass, inertia3, sid, quat4, vel4, ang4, force4, e);
+    state[2] += h * (alpha * 2.0 * e[1] + trW - dim * V * P_ext) / Wb;
+}
+
+static void npt_kick_half(int dim, int N, const double* mass, const int* sid, double* vel4, double* ang4,
+                          const double* force4, const double* torque4, double dt, double alpha, double nu) {
+    const double s = exp(-alpha * nu * 0.25 * dt);
+    for (int i = 0; i < N; ++i) {
+        const double m = mass[sid[i]];
+        double *v = vel4 + 4 * (size_t)i, *L = ang4 + 4 * (size_t)i;
+        const double *F = force4 + 4 * (size_t)i, *T = torque4 + 4 * (size_t)i;
+        for (int a = 0; a < dim; ++a) v[a] = (v[a] * s + 0.5 * dt * F[a] / m) * s;
+        for (int a = (dim == 2 ? 2 : 0); a < 3; ++a) L[a] += 0.5 * dt * T[a];
+    }
+}
+
+double orc_step_npt(const orc_shapes* S, const double* mass, const double* inertia3, int dim, int N, double box[3],
+                    double* pos4, double* quat4, double* vel4, double* ang4, const int* sid, double eps, double eps_par,
+                    double dt, int nsteps, double kT, double tau_T, double P_ext, double tau_P, double state[3],
+                    double* force4, double* torque4, double* energies) {
+    const double g = nvt_dof(dim, N, inertia3, sid), Q = g * kT * tau_T * tau_T;
+    const double Nf = (double)dim * (N - 1), alpha = 1.0 + dim / Nf, Wb = (double)dim * N * kT * tau_P * tau_P;
+    double* virial6 = (double*)malloc(sizeof(double) * 6 * (size_t)N);
+    orc_compute(S, dim, N, box, pos4, quat4, sid, eps, eps_par, 1, NULL, 0, force4, torque4, virial6, NULL);
+    double trW = sum_trace_virial(dim, N, virial6);
+#define NPT_RECORD(row)                                                                         \
+    do {                                                                                        \
+        if (energies) {                                                                         \
+            double* e_ = energies + 8 * (size_t)(row);                                          \
+            orc_energy(dim, N, mass, inertia3, sid, quat4, vel4, ang4, force4, e_);             \
+            e_[3] = state[0]; e_[4] = state[1]; e_[5] = state[2];                               \
+            e_[6] = box_volume(dim, box); e_[7] = trW;                                          \
+        }                                                                                       \
+    } while (0)
+    NPT_RECORD(0);
+    for (int step = 1; step <= nsteps; ++step) {
+        nvt_half(dim, N, mass, inertia3, sid, quat4, vel4, ang4, force4, dt, g, kT, Q, state);
+        npt_baro_half(dim, N, mass, inertia3, sid, quat4, vel4, ang4, force4, trW, box_volume(dim, box), 0.5 * dt,
+                      alpha, P_ext, Wb, state);
+        const double nu = state[2];
+        npt_kick_half(dim, N, mass, sid, vel4, ang4, force4, torque4, dt, alpha, nu);
+        /* drift: exact flow of dx/dt = v + nu x at constant v and nu */
+        const double z = 0.5 * nu * dt, ea = exp(nu * dt), eh = exp(z), sc = (z == 0.0) ? 1.0 : sinh(z) / z;
+        for (int a = 0; a < dim; ++a) box[a] *= ea;
+        for (int i = 0; i < N; ++i) {
+            double *x = pos4 + 4 * (size_t)i, *v = vel4 + 4 * (size_t)i;
+            for (int a = 0; a < dim; ++a) {
+                x[a] = x[a] * ea + v[a] * (dt * eh * sc);
+                x[a] -= box[a] * rint(x[a] / box[a]);
+            }
+            free_rotate(dim, inertia3 + 3 * sid[i], ang4 + 4 * (size_t)i, dt, quat4 + 4 * (size_t)i);
+        }
+        orc_compute(S, dim, N, box, pos4, quat4, sid, eps, eps_par, 1, NULL, 0, force4, torque4, virial6, NULL);
+        trW = sum_trace_virial(dim, N, virial6);
+        npt_kick_half(dim, N, mass, sid, vel4, ang4, force4, torque4, dt, alpha, nu);
+        npt_baro_half(dim, N, mass, inertia3, sid, quat4, vel4, ang4, force4, trW, box_volume(dim, box), 0.5 * dt,
+                      alpha, P_ext, Wb, state);
+        nvt_half(dim, N, mass, inertia3, sid, quat4, vel4, ang4, force4, dt, g, kT, Q, state);
+        NPT_RECORD(step);
+    }
+#undef NPT_RECORD
+    free(virial6);
     return g;
 }
 

@@ -47,7 +47,7 @@ def lib():
         _lib = C.CDLL(build())
         _lib.orc_point_segment.restype = C.c_double
         for name in ("orc_segment_segment", "orc_point_polygon", "orc_pair_terms", "orc_neighbors", "orc_compute",
-                     "orc_step", "orc_num_threads"):
+                     "orc_compute_cells", "orc_step", "orc_num_threads"):
             getattr(_lib, name).restype = C.c_int
         _lib.orc_wca.restype = None
         _lib.orc_energy.restype = None
@@ -161,8 +161,10 @@ def _check_min_image(state, tab):
         raise ValueError("box edge %s < 2 x interaction reach %g: minimum image invalid" % (box, reach))
 
 
-def compute(state, subset=None, use_reject=True, eps_par=DEFAULT_EPS_PAR, pos=None, quat=None):
-    """Per-particle force+energy (rows,4), torque (rows,4), virial (rows,6), counters(5) by the definition."""
+def compute(state, subset=None, use_reject=True, eps_par=DEFAULT_EPS_PAR, pos=None, quat=None, cells=False):
+    """Per-particle force+energy (rows,4), torque (rows,4), virial (rows,6), counters(5) by the definition.
+    cells=True: orc_compute_cells, the same sums over the same pairs in the same order (bit-identical to the all-pairs
+    loop with the exact reject), found through a plain cell grid instead of an O(N) scan per particle."""
     tab = state.get("_tab") or ShapeTable(state["shapes"])
     pos = _f64(state["pos"] if pos is None else pos)
     quat = _f64(state["quat"] if quat is None else quat)
@@ -173,6 +175,13 @@ def compute(state, subset=None, use_reject=True, eps_par=DEFAULT_EPS_PAR, pos=No
     f, t, w = np.zeros((rows, 4)), np.zeros((rows, 4)), np.zeros((rows, 6))
     cnt = np.zeros(5, dtype=np.int64)
     sid = np.ascontiguousarray(state["shape_id"], dtype=np.int32)
+    if cells:
+        if not use_reject:
+            raise ValueError("the cell grid only finds pairs inside the interaction reach: use_reject must stay on")
+        lib().orc_compute_cells(C.byref(tab.c), C.c_int(state["dim"]), C.c_int(n), _p(_f64(state["box"])), _p(pos),
+                                _p(quat), _p(sid), C.c_double(state["epsilon"]), C.c_double(eps_par), _p(sub),
+                                C.c_int(rows), _p(f), _p(t), _p(w), _p(cnt))
+        return f, t, w, cnt
     lib().orc_compute(C.byref(tab.c), C.c_int(state["dim"]), C.c_int(n), _p(_f64(state["box"])), _p(pos), _p(quat),
                       _p(sid), C.c_double(state["epsilon"]), C.c_double(eps_par), C.c_int(1 if use_reject else 0),
                       _p(sub), C.c_int(rows), _p(f), _p(t), _p(w), _p(cnt))
@@ -211,6 +220,27 @@ def step_nvt(state, dt, nsteps, kT, tau, thermo=(0.0, 0.0), eps_par=DEFAULT_EPS_
            _p(pos), _p(quat), _p(vel), _p(ang), _p(sid), C.c_double(state["epsilon"]), C.c_double(eps_par),
            C.c_double(dt), C.c_int(nsteps), C.c_double(kT), C.c_double(tau), _p(th), _p(f), _p(t), _p(en))
     return dict(pos=pos, quat=quat, vel=vel, angmom=ang, force=f, torque=t, energies=en, thermo=th, dof=g)
+
+
+def step_npt(state, dt, nsteps, kT, tau, pressure, tau_p, baro=(0.0, 0.0, 0.0), eps_par=DEFAULT_EPS_PAR):
+    """Nose-Hoover + MTK NPT integration of a COPY of the state (orc_step_npt; R22).  Returns dict(pos, quat,
+    vel, angmom, box, force, torque, energies [nsteps+1][8] = U, K_trans, K_rot, xi, eta, nu, V, tr W, baro = final
+    (xi, eta, nu), dof = g)."""
+    tab = state.get("_tab") or ShapeTable(state["shapes"])
+    pos, quat = _f64(state["pos"]).copy(), _f64(state["quat"]).copy()
+    vel, ang = _f64(state["vel"]).copy(), _f64(state["angmom"]).copy()
+    box = _f64(state["box"]).copy()
+    n = len(pos)
+    f, t = np.zeros((n, 4)), np.zeros((n, 4))
+    en = np.zeros((nsteps + 1, 8))
+    b = np.array(baro, dtype=np.float64)
+    sid = np.ascontiguousarray(state["shape_id"], dtype=np.int32)
+    fn = lib().orc_step_npt
+    fn.restype = C.c_double
+    g = fn(C.byref(tab.c), _p(tab.mass), _p(tab.inertia), C.c_int(state["dim"]), C.c_int(n), _p(box), _p(pos), _p(quat),
+           _p(vel), _p(ang), _p(sid), C.c_double(state["epsilon"]), C.c_double(eps_par), C.c_double(dt), C.c_int(nsteps),
+           C.c_double(kT), C.c_double(tau), C.c_double(pressure), C.c_double(tau_p), _p(b), _p(f), _p(t), _p(en))
+    return dict(pos=pos, quat=quat, vel=vel, angmom=ang, box=box, force=f, torque=t, energies=en, baro=b, dof=g)
 
 
 def energy(state, force):

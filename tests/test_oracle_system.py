@@ -346,6 +346,30 @@ def test_reject_shortcut_changes_nothing(oracle):
     assert a[3][2] == b[3][2]
 
 
+def test_cell_grid_variant_is_the_all_pairs_sum_bit_for_bit(oracle):
+    """orc_compute_cells against the definition (the all-pairs loop with the exact reject): identical bits for force,
+    torque, energy, virial and counters, on dense lattices, a mixed-shape state, boxes with fewer than three cells
+    along an axis, a shuffled random fluid with particles outside the box, and a row subset."""
+    rng = np.random.default_rng(3)
+    states = [_dense("cubes"), _dense("mixed"), _dense("pentagons"), di.dense_state("cubes", 6), di.make_config(2, scale=2)]
+    gas = di.lattice_state(3, [di.octahedron(0.5, 0.075), di.tetrahedron(0.5, 0.05)], (7, 5, 3), 1.25, seed=9,
+                           jitter=0.12, shape_fractions=(0.4, 0.6))
+    perm = rng.permutation(gas["N"])
+    for k in ("pos", "quat", "shape_id"):
+        gas[k] = gas[k][perm]
+    gas["pos"][::3, :3] += gas["box"] * rng.integers(-2, 3, (len(gas["pos"][::3]), 3))   # images outside the box
+    states.append(gas)
+    for st in states:
+        a = oracle.compute(st)
+        b = oracle.compute(st, cells=True)
+        assert a[3][0] > 0
+        for x, y in zip(a, b):
+            assert np.array_equal(x, y)
+        sub = rng.choice(st["N"], 9, replace=False).astype(np.int32)
+        c = oracle.compute(st, subset=sub, cells=True)
+        assert np.array_equal(c[0], a[0][sub]) and np.array_equal(c[1], a[1][sub]) and np.array_equal(c[2], a[2][sub])
+
+
 @pytest.mark.parametrize("kind", ["cubes", "pentagons"])
 def test_translation_and_rotation_invariance(oracle, kind):
     st = _dense(kind)
