@@ -276,8 +276,8 @@ def main():
     def timed(nwarm, nsteps, sample_clocks):
         """nwarm untimed + nsteps timed steps; (ms, clocks, launches, pair-kernel launches, their ms, counters)."""
         step(nwarm)
-        dem.set_timing(True)
-        dem.kernel_time()
+        dem.set_timing(1)
+        dem.kernel_times()
         l0 = dem.launch_count()
         sampler = ClockSampler(local) if (rank == 0 and sample_clocks) else None
         barrier()
@@ -289,10 +289,11 @@ def main():
         ms = e0.elapsed_time(e1)
         clk = sampler.stop() if sampler else None
         nl = dem.launch_count() - l0
-        npl, pms, qms = dem.kernel_time_split()   # pair-feature kernel alone, pose kernel in front of it
+        kt = dem.kernel_times()
+        npl, pms, qms = kt["pair"][0], kt["pair"][1], kt["pose"][1]   # pair-feature kernel alone, pose kernel in front of it
         tot = dem.swept_totals()
         tot["pose_ms"] = qms
-        dem.set_timing(False)
+        dem.set_timing(0)
         return max_over_ranks(ms, world, "cuda"), clk, nl, npl, pms, dem.get_counters(), tot
 
     def swept_flops(tot):

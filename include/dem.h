@@ -201,29 +201,7 @@ int dem_set_pair_kernel(dem_ctx* ctx, int which);
  * dem_compute / dem_step. */
 int dem_set_culling(dem_ctx* ctx, int enabled);
 
-/* Benchmark hygiene: when bytes > 0, dem_step overwrites a scratch buffer of that size (larger than the 126 MB L2)
- * before every time step, so that no step finds its inputs cached by the previous one.  0 (default) = off. */
-int dem_set_l2_flush(dem_ctx* ctx, int64_t bytes);
-
-/* Kernel-time accounting for bench.py: when enabled, every launch of the pair-feature kernel is bracketed by CUDA
- * events on the context's stream; dem_kernel_time returns (and resets) the number of bracketed launches and their
- * summed duration in milliseconds (synchronises). */
-int dem_set_timing(dem_ctx* ctx, int enabled);
-int dem_kernel_time(dem_ctx* ctx, int64_t* launches, double* total_ms);
-/* The same, split: *pair_ms = the pair-feature kernels alone (k_pair_fast / k_pair_cull / k_pair), *pose_ms = the pose
- * kernel in front of them (k_pose; 0 for the generic kernel, which forms the pose itself).  dem_kernel_time returns
- * their sum.  Either call resets the bracket list. */
-int dem_kernel_time_split(dem_ctx* ctx, int64_t* launches, double* pair_ms, double* pose_ms);
-/* While timing is enabled the packed search kernels' swept-term counters (dem_get_counters out[7], out[6] - out[7],
- * out[8]) are also summed over all evaluations since dem_set_timing(ctx, 1): out[0] edge-edge terms (2D: vertex-edge
- * terms), out[1] vertex-face terms, out[2] face boundary-edge tests.  HOST int64[3]; synchronises. */
-int dem_swept_totals(dem_ctx* ctx, int64_t out[3]);
-/* Number of kernels the library has launched on this context since creation (all kernels). */
-int64_t dem_launch_count(const dem_ctx* ctx);
-
-/* FP32 FMA-chain microbenchmark (roofline denominator): runs `iters` dependent-chain FFMA iterations on
- * every SM and returns the achieved FP32 TFLOP/s (2 flop per FMA); synchronises. */
-int dem_fp32_peak(dem_ctx* ctx, int iters, double* tflops);
+/* Measurement hooks (L2 flush, kernel-time accounting, launch count, FMA microbenchmark) live in dem_bench.h. */
 
 const char* dem_version(void);
 

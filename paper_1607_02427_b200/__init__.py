@@ -3,5 +3,5 @@
 The product is the C-ABI CUDA library libdem_b200.so (include/dem.h, sources in csrc/).  This package holds its
 in-tree build step (build.py) and a thin ctypes binding (binding.py).  There is no CPU implementation here.
 """
-from .binding import (DEM_F32, DEM_F64, DEM_OK, EXPORTS, Dem, DemError, from_state, lib)  # noqa: F401
+from .binding import (DEM_F32, DEM_F64, DEM_OK, EXPORTS, EXPORTS_BENCH, Dem, DemError, from_state, lib)  # noqa: F401
 from . import build  # noqa: F401  (module: build.build() compiles the library)

@@ -21,8 +21,10 @@ STATUS_NAMES = {0: "DEM_OK", -1: "DEM_EINVAL", -2: "DEM_ENOMEM", -3: "DEM_ECUDA"
 # every symbol include/dem.h declares (tests check that the built library exports all of them)
 EXPORTS = ["dem_create", "dem_destroy", "dem_last_error", "dem_set_eps_par", "dem_create_shape", "dem_build_neighbors",
            "dem_get_neighbors", "dem_copy_neighbors", "dem_compute", "dem_get_counters", "dem_step", "dem_step_nvt", "dem_energy",
-           "dem_compute_host", "dem_step_host", "dem_set_slices", "dem_set_pair_kernel", "dem_set_culling", "dem_set_l2_flush", "dem_set_timing", "dem_kernel_time", "dem_kernel_time_split", "dem_swept_totals",
-           "dem_launch_count", "dem_fp32_peak", "dem_version"]
+           "dem_compute_host", "dem_step_host", "dem_set_slices", "dem_set_pair_kernel", "dem_set_culling", "dem_version"]
+# include/dem_bench.h (measurement hooks)
+EXPORTS_BENCH = ["dem_set_l2_flush", "dem_set_timing", "dem_kernel_times", "dem_swept_totals", "dem_launch_count",
+                 "dem_fp32_peak"]
 
 _lib = None
 
@@ -34,17 +36,25 @@ class DemError(RuntimeError):
 
 
 def lib():
-    """Load libdem_b200.so (built in-tree by build.py).  Fails loudly if it is not there."""
+    """Load libdem_b200.so (built in-tree by build.py).  A library that is missing or was built from other sources than
+    the ones in the tree is rebuilt first; if that is impossible the call fails loudly (there is no CPU fallback)."""
     global _lib
     if _lib is None:
         path = _build.LIB
-        if not os.path.exists(path):
-            raise ImportError("libdem_b200.so has not been built (run `python -m paper_1607_02427_b200.build` or "
-                              "__graft_entry__.build()); there is no CPU fallback")
+        if _build.stale():
+            try:
+                _build.build()
+            except Exception as e:  # no nvcc, compile error: never fall back to anything else
+                raise ImportError("libdem_b200.so is missing or older than its sources and could not be rebuilt (%s); "
+                                  "there is no CPU fallback" % e)
         _lib = C.CDLL(path)
         _lib.dem_last_error.restype = C.c_char_p
         _lib.dem_version.restype = C.c_char_p
         _lib.dem_launch_count.restype = C.c_int64
+        want = _build.source_hash()
+        if want not in _lib.dem_version().decode():
+            raise ImportError("libdem_b200.so reports '%s' but the sources hash to %s: rebuild with "
+                              "`python -m paper_1607_02427_b200.build`" % (_lib.dem_version().decode(), want))
     return _lib
 
 
@@ -132,8 +142,9 @@ class Dem:
     def set_l2_flush(self, nbytes):
         _check(self._ctx, lib().dem_set_l2_flush(self._ctx, C.c_int64(nbytes)))
 
-    def set_timing(self, enabled):
-        _check(self._ctx, lib().dem_set_timing(self._ctx, C.c_int(1 if enabled else 0)))
+    def set_timing(self, level):
+        """0 off, 1 pose + pair kernels, 2 every kernel of a step (include/dem_bench.h)."""
+        _check(self._ctx, lib().dem_set_timing(self._ctx, C.c_int(int(level))))
 
     # ---- dem_create_shape ----------------------------------------------------------------------------------------
     def create_shape(self, verts, faces=(), edges=None, rounding=0.1, mass=1.0, inertia=(1.0, 1.0, 1.0)):
@@ -267,15 +278,13 @@ class Dem:
         _check(self._ctx, rc)
 
     # ---- accounting ------------------------------------------------------------------------------------------------------
-    def kernel_time(self):
-        n, ms = C.c_int64(), C.c_double()
-        _check(self._ctx, lib().dem_kernel_time(self._ctx, C.byref(n), C.byref(ms)))
-        return n.value, ms.value
+    KERNEL_KINDS = ("pose", "pair", "reduce", "kick_drift", "neigh", "build", "flush", "other")
 
-    def kernel_time_split(self):
-        n, pair, pose = C.c_int64(), C.c_double(), C.c_double()
-        _check(self._ctx, lib().dem_kernel_time_split(self._ctx, C.byref(n), C.byref(pair), C.byref(pose)))
-        return n.value, pair.value, pose.value
+    def kernel_times(self):
+        """dem_kernel_times: {kind: (launches, ms)} since the last call."""
+        n, ms = (C.c_int64 * 8)(), (C.c_double * 8)()
+        _check(self._ctx, lib().dem_kernel_times(self._ctx, n, ms))
+        return {k: (n[i], ms[i]) for i, k in enumerate(self.KERNEL_KINDS)}
 
     def launch_count(self):
         return int(lib().dem_launch_count(self._ctx))

@@ -86,7 +86,7 @@ __device__ __forceinline__ unsigned q_entry(int owner, int phase, int outer, int
 // degenerate, parallel).  sp: the warp's staged pose records [6][32] (plane-major, indexed by owner lane); the
 // evaluating lane reads its owner's pose from there.
 // Contributions are added to the owner in queue order, so the result does not depend on scheduling.
-__device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* q, float* sacc, unsigned* scnt, int cnt, int qn,
+static __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* q, float* sacc, unsigned* scnt, int cnt, int qn,
                                          const f4* sp, int nown) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
@@ -389,24 +389,6 @@ __device__ __forceinline__ void sweep_faces(const ShapeView<float>& S, const Sha
 // class's work list (block slices padded to whole warps: see below); pairs beyond it get their zero result records here and never reach the search kernel, so its warps carry 32
 // live pairs each.  Pose record, plane-major for coalesced loads: [6][npairs] float4 =
 // (R0 R1 R2 R3) (R4 R5 R6 R7) (R8 t0 t1 t2) (M0 M1 M2 M3) (M4 M5 M6 M7) (M8 dx dy dz); pidx[c] = the pair's index.
-struct PoseArgs {
-    const int2* pairs;
-    int npairs, slices;
-    const void* pos;
-    const void* quat;
-    BoxDev box;
-    double reach2;
-    f4* pose;
-    int* pidx;
-    int* count;  // entries of this class's work list, padding included (zeroed before the launch)
-    size_t plane;  // stride of the pose planes = capacity of the work list (pairs + 64 per k_pose block)
-    int pad;       // entries per warp tile of the kernel that follows: 32 (k_pair_fast) or 64 (k_pair_cull)
-    unsigned long long* counters;  // [0] += pairs inside the reach
-    f4* rec;
-    const int* skip;  // dem_step: non-null and *skip != 0 => the list is stale, the kernel does nothing (see step_t)
-};
-
-#define DEM_POSE_THREADS 512
 template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THREADS) k_pose(const PoseArgs a) {
     __shared__ int wcount[DEM_POSE_THREADS / 32], s_prefix;
     if (a.skip && *a.skip) return;  // the work-list count stays 0: the search kernel behind finds no tile
@@ -475,17 +457,10 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THR
     }
 }
 
-#ifdef DEM_TUNE
-__device__ int g_dbg_phases = 7;  // tuning builds only: bit 0 = edge-edge, bit 1 = vertex-face (own), bit 2 = vertex-face (other)
-#define DEM_DBG_PHASE(bit) (g_dbg_phases & (bit))
-#else
-#define DEM_DBG_PHASE(bit) true
-#endif
-
 // ---- the kernel ---------------------------------------------------------------------------------------------------------
 // One warp = 32 consecutive (pair, slice) items of one pair class (same shapes, same loop bounds).  TE / TV = packed
 // outer pairs per sweep for edges / vertices (2 TE outer edges, 2 TV outer vertices share every inner-feature load).
-template <typename PosT, int DIM, int TE, int TV, int MINB>
+template <int DIM, int TE, int TV, int MINB>
 __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     FastShared* fs = reinterpret_cast<FastShared*>(smem_raw);
@@ -597,7 +572,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
             if (DIM == 3) {
                 const int oE = B.ne, oV = B.ne + B.nv;
                 // (1) first sum of Eq. 1: edges of j (outer, packed) against edges of i (inner)
-                for (int l0 = ob, le = DEM_DBG_PHASE(1) ? min(oe, oE) : 0; l0 < le; l0 += 2 * TE) {
+                for (int l0 = ob, le = min(oe, oE); l0 < le; l0 += 2 * TE) {
                     for (int k0 = 0; k0 < A.ne; k0 += 32) {
                         u64 np2x[TE], np2y[TE], np2z[TE], d2x[TE], d2y[TE], d2z[TE], g[TE];
                         float Llo[TE], Lhi[TE];
@@ -636,7 +611,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
                     }
                 }
                 // (2) third sum of Eq. 1: vertices of j (outer, packed, i's frame) against faces of i
-                for (int o0 = max(ob, oE) - oE, on = DEM_DBG_PHASE(2) ? min(oe, oV) - oE : 0; o0 < on; o0 += 2 * TV) {
+                for (int o0 = max(ob, oE) - oE, on = min(oe, oV) - oE; o0 < on; o0 += 2 * TV) {
                     for (int f0 = 0; f0 < A.nf; f0 += 32) {
                         u64 px[TV], py[TV], pz[TV];
 #pragma unroll
@@ -661,7 +636,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
                     }
                 }
                 // (3) second sum of Eq. 1: vertices of i (outer, packed, j's frame) against faces of j
-                for (int o0 = max(ob, oV) - oV, on = DEM_DBG_PHASE(4) ? min(oe, oV + A.nv) - oV : 0; o0 < on; o0 += 2 * TV) {
+                for (int o0 = max(ob, oV) - oV, on = min(oe, oV + A.nv) - oV; o0 < on; o0 += 2 * TV) {
                     for (int f0 = 0; f0 < B.nf; f0 += 32) {
                         u64 px[TV], py[TV], pz[TV];
 #pragma unroll
@@ -911,7 +886,7 @@ __device__ __forceinline__ void write_items(CullCtx& cc, unsigned mask, int owne
         write_items(cc, m_, (OWNER), (O0), (FLAG), off_, tot_);                           \
     } while (0)
 
-template <typename PosT, int MINB, bool SAME>  // SAME: both particles of the class have the same shape
+template <int MINB, bool SAME>  // SAME: both particles of the class have the same shape
 __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a) {
     // a warp tile is 64 pairs (two per lane: owner slots lane and lane + 32), so that the item passes run fuller
     extern __shared__ __align__(16) unsigned char smem_raw[];

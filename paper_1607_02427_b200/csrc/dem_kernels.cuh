@@ -1,42 +1,15 @@
 // dem_kernels.cuh -- the CUDA kernels of libdem_b200 (sm_100a).  Host orchestration is in dem_lib.cu.
 //
-//   a2  cell list + neighbour list      k_bin, k_scan*, k_place, k_sort_cells, k_gather_sorted, k_neigh
-//       unique-pair work list           k_pair_count, k_pair_fill, k_slot_back
 //   a3-a7 pair-feature kernel           k_pair          (FP32-ALU bound; dem_math.cuh holds the arithmetic)
 //   a8  per-particle reduction          k_reduce        (warp-shuffle over 4 lanes per particle, no atomics)
-//   a9  NVE integrator                  k_kick_drift, k_kick, k_energy
+// The neighbour-list kernels (a2) are in dem_list.cuh, the integrator (a9) in dem_integrate.cuh, the packed FP32 search
+// kernels in dem_fast.cuh.
 #pragma once
 #include <cuda_runtime.h>
 
 #include "dem_math.cuh"
 
 namespace dem {
-
-#define DEM_MAX_SHAPES_K 8
-#define DEM_REC 3  // real4 per pair result record
-#define DEM_MAX_CLASSES (DEM_MAX_SHAPES_K * (DEM_MAX_SHAPES_K + 1) / 2)
-
-#define DEM_MAX_FACE_GROUPS 4
-struct ShapeDev {
-    int nv, ne, nf, nfe;
-    int off, len;  // block [off, off+len) of the device table, in real4 units: V | E | F | FE | OE
-    // runs of faces with equal boundary-edge counts (faces are stored sorted by that count): grp_n[g] faces with
-    // grp_m[g] edges each; grp_n = 0 ends the list; grp_m[0] = 0 means "more runs than fit: read each face's header"
-    int grp_m[DEM_MAX_FACE_GROUPS], grp_n[DEM_MAX_FACE_GROUPS];
-};
-
-struct ClassTable {  // indexed by pair class c = lut[s_a][s_b]
-    signed char lut[DEM_MAX_SHAPES_K][DEM_MAX_SHAPES_K];
-    int pair_base[DEM_MAX_CLASSES + 1];  // first global pair index of the class (class-major pair list)
-    int rec_base[DEM_MAX_CLASSES + 1];   // first result record of the class
-    int slices[DEM_MAX_CLASSES];         // result records per pair
-};
-
-struct BoxDev {
-    double L[3];
-    double invL[3];  // 1 / L (the bit-exact neighbour predicate R13 divides by L; everything else multiplies)
-    int dim;
-};
 
 // ---- loads --------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ d4 load4d(const float* p, int i) {
@@ -69,236 +42,7 @@ __device__ __forceinline__ double norm2_fma(double dx, double dy, double dz) {
     return __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
 }
 
-// ---- a2: cell list --------------------------------------------------------------------------------------------------
-struct GridDev {
-    int nc[3];
-    int ncell;
-};
-
-template <typename PosT>
-__global__ void k_bin(const PosT* __restrict__ pos, int N, BoxDev box, GridDev g, int* __restrict__ cell_of,
-                      int* __restrict__ cell_cnt, int* __restrict__ rank) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    const d4 x = load4d(pos, i);
-    const double xs[3] = {x.x, x.y, x.z};
-    int c[3] = {0, 0, 0};
-    for (int a = 0; a < box.dim; ++a) {
-        double f = xs[a] / box.L[a] + 0.5;
-        f -= floor(f);
-        int ca = (int)(f * g.nc[a]);
-        c[a] = min(max(ca, 0), g.nc[a] - 1);
-    }
-    const int cell = (c[2] * g.nc[1] + c[1]) * g.nc[0] + c[0];
-    cell_of[i] = cell;
-    rank[i] = atomicAdd(&cell_cnt[cell], 1);
-}
-
-// exclusive scan of int data[n] in place, blocks of 1024; block totals to sums[blockIdx]
-__global__ void k_scan_block(int* __restrict__ data, int n, int* __restrict__ sums) {
-    __shared__ int warp_tot[32];
-    const int i = blockIdx.x * 1024 + threadIdx.x;
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int v = i < n ? data[i] : 0;
-    int x = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int y = __shfl_up_sync(0xffffffffu, x, o);
-        if (lane >= o) x += y;
-    }
-    if (lane == 31) warp_tot[w] = x;
-    __syncthreads();
-    if (w == 0) {
-        int t = warp_tot[lane];
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int y = __shfl_up_sync(0xffffffffu, t, o);
-            if (lane >= o) t += y;
-        }
-        warp_tot[lane] = t;
-    }
-    __syncthreads();
-    const int base = w ? warp_tot[w - 1] : 0;
-    if (i < n) data[i] = base + x - v;
-    if (threadIdx.x == 1023 && sums) sums[blockIdx.x] = base + x;
-}
-__global__ void k_scan_add(int* __restrict__ data, int n, const int* __restrict__ sums) {
-    const int i = blockIdx.x * 1024 + threadIdx.x;
-    if (i < n) data[i] += sums[blockIdx.x];
-}
-
-__global__ void k_place(int N, const int* __restrict__ cell_of, const int* __restrict__ rank,
-                        const int* __restrict__ cell_start, int* __restrict__ order) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < N) order[cell_start[cell_of[i]] + rank[i]] = i;
-}
-
-// The atomic ranks above depend on scheduling; sorting each cell's few members by particle index makes the cell
-// list, hence the neighbour rows, the pair list and every summation order, identical from run to run.
-__global__ void k_sort_cells(int ncell, const int* __restrict__ cell_start, int* __restrict__ order) {
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= ncell) return;
-    const int b = cell_start[c], e = cell_start[c + 1];
-    for (int m = b + 1; m < e; ++m) {
-        const int v = order[m];
-        int k = m - 1;
-        while (k >= b && order[k] > v) {
-            order[k + 1] = order[k];
-            --k;
-        }
-        order[k + 1] = v;
-    }
-}
-
-template <typename PosT>
-__global__ void k_gather_sorted(const PosT* __restrict__ pos, int N, const int* __restrict__ order, d4* __restrict__ xs) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s < N) xs[s] = load4d(pos, order[s]);
-}
-
-// One thread per particle (in cell order, so a warp's candidate cells overlap in L1/L2).  Candidates from the
-// 3^dim adjacent cells; the predicate is the definition (R13) in double.  Rows are written for the ORIGINAL index.
-__global__ void k_neigh(int N, BoxDev box, GridDev g, double rc2, const int* __restrict__ order,
-                        const int* __restrict__ cell_of, const int* __restrict__ cell_start, const d4* __restrict__ xs,
-                        int stride, int* __restrict__ counts, int* __restrict__ list, int* __restrict__ max_count) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
-    const int i = order[s];
-    const d4 xi = xs[s];
-    int cell = cell_of[i];
-    const int cx = cell % g.nc[0];
-    cell /= g.nc[0];
-    const int cy = cell % g.nc[1], cz = cell / g.nc[1];
-    // per axis: all cells if there are fewer than 3, else the three adjacent ones (wrapped)
-    const int nx = g.nc[0] < 3 ? g.nc[0] : 3, ny = g.nc[1] < 3 ? g.nc[1] : 3, nz = g.nc[2] < 3 ? g.nc[2] : 3;
-    int cnt = 0;
-    int* row = list + (size_t)i * stride;
-    for (int iz = 0; iz < nz; ++iz) {
-        const int z = g.nc[2] < 3 ? iz : (cz + iz - 1 + g.nc[2]) % g.nc[2];
-        for (int iy = 0; iy < ny; ++iy) {
-            const int y = g.nc[1] < 3 ? iy : (cy + iy - 1 + g.nc[1]) % g.nc[1];
-            for (int ix = 0; ix < nx; ++ix) {
-                const int x = g.nc[0] < 3 ? ix : (cx + ix - 1 + g.nc[0]) % g.nc[0];
-                const int c2 = (z * g.nc[1] + y) * g.nc[0] + x;
-                const int b = cell_start[c2], e = cell_start[c2 + 1];
-                for (int m = b; m < e; ++m) {
-                    if (m == s) continue;
-                    const d4 xj = xs[m];
-                    const double dx = min_image_1(xi.x, xj.x, box.L[0], box.invL[0]);
-                    const double dy = min_image_1(xi.y, xj.y, box.L[1], box.invL[1]);
-                    const double dz = box.dim == 3 ? min_image_1(xi.z, xj.z, box.L[2], box.invL[2]) : 0.0;
-                    if (norm2_fma(dx, dy, dz) < rc2) {
-                        if (cnt < stride) row[cnt] = order[m];
-                        ++cnt;
-                    }
-                }
-            }
-        }
-    }
-    counts[i] = cnt;
-    if (cnt > 0) atomicMax(max_count, cnt);
-}
-
-__global__ void k_copy_rows(int N, const int* __restrict__ counts, const int* __restrict__ list, int stride,
-                            int* __restrict__ out, int out_stride) {
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= (long long)N * out_stride) return;
-    const int i = (int)(t / out_stride), k = (int)(t % out_stride);
-    out[t] = k < counts[i] ? list[(size_t)i * stride + k] : -1;
-}
-
-// ---- unique-pair work list ------------------------------------------------------------------------------------------
-// Each unordered neighbour pair {i, j} is evaluated ONCE (the method's own cost: Eq. 1/2 per pair).  The pair list is
-// class-major (class = unordered pair of shape ids) so that a warp of the pair kernel runs 32 pairs with identical
-// loop bounds and identical (warp-uniform) shape-table addresses.  `slot` tells each side where its pair's result
-// records live, so that the reduction needs no atomics.
-__global__ void k_pair_count(int N, const int* __restrict__ counts, const int* __restrict__ list, int stride,
-                             const int* __restrict__ sid, ClassTable ct, int nclass, int* __restrict__ pcnt) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    int loc[DEM_MAX_CLASSES];
-    for (int c = 0; c < nclass; ++c) loc[c] = 0;
-    const int si = sid[i];
-    const int n = min(counts[i], stride);
-    for (int k = 0; k < n; ++k) {
-        const int j = list[(size_t)i * stride + k];
-        if (j > i) loc[ct.lut[si][sid[j]]]++;
-    }
-    for (int c = 0; c < nclass; ++c) pcnt[(size_t)c * N + i] = loc[c];
-}
-
-__global__ void k_pair_fill(int N, const int* __restrict__ counts, const int* __restrict__ list, int stride,
-                            const int* __restrict__ sid, ClassTable ct, int nclass, const int* __restrict__ poff,
-                            int2* __restrict__ pairs, int* __restrict__ slot) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    int loc[DEM_MAX_CLASSES];
-    for (int c = 0; c < nclass; ++c) loc[c] = poff[(size_t)c * N + i];
-    const int si = sid[i];
-    const int n = min(counts[i], stride);
-    for (int k = 0; k < n; ++k) {
-        const int j = list[(size_t)i * stride + k];
-        if (j > i) {
-            const int sj = sid[j];
-            const int p = loc[ct.lut[si][sj]]++;
-            const bool i_first = si <= sj;  // the pair's first particle is the one with the smaller shape id
-            pairs[p] = i_first ? make_int2(i, j) : make_int2(j, i);
-            slot[(size_t)i * stride + k] = 2 * p + (i_first ? 0 : 1);
-        }
-    }
-}
-
-__global__ void k_slot_back(int N, const int* __restrict__ counts, const int* __restrict__ list, int stride,
-                            const int* __restrict__ sid, ClassTable ct, const int* __restrict__ poff,
-                            int* __restrict__ slot) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    const int si = sid[i];
-    const int n = min(counts[i], stride);
-    for (int k = 0; k < n; ++k) {
-        const int j = list[(size_t)i * stride + k];
-        if (j < i) {  // the pair is owned by j: find its position among j's owned pairs of the same class
-            const int sj = sid[j];
-            const int c = ct.lut[sj][si];
-            const int nj = min(counts[j], stride);
-            int r = 0;
-            for (int m = 0; m < nj; ++m) {
-                const int q = list[(size_t)j * stride + m];
-                if (q == i) break;
-                if (q > j && ct.lut[sj][sid[q]] == c) ++r;
-            }
-            const int p = poff[(size_t)c * N + j] + r;
-            const bool j_first = sj <= si;
-            slot[(size_t)i * stride + k] = 2 * p + (j_first ? 1 : 0);
-        }
-    }
-}
-
 // ---- a3-a7: the pair-feature kernel ---------------------------------------------------------------------------------
-template <typename real> struct PairArgs {
-    typedef typename vec4<real>::type real4;
-    const real4* table;   // device shape table
-    ShapeDev sa, sb;      // shapes of the pair's first / second particle
-    const int2* pairs;    // this class's segment of the pair list
-    int npairs;
-    int slices;           // lanes per pair (each takes a slice of the outer feature loop)
-    int n_outer;          // outer-loop length of the class
-    real4* rec;           // this class's result records: 4 real4 per (pair, slice)
-    const void* pos;
-    const void* quat;
-    BoxDev box;
-    double reach2;        // (R_a + R_b + 2^(1/6) sigma)^2 : beyond it no term can be inside the cutoff (exact, R10)
-    PairConst<real> pc;
-    real rc2_search;      // FP32 search kernel: squared candidate cutoff (WCA cutoff + slack, dem_fast.cuh)
-    real cull_a2, cull_b2;  // culling kernel: (R_first + rc_search)^2, (R_second + rc_search)^2 (circumradii)
-    const f4* pose;       // FP32 search kernel: this class's compacted pose records, pair indices and their number
-    const int* pidx;      //   (written by k_pose)
-    const int* count;
-    size_t plane;         //   stride of the pose planes
-    unsigned long long* counters;  // [0] pairs evaluated, [1] active, [2] degenerate, [3] parallel, [4..6] swept terms
-    unsigned long long* cum;       // running totals of [4..6] while bench's timing is on (else null)
-};
-
 template <typename real, typename PosT, int DIM>
 __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
     typedef typename vec4<real>::type real4;
@@ -380,14 +124,6 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
 // flags[1] = halt, flags[2] = steps completed.  dem_step queues many steps before the host looks at the flags: with
 // flags[0] set the list is stale, so the kernel changes nothing and raises halt, which turns every later
 // k_kick_drift of the chunk into a no-op; otherwise it counts the step as completed (see step_t).
-struct KickArgs {
-    double half_dt;
-    int dim;
-    d4* vel;
-    d4* ang;
-    double inv_mass[DEM_MAX_SHAPES_K];
-};
-
 template <typename real, bool KICK>
 __global__ void k_reduce(int N, const int* __restrict__ counts, const int* __restrict__ slot, int stride,
                          const int* __restrict__ sid, ClassTable ct, int nclass,
@@ -473,287 +209,6 @@ __global__ void k_reduce(int N, const int* __restrict__ counts, const int* __res
             ka.ang[i] = L;
         }
     }
-}
-
-// ---- a9: NVE integrator (reading R15) --------------------------------------------------------------------
-struct MassTable {
-    double mass[DEM_MAX_SHAPES_K];
-    double inertia[DEM_MAX_SHAPES_K][3];
-};
-
-__device__ __forceinline__ void quat_mul_d(const double* a, const double* b, double* o) {
-    o[0] = a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3];
-    o[1] = a[0] * b[1] + a[1] * b[0] + a[2] * b[3] - a[3] * b[2];
-    o[2] = a[0] * b[2] - a[1] * b[3] + a[2] * b[0] + a[3] * b[1];
-    o[3] = a[0] * b[3] + a[1] * b[2] - a[2] * b[1] + a[3] * b[0];
-}
-
-// Torque-free rotation over dt with the lab-frame angular momentum L held fixed.  Spherical tops (and 2D): exact,
-// q <- exp(dt/2 L/I0) q.  Otherwise the symmetric splitting of the free-rotor Hamiltonian into rotations about the
-// body axes x(dt/2) y(dt/2) z(dt) y(dt/2) x(dt/2) (the family of PAPER.md ref. 23).
-__device__ inline void free_rotate(int dim, const double* I, const double* L, double dt, double* q) {
-    const bool spherical = dim == 2 || (I[0] == I[1] && I[1] == I[2]);
-    if (spherical) {
-        const double I0 = I[2];
-        if (!(I0 > 0.0)) return;
-        // rotation by phi = |a| about a/|a| with a = (dt / 2 I0) L: rq = (cos phi, (sin phi / phi) a)
-        const double h = 0.5 * dt / I0;
-        const double a[3] = {h * L[0], h * L[1], h * L[2]};
-        const double p2 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2];
-        double ch, sc;  // cos phi, sin phi / phi
-        if (p2 < 0.0625) {  // Taylor series: next terms phi^12 / 12! and phi^12 / 13! are below 1.2e-16 here
-            ch = 1.0 + p2 * (-1.0 / 2 + p2 * (1.0 / 24 + p2 * (-1.0 / 720 + p2 * (1.0 / 40320 + p2 * (-1.0 / 3628800)))));
-            sc = 1.0 + p2 * (-1.0 / 6 + p2 * (1.0 / 120 + p2 * (-1.0 / 5040 + p2 * (1.0 / 362880 + p2 * (-1.0 / 39916800)))));
-        } else {
-            const double ph = sqrt(p2);
-            double sh;
-            sincos(ph, &sh, &ch);
-            sc = sh / ph;
-        }
-        const double rq[4] = {ch, sc * a[0], sc * a[1], sc * a[2]};
-        double o[4];
-        quat_mul_d(rq, q, o);
-        // |o| = |q| (1 + O(1e-16)): two Newton steps of 1/sqrt from 1 renormalise a q that is unit to float precision
-        const double n2 = o[0] * o[0] + o[1] * o[1] + o[2] * o[2] + o[3] * o[3];
-        double inv = 1.5 - 0.5 * n2;
-        inv = inv * (1.5 - 0.5 * n2 * inv * inv);
-        inv = inv * (1.5 - 0.5 * n2 * inv * inv);
-        for (int k = 0; k < 4; ++k) q[k] = o[k] * inv;
-        return;
-    }
-    double M[9], Lb[3];
-    quat_to_mat<double>(q[0], q[1], q[2], q[3], M);
-    for (int a = 0; a < 3; ++a) Lb[a] = M[a] * L[0] + M[3 + a] * L[1] + M[6 + a] * L[2];  // R^T L
-    const int axis_seq[5] = {0, 1, 2, 1, 0};
-    const double frac[5] = {0.5, 0.5, 1.0, 0.5, 0.5};
-    for (int s = 0; s < 5; ++s) {
-        const int a = axis_seq[s];
-        if (!(I[a] > 0.0)) continue;
-        const double phi = frac[s] * dt * Lb[a] / I[a];
-        double sn, cs;
-        sincos(phi, &sn, &cs);
-        const int b = (a + 1) % 3, c = (a + 2) % 3;
-        const double lb = cs * Lb[b] + sn * Lb[c], lc = -sn * Lb[b] + cs * Lb[c];
-        Lb[b] = lb;
-        Lb[c] = lc;
-        double sh, ch;
-        sincos(0.5 * phi, &sh, &ch);
-        double rq[4] = {ch, 0, 0, 0}, o[4];
-        rq[1 + a] = sh;
-        quat_mul_d(q, rq, o);  // body-axis rotation composes on the right
-        for (int k = 0; k < 4; ++k) q[k] = o[k];
-    }
-    const double n = sqrt(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
-    for (int k = 0; k < 4; ++k) q[k] /= n;
-}
-
-// Nose-Hoover thermostat (dem_step_nvt; R19): friction xi, its time integral eta, the scaling
-// of v and L that the next k_kick_drift (or k_scale_momenta) still has to apply, and the degrees of freedom g.
-struct ThermoDev {
-    double xi, eta, scale, dof;
-};
-
-// first half of velocity Verlet: v += dt/2 F/m; x += dt v (wrapped); L += dt/2 tau; free rotation of q.
-// Also raises moved[0] when a particle is farther than skin/2 from where it was at the last neighbour build.
-// Does nothing once moved[1] (halt, raised by k_reduce of an earlier step of the same chunk) is set.
-template <typename real>
-__global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict__ sid, MassTable mt,
-                             d4* __restrict__ pos, d4* __restrict__ quat, d4* __restrict__ vel, d4* __restrict__ ang,
-                             const typename vec4<real>::type* __restrict__ force,
-                             const typename vec4<real>::type* __restrict__ torque, const d4* __restrict__ pos_build,
-                             double half_skin2, int* __restrict__ moved, const ThermoDev* __restrict__ thermo) {
-    // The translational and the rotational half of a particle's update are independent: the first half of the grid
-    // does x, v (and the skin test), the second q, L -- twice the memory-level parallelism, half the dependent chain.
-    if (moved[1]) return;
-    const int half = gridDim.x >> 1;
-    const bool rot = (int)blockIdx.x >= half;
-    const int i = (blockIdx.x - (rot ? half : 0)) * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    const int s = sid[i];
-    const double sc = thermo ? thermo->scale : 1.0;  // NVT: pending thermostat scaling of v and L (k_thermostat)
-    if (!rot) {
-        const double hm = 0.5 * dt / mt.mass[s];
-        d4 x = pos[i], v = vel[i];
-        const typename vec4<real>::type F = force[i];
-        const d4 xb = pos_build[i];
-        double xs[3] = {x.x, x.y, x.z}, vs[3] = {v.x * sc, v.y * sc, v.z * sc};
-        const double Fs[3] = {(double)F.x, (double)F.y, (double)F.z};
-        for (int a = 0; a < box.dim; ++a) {
-            vs[a] += hm * Fs[a];
-            xs[a] += dt * vs[a];
-            xs[a] -= box.L[a] * rint(xs[a] * box.invL[a]);
-        }
-        x.x = xs[0]; x.y = xs[1]; x.z = xs[2];
-        v.x = vs[0]; v.y = vs[1]; v.z = vs[2];
-        pos[i] = x;
-        vel[i] = v;
-        double dx = xs[0] - xb.x, dy = xs[1] - xb.y, dz = box.dim == 3 ? xs[2] - xb.z : 0.0;
-        dx -= box.L[0] * rint(dx * box.invL[0]);
-        dy -= box.L[1] * rint(dy * box.invL[1]);
-        dz -= box.L[2] * rint(dz * box.invL[2]);
-        if (dx * dx + dy * dy + dz * dz > half_skin2) moved[0] = 1;
-    } else {
-        d4 L = ang[i], q = quat[i];
-        const typename vec4<real>::type T = torque[i];
-        double Ls[3] = {L.x * sc, L.y * sc, L.z * sc};
-        const double Ts[3] = {(double)T.x, (double)T.y, (double)T.z};
-        for (int a = (box.dim == 2 ? 2 : 0); a < 3; ++a) Ls[a] += 0.5 * dt * Ts[a];
-        double qs[4] = {q.x, q.y, q.z, q.w};
-        free_rotate(box.dim, mt.inertia[s], Ls, dt, qs);
-        L.x = Ls[0]; L.y = Ls[1]; L.z = Ls[2];
-        q.x = qs[0]; q.y = qs[1]; q.z = qs[2]; q.w = qs[3];
-        ang[i] = L;
-        quat[i] = q;
-    }
-}
-
-// NVT: per-block partial sums of K_trans + K_rot and of the rotational degrees of freedom (axes with I > 0), in double,
-// fixed order.  partial[2 b] = K, partial[2 b + 1] = degrees of freedom.
-__global__ void k_kinetic(int N, int dim, const int* __restrict__ sid, MassTable mt, const d4* __restrict__ quat,
-                          const d4* __restrict__ vel, const d4* __restrict__ ang, double* __restrict__ partial) {
-    __shared__ double sh[2][256];
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    double K = 0, dof = 0;
-    if (i < N) {
-        const int s = sid[i];
-        const d4 v = vel[i], L = ang[i], q = quat[i];
-        K = 0.5 * mt.mass[s] * (v.x * v.x + v.y * v.y + v.z * v.z);
-        double M[9];
-        quat_to_mat<double>(q.x, q.y, q.z, q.w, M);
-        for (int a = (dim == 2 ? 2 : 0); a < 3; ++a) {
-            const double Lb = M[a] * L.x + M[3 + a] * L.y + M[6 + a] * L.z;
-            const double I = mt.inertia[s][a];
-            if (I > 0.0) {
-                K += 0.5 * Lb * Lb / I;
-                dof += 1.0;
-            }
-        }
-    }
-    sh[0][threadIdx.x] = K; sh[1][threadIdx.x] = dof;
-    __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
-        if ((int)threadIdx.x < o) {
-            sh[0][threadIdx.x] += sh[0][threadIdx.x + o];
-            sh[1][threadIdx.x] += sh[1][threadIdx.x + o];
-        }
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) {
-        partial[2 * blockIdx.x] = sh[0][0];
-        partial[2 * blockIdx.x + 1] = sh[1][0];
-    }
-}
-
-// NVT: one block sums the partials of k_kinetic and advances (xi, eta) by `halves` thermostat half steps (1: the end
-// of the run, or its start; 2: the end of one step and the start of the next, which are adjacent).  The scaling of v
-// and L is left in th->scale for the next k_kick_drift / k_scale_momenta.  Does nothing when the step it follows was
-// not completed (flags[1] = halt, see k_reduce).
-__global__ void k_thermostat(int nb, const double* __restrict__ partial, int dim, int N, double dt, double kT,
-                             double tau, int halves, const int* __restrict__ flags, ThermoDev* __restrict__ th) {
-    __shared__ double sh[2][256];
-    if (flags && flags[1]) return;
-    double K = 0, dof = 0;
-    for (int b = threadIdx.x; b < nb; b += 256) {
-        K += partial[2 * b];
-        dof += partial[2 * b + 1];
-    }
-    sh[0][threadIdx.x] = K; sh[1][threadIdx.x] = dof;
-    __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
-        if ((int)threadIdx.x < o) {
-            sh[0][threadIdx.x] += sh[0][threadIdx.x + o];
-            sh[1][threadIdx.x] += sh[1][threadIdx.x + o];
-        }
-        __syncthreads();
-    }
-    if (threadIdx.x != 0) return;
-    K = sh[0][0];
-    const double g = (double)dim * (N - 1) + sh[1][0], Q = g * kT * tau * tau;
-    double xi = th->xi, eta = th->eta, scale = 1.0;
-    for (int h = 0; h < halves; ++h) {
-        xi += 0.25 * dt * (2.0 * K - g * kT) / Q;
-        const double s = exp(-xi * 0.5 * dt);
-        K *= s * s;
-        scale *= s;
-        eta += 0.5 * dt * xi;
-        xi += 0.25 * dt * (2.0 * K - g * kT) / Q;
-    }
-    th->xi = xi; th->eta = eta; th->scale = scale; th->dof = g;
-}
-
-// NVT: the scaling left by the last thermostat half step of a run.
-__global__ void k_scale_momenta(int N, d4* __restrict__ vel, d4* __restrict__ ang, const ThermoDev* __restrict__ th) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    const double s = th->scale;
-    d4 v = vel[i], L = ang[i];
-    v.x *= s; v.y *= s; v.z *= s;
-    L.x *= s; L.y *= s; L.z *= s;
-    vel[i] = v;
-    ang[i] = L;
-}
-
-// U, K_trans, K_rot: per-block partial sums in double (fixed order), summed on the host.
-template <typename real, typename PosT>
-__global__ void k_energy(int N, int dim, const int* __restrict__ sid, MassTable mt, const PosT* __restrict__ quat,
-                         const PosT* __restrict__ vel, const PosT* __restrict__ ang,
-                         const typename vec4<real>::type* __restrict__ force, double* __restrict__ partial) {
-    __shared__ double sh[3][256];
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    double U = 0, Kt = 0, Kr = 0;
-    if (i < N) {
-        const int s = sid[i];
-        const d4 v = load4d(vel, i), L = load4d(ang, i), q = load4d(quat, i);
-        U = (double)force[i].w;
-        Kt = 0.5 * mt.mass[s] * (v.x * v.x + v.y * v.y + v.z * v.z);
-        double M[9];
-        quat_to_mat<double>(q.x, q.y, q.z, q.w, M);
-        for (int a = (dim == 2 ? 2 : 0); a < 3; ++a) {
-            const double Lb = M[a] * L.x + M[3 + a] * L.y + M[6 + a] * L.z;
-            const double I = mt.inertia[s][a];
-            if (I > 0.0) Kr += 0.5 * Lb * Lb / I;
-        }
-    }
-    sh[0][threadIdx.x] = U; sh[1][threadIdx.x] = Kt; sh[2][threadIdx.x] = Kr;
-    __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
-        if ((int)threadIdx.x < o)
-            for (int a = 0; a < 3; ++a) sh[a][threadIdx.x] += sh[a][threadIdx.x + o];
-        __syncthreads();
-    }
-    if (threadIdx.x == 0)
-        for (int a = 0; a < 3; ++a) partial[3 * blockIdx.x + a] = sh[a][0];
-}
-
-// ---- precision conversion of state arrays (DEM_F32 contexts integrate in double, R15b) --------------------------------
-__global__ void k_f4_to_d4(int n, const f4* __restrict__ in, d4* __restrict__ out) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const f4 v = in[i];
-    d4 r;
-    r.x = v.x; r.y = v.y; r.z = v.z; r.w = v.w;
-    out[i] = r;
-}
-__global__ void k_d4_to_f4(int n, const d4* __restrict__ in, f4* __restrict__ out) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const d4 v = in[i];
-    f4 r;
-    r.x = (float)v.x; r.y = (float)v.y; r.z = (float)v.z; r.w = (float)v.w;
-    out[i] = r;
-}
-
-// ---- FP32 FMA-chain microbenchmark (roofline denominator) --------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_fma_peak(int iters, float seed, float* __restrict__ out) {
-    float a0 = seed + threadIdx.x, a1 = a0 + 1.f, a2 = a0 + 2.f, a3 = a0 + 3.f, a4 = a0 + 4.f, a5 = a0 + 5.f,
-          a6 = a0 + 6.f, a7 = a0 + 7.f;
-    const float m = 0.999f + seed * 1e-9f, c = seed;
-    for (int k = 0; k < iters; ++k) {
-        a0 = fmaf(a0, m, c); a1 = fmaf(a1, m, c); a2 = fmaf(a2, m, c); a3 = fmaf(a3, m, c);
-        a4 = fmaf(a4, m, c); a5 = fmaf(a5, m, c); a6 = fmaf(a6, m, c); a7 = fmaf(a7, m, c);
-    }
-    const float s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
-    if (s == 123.456f) out[0] = s;  // never true; keeps the chains alive
 }
 
 }  // namespace dem

@@ -1,121 +1,14 @@
 // dem_lib.cu -- C ABI (include/dem.h) and host orchestration of libdem_b200.  Kernels: dem_kernels.cuh.
 // There is no CPU path: every computing entry point launches CUDA kernels and fails with DEM_ECUDA without a device.
-#include <cuda_runtime.h>
-
-#include <cstdarg>
-#include <cstdio>
-#include <cstring>
-#include <string>
-#include <vector>
-
-#include "../../include/dem.h"
-#include "dem_fast.cuh"
-#include "dem_kernels.cuh"
-#include "dem_shape.h"
-
 #include <type_traits>
+
+#include "dem_ctx.h"
+#include "dem_integrate.cuh"
+#include "dem_list.cuh"
 
 using namespace dem;
 
 namespace {
-
-struct DevBuf {  // grow-only device buffer
-    void* p = nullptr;
-    size_t cap = 0;
-    cudaError_t reserve(size_t bytes) {
-        if (bytes <= cap) return cudaSuccess;
-        if (p) cudaFree(p);
-        p = nullptr;
-        cap = 0;
-        size_t want = bytes + bytes / 8 + 256;
-        cudaError_t e = cudaMalloc(&p, want);
-        if (e == cudaSuccess) cap = want;
-        return e;
-    }
-    void release() {
-        if (p) cudaFree(p);
-        p = nullptr;
-        cap = 0;
-    }
-    template <typename T> T* as() const { return static_cast<T*>(p); }
-};
-
-}  // namespace
-
-struct dem_ctx {
-    int dim = 3, prec = DEM_F32;
-    double eps = 1.0, eps_par = 1e-6;
-    cudaStream_t stream = nullptr;
-    std::string err;
-    std::vector<HostShape> shapes;
-    bool table_dirty = true;
-    std::vector<ShapeDev> shape_dev;
-    DevBuf table;
-    MassTable mt;
-    // neighbour list state
-    bool have_list = false;
-    int N = 0, stride = 16, max_count = 0;
-    double box[3] = {0, 0, 0}, r_cut = 0;
-    GridDev grid;
-    DevBuf cell_of, rank, cell_start, order, xs, counts, list, slot, scratch_scan, pcnt, pairs, rec, flags, counters, thermo;
-    DevBuf cum;         // running totals of the swept-term counters while timing is on
-    DevBuf pose, pidx;  // FP32 search kernel: compacted pose records per class (k_pose)
-    ClassTable ct;
-    int nclass = 0;
-    int class_sa[DEM_MAX_CLASSES], class_sb[DEM_MAX_CLASSES], class_np[DEM_MAX_CLASSES];
-    long long npairs_total = 0, nrec_total = 0;
-    int force_slices = 0;  // 0 = heuristic
-    bool cull = true;             // packed search kernel in 3D: exact per-feature culling (dem_set_culling)
-    bool generic_kernel = false;  // DEM_F32 contexts: use the generic k_pair instead of the packed search kernel
-    size_t l2_flush_bytes = 0;  // bench hygiene: overwrite this many bytes of scratch before every time step
-    DevBuf l2_scratch;
-    // dem_step state (double) for DEM_F32 contexts, plus forces and the positions of the last build
-    DevBuf st_pos, st_quat, st_vel, st_ang, st_force, st_torque, pos_build, epart;
-    // host-buffer entry points
-    DevBuf h_pos, h_quat, h_vel, h_ang, h_sid, h_force, h_torque, h_virial;
-    // accounting
-    int64_t launches = 0;
-    bool timing = false;
-    struct EvTriple { cudaEvent_t first, mid, second; };  // before k_pose, between k_pose and the pair kernel, after
-    std::vector<EvTriple> ev_pool;
-    size_t ev_used = 0;
-    int64_t last_terms = 0;
-    int sm_count = 148;
-    int* h_moved = nullptr;        // pinned host copy of dem_step's flags (moved, halt, steps completed)
-    cudaStream_t copy_stream = nullptr;  // dem_step_host: second H2D stream (velocities, angular momenta)
-    cudaEvent_t ev_copy = nullptr;
-    bool ev_copy_pending = false;
-    double nvt_dof = 0;            // degrees of freedom counted by the last dem_step_nvt
-    int rebuild_interval = 8;      // steps between the last two neighbour rebuilds of dem_step (sizes its chunks)
-};
-
-namespace {
-
-int fail(dem_ctx* c, int code, const char* fmt, ...) {
-    char buf[512];
-    va_list ap;
-    va_start(ap, fmt);
-    vsnprintf(buf, sizeof buf, fmt, ap);
-    va_end(ap);
-    if (c) c->err = buf;
-    return code;
-}
-
-#define CU(call)                                                                                        \
-    do {                                                                                                \
-        cudaError_t e_ = (call);                                                                        \
-        if (e_ != cudaSuccess)                                                                          \
-            return fail(ctx, e_ == cudaErrorMemoryAllocation ? DEM_ENOMEM : DEM_ECUDA, "%s: %s", #call, \
-                        cudaGetErrorString(e_));                                                        \
-    } while (0)
-#define CHECK(call)             \
-    do {                        \
-        int rc_ = (call);       \
-        if (rc_ != DEM_OK) return rc_; \
-    } while (0)
-#define LAUNCHED(ctx) ((ctx)->launches++)
-
-inline int nblk(long long n, int b) { return (int)((n + b - 1) / b); }
 
 // in-place exclusive scan of data[0..n); data must have room for n entries; uses ctx->scratch_scan
 int scan_exclusive(dem_ctx* ctx, int* data, int n, int* scratch, size_t scratch_ints) {
@@ -189,27 +82,6 @@ int sync_tables(dem_ctx* ctx) {
     return DEM_OK;
 }
 
-double reach_of(const HostShape& a, const HostShape& b) {
-    return a.circumradius + b.circumradius + std::pow(2.0, 1.0 / 6.0) * (a.rounding + b.rounding);
-}
-double max_reach(const dem_ctx* ctx) {
-    double r = 0;
-    for (auto& a : ctx->shapes)
-        for (auto& b : ctx->shapes) r = std::max(r, reach_of(a, b));
-    return r;
-}
-
-// nominal Eq. 1 / Eq. 2 terms of one pair of the class, and the outer-loop length the pair kernel slices
-long long class_terms(const dem_ctx* ctx, int c) {
-    const HostShape &A = ctx->shapes[ctx->class_sa[c]], &B = ctx->shapes[ctx->class_sb[c]];
-    if (ctx->dim == 3) return (long long)A.ne * B.ne + (long long)A.nv * B.nf + (long long)B.nv * A.nf;
-    return (long long)A.nv * B.ne + (long long)B.nv * A.ne;
-}
-int class_outer(const dem_ctx* ctx, int c) {
-    const HostShape &A = ctx->shapes[ctx->class_sa[c]], &B = ctx->shapes[ctx->class_sb[c]];
-    return ctx->dim == 3 ? B.ne + B.nv + A.nv : B.nv + A.nv;
-}
-
 // ---- neighbour build ----------------------------------------------------------------------------------------------
 template <typename PosT>
 int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, const double box[3], double r_cut,
@@ -224,15 +96,12 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
     if (check_rcut && r_cut < max_reach(ctx) * (1.0 - 1e-12))
         return fail(ctx, DEM_ERCUT, "r_cut = %.17g < interaction reach %.17g", r_cut, max_reach(ctx));
     cudaStream_t st = ctx->stream;
+    cudaEvent_t b0 = ev_mark(ctx, 2);
     ctx->have_list = false;
     ctx->N = N;
     for (int a = 0; a < 3; ++a) ctx->box[a] = box[a];
     ctx->r_cut = r_cut;
-    BoxDev bx;
-    bx.dim = ctx->dim;
-    for (int a = 0; a < 3; ++a) bx.L[a] = box[a];
-    if (ctx->dim == 2) bx.L[2] = 1.0;
-    for (int a = 0; a < 3; ++a) bx.invL[a] = 1.0 / bx.L[a];
+    const BoxDev bx = box_dev(ctx->dim, box);
     // cells at least r_cut wide (with a relative margin far above double rounding), at most ~2 N + 64 cells in all
     GridDev g;
     g.nc[0] = g.nc[1] = g.nc[2] = 1;
@@ -281,10 +150,12 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
         CU(ctx->list.reserve(sizeof(int) * (size_t)N * ctx->stride));
         CU(ctx->slot.reserve(sizeof(int) * (size_t)N * ctx->stride));
         CU(cudaMemsetAsync(flags, 0, sizeof(int) * 16, st));
+        cudaEvent_t n0 = ev_mark(ctx, 2);
         k_neigh<<<nblk(N, 128), 128, 0, st>>>(N, bx, g, r_cut * r_cut, ctx->order.as<int>(), ctx->cell_of.as<int>(),
                                               cell_start, ctx->xs.as<d4>(), ctx->stride, ctx->counts.as<int>(),
                                               ctx->list.as<int>(), flags);
         LAUNCHED(ctx);
+        ev_span(ctx, KT_NEIGH, n0, ev_mark(ctx, 2));
         int mc = 0;
         CU(cudaMemcpyAsync(&mc, flags, sizeof(int), cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
@@ -298,13 +169,17 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
     CU(ctx->pcnt.reserve(sizeof(int) * ((size_t)nc * N + 1)));
     int* pcnt = ctx->pcnt.as<int>();
     CU(cudaMemsetAsync(pcnt + (size_t)nc * N, 0, sizeof(int), st));
-    k_pair_count<<<nblk(N, B), B, 0, st>>>(N, ctx->counts.as<int>(), ctx->list.as<int>(), ctx->stride, sid, ctx->ct, nc, pcnt);
+    k_pair_count<<<nblk(N, B), B, 0, st>>>(N, ctx->counts.as<int>(), ctx->list.as<int>(), ctx->stride, sid, ctx->ct, nc,
+                                           (int)ctx->shapes.size(), pcnt, flags + 1);
     LAUNCHED(ctx);
     CHECK(scan_exclusive(ctx, pcnt, nc * N + 1, ctx->scratch_scan.as<int>(), scan_ints));
     int bases[DEM_MAX_CLASSES + 1];
     for (int c = 0; c <= nc; ++c)
         CU(cudaMemcpyAsync(&bases[c], pcnt + (size_t)c * N, sizeof(int), cudaMemcpyDeviceToHost, st));
+    int bad_shape = 0;
+    CU(cudaMemcpyAsync(&bad_shape, flags + 1, sizeof(int), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    if (bad_shape) return fail(ctx, DEM_EINVAL, "shape_id holds an id outside the %d registered shapes", (int)ctx->shapes.size());
     ctx->npairs_total = bases[nc];
     long long nrec = 0, terms = 0;
     for (int c = 0; c < nc; ++c) {
@@ -342,175 +217,8 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
                                           ctx->slot.as<int>());
     LAUNCHED(ctx);
     CU(cudaGetLastError());
+    ev_span(ctx, KT_BUILD, b0, ev_mark(ctx, 2));
     ctx->have_list = true;
-    return DEM_OK;
-}
-
-// ---- force evaluation ---------------------------------------------------------------------------------------------
-template <typename real, typename PosT>
-int compute_t(dem_ctx* ctx, const PosT* pos, const PosT* quat, const int32_t* sid, int N, void* force, void* torque,
-              void* virial, int* skip = nullptr, const KickArgs* kick = nullptr) {
-    typedef typename vec4<real>::type real4;
-    if (!ctx->have_list) return fail(ctx, DEM_ESTALE, "no neighbour list: call dem_build_neighbors first");
-    if (N != ctx->N) return fail(ctx, DEM_ESTALE, "N = %d differs from the last build (%d)", N, ctx->N);
-    if (!pos || !quat || !sid || !force || !torque) return fail(ctx, DEM_EINVAL, "null particle array");
-    cudaStream_t st = ctx->stream;
-    // counters[0..7] (unsigned long long) followed by the per-class lengths of the k_pose work lists (int): one memset
-    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES, st));
-    int* ccount = reinterpret_cast<int*>(ctx->counters.as<unsigned long long>() + 8);
-    // capacity of a class's work list: its pairs plus the padding of every k_pose block to a whole warp
-    auto list_cap = [&](int c) { return (size_t)ctx->class_np[c] + 64u * (size_t)nblk(ctx->class_np[c], DEM_POSE_THREADS); };
-    size_t list_base[DEM_MAX_CLASSES + 1];
-    list_base[0] = 0;
-    for (int c = 0; c < ctx->nclass; ++c) list_base[c + 1] = list_base[c] + list_cap(c);
-    const bool search = std::is_same<real, float>::value && !ctx->generic_kernel;
-    if (search) {
-        CU(ctx->pose.reserve(sizeof(f4) * 6 * std::max<size_t>(list_base[ctx->nclass], 1)));
-        CU(ctx->pidx.reserve(sizeof(int) * std::max<size_t>(list_base[ctx->nclass], 1)));
-    }
-    BoxDev bx;
-    bx.dim = ctx->dim;
-    for (int a = 0; a < 3; ++a) bx.L[a] = ctx->box[a];
-    if (ctx->dim == 2) bx.L[2] = 1.0;
-    for (int a = 0; a < 3; ++a) bx.invL[a] = 1.0 / bx.L[a];
-    for (int c = 0; c < ctx->nclass; ++c) {
-        const int np = ctx->class_np[c];
-        if (np == 0) continue;
-        const HostShape &HA = ctx->shapes[ctx->class_sa[c]], &HB = ctx->shapes[ctx->class_sb[c]];
-        PairArgs<real> a;
-        a.table = ctx->table.as<real4>();
-        a.sa = ctx->shape_dev[ctx->class_sa[c]];
-        a.sb = ctx->shape_dev[ctx->class_sb[c]];
-        a.pairs = ctx->pairs.as<int2>() + ctx->ct.pair_base[c];
-        a.npairs = np;
-        a.slices = ctx->ct.slices[c];
-        a.n_outer = class_outer(ctx, c);
-        a.rec = ctx->rec.as<real4>() + DEM_REC * (size_t)ctx->ct.rec_base[c];
-        a.pos = pos;
-        a.quat = quat;
-        a.box = bx;
-        const double reach = reach_of(HA, HB), sigma = HA.rounding + HB.rounding;
-        a.reach2 = reach * reach;
-        a.pc.rc2 = (real)(std::cbrt(2.0) * sigma * sigma);
-        a.pc.sig2 = (real)(sigma * sigma);
-        a.pc.eps = (real)ctx->eps;
-        a.pc.eps_par = (real)ctx->eps_par;
-        a.pc.degen2 = (real)((1e-6 * sigma) * (1e-6 * sigma));
-        a.counters = ctx->counters.as<unsigned long long>();
-        a.cum = (ctx->timing && ctx->cum.p) ? ctx->cum.as<unsigned long long>() : nullptr;
-        // candidate cutoff of the FP32 search kernel: FP32 rounding of the packed formulation (1e-3 relative) plus
-        // its error on near-parallel edges, at most sin(angle) x edge length with the angle below ~1e-3 where the
-        // line-line solve loses its digits; 4e-3 x longest edge leaves a factor 4
-        const double rc = std::pow(2.0, 1.0 / 6.0) * sigma;
-        const double rcs = rc * (1.0 + 1e-3) + (ctx->dim == 3 ? 4e-3 * std::max(HA.max_edge, HB.max_edge) : 0.0);
-        a.rc2_search = (real)(rcs * rcs);
-        size_t smem = sizeof(real4) * (size_t)(a.sa.len + (a.sa.off == a.sb.off ? 0 : a.sb.len));
-        const long long items = (long long)((np + 31) & ~31) * a.slices;
-        const int threads = 128;
-        int grid = (int)std::min<long long>(nblk(items, threads), (long long)ctx->sm_count * 64);
-        void (*kern)(const PairArgs<real>) = ctx->dim == 3 ? k_pair<real, PosT, 3> : k_pair<real, PosT, 2>;
-        PoseArgs pa;
-        if constexpr (std::is_same<real, float>::value) {
-            if (search) {
-                a.pose = ctx->pose.as<f4>() + 6 * list_base[c];
-                a.pidx = ctx->pidx.as<int>() + list_base[c];
-                a.plane = list_cap(c);
-                a.count = ccount + c;
-                pa.pairs = a.pairs; pa.npairs = np; pa.slices = a.slices; pa.pos = pos; pa.quat = quat; pa.box = bx;
-                pa.reach2 = a.reach2;
-                pa.pose = ctx->pose.as<f4>() + 6 * list_base[c];
-                pa.pidx = ctx->pidx.as<int>() + list_base[c];
-                pa.count = ccount + c;
-                pa.plane = list_cap(c);
-                pa.pad = (ctx->dim == 3 && ctx->cull) ? 64 : 32;
-                pa.counters = a.counters;
-                pa.rec = reinterpret_cast<f4*>(a.rec);
-                pa.skip = skip;
-                smem += fast_smem_header();
-                // packed outer pairs per sweep: 3 when the vertex counts fill tiles of 6 at least as well as tiles of 4
-                auto waste = [](int n, int tile) { return ((n + tile - 1) / tile) * tile - n; };
-                const int nva = HA.nv, nvb = HB.nv;
-                const bool tv3 = waste(nva, 6) + waste(nvb, 6) <= waste(nva, 4) + waste(nvb, 4);
-                if (ctx->dim == 3)
-                    kern = tv3 ? k_pair_fast<PosT, 3, 2, 3, 4> : k_pair_fast<PosT, 3, 2, 2, 4>;
-                else
-                    kern = tv3 ? k_pair_fast<PosT, 2, 2, 3, 4> : k_pair_fast<PosT, 2, 2, 2, 4>;
-                int resident = 64;  // grid cap in blocks per SM (measured on cfg4: one tile per warp beats one persistent wave)
-#ifdef DEM_TUNE
-                if (const char* v = getenv("DEM_VARIANT")) {
-                    if (ctx->dim == 3 && sizeof(PosT) == 8) {
-                        switch (atoi(v)) {
-                            case 0: kern = k_pair_fast<PosT, 3, 2, 3, 3>; break;
-                            case 1: kern = k_pair_fast<PosT, 3, 2, 3, 4>; break;
-                            case 2: kern = k_pair_fast<PosT, 3, 1, 3, 4>; break;
-                            case 5: kern = k_pair_fast<PosT, 3, 2, 2, 4>; break;
-                            case 7: kern = k_pair_fast<PosT, 3, 3, 3, 3>; break;
-                        }
-                    }
-                }
-                if (const char* v = getenv("DEM_RESIDENT")) resident = atoi(v);
-                if (const char* v = getenv("DEM_PHASES")) {
-                    const int ph = atoi(v);
-                    cudaMemcpyToSymbolAsync(g_dbg_phases, &ph, sizeof ph, 0, cudaMemcpyHostToDevice, st);
-                }
-#endif
-                if (ctx->dim == 3 && ctx->cull) {
-                    // measured on cfg4: 167 registers without spills beat 128 / 96 / 80 with
-                    kern = a.sa.off == a.sb.off ? k_pair_cull<PosT, 3, true> : k_pair_cull<PosT, 3, false>;
-#ifdef DEM_TUNE
-                    if (const char* v = getenv("DEM_CULL_MINB")) {
-                        if (atoi(v) == 4) kern = a.sa.off == a.sb.off ? k_pair_cull<PosT, 4, true> : k_pair_cull<PosT, 4, false>;
-                        if (atoi(v) == 5) kern = a.sa.off == a.sb.off ? k_pair_cull<PosT, 5, true> : k_pair_cull<PosT, 5, false>;
-                    }
-#endif
-                    smem += cull_smem_header() - fast_smem_header();
-                    const double ra = HA.circumradius + rcs, rb = HB.circumradius + rcs;
-                    a.cull_a2 = (real)(ra * ra);
-                    a.cull_b2 = (real)(rb * rb);
-                }
-                // the padded work list bounds the tiles; a warp of k_pair_cull takes 64 entries, of k_pair_fast 32
-                const long long list_items = (long long)list_cap(c) * a.slices / (ctx->dim == 3 && ctx->cull ? 2 : 1);
-                grid = (int)std::min<long long>(nblk(list_items, threads), (long long)ctx->sm_count * resident);
-            }
-        }
-        if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        cudaEvent_t e0 = nullptr, em = nullptr, e1 = nullptr;
-        if (ctx->timing) {
-            if (ctx->ev_used == ctx->ev_pool.size()) {
-                cudaEvent_t x, y, z;
-                CU(cudaEventCreate(&x));
-                CU(cudaEventCreate(&y));
-                CU(cudaEventCreate(&z));
-                ctx->ev_pool.push_back({x, y, z});
-            }
-            e0 = ctx->ev_pool[ctx->ev_used].first;
-            em = ctx->ev_pool[ctx->ev_used].mid;
-            e1 = ctx->ev_pool[ctx->ev_used].second;
-            ctx->ev_used++;
-            CU(cudaEventRecord(e0, st));
-        }
-        if (search) {  // a3 (relative poses, compaction) runs as its own kernel in front of the search kernel
-            if (ctx->dim == 3)
-                k_pose<PosT, 3><<<nblk(np, DEM_POSE_THREADS), DEM_POSE_THREADS, 0, st>>>(pa);
-            else
-                k_pose<PosT, 2><<<nblk(np, DEM_POSE_THREADS), DEM_POSE_THREADS, 0, st>>>(pa);
-            LAUNCHED(ctx);
-        }
-        if (ctx->timing) CU(cudaEventRecord(em, st));
-        kern<<<grid, threads, smem, st>>>(a);
-        LAUNCHED(ctx);
-        if (ctx->timing) CU(cudaEventRecord(e1, st));
-    }
-    if (kick)
-        k_reduce<real, true><<<nblk(4LL * N, 128), 128, 0, st>>>(
-            N, ctx->counts.as<int>(), ctx->slot.as<int>(), ctx->stride, sid, ctx->ct, ctx->nclass, ctx->rec.as<real4>(),
-            static_cast<real4*>(force), static_cast<real4*>(torque), static_cast<real*>(virial), skip, *kick);
-    else
-        k_reduce<real, false><<<nblk(4LL * N, 128), 128, 0, st>>>(
-            N, ctx->counts.as<int>(), ctx->slot.as<int>(), ctx->stride, sid, ctx->ct, ctx->nclass, ctx->rec.as<real4>(),
-            static_cast<real4*>(force), static_cast<real4*>(torque), static_cast<real*>(virial), skip, KickArgs());
-    LAUNCHED(ctx);
-    CU(cudaGetLastError());
     return DEM_OK;
 }
 
@@ -550,13 +258,9 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     real4* F = ctx->st_force.as<real4>();
     real4* T = ctx->st_torque.as<real4>();
     const double r_list = max_reach(ctx) + skin;
-    BoxDev bx;
-    bx.dim = ctx->dim;
-    for (int a = 0; a < 3; ++a) bx.L[a] = box[a];
-    if (ctx->dim == 2) bx.L[2] = 1.0;
-    for (int a = 0; a < 3; ++a) bx.invL[a] = 1.0 / bx.L[a];
+    const BoxDev bx = box_dev(ctx->dim, box);
     CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
-    CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr)));
+    CHECK(evaluate(ctx, x, q, true, sid, N, F, T, nullptr, nullptr, nullptr));
     // The list build and the first evaluation need positions and orientations only: dem_step_host copies velocities
     // and angular momenta on a second stream meanwhile, and they are waited for (and converted) here.
     if (ctx->ev_copy_pending) {
@@ -610,11 +314,17 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
         const int chunk = std::min(remaining, std::min(64, std::max(hint - since, std::max(1, hint / 8))));
         CU(cudaMemsetAsync(flags, 0, 3 * sizeof(int), st));
         for (int s = 0; s < chunk; ++s) {
-            if (ctx->l2_flush_bytes) CU(cudaMemsetAsync(ctx->l2_scratch.p, s & 0xff, ctx->l2_flush_bytes, st));
+            if (ctx->l2_flush_bytes) {
+                cudaEvent_t f0 = ev_mark(ctx, 2);
+                CU(cudaMemsetAsync(ctx->l2_scratch.p, s & 0xff, ctx->l2_flush_bytes, st));
+                ev_span(ctx, KT_FLUSH, f0, ev_mark(ctx, 2));
+            }
+            cudaEvent_t k0 = ev_mark(ctx, 2);
             k_kick_drift<real><<<2 * nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T,
                                                          ctx->pos_build.as<d4>(), half_skin2, flags, th);
             LAUNCHED(ctx);
-            CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr, flags, &ka)));
+            ev_span(ctx, KT_KICK_DRIFT, k0, ev_mark(ctx, 2));
+            CHECK(evaluate(ctx, x, q, true, sid, N, F, T, nullptr, flags, &ka));
             if (th) CHECK(thermostat(nsteps - remaining + s == nsteps - 1 ? 1 : 2, flags));
         }
         CU(cudaMemcpyAsync(ctx->h_moved, flags, 3 * sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -624,7 +334,7 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
             return fail(ctx, DEM_ECUDA, "dem_step: inconsistent step flags (done %d of %d, moved %d)", done, chunk, ctx->h_moved[0]);
         if (ctx->h_moved[0]) {
             CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
-            CHECK((compute_t<real, double>(ctx, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(q), sid, N, F, T, nullptr, nullptr, &ka)));
+            CHECK(evaluate(ctx, x, q, true, sid, N, F, T, nullptr, nullptr, &ka));
             done += 1;
             if (th) CHECK(thermostat(nsteps - remaining + done == nsteps ? 1 : 2, nullptr));
             ctx->rebuild_interval = since + done;
@@ -685,7 +395,11 @@ int energy_t(dem_ctx* ctx, const PosT* quat, const PosT* vel, const PosT* ang, c
 // =====================================================================================================================
 extern "C" {
 
-const char* dem_version(void) { return "dem_b200 0.1 (sm_100a)"; }
+#ifndef DEM_SOURCE_HASH
+#define DEM_SOURCE_HASH "unknown"
+#endif
+// the hash is that of the sources the library was built from (build.py); binding.lib() refuses a library that lags them
+const char* dem_version(void) { return "dem_b200 0.2 (sm_100a) src " DEM_SOURCE_HASH; }
 
 int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda_stream) {
     if (!out) return DEM_EINVAL;
@@ -714,11 +428,7 @@ int dem_destroy(dem_ctx* c) {
     if (c->h_moved) cudaFreeHost(c->h_moved);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->ev_copy) cudaEventDestroy(c->ev_copy);
-    for (auto& e : c->ev_pool) {
-        cudaEventDestroy(e.mid);
-        cudaEventDestroy(e.first);
-        cudaEventDestroy(e.second);
-    }
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return DEM_OK;
 }
@@ -803,11 +513,7 @@ int dem_copy_neighbors(dem_ctx* ctx, int32_t* counts_out, int32_t* list_out, int
 int dem_compute(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* shape_id, int N, void* force_energy,
                 void* torque, void* virial6) {
     if (!ctx) return DEM_EINVAL;
-    if (ctx->prec == DEM_F64)
-        return compute_t<double, double>(ctx, static_cast<const double*>(pos), static_cast<const double*>(quat), shape_id,
-                                         N, force_energy, torque, virial6);
-    return compute_t<float, float>(ctx, static_cast<const float*>(pos), static_cast<const float*>(quat), shape_id, N,
-                                   force_energy, torque, virial6);
+    return evaluate(ctx, pos, quat, ctx->prec == DEM_F64, shape_id, N, force_energy, torque, virial6, nullptr, nullptr);
 }
 
 int dem_get_counters(dem_ctx* ctx, int64_t out[9]) {
@@ -948,88 +654,6 @@ int dem_step_host(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, 
     if (force_energy) CU(cudaMemcpyAsync(force_energy, ctx->h_force.p, r4 * N, cudaMemcpyDeviceToHost, st));
     if (torque) CU(cudaMemcpyAsync(torque, ctx->h_torque.p, r4 * N, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
-    return DEM_OK;
-}
-
-int dem_set_l2_flush(dem_ctx* ctx, int64_t bytes) {
-    if (!ctx || bytes < 0) return fail(ctx, DEM_EINVAL, "bytes must be >= 0");
-    ctx->l2_flush_bytes = (size_t)bytes;
-    return DEM_OK;
-}
-
-int dem_set_timing(dem_ctx* ctx, int enabled) {
-    if (!ctx) return DEM_EINVAL;
-    ctx->timing = enabled != 0;
-    if (ctx->timing) {
-        CU(ctx->cum.reserve(sizeof(unsigned long long) * 4));
-        CU(cudaMemsetAsync(ctx->cum.p, 0, sizeof(unsigned long long) * 4, ctx->stream));
-    }
-    return DEM_OK;
-}
-
-int dem_swept_totals(dem_ctx* ctx, int64_t out[3]) {
-    if (!ctx || !out) return DEM_EINVAL;
-    out[0] = out[1] = out[2] = 0;
-    if (!ctx->cum.p) return DEM_OK;
-    unsigned long long h[3];
-    CU(cudaMemcpyAsync(h, ctx->cum.p, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
-    CU(cudaStreamSynchronize(ctx->stream));
-    for (int k = 0; k < 3; ++k) out[k] = (int64_t)h[k];
-    return DEM_OK;
-}
-
-int dem_kernel_time_split(dem_ctx* ctx, int64_t* launches, double* pair_ms, double* pose_ms) {
-    if (!ctx || !launches || !pair_ms || !pose_ms) return DEM_EINVAL;
-    CU(cudaStreamSynchronize(ctx->stream));
-    double tp = 0, tq = 0;
-    for (size_t k = 0; k < ctx->ev_used; ++k) {
-        float a = 0, b = 0;
-        CU(cudaEventElapsedTime(&a, ctx->ev_pool[k].first, ctx->ev_pool[k].mid));
-        CU(cudaEventElapsedTime(&b, ctx->ev_pool[k].mid, ctx->ev_pool[k].second));
-        tq += a;
-        tp += b;
-    }
-    *launches = (int64_t)ctx->ev_used;
-    *pair_ms = tp;
-    *pose_ms = tq;
-    ctx->ev_used = 0;
-    return DEM_OK;
-}
-
-int dem_kernel_time(dem_ctx* ctx, int64_t* launches, double* total_ms) {
-    if (!total_ms) return DEM_EINVAL;
-    double pose = 0;
-    CHECK(dem_kernel_time_split(ctx, launches, total_ms, &pose));
-    *total_ms += pose;
-    return DEM_OK;
-}
-
-int64_t dem_launch_count(const dem_ctx* ctx) { return ctx ? ctx->launches : 0; }
-
-int dem_fp32_peak(dem_ctx* ctx, int iters, double* tflops) {
-    if (!ctx || !tflops || iters < 1) return DEM_EINVAL;
-    int dev = 0, sms = 0;
-    CU(cudaGetDevice(&dev));
-    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CU(ctx->flags.reserve(sizeof(int) * 16));
-    cudaEvent_t e0, e1;
-    CU(cudaEventCreate(&e0));
-    CU(cudaEventCreate(&e1));
-    const int grid = sms * 8, threads = 256;
-    float best = 1e30f;
-    for (int rep = 0; rep < 4; ++rep) {
-        CU(cudaEventRecord(e0, ctx->stream));
-        k_fma_peak<<<grid, threads, 0, ctx->stream>>>(iters, 1.0f, ctx->flags.as<float>());
-        LAUNCHED(ctx);
-        CU(cudaEventRecord(e1, ctx->stream));
-        CU(cudaEventSynchronize(e1));
-        float ms = 0;
-        CU(cudaEventElapsedTime(&ms, e0, e1));
-        if (rep > 0 && ms < best) best = ms;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    *tflops = 2.0 * 8.0 * (double)iters * (double)grid * threads / (best * 1e-3) / 1e12;
     return DEM_OK;
 }
 

@@ -11,27 +11,21 @@
 // reason and its rare active terms are rotated back.  The result (F, T, u) is in i's frame; the kernel rotates it to
 // the lab frame once per pair.
 //
-// The functions are __host__ __device__ so that the same source can be exercised on a CPU while developing; the
-// library itself only ever calls them from kernels (there is no CPU path in the product).
+// Device code only: the library calls these from its kernels and nothing else does (there is no CPU path in the
+// product, and the oracle shares no code with this file).
 #pragma once
 #include <math.h>
 #include <stdint.h>
 
-#if defined(__CUDACC__)
-#define DEM_HD __host__ __device__ __forceinline__
-#define DEM_HD_NOINLINE __host__ __device__ __noinline__
-#else
-#define DEM_HD inline
-#define DEM_HD_NOINLINE
+#include "dem_types.h"
+
+#if !defined(__CUDACC__)
+#error "dem_math.cuh is device code: compile it with nvcc"
 #endif
+#define DEM_HD __device__ __forceinline__
+#define DEM_HD_NOINLINE __device__ __noinline__
 
 namespace dem {
-
-struct alignas(16) f4 { float x, y, z, w; };
-struct alignas(16) d4 { double x, y, z, w; };
-template <typename real> struct vec4;
-template <> struct vec4<float> { typedef f4 type; };
-template <> struct vec4<double> { typedef d4 type; };
 
 // ---- scalar helpers ---------------------------------------------------------------------------------------------
 DEM_HD float rmin(float a, float b) { return fminf(a, b); }
@@ -83,14 +77,6 @@ template <typename real> struct ShapeView {
 template <typename real> struct PairAcc {
     real F[3], T[3], u;  // force on i, torque on i about x_i (i's body frame), pair energy U_ij
     unsigned nactive, ndegen, npar;
-};
-
-template <typename real> struct PairConst {
-    real rc2;      // (2^(1/6) sigma_ij)^2 = 2^(1/3) sigma^2     (Eq. 4, compared squared: R7)
-    real sig2;     // sigma_ij^2, sigma_ij = rho_i + rho_j       (R6)
-    real eps;      // epsilon
-    real eps_par;  // near-parallel threshold                    (R5)
-    real degen2;   // (1e-6 sigma)^2                             (R11)
 };
 
 // WCA for one term inside the cutoff; ci = interaction point on i (i frame, relative to x_i), del = c_i - c_j.
