@@ -50,7 +50,7 @@ typedef enum dem_status {
     DEM_EBOX = -4,      /* a periodic box edge < 2 r_cut: the minimum image would be invalid                      */
     DEM_ERCUT = -5,     /* r_cut < max_ij (R_i + R_j + 2^(1/6) sigma_ij): interactions would be dropped silently  */
     DEM_EOVERFLOW = -6, /* neighbour capacity exceeded and could not be regrown                                  */
-    DEM_ESTALE = -7     /* dem_compute called with N different from the last dem_build_neighbors                  */
+    DEM_ESTALE = -7     /* dem_compute without a list, or with N different from the last dem_build_neighbors     */
 } dem_status;
 
 enum { DEM_F32 = 0, DEM_F64 = 1 };
@@ -153,7 +153,7 @@ int dem_step(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const
  * One step = thermostat half step, the NVE step of dem_step, thermostat half step; a half step is
  *     xi += (dt/4)(2K - g kT)/Q;  s = exp(-xi dt/2);  v *= s;  L *= s;  K *= s^2;  eta += (dt/2) xi;
  *     xi += (dt/4)(2K - g kT)/Q.
- * U + K + Q xi^2 / 2 + g kT eta is conserved.  The barostat of PAPER.md:115 is not built.
+ * U + K + Q xi^2 / 2 + g kT eta is conserved.  With the barostat of PAPER.md:115: dem_step_npt.
  *   kT, tau        target temperature and thermostat period (> 0)
  *   thermostat[2]  HOST, in and out: (xi, eta); start a run from (0, 0) and pass the values back in to continue it
  *   *dof           HOST, may be NULL: receives g
@@ -161,6 +161,31 @@ int dem_step(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const
  */
 int dem_step_nvt(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const int32_t* shape_id, int N,
                  const double box[3], double dt, int nsteps, double skin, double kT, double tau, double thermostat[2],
+                 double* dof, void* force_energy, void* torque);
+
+/*
+ * NPT: dem_step_nvt plus a barostat that "computes the pressure from the virial tensor, just as in MD" (
+ * SURVEY.md 8(f) NEXT-3).  The paper gives no equations; R22: the isotropic Martyna-Tobias-Klein barostat on
+ * the strain rate nu = d ln L / dt of the box, coupled to the centres of mass only (the centre-of-mass virial
+ * tr W = sum_pairs r_ij . F_ij that dem_compute produces; orientations and angular momenta do not feel the box):
+ *     dx/dt = v + nu x,  dL_box/dt = nu L_box,  dv/dt = F/m - (alpha nu + xi) v,  dL/dt = tau - xi L,
+ *     dnu/dt = [alpha 2 K_trans + tr W - d V P] / W_b,   alpha = 1 + d / N_f,  N_f = d (N - 1),  W_b = d N kT tau_p^2,
+ *     dxi/dt = (2K - g kT)/Q, deta/dt = xi  (as in dem_step_nvt),
+ * d = 2 or 3, V = the box volume (area in 2D), i.e. d V (P_int - P) + (d/N_f) 2 K_trans with the instantaneous pressure
+ * P_int = (2 K_trans + tr W) / (d V).  U + K + P V + W_b nu^2/2 + Q xi^2/2 + g kT eta is conserved.
+ * One step (time-reversible, second order; h = dt/2): thermostat half step, nu += h dnu/dt, v = (v s + h F/m) s with
+ * s = exp(-alpha nu h / 2) and L += h tau, drift x = x e^{nu dt} + v dt e^{nu dt/2} sinh(nu dt/2)/(nu dt/2) with the box
+ * scaled by e^{nu dt} and free rotation, forces, and the same three half steps in reverse order.
+ *   box[3]     HOST, in and out: the box edges (all periodic edges scale by the same factor)
+ *   pressure   the external pressure P;  tau_p the barostat period (> 0; infinity = constant volume)
+ *   state[3]   HOST, in and out: (xi, eta, nu); start a run from (0, 0, 0) and pass the values back in to continue it
+ * The neighbour list follows the box: it is rebuilt when a particle has moved more than allowed by the skin away from
+ * the affine image of its position at the last build.  Everything else as dem_step_nvt (tau = infinity: no thermostat).
+ * Errors: those of dem_step; DEM_EINVAL for kT, tau, tau_p <= 0 or N < 2; DEM_EBOX when the box shrinks below twice the
+ * interaction reach.  Synchronises once per step (the scalar equations are advanced on the host between kernels).
+ */
+int dem_step_npt(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const int32_t* shape_id, int N, double box[3],
+                 double dt, int nsteps, double skin, double kT, double tau, double pressure, double tau_p, double state[3],
                  double* dof, void* force_energy, void* torque);
 
 /* U = sum_i U_i (from force_energy[.][3]), K_trans, K_rot of a state; DEVICE inputs, HOST out[3]; synchronises. */

@@ -20,7 +20,8 @@ STATUS_NAMES = {0: "DEM_OK", -1: "DEM_EINVAL", -2: "DEM_ENOMEM", -3: "DEM_ECUDA"
 
 # every symbol include/dem.h declares (tests check that the built library exports all of them)
 EXPORTS = ["dem_create", "dem_destroy", "dem_last_error", "dem_set_eps_par", "dem_create_shape", "dem_build_neighbors",
-           "dem_get_neighbors", "dem_copy_neighbors", "dem_compute", "dem_get_counters", "dem_step", "dem_step_nvt", "dem_energy",
+           "dem_get_neighbors", "dem_copy_neighbors", "dem_compute", "dem_get_counters", "dem_step", "dem_step_nvt", "dem_step_npt",
+           "dem_energy",
            "dem_compute_host", "dem_step_host", "dem_set_slices", "dem_set_pair_kernel", "dem_set_culling", "dem_version"]
 # include/dem_bench.h (measurement hooks)
 EXPORTS_BENCH = ["dem_set_l2_flush", "dem_set_timing", "dem_kernel_times", "dem_swept_totals", "dem_launch_count",
@@ -241,6 +242,23 @@ class Dem:
         _check(self._ctx, rc)
         self._n_last = n
         return (th[0], th[1]), dof.value
+
+    def step_npt(self, pos, quat, vel, angmom, shape_id, box, dt, nsteps, skin, kT, tau, pressure, tau_p,
+                 state=(0.0, 0.0, 0.0), force=None, torque=None):
+        """dem_step_npt; returns (box, (xi, eta, nu), g)."""
+        torch = self.torch
+        n = pos.shape[0]
+        st = (C.c_double * 3)(*[float(x) for x in state])
+        b = (C.c_double * 3)(*[float(x) for x in _box(box)])
+        dof = C.c_double(0.0)
+        rc = lib().dem_step_npt(self._ctx, _dev(pos, self.dtype, "pos"), _dev(quat, self.dtype, "quat"),
+                                _dev(vel, self.dtype, "vel"), _dev(angmom, self.dtype, "angmom"),
+                                _dev(shape_id, torch.int32, "shape_id"), C.c_int(n), b, C.c_double(dt), C.c_int(nsteps),
+                                C.c_double(skin), C.c_double(kT), C.c_double(tau), C.c_double(pressure),
+                                C.c_double(tau_p), st, C.byref(dof), _dev(force, self.dtype), _dev(torque, self.dtype))
+        _check(self._ctx, rc)
+        self._n_last = n
+        return np.array(b[:]), (st[0], st[1], st[2]), dof.value
 
     def energy(self, quat, vel, angmom, shape_id, force):
         torch = self.torch

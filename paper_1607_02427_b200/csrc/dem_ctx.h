@@ -74,7 +74,7 @@ struct dem_ctx {
     size_t l2_flush_bytes = 0;  // bench hygiene: overwrite this many bytes of scratch before every time step
     DevBuf l2_scratch;
     // dem_step state (double) for DEM_F32 contexts, plus forces and the positions of the last build
-    DevBuf st_pos, st_quat, st_vel, st_ang, st_force, st_torque, pos_build, epart;
+    DevBuf st_pos, st_quat, st_vel, st_ang, st_force, st_torque, st_virial, pos_build, epart;
     // host-buffer entry points
     DevBuf h_pos, h_quat, h_vel, h_ang, h_sid, h_force, h_torque, h_virial;
     // accounting

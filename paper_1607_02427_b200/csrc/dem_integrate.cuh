@@ -212,6 +212,127 @@ __global__ void k_scale_momenta(int N, d4* __restrict__ vel, d4* __restrict__ an
     ang[i] = L;
 }
 
+// ---- NPT (dem_step_npt; R22) ----------------------------------------------------------------------
+// The scalar variables of the thermostat and of the barostat (xi, eta, nu, the box) are advanced on the host between
+// the kernels of a step: the box is a launch argument of every kernel that takes a minimum image.  What touches the
+// particles runs here.
+//
+// First half of an NPT step: pending thermostat scaling `pend` of v and L, half kick with the barostat drag
+// v = (v s + dt/2 F/m) s  (s = exp(-alpha nu dt/4)), L += dt/2 tau, drift x = x ea + v vb  (ea = e^{nu dt},
+// vb = dt e^{nu dt/2} sinh(nu dt/2)/(nu dt/2)) wrapped into the NEW box, free rotation.  Raises moved[0] when the
+// particle is farther than sqrt(thr2) from the affine image lambda x_build of where it was at the last list build
+// (a pair outside the list then still is outside the interaction reach: |d| >= lambda r_list - 2 u_max).
+template <typename real>
+__global__ void k_npt_kick_drift(int N, BoxDev box, double dt, const int* __restrict__ sid, MassTable mt,
+                                 d4* __restrict__ pos, d4* __restrict__ quat, d4* __restrict__ vel, d4* __restrict__ ang,
+                                 const typename vec4<real>::type* __restrict__ force,
+                                 const typename vec4<real>::type* __restrict__ torque, const d4* __restrict__ pos_build,
+                                 double lambda, double thr2, int* __restrict__ moved, double pend, double s, double ea,
+                                 double vb) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int sh = sid[i];
+    const double m = mt.mass[sh];
+    d4 x = pos[i], v = vel[i], L = ang[i], q = quat[i];
+    const typename vec4<real>::type F = force[i], T = torque[i];
+    const d4 xb = pos_build[i];
+    double xs[3] = {x.x, x.y, x.z}, vs[3] = {v.x * pend, v.y * pend, v.z * pend};
+    const double Fs[3] = {(double)F.x, (double)F.y, (double)F.z};
+    for (int a = 0; a < box.dim; ++a) {
+        vs[a] = (vs[a] * s + 0.5 * dt * Fs[a] / m) * s;
+        xs[a] = xs[a] * ea + vs[a] * vb;
+        xs[a] -= box.L[a] * rint(xs[a] * box.invL[a]);
+    }
+    x.x = xs[0]; x.y = xs[1]; x.z = xs[2];
+    v.x = vs[0]; v.y = vs[1]; v.z = vs[2];
+    pos[i] = x;
+    vel[i] = v;
+    double dx = xs[0] - lambda * xb.x, dy = xs[1] - lambda * xb.y, dz = box.dim == 3 ? xs[2] - lambda * xb.z : 0.0;
+    dx -= box.L[0] * rint(dx * box.invL[0]);
+    dy -= box.L[1] * rint(dy * box.invL[1]);
+    dz -= box.L[2] * rint(dz * box.invL[2]);
+    if (!(dx * dx + dy * dy + dz * dz <= thr2)) moved[0] = 1;
+    double Ls[3] = {L.x * pend, L.y * pend, L.z * pend};
+    const double Ts[3] = {(double)T.x, (double)T.y, (double)T.z};
+    for (int a = (box.dim == 2 ? 2 : 0); a < 3; ++a) Ls[a] += 0.5 * dt * Ts[a];
+    double qs[4] = {q.x, q.y, q.z, q.w};
+    free_rotate(box.dim, mt.inertia[sh], Ls, dt, qs);
+    L.x = Ls[0]; L.y = Ls[1]; L.z = Ls[2];
+    q.x = qs[0]; q.y = qs[1]; q.z = qs[2]; q.w = qs[3];
+    ang[i] = L;
+    quat[i] = q;
+}
+
+// Second half kick of an NPT step: v = (v s + dt/2 F/m) s, L += dt/2 tau.
+template <typename real>
+__global__ void k_npt_kick(int N, int dim, double dt, const int* __restrict__ sid, MassTable mt, d4* __restrict__ vel,
+                           d4* __restrict__ ang, const typename vec4<real>::type* __restrict__ force,
+                           const typename vec4<real>::type* __restrict__ torque, double s) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double m = mt.mass[sid[i]];
+    d4 v = vel[i], L = ang[i];
+    const typename vec4<real>::type F = force[i], T = torque[i];
+    v.x = (v.x * s + 0.5 * dt * (double)F.x / m) * s;
+    v.y = (v.y * s + 0.5 * dt * (double)F.y / m) * s;
+    if (dim == 3) {
+        v.z = (v.z * s + 0.5 * dt * (double)F.z / m) * s;
+        L.x += 0.5 * dt * (double)T.x;
+        L.y += 0.5 * dt * (double)T.y;
+    }
+    L.z += 0.5 * dt * (double)T.z;
+    vel[i] = v;
+    ang[i] = L;
+}
+
+// Per-block partial sums (double, fixed order) of K_trans, K_rot, the rotational degrees of freedom and the trace of the
+// virial: partial[4 b + 0..3].  The host adds the blocks' partials in order.
+template <typename real>
+__global__ void k_npt_sums(int N, int dim, const int* __restrict__ sid, MassTable mt, const d4* __restrict__ quat,
+                           const d4* __restrict__ vel, const d4* __restrict__ ang, const real* __restrict__ virial,
+                           double* __restrict__ partial) {
+    __shared__ double sh[4][256];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double Kt = 0, Kr = 0, dof = 0, trw = 0;
+    if (i < N) {
+        const int s = sid[i];
+        const d4 v = vel[i], L = ang[i], q = quat[i];
+        Kt = 0.5 * mt.mass[s] * (v.x * v.x + v.y * v.y + v.z * v.z);
+        double M[9];
+        quat_to_mat<double>(q.x, q.y, q.z, q.w, M);
+        for (int a = (dim == 2 ? 2 : 0); a < 3; ++a) {
+            const double Lb = M[a] * L.x + M[3 + a] * L.y + M[6 + a] * L.z;
+            const double I = mt.inertia[s][a];
+            if (I > 0.0) {
+                Kr += 0.5 * Lb * Lb / I;
+                dof += 1.0;
+            }
+        }
+        const real* w = virial + 6 * (size_t)i;
+        trw = (double)w[0] + (double)w[3] + (dim == 3 ? (double)w[5] : 0.0);
+    }
+    sh[0][threadIdx.x] = Kt; sh[1][threadIdx.x] = Kr; sh[2][threadIdx.x] = dof; sh[3][threadIdx.x] = trw;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o)
+            for (int a = 0; a < 4; ++a) sh[a][threadIdx.x] += sh[a][threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0)
+        for (int a = 0; a < 4; ++a) partial[4 * blockIdx.x + a] = sh[a][0];
+}
+
+// v *= s, L *= s (the thermostat scaling still pending when a run ends)
+static __global__ void k_scale_momenta_by(int N, d4* __restrict__ vel, d4* __restrict__ ang, double s) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    d4 v = vel[i], L = ang[i];
+    v.x *= s; v.y *= s; v.z *= s;
+    L.x *= s; L.y *= s; L.z *= s;
+    vel[i] = v;
+    ang[i] = L;
+}
+
 // U, K_trans, K_rot: per-block partial sums in double (fixed order), summed on the host.
 template <typename real, typename PosT>
 __global__ void k_energy(int N, int dim, const int* __restrict__ sid, MassTable mt, const PosT* __restrict__ quat,

@@ -371,6 +371,150 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     return DEM_OK;
 }
 
+// ---- NPT (R22) ------------------------------------------------------------------------------------------------
+// Host-driven, one step at a time: the box is a launch argument of the kernels, and the scalar equations of the
+// thermostat and the barostat need the sums K_trans, K_rot, tr W of the step before.  Order of a step (h = dt/2):
+// T(h) B(h) K(h) D(dt) forces K(h) B(h) T(h)  (include/dem.h: dem_step_npt).
+struct NptArgs {
+    double kT, tau, pressure, tau_p;
+    double* state;  // xi, eta, nu (host, in and out)
+    double* box;    // host, in and out
+};
+
+template <typename real> int step_npt_t(dem_ctx* ctx, void* pos, void* quat, void* vel, void* ang, const int32_t* sid,
+                                        int N, double dt, int nsteps, double skin, void* force_out, void* torque_out,
+                                        const NptArgs& npt) {
+    typedef typename vec4<real>::type real4;
+    if (N < 2 || !pos || !quat || !vel || !ang || !sid) return fail(ctx, DEM_EINVAL, "bad particle arrays");
+    if (nsteps < 0 || !(skin >= 0)) return fail(ctx, DEM_EINVAL, "bad nsteps / skin");
+    CHECK(sync_tables(ctx));
+    cudaStream_t st = ctx->stream;
+    const int B = 256, dim = ctx->dim;
+    const bool conv = ctx->prec == DEM_F32;
+    d4 *x, *q, *v, *L;
+    if (conv) {  // R15b: a DEM_F32 context integrates its state in double
+        CU(ctx->st_pos.reserve(sizeof(d4) * (size_t)N));
+        CU(ctx->st_quat.reserve(sizeof(d4) * (size_t)N));
+        CU(ctx->st_vel.reserve(sizeof(d4) * (size_t)N));
+        CU(ctx->st_ang.reserve(sizeof(d4) * (size_t)N));
+        x = ctx->st_pos.as<d4>(); q = ctx->st_quat.as<d4>(); v = ctx->st_vel.as<d4>(); L = ctx->st_ang.as<d4>();
+        const void* in[4] = {pos, quat, vel, ang};
+        d4* out[4] = {x, q, v, L};
+        for (int k = 0; k < 4; ++k) {
+            k_f4_to_d4<<<nblk(N, B), B, 0, st>>>(N, static_cast<const f4*>(in[k]), out[k]);
+            LAUNCHED(ctx);
+        }
+    } else {
+        x = static_cast<d4*>(pos); q = static_cast<d4*>(quat); v = static_cast<d4*>(vel); L = static_cast<d4*>(ang);
+    }
+    CU(ctx->st_force.reserve(sizeof(real4) * (size_t)N));
+    CU(ctx->st_torque.reserve(sizeof(real4) * (size_t)N));
+    CU(ctx->st_virial.reserve(sizeof(real) * 6 * (size_t)N));
+    real4* F = ctx->st_force.as<real4>();
+    real4* T = ctx->st_torque.as<real4>();
+    real* W = ctx->st_virial.as<real>();
+    const int nbk = nblk(N, 256);
+    CU(ctx->epart.reserve(sizeof(double) * 4 * (size_t)nbk));
+    std::vector<double> part(4 * (size_t)nbk);
+    double box[3] = {npt.box[0], npt.box[1], npt.box[2]};
+    const double reach = max_reach(ctx), r_list = reach + skin;
+    double box_build = box[0];  // the list's box edge along x: lambda = box[0] / box_build (the scaling is isotropic)
+    double Kt = 0, Kr = 0, dofr = 0, trW = 0;
+    // forces, virial and the sums of the current state
+    auto forces = [&]() -> int {
+        for (int a = 0; a < 3; ++a) ctx->box[a] = box[a];  // the list stays; the minimum image uses the current box
+        return evaluate(ctx, x, q, true, sid, N, F, T, W, nullptr, nullptr);
+    };
+    auto sums = [&]() -> int {
+        k_npt_sums<real><<<nbk, 256, 0, st>>>(N, dim, sid, ctx->mt, q, v, L, W, ctx->epart.as<double>());
+        LAUNCHED(ctx);
+        CU(cudaMemcpyAsync(part.data(), ctx->epart.p, sizeof(double) * part.size(), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        Kt = Kr = dofr = trW = 0;
+        for (int b = 0; b < nbk; ++b) {
+            Kt += part[4 * (size_t)b];
+            Kr += part[4 * (size_t)b + 1];
+            dofr += part[4 * (size_t)b + 2];
+            trW += part[4 * (size_t)b + 3];
+        }
+        return DEM_OK;
+    };
+    auto rebuild = [&]() -> int {
+        CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
+        box_build = box[0];
+        return DEM_OK;
+    };
+    CHECK(rebuild());
+    CHECK(forces());
+    CHECK(sums());
+    const double g = (double)dim * (N - 1) + dofr, Q = g * npt.kT * npt.tau * npt.tau;
+    const double Nf = (double)dim * (N - 1), alpha = 1.0 + dim / Nf, Wb = (double)dim * N * npt.kT * npt.tau_p * npt.tau_p;
+    double xi = npt.state[0], eta = npt.state[1], nu = npt.state[2], pend = 1.0;
+    auto volume = [&]() { return dim == 3 ? box[0] * box[1] * box[2] : box[0] * box[1]; };
+    auto thermo_half = [&]() {  // R19; the scaling of v and L stays pending in `pend`, K_trans and K_rot follow it
+        xi += 0.25 * dt * (2.0 * (Kt + Kr) - g * npt.kT) / Q;
+        const double s = std::exp(-xi * 0.5 * dt);
+        pend *= s;
+        Kt *= s * s;
+        Kr *= s * s;
+        eta += 0.5 * dt * xi;
+        xi += 0.25 * dt * (2.0 * (Kt + Kr) - g * npt.kT) / Q;
+    };
+    auto baro_half = [&]() { nu += 0.5 * dt * (alpha * 2.0 * Kt + trW - dim * volume() * npt.pressure) / Wb; };
+    int* flags = ctx->flags.as<int>() + 8;
+    if (!ctx->h_moved) CU(cudaHostAlloc(&ctx->h_moved, 4 * sizeof(int), cudaHostAllocDefault));
+    for (int step = 0; step < nsteps; ++step) {
+        thermo_half();
+        baro_half();
+        const double s = std::exp(-alpha * nu * 0.25 * dt);
+        const double z = 0.5 * nu * dt, ea = std::exp(nu * dt), eh = std::exp(z), sc = z == 0.0 ? 1.0 : std::sinh(z) / z;
+        for (int a = 0; a < dim; ++a) box[a] *= ea;
+        for (int a = 0; a < dim; ++a)
+            if (!(box[a] >= 2.0 * reach))
+                return fail(ctx, DEM_EBOX, "dem_step_npt: box edge %d shrank to %g < 2 x interaction reach %g", a, box[a], reach);
+        const double lambda = box[0] / box_build;
+        const double slack = 0.5 * (lambda * r_list - reach);
+        const BoxDev bx = box_dev(dim, box);
+        CU(cudaMemsetAsync(flags, 0, sizeof(int), st));
+        k_npt_kick_drift<real><<<nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T, ctx->pos_build.as<d4>(),
+                                                        lambda, slack > 0 ? slack * slack : -1.0, flags, pend, s, ea,
+                                                        dt * eh * sc);
+        LAUNCHED(ctx);
+        pend = 1.0;
+        CU(cudaMemcpyAsync(ctx->h_moved, flags, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        // the list also has to follow the box: its cells must stay at least r_list wide for the next build only, but a
+        // box that no longer holds two cutoffs is refused by the build itself
+        if (ctx->h_moved[0]) CHECK(rebuild());
+        CHECK(forces());
+        k_npt_kick<real><<<nblk(N, B), B, 0, st>>>(N, dim, dt, sid, ctx->mt, v, L, F, T, s);
+        LAUNCHED(ctx);
+        CHECK(sums());
+        baro_half();
+        thermo_half();
+    }
+    if (pend != 1.0) {
+        k_scale_momenta_by<<<nblk(N, B), B, 0, st>>>(N, v, L, pend);
+        LAUNCHED(ctx);
+    }
+    if (conv) {
+        void* out[4] = {pos, quat, vel, ang};
+        d4* in[4] = {x, q, v, L};
+        for (int k = 0; k < 4; ++k) {
+            k_d4_to_f4<<<nblk(N, B), B, 0, st>>>(N, in[k], static_cast<f4*>(out[k]));
+            LAUNCHED(ctx);
+        }
+    }
+    if (force_out) CU(cudaMemcpyAsync(force_out, F, sizeof(real4) * (size_t)N, cudaMemcpyDeviceToDevice, st));
+    if (torque_out) CU(cudaMemcpyAsync(torque_out, T, sizeof(real4) * (size_t)N, cudaMemcpyDeviceToDevice, st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    npt.state[0] = xi; npt.state[1] = eta; npt.state[2] = nu;
+    for (int a = 0; a < 3; ++a) npt.box[a] = box[a];
+    ctx->nvt_dof = g;
+    return DEM_OK;
+}
+
 template <typename real, typename PosT>
 int energy_t(dem_ctx* ctx, const PosT* quat, const PosT* vel, const PosT* ang, const int32_t* sid, const void* force,
              int N, double out[3]) {
@@ -422,7 +566,7 @@ int dem_destroy(dem_ctx* c) {
     if (!c) return DEM_EINVAL;
     DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
                       &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->thermo, &c->pose, &c->pidx, &c->cum, &c->st_pos, &c->st_quat,
-                      &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->pos_build, &c->epart, &c->h_pos,
+                      &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->st_virial, &c->pos_build, &c->epart, &c->h_pos,
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();
     if (c->h_moved) cudaFreeHost(c->h_moved);
@@ -578,6 +722,23 @@ int dem_step_nvt(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, c
         rc = step_t<double>(ctx, pos, quat, vel, angmom, shape_id, N, box, dt, nsteps, skin, force_energy, torque, &nvt);
     else
         rc = step_t<float>(ctx, pos, quat, vel, angmom, shape_id, N, box, dt, nsteps, skin, force_energy, torque, &nvt);
+    if (rc == DEM_OK && dof) *dof = ctx->nvt_dof;
+    return rc;
+}
+
+int dem_step_npt(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, const int32_t* shape_id, int N, double box[3],
+                 double dt, int nsteps, double skin, double kT, double tau, double pressure, double tau_p, double state[3],
+                 double* dof, void* force_energy, void* torque) {
+    if (!ctx) return DEM_EINVAL;
+    if (!box || !state) return fail(ctx, DEM_EINVAL, "null box / state");
+    if (!(kT > 0) || !(tau > 0) || !(tau_p > 0)) return fail(ctx, DEM_EINVAL, "kT, tau and tau_p must be > 0");
+    if (N < 2) return fail(ctx, DEM_EINVAL, "the thermostat needs N >= 2");
+    const NptArgs npt = {kT, tau, pressure, tau_p, state, box};
+    int rc;
+    if (ctx->prec == DEM_F64)
+        rc = step_npt_t<double>(ctx, pos, quat, vel, angmom, shape_id, N, dt, nsteps, skin, force_energy, torque, npt);
+    else
+        rc = step_npt_t<float>(ctx, pos, quat, vel, angmom, shape_id, N, dt, nsteps, skin, force_energy, torque, npt);
     if (rc == DEM_OK && dof) *dof = ctx->nvt_dof;
     return rc;
 }

@@ -132,21 +132,25 @@ def _drift(pkg, st, dt, eps_par=None):
 @pytest.mark.parametrize("kind,cells,dt,eps_par", [("squares", 10, 2e-5, None), ("octahedra", 5, 1.6e-5, None),
                                                    ("cubes", 5, 4e-6, 0.0)])
 def test_dense_state_drift_gate_f64(pkg, kind, cells, dt, eps_par):
-    """Interacting dense states (hundreds of active terms), FP64, 10^4 steps: drift per particle below 1e-4
-    (north_star).  dt is small because these lattices start strongly compressed (U/N = 3.3 eps for the squares,
-    28 eps for the cubes with 18 neighbours each): the truncation error of velocity Verlet on these states scales as
-    dt^2 (measured on the GPU: octahedra -7.1e-5 / -1.7e-5 / -4.4e-6 at dt = 1.6e-5 / 8e-6 / 4e-6).
-    The near-aligned cubes run with the parallel-edge rule off (eps_par = 0), which makes the force the exact gradient
-    of U; the rule's own energy cost is the next test."""
+    """That north_star's bar (max |E(t) - E(0)|/N < 1e-4 over 10^4 steps) CAN be met on interacting dense states
+    (hundreds of active terms, FP64) -- at the dt their stiffness needs.  These lattices start strongly compressed
+    (U/N = 3.3 epsilon for the squares, 28 epsilon for the cubes with 18 neighbours each), and the truncation error of
+    velocity Verlet on them goes as dt^2 (the same states at the configs' dt = 2e-4 are measured, not
+    gated at 1e-4, in test_dense_states_at_a_config_timestep_with_the_parallel_rule_on).  The dt values below were
+    chosen AFTER measuring (octahedra: -7.1e-5 / -1.7e-5 / -4.4e-6 at dt = 1.6e-5 / 8e-6 / 4e-6), and the near-aligned
+    cubes run with the parallel-edge rule OFF (eps_par = 0: the force is then the exact gradient of U); with the rule
+    on they do not meet the bar at any dt tried (next test).  DESIGN.md R18 records this."""
     worst = _drift(pkg, di.dense_state(kind, cells), dt, eps_par)
     assert worst < 1e-4, worst
 
 
 def test_parallel_edge_rule_energy_cost(pkg):
     """PAPER.md:59 moves the interaction point discontinuously when two edges cross the 'sufficiently parallel'
-    threshold (R5).  In the near-aligned dense cube state (all rotations <= 0.05 rad) edges cross it all the
-    time; measured on the GPU at dt = 4e-6 the total energy then wanders by +-2.7e-4 eps per particle over 10^4 steps
-    (5e-5 with the rule off, previous test).  Gate: the cost stays below 2e-3 eps per particle."""
+    threshold (R5), so inside that branch the force is not the gradient of U.  In the near-aligned dense cube
+    state (all rotations <= 0.05 rad) edges cross the threshold all the time: measured at dt = 4e-6 the total energy
+    wanders by 2.7e-4 epsilon per particle over 10^4 steps with the rule on (5e-5 with it off, previous test): this
+    state does NOT meet north_star's 1e-4 with the paper's rule on.  The assertion only bounds the cost of the rule
+    (an order of magnitude above the reading); it is a record, not a pass of the bar."""
     worst = _drift(pkg, di.dense_state("cubes", 5), 4e-6)
     assert worst < 2e-3, worst
 
@@ -165,22 +169,26 @@ def test_step_host_matches_device(pkg):
     dem.close()
 
 
-@pytest.mark.parametrize("k,skin", [(3, 0.2), (4, 0.3)])
-def test_full_size_fp32_runs_of_the_configs(pkg, oracle, k, skin):
-    """BASELINE.json configs 3 and 4 as stated: FP32, force evaluation + 1000 NVE steps at the config's dt (the launch
-    configuration bench.py times).  Reported: max_t |E(t) - E(0)| / N (R18 gates the drift in FP64 only; the
-    FP32 contexts integrate in double with FP32 forces, so a loose bound of 1e-3 eps per particle is asserted).
-    P1: the state REACHED by the run -- particles have moved, pairs have left the reach, contacts have
-    formed -- is evaluated again and sampled rows are compared with the oracle at the north_star tolerance."""
-    import torch
+def _lsq_drift(steps, e_per_particle):
+    """Least-squares slope of E/N against the step number, times 10^4 steps: PAPER.md:85 reports the long-term drift as
+    a rate ((E(t) - E(0))/N per unit time); north_star's bar is that rate over 10^4 steps."""
+    return float(np.polyfit(steps, e_per_particle, 1)[0] * 1e4)
+
+
+@pytest.mark.parametrize("k,skin,nsteps", [(3, 0.2, 1000), (4, 0.3, 1000), (5, 0.3, 400)])
+def test_full_size_fp32_runs_of_the_configs(pkg, oracle, k, skin, nsteps):
+    """BASELINE.json configs 3, 4 and 5 at full size: FP32, force evaluation + NVE steps at the config's dt (the launch
+    configuration bench.py times; config 5 names no run length: 400 steps).  P1: the state REACHED by
+    the run -- particles have moved, pairs have left the reach, contacts have formed -- is evaluated again and EVERY
+    row is compared with the oracle at the north_star tolerance, with the scales taken from the oracle's side."""
+    from _gpu_util import scales
 
     st = round_state(di.make_config(k), "f32")
-    got = _run(pkg, st, "f32", st["dt"], 1000, skin=skin, chunks=10)
+    got = _run(pkg, st, "f32", st["dt"], nsteps, skin=skin, chunks=10)
     e = got["energies"].sum(1)
-    drift = np.abs(e - got["e0"]).max() / st["N"]
-    print("config %d: N = %d, 1000 steps, dt = %g: max |E(t) - E(0)| / N = %.3e" % (k, st["N"], st["dt"], drift))
-    assert np.isfinite(e).all() and drift < 1e-3, drift
-    # P1: parity on the reached state
+    dev = np.abs(e - got["e0"]).max() / st["N"]
+    print("config %d: N = %d, %d steps, dt = %g: max |E(t) - E(0)| / N = %.3e" % (k, st["N"], nsteps, st["dt"], dev))
+    assert np.isfinite(e).all() and dev < 1e-3, dev
     end = dict(st)
     for key in ("pos", "quat", "vel", "angmom"):
         end[key] = got[key]
@@ -189,16 +197,58 @@ def test_full_size_fp32_runs_of_the_configs(pkg, oracle, k, skin):
     f, tq, w = dem.compute(t["pos"], t["quat"], t["shape_id"])
     cnt = dem.get_counters()
     dem.close()
-    f, tq = f.cpu().numpy().astype(np.float64), tq.cpu().numpy().astype(np.float64)
-    sub = np.sort(np.random.default_rng(40 + k).choice(st["N"], 128, replace=False)).astype(np.int32)
-    of, ot, _, _ = oracle.compute(end, subset=sub)
-    sig = min(2 * s["rounding"] for s in st["shapes"])
-    fs = max(np.abs(f[:, :3]).max(), 1.0 / sig)
-    ts = max(np.abs(tq[:, :3]).max(), 1.0)
-    assert np.abs(f[sub, :3] - of[:, :3]).max() / fs < 1e-4
-    assert np.abs(tq[sub, :3] - ot[:, :3]).max() / ts < 1e-4
-    assert np.abs(f[sub, 3] - of[:, 3]).max() / max(np.abs(of[:, 3]).max(), 1.0) < 1e-4
-    assert cnt["active"] > 0
+    f, tq, w = (a.cpu().numpy().astype(np.float64) for a in (f, tq, w))
+    of, ot, ow, ocnt = oracle.compute(end, cells=True)           # every row, bit-identical to the all-pairs definition
+    fs, ts, us = scales(end, of, ot)                             # denominators from the oracle alone
+    active = int((np.abs(of[:, :3]).sum(1) > 0).sum())
+    print("config %d reached state: %d interacting particles, %d active terms" % (k, active, ocnt[2] // 2))
+    assert active >= 500, active
+    assert np.abs(f[:, :3] - of[:, :3]).max() / fs < 1e-4
+    assert np.abs(tq[:, :3] - ot[:, :3]).max() / ts < 1e-4
+    assert np.abs(f[:, 3] - of[:, 3]).max() / us < 1e-4
+    assert np.abs(w - ow).max() / max(np.abs(ow).max(), 1.0) < 1e-4
+    assert 2 * cnt["active"] == ocnt[2] and 2 * cnt["degenerate"] == ocnt[3] and 2 * cnt["parallel"] == ocnt[4]
+
+
+def test_config3_drift_is_truncation_not_precision(pkg):
+    """Config 3 (FP32, dt = 5e-4) shows max |E(t) - E(0)|/N = 2.3e-4, above north_star's 1e-4.  What that number is:
+    (i) the same run in a DEM_F64 context reads the same value, so it is not single precision; (ii) at dt/2 it drops by
+    ~4: the O(dt^2) offset of a second-order integrator started from a lattice, reached within the first
+    few hundred steps; (iii) it does not grow: the least-squares drift over 10^4 steps -- the measure PAPER.md:85
+    reports -- is below 1e-4 per particle (R18)."""
+    st = di.make_config(3)
+    steps = np.arange(1, 51) * 200
+    r32 = _run(pkg, st, "f32", st["dt"], 10000, skin=0.2, chunks=50)
+    r64 = _run(pkg, st, "f64", st["dt"], 10000, skin=0.2, chunks=50)
+    e32, e64 = r32["energies"].sum(1) / st["N"], r64["energies"].sum(1) / st["N"]
+    d32, d64 = np.abs(e32 - r32["e0"] / st["N"]).max(), np.abs(e64 - r64["e0"] / st["N"]).max()
+    s32, s64 = _lsq_drift(steps, e32), _lsq_drift(steps, e64)
+    half = _run(pkg, st, "f64", st["dt"] / 2, 4000, skin=0.2, chunks=20)
+    dh = np.abs(half["energies"].sum(1) - half["e0"]).max() / st["N"]
+    print("config 3, 10^4 steps: max dev f32 %.3e f64 %.3e; lsq drift per 10^4 steps f32 %.3e f64 %.3e; f64 at dt/2 "
+          "(2000 tau-equivalent steps) max dev %.3e" % (d32, d64, s32, s64, dh))
+    assert abs(d32 - d64) < 0.1 * d64, (d32, d64)
+    assert 2.8 < d64 / dh < 5.5, (d64, dh)
+    assert abs(s32) < 1e-4 and abs(s64) < 1e-4, (s32, s64)
+
+
+@pytest.mark.parametrize("kind,cells", [("cubes", 5), ("octahedra", 5), ("squares", 10)])
+def test_dense_states_at_a_config_timestep_with_the_parallel_rule_on(pkg, kind, cells):
+    """The dense parity states at dt = 2e-4 (the dt of configs 4 and 5), FP64, parallel-edge rule ON, 10^4 steps.  They
+    start strongly compressed (U/N = 28 / 8 / 3.3 epsilon for cubes / octahedra / squares, contacts at 0.77 sigma where
+    the force is ~30x that at sigma), unlike the configs' fluids, so their truncation error at this dt is far above
+    north_star's bar (measured max |E(t) - E(0)|/N: 7.8e-2, 1.1e-2, 1.8e-3).  What is asserted is what the paper states
+    (PAPER.md:83): the error is second order -- halving dt divides it by ~4 -- and small against E/N itself."""
+    st = di.dense_state(kind, cells)
+    dev = []
+    for dt in (2e-4, 1e-4):
+        out = _run(pkg, st, "f64", dt, 10000, skin=0.3, chunks=50)
+        e = out["energies"].sum(1)
+        dev.append(np.abs(e - out["e0"]).max() / st["N"])
+    print("dense %s, parallel rule on: max |E(t) - E(0)|/N = %.3e (dt 2e-4), %.3e (dt 1e-4); E/N = %.2f"
+          % (kind, dev[0], dev[1], out["e0"] / st["N"]))
+    assert 2.8 < dev[0] / dev[1] < 5.5, dev
+    assert dev[0] < 5e-3 * abs(out["e0"]) / st["N"], dev
 
 
 @pytest.mark.parametrize("shape", di.TABLE1_SHAPES)
@@ -279,6 +329,91 @@ def test_nvt_fp32_reaches_the_target_temperature(pkg):
     assert abs(e.sum() - e0.sum()) / n > 1.0
 
 
+@pytest.mark.parametrize("kind,cells,spacing,dt", [("cubes", 4, 1.38, 5e-4), ("squares", 8, None, 5e-4),
+                                                   ("mixed", 4, None, 2.5e-4)])
+def test_npt_matches_oracle_f64(pkg, oracle, kind, cells, spacing, dt):
+    """dem_step_npt (R22) against orc_step_npt: trajectory, box, thermostat and barostat variables.
+    The run is split over three calls (state and box handed back in) with a thin skin, so that the list is rebuilt
+    while the box is moving."""
+    import torch
+
+    st = di.dense_state(kind, cells, spacing=spacing)
+    kT, tau, p, tau_p, n = 0.8, 0.1, 4.0, 0.25, 90
+    ref = oracle.step_npt(st, dt, n, kT, tau, p, tau_p)
+    dem, t = pkg.from_state(st, "f64")
+    f = torch.empty((st["N"], 4), dtype=torch.float64, device="cuda")
+    box, state, l0 = st["box"].copy(), (0.0, 0.0, 0.0), dem.launch_count()
+    for part in range(3):
+        box, state, dof = dem.step_npt(t["pos"], t["quat"], t["vel"], t["angmom"], t["shape_id"], box, dt, n // 3, 0.05,
+                                       kT, tau, p, tau_p, state, f)
+        row = ref["energies"][(part + 1) * (n // 3)]
+        e = dem.energy(t["quat"], t["vel"], t["angmom"], t["shape_id"], f)
+        assert np.allclose(e, row[:3], rtol=1e-9, atol=1e-9)
+        assert all(abs(state[k] - row[3 + k]) < 1e-9 for k in range(3)), (state, row)
+        vol = np.prod(box[:st["dim"]])
+        assert abs(vol - row[6]) < 1e-9 * row[6]
+    assert dof == ref["dof"]
+    assert np.allclose(box, ref["box"], rtol=1e-12)
+    for k in ("pos", "quat", "vel", "angmom"):
+        assert np.abs(t[k].cpu().numpy() - ref[k]).max() < 1e-8, k
+    assert abs(ref["baro"][2]) > 1e-3 and abs(ref["box"][0] / st["box"][0] - 1.0) > 1e-3      # the barostat acted
+    dem.close()
+
+
+def test_npt_infinite_barostat_period_is_nvt(pkg):
+    """tau_p = inf: nu stays 0, the box stays put and dem_step_npt walks the trajectory of dem_step_nvt."""
+    import math
+    import torch
+
+    st = di.dense_state("cubes", 4, spacing=1.38)
+    out = []
+    for npt in (False, True):
+        dem, t = pkg.from_state(st, "f64")
+        f = torch.empty((st["N"], 4), dtype=torch.float64, device="cuda")
+        args = (t["pos"], t["quat"], t["vel"], t["angmom"], t["shape_id"], st["box"], 5e-4, 60, 0.2)
+        if npt:
+            box, state, _ = dem.step_npt(*args, 0.8, 0.1, 3.0, math.inf, (0.0, 0.0, 0.0), f)
+            assert np.array_equal(box, st["box"]) and state[2] == 0.0
+            th = state[:2]
+        else:
+            th, _ = dem.step_nvt(*args, 0.8, 0.1, (0.0, 0.0), f)
+        out.append((th, {k: t[k].cpu().numpy() for k in ("pos", "quat", "vel", "angmom")}))
+        dem.close()
+    assert np.allclose(out[0][0], out[1][0], rtol=1e-12, atol=1e-14)
+    for k in ("pos", "quat", "vel", "angmom"):
+        assert np.abs(out[0][1][k] - out[1][1][k]).max() < 1e-11, k
+
+
+def test_npt_fp32_reaches_the_target_pressure(pkg):
+    """FP32 context, 4096 cubes of the Table I stand-in, compressed by the barostat: the conserved quantity
+    U + K + P V + W_b nu^2/2 + Q xi^2/2 + g kT eta stays put while the volume changes by tens of percent (the list is
+    rebuilt as the box moves), and the scaling stays isotropic."""
+    import torch
+
+    st = di.table1_state("cube", 4096)
+    n = st["N"]
+    kT, tau, tau_p = 1.0, 0.1, 0.5
+    v0 = float(np.prod(st["box"]))
+    p = 2.0 * n * kT / v0                       # twice the ideal-gas pressure of the start state: the box must shrink
+    dem, t = pkg.from_state(st, "f32")
+    f = torch.empty((n, 4), dtype=torch.float32, device="cuda")
+    args = (t["pos"], t["quat"], t["vel"], t["angmom"], t["shape_id"])
+    dem.step(*args, st["box"], st["dt"], 0, 0.3, f)
+    e0 = dem.energy(t["quat"], t["vel"], t["angmom"], t["shape_id"], f).sum()
+    box, state, cons, vols = st["box"].copy(), (0.0, 0.0, 0.0), [], []
+    for _ in range(30):
+        box, state, g = dem.step_npt(*args, box, st["dt"], 200, 0.3, kT, tau, p, tau_p, state, f)
+        e = dem.energy(t["quat"], t["vel"], t["angmom"], t["shape_id"], f)
+        vol = float(np.prod(box))
+        vols.append(vol)
+        cons.append(e.sum() + p * vol + 0.5 * 3 * n * kT * tau_p ** 2 * state[2] ** 2
+                    + 0.5 * g * kT * tau ** 2 * state[0] ** 2 + g * kT * state[1])
+    dem.close()
+    assert min(vols) < 0.8 * v0, vols
+    assert np.abs(np.array(cons) - (e0 + p * v0)).max() / n < 5e-3, cons
+    assert np.allclose(box / st["box"], (vols[-1] / v0) ** (1.0 / 3.0), rtol=1e-9)
+
+
 @pytest.mark.parametrize("kind", ["squares", "tetrahedra"])
 def test_fig3_energy_fluctuations_scale_with_dt_squared(pkg, kind):
     """PAPER.md:83-85 (Fig. 3): for a second-order integrator sigma(E/N) over a short NVE run grows as dt^2 until rounding
@@ -294,11 +429,13 @@ def test_fig3_energy_fluctuations_scale_with_dt_squared(pkg, kind):
 
 def test_config4_fp32_drift_over_ten_thousand_steps(pkg):
     """north_star's drift bar (< 1e-4 epsilon per particle over 10^4 NVE steps) on the bench workload itself, in the
-    precision and launch configuration bench.py times: config 4, DEM_F32 context, dt = 2e-4, skin 0.3."""
+    precision and launch configuration bench.py times: config 4, DEM_F32 context, dt = 2e-4, skin 0.3.  Both measures:
+    the largest deviation from E(0) and the least-squares drift."""
     st = di.make_config(4)
     got = _run(pkg, st, "f32", st["dt"], 10000, skin=0.3, chunks=20)
     e = got["energies"].sum(1)
-    drift = np.abs(e - got["e0"]).max() / st["N"]
-    print("config 4, fp32, 10^4 steps: max |E(t) - E(0)| / N = %.3e" % drift)
-    assert drift < 1e-4, drift
+    dev = np.abs(e - got["e0"]).max() / st["N"]
+    slope = _lsq_drift(np.arange(1, 21) * 500, e / st["N"])
+    print("config 4, fp32, 10^4 steps: max |E(t) - E(0)| / N = %.3e, lsq drift per 10^4 steps %.3e" % (dev, slope))
+    assert dev < 1e-4 and abs(slope) < 1e-4, (dev, slope)
     assert got["energies"][-1][0] / st["N"] > 0.01          # a fluid in contact by then, not the initial lattice
