@@ -385,7 +385,8 @@ def test_npt_infinite_barostat_period_is_nvt(pkg):
 
 
 def test_npt_fp32_reaches_the_target_pressure(pkg):
-    """FP32 context, 4096 cubes of the Table I stand-in, compressed by the barostat: the conserved quantity
+    """FP32 context, 4096 cubes of the Table I stand-in (volume fraction 0.5: its pressure is several times the ideal-gas
+    value) under a barostat set to twice the ideal-gas pressure, so the box must grow: the conserved quantity
     U + K + P V + W_b nu^2/2 + Q xi^2/2 + g kT eta stays put while the volume changes by tens of percent (the list is
     rebuilt as the box moves), and the scaling stays isotropic."""
     import torch
@@ -394,7 +395,7 @@ def test_npt_fp32_reaches_the_target_pressure(pkg):
     n = st["N"]
     kT, tau, tau_p = 1.0, 0.1, 0.5
     v0 = float(np.prod(st["box"]))
-    p = 2.0 * n * kT / v0                       # twice the ideal-gas pressure of the start state: the box must shrink
+    p = 2.0 * n * kT / v0                       # twice the ideal-gas pressure of the start state
     dem, t = pkg.from_state(st, "f32")
     f = torch.empty((n, 4), dtype=torch.float32, device="cuda")
     args = (t["pos"], t["quat"], t["vel"], t["angmom"], t["shape_id"])
@@ -409,7 +410,7 @@ def test_npt_fp32_reaches_the_target_pressure(pkg):
         cons.append(e.sum() + p * vol + 0.5 * 3 * n * kT * tau_p ** 2 * state[2] ** 2
                     + 0.5 * g * kT * tau ** 2 * state[0] ** 2 + g * kT * state[1])
     dem.close()
-    assert min(vols) < 0.8 * v0, vols
+    assert max(vols) > 1.2 * v0, vols
     assert np.abs(np.array(cons) - (e0 + p * v0)).max() / n < 5e-3, cons
     assert np.allclose(box / st["box"], (vols[-1] / v0) ** (1.0 / 3.0), rtol=1e-9)
 
