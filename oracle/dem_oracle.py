@@ -19,12 +19,18 @@ DEFAULT_EPS_PAR = 1e-6  # reading R5: parallel <=> |d1 x d2|^2 < eps_par |d1|^2 
 
 
 def build(force=False):
-    """Compile the oracle with gcc (-O2, no FMA contraction, no fast-math)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        tmp = _LIB + ".tmp%d" % os.getpid()
-        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", _SRC, "-o", tmp, "-lm"])
-        os.replace(tmp, _LIB)
-    return _LIB
+    """Compile the oracle with gcc (-O2, no FMA contraction, no fast-math).  With DEM_ORACLE_SANITIZE=1 in the
+    environment a second library is built with -fsanitize=address,undefined and used instead (run python with
+    LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0; profiles/r02_sanitizers.md)."""
+    san = os.environ.get("DEM_ORACLE_SANITIZE") == "1"
+    out = _LIB.replace(".so", "_san.so") if san else _LIB
+    flags = (["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"]
+             if san else ["-O2"])
+    if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(_SRC):
+        tmp = out + ".tmp%d" % os.getpid()
+        subprocess.check_call(["gcc"] + flags + ["-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", _SRC, "-o", tmp, "-lm"])
+        os.replace(tmp, out)
+    return out
 
 
 class _Shapes(C.Structure):

@@ -13,15 +13,21 @@ import hashlib
 import os
 import shutil
 import subprocess
+import time
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.normpath(os.path.join(HERE, "..", "include"))
-OBJDIR = os.path.join(CSRC, "build")
-LIB = os.path.join(HERE, "libdem_b200.so")
+OBJDIR = os.path.join(CSRC, "build")  # object names carry a hash of the flags, so the two builds do not collide
+# DEM_CHECKED=1 in the environment selects the checked build (device-side bounds checks of every index into the kernels'
+# hand-rolled shared-memory structures, csrc/dem_types.h: DEM_ASSERT): another library file, built from the same
+# sources with -DDEM_CHECKED, which binding.lib() then loads instead.  `python -m pytest tests -m gpu` under
+# DEM_CHECKED=1 is the repo's substitute for a compute-sanitizer memcheck run (profiles/r02_sanitizers.md).
+CHECKED = os.environ.get("DEM_CHECKED") == "1"
+LIB = os.path.join(HERE, "libdem_b200_checked.so" if CHECKED else "libdem_b200.so")
 HASHFILE = LIB + ".hash"
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
-              "-Xptxas", "-v"]
+              "-Xptxas", "-v"] + (["-DDEM_CHECKED"] if CHECKED else [])
 
 
 def _nvcc():
@@ -76,7 +82,8 @@ def build(force=False, verbose=False):
         obj = os.path.join(OBJDIR, "%s.%s.o" % (base, key))
         if force or not os.path.exists(obj):
             for old in glob.glob(os.path.join(OBJDIR, base + ".*.o")):
-                os.remove(old)
+                if time.time() - os.path.getmtime(old) > 3600:  # objects of abandoned source states
+                    os.remove(old)
             jobs.append((src, obj))
         else:
             jobs.append((None, obj))

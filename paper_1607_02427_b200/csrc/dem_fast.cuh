@@ -90,6 +90,7 @@ static __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* 
                                          const f4* sp, int nown) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
+    DEM_ASSERT(cnt >= 0 && cnt <= 32 && cnt <= qn && qn <= DEM_QCAP);
     const unsigned e = lane < cnt ? q[lane] : DEM_Q_INVALID;
     const int rem = qn - cnt;
     const unsigned v0 = lane < rem ? q[cnt + lane] : 0u, v1 = lane + 32 < rem ? q[cnt + 32 + lane] : 0u;
@@ -98,6 +99,7 @@ static __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* 
     if (lane + 32 < rem) q[32 + lane] = v1;
     __syncwarp();
     const int owner = e == DEM_Q_INVALID ? lane : (int)(e >> 26);
+    DEM_ASSERT(owner >= 0 && owner < nown);
     float R[9], t[3];
     {
         const f4 p0 = sp[owner], p1 = sp[nown + owner], p2 = sp[2 * nown + owner];
@@ -110,6 +112,10 @@ static __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* 
     if (e != DEM_Q_INVALID) {
         const int phase = (int)((e >> 23) & 7u), o = (int)((e >> 12) & 0x7ffu), k = (int)(e & 0xfffu);
         const ShapeView<float> A = fs->A, B = fs->B;
+        DEM_ASSERT(phase == PH_EE ? (o < B.ne && k < A.ne)
+                   : phase == PH_VF_OWN ? (o < B.nv && k < A.nf)
+                   : phase == PH_VF_OTHER ? (o < A.nv && k < B.nf)
+                   : phase == PH_VE_OWN ? (o < B.nv && k < A.ne) : (phase == PH_VE_OTHER && o < A.nv && k < B.ne));
         const PairConst<float> pc = fs->pc;
         float p[3];
         if (phase == PH_EE) {
@@ -187,6 +193,7 @@ __device__ __forceinline__ void push_one(WarpCtx& w, int phase_a, int phase_b, u
         const bool ha = have && ok_a, hb = have && ok_b;
         const unsigned ba = __ballot_sync(full, ha), bb = __ballot_sync(full, hb);
         const int na = __popc(ba);
+        DEM_ASSERT(w.qn >= 0 && w.qn + na + __popc(bb) <= DEM_QCAP);
         if (ha) w.q[w.qn + __popc(ba & lt)] = q_entry(wa, phase_a, oa, k);
         if (hb) w.q[w.qn + na + __popc(bb & lt)] = q_entry(wb, phase_b, ob, k);
         w.qn += na + __popc(bb);
@@ -446,6 +453,7 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THR
         for (int k = 0; k < warp; ++k) wb += wcount[k];
         const int c = wb + __popc(m & ((1u << lane) - 1u));
         const size_t n = a.plane;
+        DEM_ASSERT(c >= 0 && (size_t)c < n && s_prefix + tot_pad <= (int)n);
         f4 v;
         v.x = R[0]; v.y = R[1]; v.z = R[2]; v.w = R[3]; a.pose[c] = v;
         v.x = R[4]; v.y = R[5]; v.z = R[6]; v.w = R[7]; a.pose[n + c] = v;
@@ -515,6 +523,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
     auto stage = [&](int buf, long long wt_) {
         if (wt_ < n_wtiles) {
             const int c_ = (int)((wt_ * 32 + lane) % np_pad);
+            DEM_ASSERT(c_ >= 0 && (size_t)count <= plane);
             if (c_ < count) {
 #pragma unroll
                 for (int k = 0; k < 6; ++k)
@@ -724,6 +733,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
                 const float Mi[9] = {p3.x, p3.y, p3.z, p3.w, p4.x, p4.y, p4.z, p4.w, p5.x};
                 float out[10];
                 pair_finish<float>(Mi, t, F, T, w.sacc[6 * 32 + lane], out);
+                DEM_ASSERT(spidx[buf * 32 + lane] < a.npairs && slice < a.slices);
                 f4* rec = a.rec + DEM_REC * ((size_t)spidx[buf * 32 + lane] * a.slices + slice);
                 f4 r0, r1, r2;
                 r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
@@ -792,6 +802,10 @@ __device__ __forceinline__ void sweep_items(WarpCtx& w, CullCtx& cc, const Shape
         const bool ok_a = ia < cc.iqn, ok_b = ib < cc.iqn;
         const unsigned ea = ok_a ? cc.iq[ia] : 0u, eb = ok_b ? cc.iq[ib] : ea;
         const int wa = (int)(ea >> 16), oa = (int)(ea & 0xffffu), wb = (int)(eb >> 16), ob = (int)(eb & 0xffffu);
+        DEM_ASSERT(wa >= 0 && wa < w.nown && wb >= 0 && wb < w.nown);
+        DEM_ASSERT(PHASE == PH_EE ? (oa < B.ne && ob < B.ne)
+                   : PHASE == PH_VF_OWN ? (oa < B.nv && ob < B.nv)
+                   : PHASE == PH_VF_OTHER ? (oa < A.nv && ob < A.nv) : ((oa & 0x7fff) < A.nv && (ob & 0x7fff) < A.nv));
         float Ra[9], ta[3], Rb[9], tb[3];
         load_pose(w.sp, w.nown, wa, Ra, ta);
         load_pose(w.sp, w.nown, wb, Rb, tb);
@@ -869,6 +883,7 @@ __device__ __forceinline__ int count_items(const WarpCtx& w, unsigned mask, int&
 __device__ __forceinline__ void write_items(CullCtx& cc, unsigned mask, int owner, int o0, unsigned flag, int offset,
                                             int total) {
     int pos = cc.iqn + offset;
+    DEM_ASSERT(cc.iqn >= 0 && cc.iqn + total <= DEM_IQCAP && offset >= 0 && offset + __popc(mask) <= total);
     while (mask) {
         const int b = __ffs(mask) - 1;
         mask &= mask - 1u;
@@ -943,6 +958,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             const int own = lane + 32 * h, c_ = cbase + own;
+            DEM_ASSERT(c_ >= 0 && c_ < count && (size_t)count <= plane);
 #pragma unroll
             for (int k = 0; k < 6; ++k)
                 asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
@@ -1057,6 +1073,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
             const float Mi[9] = {p3.x, p3.y, p3.z, p3.w, p4.x, p4.y, p4.z, p4.w, p5.x};
             float out[10];
             pair_finish<float>(Mi, tq[h], F, T, w.sacc[6 * 64 + own], out);
+            DEM_ASSERT(spidx[own] < a.npairs && slice < a.slices);
             f4* rec = a.rec + DEM_REC * ((size_t)spidx[own] * a.slices + slice);
             f4 r0, r1, r2;
             r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];

@@ -149,6 +149,7 @@ __global__ void k_reduce(int N, const int* __restrict__ counts, const int* __res
             int c = 0;
             while (c + 1 < nclass && p >= ct.pair_base[c + 1]) ++c;
             const int S = ct.slices[c];
+            DEM_ASSERT(sl >= 0 && p < ct.pair_base[nclass] && p >= ct.pair_base[c]);
             const real4* r = rec + DEM_REC * ((size_t)ct.rec_base[c] + (size_t)(p - ct.pair_base[c]) * S);
             for (int s = 0; s < S; ++s, r += DEM_REC) {
                 const real4 r0 = r[0], r1 = r[1], r2 = r[2];

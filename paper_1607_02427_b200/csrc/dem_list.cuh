@@ -181,6 +181,7 @@ __global__ void k_pair_fill(int N, const int* __restrict__ counts, const int* __
         if (j > i) {
             const int sj = sid[j];
             const int p = loc[ct.lut[si][sj]]++;
+            DEM_ASSERT(p >= 0 && p < ct.pair_base[nclass]);
             const bool i_first = si <= sj;  // the pair's first particle is the one with the smaller shape id
             pairs[p] = i_first ? make_int2(i, j) : make_int2(j, i);
             slot[(size_t)i * stride + k] = 2 * p + (i_first ? 0 : 1);
@@ -208,6 +209,7 @@ __global__ void k_slot_back(int N, const int* __restrict__ counts, const int* __
                 if (q > j && ct.lut[sj][sid[q]] == c) ++r;
             }
             const int p = poff[(size_t)c * N + j] + r;
+            DEM_ASSERT(r < nj && p >= ct.pair_base[c] && p < ct.pair_base[c + 1]);
             const bool j_first = sj <= si;
             slot[(size_t)i * stride + k] = 2 * p + (j_first ? 1 : 0);
         }

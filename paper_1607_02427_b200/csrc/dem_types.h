@@ -4,6 +4,24 @@
 #include <stdint.h>
 #include <vector_types.h>  // int2
 
+// Checked build (python -m paper_1607_02427_b200.build --checked, loaded with DEM_CHECKED=1): every index into the
+// hand-rolled warp-synchronous shared-memory structures (candidate queue, item list, staged poses) and into the pair /
+// record / work-list arrays is bounds-checked on the device; a violation prints its location and traps, which the host
+// sees as a CUDA error.  The release build compiles the checks away.  (compute-sanitizer is not available on the GPU
+// pool this library is developed on; profiles/r02_sanitizers.md.)
+#ifdef DEM_CHECKED
+#include <cstdio>
+#define DEM_ASSERT(cond)                                                                    \
+    do {                                                                                    \
+        if (!(cond)) {                                                                      \
+            printf("DEM_ASSERT failed: %s  (%s:%d)\n", #cond, __FILE__, __LINE__);          \
+            __trap();                                                                       \
+        }                                                                                   \
+    } while (0)
+#else
+#define DEM_ASSERT(cond) ((void)0)
+#endif
+
 namespace dem {
 
 struct alignas(16) f4 { float x, y, z, w; };

@@ -315,12 +315,20 @@ def test_error_codes(pkg):
     dem.close()
 
 
-def test_run_to_run_bit_reproducible(pkg):
-    """No atomics on the accumulation path and a sorted cell list: two runs give identical bits."""
-    st = di.dense_state("mixed", 5)
-    a = gpu_compute(st, "f32")
-    b = gpu_compute(st, "f32")
-    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+@pytest.mark.parametrize("kind,cells,kw", [("mixed", 5, dict(cull=True)), ("mixed", 5, dict(cull=False)),
+                                           ("cubes", 6, dict(cull=True, slices=3)), ("pentagons", 12, dict(kernel=0)),
+                                           ("octahedra", 6, dict(cull=True))])
+def test_run_to_run_bit_reproducible(pkg, kind, cells, kw):
+    """No atomics on the accumulation path, a sorted cell list, ballot-ranked queues: repeated runs give identical bits
+    for force, torque, virial and counters.  The warp-synchronous shared-memory structures of the search kernels
+    (candidate queue, item list, double-buffered pose stages) are the likeliest place for a data race, and a race there
+    would show up as run-to-run differences; six runs on states with hundreds of queued candidates per warp."""
+    st = di.dense_state(kind, cells)
+    runs = [gpu_compute(st, "f32", **kw) for _ in range(6)]
+    assert runs[0][3]["active"] > 50
+    for r in runs[1:]:
+        assert np.array_equal(runs[0][0], r[0]) and np.array_equal(runs[0][1], r[1]) and np.array_equal(runs[0][2], r[2])
+        assert runs[0][3] == r[3]
 
 
 def test_host_buffer_entry_point_matches_device_path(pkg):
