@@ -61,7 +61,7 @@ struct dem_ctx {
     int N = 0, stride = 16, max_count = 0;
     double box[3] = {0, 0, 0}, r_cut = 0;
     GridDev grid;
-    DevBuf cell_of, rank, cell_start, order, xs, counts, list, slot, scratch_scan, pcnt, pairs, rec, flags, counters, thermo;
+    DevBuf cell_of, rank, cell_start, order, xs, counts, list, slot, scratch_scan, pcnt, pairs, rec, rflag, flags, counters, thermo;
     DevBuf cum;         // running totals of the swept-term counters while timing is on
     DevBuf pose, pidx;  // FP32 search kernel: compacted pose records per class (k_pose)
     ClassTable ct;

@@ -48,6 +48,7 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
         a.slices = ctx->ct.slices[c];
         a.n_outer = class_outer(ctx, c);
         a.rec = ctx->rec.as<real4>() + DEM_REC * (size_t)ctx->ct.rec_base[c];
+        a.rflag = ctx->rflag.as<unsigned char>() + (size_t)ctx->ct.rec_base[c];
         a.pos = pos;
         a.quat = quat;
         a.box = bx;
@@ -88,7 +89,7 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
                 pa.plane = list_cap(c);
                 pa.pad = cull ? 64 : 32;  // a warp of k_pair_cull takes 64 entries, of k_pair_fast 32
                 pa.counters = a.counters;
-                pa.rec = reinterpret_cast<f4*>(a.rec);
+                pa.rflag = a.rflag;
                 pa.skip = skip;
                 launch_pose(ctx->dim, pos_is_double, nblk(np, pose_block), st, pa);
                 LAUNCHED(ctx);
@@ -125,11 +126,11 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
     if (kick)
         k_reduce<real, true><<<nblk(4LL * N, 128), 128, 0, st>>>(
             N, ctx->counts.as<int>(), ctx->slot.as<int>(), ctx->stride, sid, ctx->ct, ctx->nclass, ctx->rec.as<real4>(),
-            static_cast<real4*>(force), static_cast<real4*>(torque), static_cast<real*>(virial), skip, *kick);
+            ctx->rflag.as<unsigned char>(), static_cast<real4*>(force), static_cast<real4*>(torque), static_cast<real*>(virial), skip, *kick);
     else
         k_reduce<real, false><<<nblk(4LL * N, 128), 128, 0, st>>>(
             N, ctx->counts.as<int>(), ctx->slot.as<int>(), ctx->stride, sid, ctx->ct, ctx->nclass, ctx->rec.as<real4>(),
-            static_cast<real4*>(force), static_cast<real4*>(torque), static_cast<real*>(virial), skip, KickArgs());
+            ctx->rflag.as<unsigned char>(), static_cast<real4*>(force), static_cast<real4*>(torque), static_cast<real*>(virial), skip, KickArgs());
     LAUNCHED(ctx);
     ev_span(ctx, KT_REDUCE, r0, ev_mark(ctx, 2));
     CU(cudaGetLastError());

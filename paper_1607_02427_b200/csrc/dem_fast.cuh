@@ -85,9 +85,10 @@ __device__ __forceinline__ unsigned q_entry(int owner, int phase, int outer, int
 // per-lane accumulators [7][32] = (F.xyz, T.xyz, u) in the owner's body frame; scnt: this warp's counters (active,
 // degenerate, parallel).  sp: the warp's staged pose records [6][32] (plane-major, indexed by owner lane); the
 // evaluating lane reads its owner's pose from there.
-// Contributions are added to the owner in queue order, so the result does not depend on scheduling.
-static __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* q, float* sacc, unsigned* scnt, int cnt, int qn,
-                                         const f4* sp, int nown) {
+// Contributions are added to the owner in queue order, so the result does not depend on scheduling.  Returns, per lane,
+// which of its owner slots received a contribution (only those pairs get a result record).
+static __device__ __noinline__ unsigned drain_terms(const FastShared* fs, unsigned* q, float* sacc, unsigned* scnt, int cnt,
+                                                    int qn, const f4* sp, int nown) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     DEM_ASSERT(cnt >= 0 && cnt <= 32 && cnt <= qn && qn <= DEM_QCAP);
@@ -148,6 +149,7 @@ static __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* 
         scnt[2] += np;
     }
     unsigned act = __ballot_sync(full, loc.nactive != 0u);
+    unsigned touched = 0u;  // bit h: this lane's owner slot lane + 32 h received a contribution
     while (act) {
         const int s = __ffs(act) - 1;
         act &= act - 1;
@@ -160,9 +162,11 @@ static __device__ __noinline__ void drain_terms(const FastShared* fs, unsigned* 
             sacc[0 * nown + ow] += fx; sacc[1 * nown + ow] += fy; sacc[2 * nown + ow] += fz;
             sacc[3 * nown + ow] += tx; sacc[4 * nown + ow] += ty; sacc[5 * nown + ow] += tz;
             sacc[6 * nown + ow] += uu;
+            touched |= 1u << (ow >> 5);
         }
     }
     __syncwarp();
+    return touched;
 }
 
 // per-warp state of the search loops
@@ -173,8 +177,9 @@ struct WarpCtx {
     unsigned* scnt;
     int qn;    // queued candidates (warp-uniform)
     int lane;
-    const f4* sp;  // staged pose records of the current tile, [6][nown]
+    const f4* sp;  // staged pose records of the current tile, [3][nown] (R, t)
     int nown;      // pairs per warp tile: 32 (k_pair_fast) or 64 (k_pair_cull)
+    unsigned touched;  // bit h: owner slot lane + 32 h of this lane has received a contribution in the current tile
 };
 
 // ---- queue: append the candidates flagged in mask[] and evaluate while a full warp of them is waiting ------------------
@@ -199,7 +204,7 @@ __device__ __forceinline__ void push_one(WarpCtx& w, int phase_a, int phase_b, u
         w.qn += na + __popc(bb);
         __syncwarp();
         while (w.qn >= 32) {
-            drain_terms(w.fs, w.q, w.sacc, w.scnt, 32, w.qn, w.sp, w.nown);
+            w.touched |= drain_terms(w.fs, w.q, w.sacc, w.scnt, 32, w.qn, w.sp, w.nown);
             w.qn -= 32;
         }
     }
@@ -393,7 +398,8 @@ __device__ __forceinline__ void sweep_faces(const ShapeView<float>& S, const Sha
 // ---- a3: relative pose of every pair of a class, compacted -----------------------------------------------------------
 // One thread per unique pair: minimum-image separation d, exact reach test (R10), relative pose R = R_i^T R_j,
 // t = R_i^T d and R_i in FP64, rounded once to float.  Pairs inside the reach are compacted into the
-// class's work list (block slices padded to whole warps: see below); pairs beyond it get their zero result records here and never reach the search kernel, so its warps carry 32
+// class's work list (block slices padded to whole warps: see below); pairs beyond it get their result-record flag cleared
+// here (nothing is written for them, the reduction skips them) and never reach the search kernel, so its warps carry 32
 // live pairs each.  Pose record, plane-major for coalesced loads: [6][npairs] float4 =
 // (R0 R1 R2 R3) (R4 R5 R6 R7) (R8 t0 t1 t2) (M0 M1 M2 M3) (M4 M5 M6 M7) (M8 dx dy dz); pidx[c] = the pair's index.
 template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THREADS) k_pose(const PoseArgs a) {
@@ -436,15 +442,8 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THR
     if (valid) {
         const double qa[4] = {qi.x, qi.y, qi.z, qi.w}, qb[4] = {qj.x, qj.y, qj.z, qj.w};
         pair_pose<float>(qa, qb, d, Mi, R, t);
-    } else if (p < a.npairs) {
-        f4 r0, r1, r2;
-        r0.x = r0.y = r0.z = r0.w = 0.f;
-        r1.x = r1.y = r1.z = 0.f; r1.w = (float)d[0];
-        r2.x = (float)d[1]; r2.y = (float)d[2]; r2.z = r2.w = 0.f;
-        for (int sl = 0; sl < a.slices; ++sl) {
-            f4* rec = a.rec + DEM_REC * ((size_t)p * a.slices + sl);
-            rec[0] = r0; rec[1] = r1; rec[2] = r2;
-        }
+    } else if (p < a.npairs) {  // beyond the reach: contributes nothing, no record is written
+        for (int sl = 0; sl < a.slices; ++sl) a.rflag[(size_t)p * a.slices + sl] = 0;
     }
     __syncthreads();
     if ((int)threadIdx.x < tot_pad - tot) a.pidx[s_prefix + tot + threadIdx.x] = -1;
@@ -475,8 +474,8 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
     unsigned* queue = reinterpret_cast<unsigned*>(smem_raw + 256);  // 4 warps x DEM_QCAP
     float* sacc_all = reinterpret_cast<float*>(queue + 4 * DEM_QCAP);  // 4 warps x 7 x 32
     unsigned* scnt_all = reinterpret_cast<unsigned*>(sacc_all + 4 * 7 * 32);  // 4 warps x 4
-    f4* stage_pose = reinterpret_cast<f4*>(scnt_all + 16);                 // 4 warps x [2][6][32] float4
-    int* stage_pidx = reinterpret_cast<int*>(stage_pose + 4 * 2 * 6 * 32);  // 4 warps x [2][32]
+    f4* stage_pose = reinterpret_cast<f4*>(scnt_all + 16);                 // 4 warps x [2][3][32] float4 (R, t)
+    int* stage_pidx = reinterpret_cast<int*>(stage_pose + 4 * 2 * 3 * 32);  // 4 warps x [2][32]
     f4* sm = reinterpret_cast<f4*>(stage_pidx + 4 * 2 * 32);
     static_assert(sizeof(FastShared) <= 256, "FastShared header");
     // stage the shape-feature tables of the class (a1) into shared memory
@@ -518,7 +517,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
     // cap).  The pose records of a warp's next tile are copied global -> shared with cp.async while the current tile is
     // being swept; each lane copies and later reads only its own records.
     const long long wt_stride = (long long)gridDim.x * 4;
-    f4* spose = stage_pose + warp * (2 * 6 * 32);   // [2][6][32]
+    f4* spose = stage_pose + warp * (2 * 3 * 32);   // [2][3][32]
     int* spidx = stage_pidx + warp * (2 * 32);      // [2][32]
     auto stage = [&](int buf, long long wt_) {
         if (wt_ < n_wtiles) {
@@ -526,9 +525,9 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
             DEM_ASSERT(c_ >= 0 && (size_t)count <= plane);
             if (c_ < count) {
 #pragma unroll
-                for (int k = 0; k < 6; ++k)
+                for (int k = 0; k < 3; ++k)  // R and t; R_i and d (planes 3-5) are fetched only by pairs that contribute
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
-                                     spose + (buf * 6 + k) * 32 + lane)), "l"(a.pose + k * plane + c_));
+                                     spose + (buf * 3 + k) * 32 + lane)), "l"(a.pose + k * plane + c_));
                 asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(
                                  spidx + buf * 32 + lane)), "l"(a.pidx + c_));
             }
@@ -544,13 +543,14 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
         stage(buf ^ 1, wt + wt_stride);
         asm volatile("cp.async.wait_group 1;" ::: "memory");
         __syncwarp();  // the cooperative evaluation reads other lanes' staged poses
-        w.sp = spose + buf * 6 * 32;
+        w.sp = spose + buf * 3 * 32;
+        w.touched = 0u;
         const bool valid = in_list && spidx[buf * 32 + lane] >= 0;  // the work list is padded to whole warps per k_pose block
         if (!__any_sync(full, valid)) continue;                    // a tile of padding only
         float R[9], t[3];
         if (valid) {
-            const f4 p0 = spose[(buf * 6 + 0) * 32 + lane], p1 = spose[(buf * 6 + 1) * 32 + lane],
-                     p2 = spose[(buf * 6 + 2) * 32 + lane];
+            const f4 p0 = spose[(buf * 3 + 0) * 32 + lane], p1 = spose[(buf * 3 + 1) * 32 + lane],
+                     p2 = spose[(buf * 3 + 2) * 32 + lane];
             R[0] = p0.x; R[1] = p0.y; R[2] = p0.z; R[3] = p0.w; R[4] = p1.x; R[5] = p1.y; R[6] = p1.z; R[7] = p1.w;
             R[8] = p2.x; t[0] = p2.y; t[1] = p2.z; t[2] = p2.w;
         } else {  // lanes without work sweep a far-away dummy so that the warp stays converged
@@ -718,28 +718,36 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
                 }
             }
             if (w.qn > 0) {
-                drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp, w.nown);
+                w.touched |= drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp, w.nown);
                 w.qn = 0;
             }
-            float F[3], T[3];
-#pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                F[k] = w.sacc[k * 32 + lane];
-                T[k] = w.sacc[(3 + k) * 32 + lane];
-            }
             if (valid) {
-                const f4 p3 = spose[(buf * 6 + 3) * 32 + lane], p4 = spose[(buf * 6 + 4) * 32 + lane],
-                         p5 = spose[(buf * 6 + 5) * 32 + lane];
-                const float Mi[9] = {p3.x, p3.y, p3.z, p3.w, p4.x, p4.y, p4.z, p4.w, p5.x};
-                float out[10];
-                pair_finish<float>(Mi, t, F, T, w.sacc[6 * 32 + lane], out);
-                DEM_ASSERT(spidx[buf * 32 + lane] < a.npairs && slice < a.slices);
-                f4* rec = a.rec + DEM_REC * ((size_t)spidx[buf * 32 + lane] * a.slices + slice);
-                f4 r0, r1, r2;
-                r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
-                r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = p5.y;
-                r2.x = p5.z; r2.y = p5.w; r2.z = r2.w = 0.f;
-                rec[0] = r0; rec[1] = r1; rec[2] = r2;
+                // a pair none of whose terms is inside the cutoff contributes nothing: its record flag is cleared and
+                // no record is written (the reduction skips it)
+                const int pi = spidx[buf * 32 + lane];
+                DEM_ASSERT(pi < a.npairs && slice < a.slices);
+                const size_t ri = (size_t)pi * a.slices + slice;
+                a.rflag[ri] = (unsigned char)(w.touched & 1u);
+                if (w.touched & 1u) {
+                    float F[3], T[3];
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) {
+                        F[k] = w.sacc[k * 32 + lane];
+                        T[k] = w.sacc[(3 + k) * 32 + lane];
+                    }
+                    const int c_ = (int)((wt * 32 + lane) % np_pad);
+                    const f4 p3 = a.pose[3 * plane + c_], p4 = a.pose[4 * plane + c_],
+                             p5 = a.pose[5 * plane + c_];
+                    const float Mi[9] = {p3.x, p3.y, p3.z, p3.w, p4.x, p4.y, p4.z, p4.w, p5.x};
+                    float out[10];
+                    pair_finish<float>(Mi, t, F, T, w.sacc[6 * 32 + lane], out);
+                    f4* rec = a.rec + DEM_REC * ri;
+                    f4 r0, r1, r2;
+                    r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
+                    r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = p5.y;
+                    r2.x = p5.z; r2.y = p5.w; r2.z = r2.w = 0.f;
+                    rec[0] = r0; rec[1] = r1; rec[2] = r2;
+                }
             }
         }
     }
@@ -765,7 +773,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
 // bytes of dynamic shared memory k_pair_fast needs in front of the staged tables
 static inline size_t fast_smem_header() {
     return 256 + sizeof(unsigned) * 4 * DEM_QCAP + sizeof(float) * 4 * 7 * 32 + sizeof(unsigned) * 16 +
-           sizeof(f4) * 4 * 2 * 6 * 32 + sizeof(int) * 4 * 2 * 32;
+           sizeof(f4) * 4 * 2 * 3 * 32 + sizeof(int) * 4 * 2 * 32;
 }
 
 // ---- the kernel with exact per-feature culling (3D) ----------------------------------------------------------------------
@@ -909,8 +917,8 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     unsigned* queue = reinterpret_cast<unsigned*>(smem_raw + 256);        // 4 warps x DEM_QCAP
     float* sacc_all = reinterpret_cast<float*>(queue + 4 * DEM_QCAP);      // 4 warps x 7 x 64
     unsigned* scnt_all = reinterpret_cast<unsigned*>(sacc_all + 4 * 7 * 64);  // 4 warps x 4
-    f4* stage_pose = reinterpret_cast<f4*>(scnt_all + 16);                 // 4 warps x [6][64] float4
-    int* stage_pidx = reinterpret_cast<int*>(stage_pose + 4 * 6 * 64);      // 4 warps x [64]
+    f4* stage_pose = reinterpret_cast<f4*>(scnt_all + 16);                 // 4 warps x [3][64] float4 (R, t)
+    int* stage_pidx = reinterpret_cast<int*>(stage_pose + 4 * 3 * 64);      // 4 warps x [64]
     unsigned* items = reinterpret_cast<unsigned*>(stage_pidx + 4 * 64);     // 4 warps x DEM_IQCAP
     f4* sm = reinterpret_cast<f4*>(items + 4 * DEM_IQCAP);
     const bool same = SAME;
@@ -949,7 +957,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     const int count = *a.count;  // a multiple of 64 (k_pose pads its block slices)
     const long long n_wtiles = (long long)(count >> 6) * a.slices;
     const size_t plane = a.plane;
-    f4* spose = stage_pose + warp * (6 * 64);
+    f4* spose = stage_pose + warp * (3 * 64);
     int* spidx = stage_pidx + warp * 64;
     w.sp = spose;
     for (long long wt = (long long)blockIdx.x * 4 + warp; wt < n_wtiles; wt += (long long)gridDim.x * 4) {
@@ -960,7 +968,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
             const int own = lane + 32 * h, c_ = cbase + own;
             DEM_ASSERT(c_ >= 0 && c_ < count && (size_t)count <= plane);
 #pragma unroll
-            for (int k = 0; k < 6; ++k)
+            for (int k = 0; k < 3; ++k)  // R and t; R_i and d (planes 3-5) are fetched only by pairs that contribute
                 asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
                                  spose + k * 64 + own)), "l"(a.pose + k * plane + c_));
             asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(spidx + own)),
@@ -973,6 +981,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
         valid[0] = spidx[lane] >= 0;  // the work list is padded to whole tiles per k_pose block (pidx = -1)
         valid[1] = spidx[lane + 32] >= 0;
         if (!__any_sync(full, valid[0] || valid[1])) continue;
+        w.touched = 0u;
 #pragma unroll
         for (int k = 0; k < 7; ++k) w.sacc[k * 64 + lane] = w.sacc[k * 64 + lane + 32] = 0.f;
         const int ob = (int)((long long)slice * a.n_outer / a.slices);
@@ -1056,25 +1065,30 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
             sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
         }
         if (w.qn > 0) {
-            drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp, w.nown);
+            w.touched |= drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp, w.nown);
             w.qn = 0;
         }
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             if (!valid[h]) continue;
             const int own = lane + 32 * h;
+            DEM_ASSERT(spidx[own] < a.npairs && slice < a.slices);
+            const size_t ri = (size_t)spidx[own] * a.slices + slice;
+            const bool hit = (w.touched >> h) & 1u;
+            a.rflag[ri] = (unsigned char)hit;  // no contribution: no record is written, the reduction skips the pair
+            if (!hit) continue;
             float F[3], T[3];
 #pragma unroll
             for (int k = 0; k < 3; ++k) {
                 F[k] = w.sacc[k * 64 + own];
                 T[k] = w.sacc[(3 + k) * 64 + own];
             }
-            const f4 p3 = spose[3 * 64 + own], p4 = spose[4 * 64 + own], p5 = spose[5 * 64 + own];
+            const int c_ = cbase + own;
+            const f4 p3 = a.pose[3 * plane + c_], p4 = a.pose[4 * plane + c_], p5 = a.pose[5 * plane + c_];
             const float Mi[9] = {p3.x, p3.y, p3.z, p3.w, p4.x, p4.y, p4.z, p4.w, p5.x};
             float out[10];
             pair_finish<float>(Mi, tq[h], F, T, w.sacc[6 * 64 + own], out);
-            DEM_ASSERT(spidx[own] < a.npairs && slice < a.slices);
-            f4* rec = a.rec + DEM_REC * ((size_t)spidx[own] * a.slices + slice);
+            f4* rec = a.rec + DEM_REC * ri;
             f4 r0, r1, r2;
             r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
             r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = p5.y;
@@ -1102,7 +1116,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
 // bytes of dynamic shared memory k_pair_cull needs in front of the staged tables
 static inline size_t cull_smem_header() {
     return 256 + sizeof(unsigned) * 4 * DEM_QCAP + sizeof(float) * 4 * 7 * 64 + sizeof(unsigned) * 16 +
-           sizeof(f4) * 4 * 6 * 64 + sizeof(int) * 4 * 64 + sizeof(unsigned) * 4 * DEM_IQCAP;
+           sizeof(f4) * 4 * 3 * 64 + sizeof(int) * 4 * 64 + sizeof(unsigned) * 4 * DEM_IQCAP;
 }
 
 }  // namespace dem

@@ -77,6 +77,7 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
         real out[10];
 #pragma unroll
         for (int k = 0; k < 10; ++k) out[k] = real(0);
+        unsigned nact = 0u;
         if (d[0] * d[0] + d[1] * d[1] + d[2] * d[2] < a.reach2) {
             const d4 qi = load4d(static_cast<const PosT*>(a.quat), ij.x), qj = load4d(static_cast<const PosT*>(a.quat), ij.y);
             const double qa[4] = {qi.x, qi.y, qi.z, qi.w}, qb[4] = {qj.x, qj.y, qj.z, qj.w};
@@ -88,15 +89,21 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
             c_act += cnt[0];
             c_deg += cnt[1];
             c_par += cnt[2];
+            nact = cnt[0];
         }
         // result record (DEM_REC real4 each): (F_i, U_ij) (tau_i, d.x) (d.y, d.z, 0, 0); the reduction derives the other
-        // side: F_j = -F_i, tau_j = -tau_i + d x F_i
-        real4* rec = a.rec + DEM_REC * ((size_t)p * a.slices + slice);
-        real4 r0, r1, r2;
-        r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
-        r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = (real)d[0];
-        r2.x = (real)d[1]; r2.y = (real)d[2]; r2.z = r2.w = real(0);
-        rec[0] = r0; rec[1] = r1; rec[2] = r2;
+        // side: F_j = -F_i, tau_j = -tau_i + d x F_i.  Written only when a term is inside the cutoff; the flag tells the
+        // reduction whether there is a record to read.
+        const size_t ri = (size_t)p * a.slices + slice;
+        a.rflag[ri] = nact ? 1 : 0;
+        if (nact) {
+            real4* rec = a.rec + DEM_REC * ri;
+            real4 r0, r1, r2;
+            r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
+            r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = (real)d[0];
+            r2.x = (real)d[1]; r2.y = (real)d[2]; r2.z = r2.w = real(0);
+            rec[0] = r0; rec[1] = r1; rec[2] = r2;
+        }
     }
     // counters: one atomic per warp per counter, after the hot loop
 #pragma unroll
@@ -117,7 +124,8 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
 // ---- a8: per-particle reduction -------------------------------------------------------------------------------------
 // a particle's total is the sum over its neighbours.  4 lanes per particle walk its neighbour row, each
 // reads the result records of its pairs (which side of the pair it is comes from `slot`, the pair's class from the
-// class-major pair index), and the 4 partial sums are combined with warp shuffles.  The summation order is fixed, so
+// class-major pair index; pairs whose record flag is 0 contribute nothing and have no record), and the 4 partial sums
+// are combined with warp shuffles.  The summation order is fixed, so
 // results are bit-reproducible from run to run.  With KICK the lane that stores the result also applies the second
 // half kick of velocity Verlet (v += dt/2 F/m, L += dt/2 tau), which saves a pass over the state.
 // `flags` (dem_step only, else null): flags[0] = "some particle left its skin in this step's drift" (k_kick_drift),
@@ -127,7 +135,8 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
 template <typename real, bool KICK>
 __global__ void k_reduce(int N, const int* __restrict__ counts, const int* __restrict__ slot, int stride,
                          const int* __restrict__ sid, ClassTable ct, int nclass,
-                         const typename vec4<real>::type* __restrict__ rec, typename vec4<real>::type* __restrict__ force,
+                         const typename vec4<real>::type* __restrict__ rec, const unsigned char* __restrict__ rflag,
+                         typename vec4<real>::type* __restrict__ force,
                          typename vec4<real>::type* __restrict__ torque, real* __restrict__ virial,
                          int* __restrict__ flags, KickArgs ka) {
     typedef typename vec4<real>::type real4;
@@ -150,8 +159,10 @@ __global__ void k_reduce(int N, const int* __restrict__ counts, const int* __res
             while (c + 1 < nclass && p >= ct.pair_base[c + 1]) ++c;
             const int S = ct.slices[c];
             DEM_ASSERT(sl >= 0 && p < ct.pair_base[nclass] && p >= ct.pair_base[c]);
-            const real4* r = rec + DEM_REC * ((size_t)ct.rec_base[c] + (size_t)(p - ct.pair_base[c]) * S);
+            const size_t r0i = (size_t)ct.rec_base[c] + (size_t)(p - ct.pair_base[c]) * S;
+            const real4* r = rec + DEM_REC * r0i;
             for (int s = 0; s < S; ++s, r += DEM_REC) {
+                if (!rflag[r0i + s]) continue;  // this (pair, slice) contributes nothing: no record was written
                 const real4 r0 = r[0], r1 = r[1], r2 = r[2];
                 const real dx = r1.w, dy = r2.x, dz = r2.y;
                 if (side) {  // this particle is the pair's second one: F_j = -F_i, tau_j = -tau_i + d x F_i

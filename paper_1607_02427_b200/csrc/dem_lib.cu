@@ -210,6 +210,7 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
     if (nrec * DEM_REC > 0x7fffffffLL) return fail(ctx, DEM_EOVERFLOW, "too many pair records");
     CU(ctx->pairs.reserve(sizeof(int2) * (size_t)std::max<long long>(ctx->npairs_total, 1)));
     CU(ctx->rec.reserve((ctx->prec == DEM_F64 ? sizeof(d4) : sizeof(f4)) * DEM_REC * (size_t)std::max<long long>(nrec, 1)));
+    CU(ctx->rflag.reserve((size_t)std::max<long long>(nrec, 1)));
     k_pair_fill<<<nblk(N, B), B, 0, st>>>(N, ctx->counts.as<int>(), ctx->list.as<int>(), ctx->stride, sid, ctx->ct, nc,
                                           pcnt, ctx->pairs.as<int2>(), ctx->slot.as<int>());
     LAUNCHED(ctx);
@@ -565,7 +566,7 @@ int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda
 int dem_destroy(dem_ctx* c) {
     if (!c) return DEM_EINVAL;
     DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
-                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->flags, &c->counters, &c->thermo, &c->pose, &c->pidx, &c->cum, &c->st_pos, &c->st_quat,
+                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->rflag, &c->flags, &c->counters, &c->thermo, &c->pose, &c->pidx, &c->cum, &c->st_pos, &c->st_quat,
                       &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->st_virial, &c->pos_build, &c->epart, &c->h_pos,
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();

@@ -84,6 +84,8 @@ template <typename real> struct PairArgs {
     int slices;           // lanes per pair (each takes a slice of the outer feature loop)
     int n_outer;          // outer-loop length of the class
     real4* rec;           // this class's result records: DEM_REC real4 per (pair, slice)
+    unsigned char* rflag; // one byte per result record: 1 = the record was written and carries a contribution, 0 = the
+                          //   (pair, slice) contributes nothing and its record was NOT written (the reduction skips it)
     const void* pos;
     const void* quat;
     BoxDev box;
@@ -113,7 +115,7 @@ struct PoseArgs {
     size_t plane;  // stride of the pose planes = capacity of the work list (pairs + 64 per k_pose block)
     int pad;       // entries per warp tile of the kernel that follows: 32 (k_pair_fast) or 64 (k_pair_cull)
     unsigned long long* counters;  // [0] += pairs inside the reach
-    f4* rec;
+    unsigned char* rflag;  // result-record flags of the class: pairs beyond the reach get 0 here (no record is written)
     const int* skip;  // dem_step: non-null and *skip != 0 => the list is stale, the kernel does nothing (see step_t)
 };
 
