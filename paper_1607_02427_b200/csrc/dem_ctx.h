@@ -171,9 +171,9 @@ inline BoxDev box_dev(int dim, const double box[3]) {
 
 // ---- dem_eval.cu: one force evaluation over the current list (steps a3-a8) ---------------------------------------------
 // pos / quat are float[N][4] or double[N][4] (pos_is_double); force / torque / virial are `real` of the context.
-// skip / kick: dem_step's device flags and fused second half kick (null outside dem_step).
+// fin (null outside dem_step): what the reduction kernel does behind the reduction (FinArgs: integrator, device flags).
 int evaluate(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_double, const int32_t* sid, int N, void* force,
-             void* torque, void* virial, int* skip, const KickArgs* kick);
+             void* torque, void* virial, const FinArgs* fin);
 
 // ---- kernel launchers (one translation unit per kernel family) ------------------------------------------------------------
 void launch_pose(int dim, bool pos_is_double, int grid, cudaStream_t st, const PoseArgs& pa);

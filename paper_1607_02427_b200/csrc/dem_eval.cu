@@ -12,12 +12,13 @@ namespace {
 
 template <typename real>
 int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_double, const int32_t* sid, int N,
-               void* force, void* torque, void* virial, int* skip, const KickArgs* kick) {
+               void* force, void* torque, void* virial, const FinArgs* fin) {
     typedef typename vec4<real>::type real4;
     if (!ctx->have_list) return fail(ctx, DEM_ESTALE, "no neighbour list: call dem_build_neighbors first");
     if (N != ctx->N) return fail(ctx, DEM_ESTALE, "N = %d differs from the last build (%d)", N, ctx->N);
     if (!pos || !quat || !sid || !force || !torque) return fail(ctx, DEM_EINVAL, "null particle array");
     cudaStream_t st = ctx->stream;
+    const int* skip = fin ? fin->bail : nullptr;
     // counters[0..7] (unsigned long long) followed by the per-class lengths of the k_pose work lists (int): one memset
     CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES, st));
     int* ccount = reinterpret_cast<int*>(ctx->counters.as<unsigned long long>() + 8);
@@ -123,14 +124,24 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
         ev_span(ctx, KT_PAIR, em, e1);
     }
     cudaEvent_t r0 = ev_mark(ctx, 2);
-    if (kick)
-        k_reduce<real, true><<<nblk(4LL * N, 128), 128, 0, st>>>(
-            N, ctx->counts.as<int>(), ctx->slot.as<int>(), ctx->stride, sid, ctx->ct, ctx->nclass, ctx->rec.as<real4>(),
-            ctx->rflag.as<unsigned char>(), static_cast<real4*>(force), static_cast<real4*>(torque), static_cast<real*>(virial), skip, *kick);
-    else
-        k_reduce<real, false><<<nblk(4LL * N, 128), 128, 0, st>>>(
-            N, ctx->counts.as<int>(), ctx->slot.as<int>(), ctx->stride, sid, ctx->ct, ctx->nclass, ctx->rec.as<real4>(),
-            ctx->rflag.as<unsigned char>(), static_cast<real4*>(force), static_cast<real4*>(torque), static_cast<real*>(virial), skip, KickArgs());
+    {
+        FinArgs fa;
+        if (fin) fa = *fin;
+        else memset(&fa, 0, sizeof fa);
+        const int grid = nblk(N, 256);
+        const int* counts = ctx->counts.as<int>();
+        const int* slot = ctx->slot.as<int>();
+        const real4* rec = ctx->rec.as<real4>();
+        const unsigned char* rf = ctx->rflag.as<unsigned char>();
+        real4 *F = static_cast<real4*>(force), *T = static_cast<real4*>(torque);
+        real* W = static_cast<real*>(virial);
+        if (fa.mode == 2)
+            k_finish<real, 2><<<grid, 256, 0, st>>>(N, counts, slot, sid, ctx->ct, ctx->nclass, rec, rf, F, T, W, fa);
+        else if (fa.mode == 1)
+            k_finish<real, 1><<<grid, 256, 0, st>>>(N, counts, slot, sid, ctx->ct, ctx->nclass, rec, rf, F, T, W, fa);
+        else
+            k_finish<real, 0><<<grid, 256, 0, st>>>(N, counts, slot, sid, ctx->ct, ctx->nclass, rec, rf, F, T, W, fa);
+    }
     LAUNCHED(ctx);
     ev_span(ctx, KT_REDUCE, r0, ev_mark(ctx, 2));
     CU(cudaGetLastError());
@@ -140,9 +151,9 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
 }  // namespace
 
 int evaluate(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_double, const int32_t* sid, int N, void* force,
-             void* torque, void* virial, int* skip, const KickArgs* kick) {
-    if (ctx->prec == DEM_F64) return evaluate_t<double>(ctx, pos, quat, true, sid, N, force, torque, virial, skip, kick);
-    return evaluate_t<float>(ctx, pos, quat, pos_is_double, sid, N, force, torque, virial, skip, kick);
+             void* torque, void* virial, const FinArgs* fin) {
+    if (ctx->prec == DEM_F64) return evaluate_t<double>(ctx, pos, quat, true, sid, N, force, torque, virial, fin);
+    return evaluate_t<float>(ctx, pos, quat, pos_is_double, sid, N, force, torque, virial, fin);
 }
 
 }  // namespace dem

@@ -6,84 +6,22 @@
 namespace dem {
 
 // ---- a9: NVE integrator (reading R15) --------------------------------------------------------------------
-__device__ __forceinline__ void quat_mul_d(const double* a, const double* b, double* o) {
-    o[0] = a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3];
-    o[1] = a[0] * b[1] + a[1] * b[0] + a[2] * b[3] - a[3] * b[2];
-    o[2] = a[0] * b[2] - a[1] * b[3] + a[2] * b[0] + a[3] * b[1];
-    o[3] = a[0] * b[3] + a[1] * b[2] - a[2] * b[1] + a[3] * b[0];
-}
-
-// Torque-free rotation over dt with the lab-frame angular momentum L held fixed.  Spherical tops (and 2D): exact,
-// q <- exp(dt/2 L/I0) q.  Otherwise the symmetric splitting of the free-rotor Hamiltonian into rotations about the
-// body axes x(dt/2) y(dt/2) z(dt) y(dt/2) x(dt/2) (the family of PAPER.md ref. 23).
-__device__ inline void free_rotate(int dim, const double* I, const double* L, double dt, double* q) {
-    const bool spherical = dim == 2 || (I[0] == I[1] && I[1] == I[2]);
-    if (spherical) {
-        const double I0 = I[2];
-        if (!(I0 > 0.0)) return;
-        // rotation by phi = |a| about a/|a| with a = (dt / 2 I0) L: rq = (cos phi, (sin phi / phi) a)
-        const double h = 0.5 * dt / I0;
-        const double a[3] = {h * L[0], h * L[1], h * L[2]};
-        const double p2 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2];
-        double ch, sc;  // cos phi, sin phi / phi
-        if (p2 < 0.0625) {  // Taylor series: next terms phi^12 / 12! and phi^12 / 13! are below 1.2e-16 here
-            ch = 1.0 + p2 * (-1.0 / 2 + p2 * (1.0 / 24 + p2 * (-1.0 / 720 + p2 * (1.0 / 40320 + p2 * (-1.0 / 3628800)))));
-            sc = 1.0 + p2 * (-1.0 / 6 + p2 * (1.0 / 120 + p2 * (-1.0 / 5040 + p2 * (1.0 / 362880 + p2 * (-1.0 / 39916800)))));
-        } else {
-            const double ph = sqrt(p2);
-            double sh;
-            sincos(ph, &sh, &ch);
-            sc = sh / ph;
-        }
-        const double rq[4] = {ch, sc * a[0], sc * a[1], sc * a[2]};
-        double o[4];
-        quat_mul_d(rq, q, o);
-        // |o| = |q| (1 + O(1e-16)): two Newton steps of 1/sqrt from 1 renormalise a q that is unit to float precision
-        const double n2 = o[0] * o[0] + o[1] * o[1] + o[2] * o[2] + o[3] * o[3];
-        double inv = 1.5 - 0.5 * n2;
-        inv = inv * (1.5 - 0.5 * n2 * inv * inv);
-        inv = inv * (1.5 - 0.5 * n2 * inv * inv);
-        for (int k = 0; k < 4; ++k) q[k] = o[k] * inv;
-        return;
-    }
-    double M[9], Lb[3];
-    quat_to_mat<double>(q[0], q[1], q[2], q[3], M);
-    for (int a = 0; a < 3; ++a) Lb[a] = M[a] * L[0] + M[3 + a] * L[1] + M[6 + a] * L[2];  // R^T L
-    const int axis_seq[5] = {0, 1, 2, 1, 0};
-    const double frac[5] = {0.5, 0.5, 1.0, 0.5, 0.5};
-    for (int s = 0; s < 5; ++s) {
-        const int a = axis_seq[s];
-        if (!(I[a] > 0.0)) continue;
-        const double phi = frac[s] * dt * Lb[a] / I[a];
-        double sn, cs;
-        sincos(phi, &sn, &cs);
-        const int b = (a + 1) % 3, c = (a + 2) % 3;
-        const double lb = cs * Lb[b] + sn * Lb[c], lc = -sn * Lb[b] + cs * Lb[c];
-        Lb[b] = lb;
-        Lb[c] = lc;
-        double sh, ch;
-        sincos(0.5 * phi, &sh, &ch);
-        double rq[4] = {ch, 0, 0, 0}, o[4];
-        rq[1 + a] = sh;
-        quat_mul_d(q, rq, o);  // body-axis rotation composes on the right
-        for (int k = 0; k < 4; ++k) q[k] = o[k];
-    }
-    const double n = sqrt(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
-    for (int k = 0; k < 4; ++k) q[k] /= n;
-}
-
 // first half of velocity Verlet: v += dt/2 F/m; x += dt v (wrapped); L += dt/2 tau; free rotation of q.
-// Also raises moved[0] when a particle is farther than skin/2 from where it was at the last neighbour build.
-// Does nothing once moved[1] (halt, raised by k_reduce of an earlier step of the same chunk) is set.
+// Raises *raise when a particle is farther than skin/2 from where it was at the last neighbour build.
+// Does nothing when *bail is set (the list went stale in an earlier step of the same chunk; see FinArgs).
 template <typename real>
 __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict__ sid, MassTable mt,
                              d4* __restrict__ pos, d4* __restrict__ quat, d4* __restrict__ vel, d4* __restrict__ ang,
                              const typename vec4<real>::type* __restrict__ force,
                              const typename vec4<real>::type* __restrict__ torque, const d4* __restrict__ pos_build,
-                             double half_skin2, int* __restrict__ moved, const ThermoDev* __restrict__ thermo) {
+                             double half_skin2, const int* __restrict__ bail, int* __restrict__ raise,
+                             const ThermoDev* __restrict__ thermo) {
     // The translational and the rotational half of a particle's update are independent: the first half of the grid
     // does x, v (and the skin test), the second q, L -- twice the memory-level parallelism, half the dependent chain.
-    if (moved[1]) return;
+    if (bail && *bail) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) *raise = 1;  // pass the word on: the next evaluation looks at *raise
+        return;
+    }
     const int half = gridDim.x >> 1;
     const bool rot = (int)blockIdx.x >= half;
     const int i = (blockIdx.x - (rot ? half : 0)) * blockDim.x + threadIdx.x;
@@ -110,7 +48,7 @@ __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict
         dx -= box.L[0] * rint(dx * box.invL[0]);
         dy -= box.L[1] * rint(dy * box.invL[1]);
         dz -= box.L[2] * rint(dz * box.invL[2]);
-        if (dx * dx + dy * dy + dz * dz > half_skin2) moved[0] = 1;
+        if (dx * dx + dy * dy + dz * dz > half_skin2) *raise = 1;
     } else {
         d4 L = ang[i], q = quat[i];
         const typename vec4<real>::type T = torque[i];
@@ -166,11 +104,11 @@ __global__ void k_kinetic(int N, int dim, const int* __restrict__ sid, MassTable
 // NVT: one block sums the partials of k_kinetic and advances (xi, eta) by `halves` thermostat half steps (1: the end
 // of the run, or its start; 2: the end of one step and the start of the next, which are adjacent).  The scaling of v
 // and L is left in th->scale for the next k_kick_drift / k_scale_momenta.  Does nothing when the step it follows was
-// not completed (flags[1] = halt, see k_reduce).
+// not completed (*bail set, see FinArgs).
 __global__ void k_thermostat(int nb, const double* __restrict__ partial, int dim, int N, double dt, double kT,
-                             double tau, int halves, const int* __restrict__ flags, ThermoDev* __restrict__ th) {
+                             double tau, int halves, const int* __restrict__ bail, ThermoDev* __restrict__ th) {
     __shared__ double sh[2][256];
-    if (flags && flags[1]) return;
+    if (bail && *bail) return;
     double K = 0, dof = 0;
     for (int b = threadIdx.x; b < nb; b += 256) {
         K += partial[2 * b];

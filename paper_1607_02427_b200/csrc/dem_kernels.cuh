@@ -1,13 +1,14 @@
 // dem_kernels.cuh -- the CUDA kernels of libdem_b200 (sm_100a).  Host orchestration is in dem_lib.cu.
 //
 //   a3-a7 pair-feature kernel           k_pair          (FP32-ALU bound; dem_math.cuh holds the arithmetic)
-//   a8  per-particle reduction          k_reduce        (warp-shuffle over 4 lanes per particle, no atomics)
+//   a8  per-particle reduction          k_finish        (one thread per particle, no atomics; fused with the integrator)
 // The neighbour-list kernels (a2) are in dem_list.cuh, the integrator (a9) in dem_integrate.cuh, the packed FP32 search
 // kernels in dem_fast.cuh.
 #pragma once
 #include <cuda_runtime.h>
 
 #include "dem_math.cuh"
+#include "dem_rigid.cuh"
 
 namespace dem {
 
@@ -121,48 +122,80 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
     }
 }
 
-// ---- a8: per-particle reduction -------------------------------------------------------------------------------------
-// a particle's total is the sum over its neighbours.  4 lanes per particle walk its neighbour row, each
-// reads the result records of its pairs (which side of the pair it is comes from `slot`, the pair's class from the
-// class-major pair index; pairs whose record flag is 0 contribute nothing and have no record), and the 4 partial sums
-// are combined with warp shuffles.  The summation order is fixed, so
-// results are bit-reproducible from run to run.  With KICK the lane that stores the result also applies the second
-// half kick of velocity Verlet (v += dt/2 F/m, L += dt/2 tau), which saves a pass over the state.
-// `flags` (dem_step only, else null): flags[0] = "some particle left its skin in this step's drift" (k_kick_drift),
-// flags[1] = halt, flags[2] = steps completed.  dem_step queues many steps before the host looks at the flags: with
-// flags[0] set the list is stale, so the kernel changes nothing and raises halt, which turns every later
-// k_kick_drift of the chunk into a no-op; otherwise it counts the step as completed (see step_t).
-template <typename real, bool KICK>
-__global__ void k_reduce(int N, const int* __restrict__ counts, const int* __restrict__ slot, int stride,
-                         const int* __restrict__ sid, ClassTable ct, int nclass,
-                         const typename vec4<real>::type* __restrict__ rec, const unsigned char* __restrict__ rflag,
-                         typename vec4<real>::type* __restrict__ force,
-                         typename vec4<real>::type* __restrict__ torque, real* __restrict__ virial,
-                         int* __restrict__ flags, KickArgs ka) {
+// ---- a8 (+ a9): per-particle reduction, fused with the integrator ------------------------------------------------------
+// a particle's total is the sum over its neighbours.  One thread per particle walks its neighbour slots
+// (slot[k][i], neighbour-major so that a warp's loads coalesce: 2 x pair index + which side of the pair the particle is;
+// the pair's class follows from the class-major pair index), looks up each pair's record flag and reads the 48-byte
+// record only where a term was inside the cutoff.  The loads of a batch of four neighbours are issued before any is
+// used.  The summation order is fixed (no atomics), so results are bit-reproducible from run to run.
+// Inside dem_step the same thread goes on with the integrator (FinArgs: second half kick; in mode 2 also the first
+// half kick of the next step, the drift, the free rotation and the skin test), which saves the passes over F, tau, v
+// and L that separate kernels would need.  Forces and torques are stored only in modes 0 and 1 (mode 2 consumes them
+// in registers; the step that ends a dem_step call runs in mode 1).
+template <typename real, int MODE>
+__global__ void __launch_bounds__(256) k_finish(int N, const int* __restrict__ counts, const int* __restrict__ slot,
+                                                const int* __restrict__ sid, ClassTable ct, int nclass,
+                                                const typename vec4<real>::type* __restrict__ rec,
+                                                const unsigned char* __restrict__ rflag,
+                                                typename vec4<real>::type* __restrict__ force,
+                                                typename vec4<real>::type* __restrict__ torque, real* __restrict__ virial,
+                                                FinArgs fa) {
     typedef typename vec4<real>::type real4;
-    const int gid = blockIdx.x * blockDim.x + threadIdx.x;
-    if (flags) {
-        if (flags[0]) {
-            if (gid == 0) flags[1] = 1;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (MODE != 0) {
+        if (fa.bail && *fa.bail) {               // the list went stale before this step: change nothing, and pass
+            if (i == 0 && fa.raise) *fa.raise = 1;  // the word on (the next evaluation looks at the other flag)
             return;
         }
-        if (gid == 0) flags[2] += 1;  // nothing in this kernel reads flags[2]
+        if (i == 0 && fa.done) *fa.done += 1;    // nothing in this kernel reads it
     }
-    const int i = gid >> 2, sub = gid & 3;
+    if (i >= N) return;
+    // state loads first: they do not depend on the reduction
+    d4 v, L, x, q, xb;
+    int sh = 0;
+    if (MODE >= 1) {
+        v = fa.vel[i];
+        L = fa.ang[i];
+        sh = sid[i];
+    }
+    if (MODE == 2) {
+        x = fa.pos[i];
+        q = fa.quat[i];
+        xb = fa.pos_build[i];
+    }
     real F[3] = {0, 0, 0}, T[3] = {0, 0, 0}, U = 0, W[6] = {0, 0, 0, 0, 0, 0};
-    if (i < N) {
-        const int n = min(counts[i], stride);
-        for (int k = sub; k < n; k += 4) {
-            const int sl = slot[(size_t)i * stride + k];
-            const int p = sl >> 1, side = sl & 1;
-            int c = 0;
-            while (c + 1 < nclass && p >= ct.pair_base[c + 1]) ++c;
-            const int S = ct.slices[c];
-            DEM_ASSERT(sl >= 0 && p < ct.pair_base[nclass] && p >= ct.pair_base[c]);
-            const size_t r0i = (size_t)ct.rec_base[c] + (size_t)(p - ct.pair_base[c]) * S;
-            const real4* r = rec + DEM_REC * r0i;
-            for (int s = 0; s < S; ++s, r += DEM_REC) {
-                if (!rflag[r0i + s]) continue;  // this (pair, slice) contributes nothing: no record was written
+    const int n = counts[i];
+    for (int k0 = 0; k0 < n; k0 += 4) {
+        int sl[4];
+        size_t ri[4];
+        int S[4];
+        unsigned any[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) sl[u] = k0 + u < n ? slot[(size_t)(k0 + u) * N + i] : -1;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            any[u] = 0u;
+            S[u] = 0;
+            ri[u] = 0;
+            if (sl[u] >= 0) {
+                const int p = sl[u] >> 1;
+                int c = 0;
+                while (c + 1 < nclass && p >= ct.pair_base[c + 1]) ++c;
+                DEM_ASSERT(p < ct.pair_base[nclass] && p >= ct.pair_base[c]);
+                S[u] = ct.slices[c];
+                ri[u] = (size_t)ct.rec_base[c] + (size_t)(p - ct.pair_base[c]) * S[u];
+                // bit s: slice s of the pair has a record (more than 32 slices: every flag is looked at below)
+                for (int s = 0; s < S[u] && s < 32; ++s) any[u] |= (unsigned)(rflag[ri[u] + s] != 0) << s;
+                if (S[u] > 32) any[u] |= 0x80000000u;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (!any[u]) continue;  // this pair contributes nothing: no record was written
+            const int side = sl[u] & 1;
+            for (int s = 0; s < S[u]; ++s) {
+                if (S[u] <= 32 ? !((any[u] >> s) & 1u) : !rflag[ri[u] + s]) continue;
+                const real4* r = rec + DEM_REC * (ri[u] + s);
                 const real4 r0 = r[0], r1 = r[1], r2 = r[2];
                 const real dx = r1.w, dy = r2.x, dz = r2.y;
                 if (side) {  // this particle is the pair's second one: F_j = -F_i, tau_j = -tau_i + d x F_i
@@ -183,20 +216,7 @@ __global__ void k_reduce(int N, const int* __restrict__ counts, const int* __res
             }
         }
     }
-#pragma unroll
-    for (int o = 1; o <= 2; o <<= 1) {
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            F[a] += __shfl_xor_sync(0xffffffffu, F[a], o);
-            T[a] += __shfl_xor_sync(0xffffffffu, T[a], o);
-        }
-        U += __shfl_xor_sync(0xffffffffu, U, o);
-        if (virial) {
-#pragma unroll
-            for (int a = 0; a < 6; ++a) W[a] += __shfl_xor_sync(0xffffffffu, W[a], o);
-        }
-    }
-    if (i < N && sub == 0) {
+    if (MODE != 2) {
         real4 f, t;
         f.x = F[0]; f.y = F[1]; f.z = F[2]; f.w = U;
         t.x = T[0]; t.y = T[1]; t.z = T[2]; t.w = real(0);
@@ -206,20 +226,37 @@ __global__ void k_reduce(int N, const int* __restrict__ counts, const int* __res
 #pragma unroll
             for (int a = 0; a < 6; ++a) virial[(size_t)i * 6 + a] = W[a];
         }
-        if (KICK) {
-            const double hm = ka.half_dt * ka.inv_mass[sid[i]];
-            d4 v = ka.vel[i], L = ka.ang[i];
-            v.x += hm * (double)F[0];
-            v.y += hm * (double)F[1];
-            if (ka.dim == 3) {
-                v.z += hm * (double)F[2];
-                L.x += ka.half_dt * (double)T[0];
-                L.y += ka.half_dt * (double)T[1];
+    }
+    if (MODE >= 1) {
+        const double hm = 0.5 * fa.dt / fa.mt.mass[sh];
+        double vs[3] = {v.x, v.y, v.z}, Ls[3] = {L.x, L.y, L.z};
+        const double Fs[3] = {(double)F[0], (double)F[1], (double)F[2]}, Ts[3] = {(double)T[0], (double)T[1], (double)T[2]};
+        for (int a = 0; a < fa.dim; ++a) vs[a] += hm * Fs[a];                       // second half kick: the step is done
+        for (int a = (fa.dim == 2 ? 2 : 0); a < 3; ++a) Ls[a] += 0.5 * fa.dt * Ts[a];
+        if (MODE == 2) {  // first half of the next step (the same arithmetic as k_kick_drift)
+            double xs[3] = {x.x, x.y, x.z};
+            for (int a = 0; a < fa.dim; ++a) {
+                vs[a] += hm * Fs[a];
+                xs[a] += fa.dt * vs[a];
+                xs[a] -= fa.box.L[a] * rint(xs[a] * fa.box.invL[a]);
             }
-            L.z += ka.half_dt * (double)T[2];
-            ka.vel[i] = v;
-            ka.ang[i] = L;
+            x.x = xs[0]; x.y = xs[1]; x.z = xs[2];
+            fa.pos[i] = x;
+            double dx = xs[0] - xb.x, dy = xs[1] - xb.y, dz = fa.dim == 3 ? xs[2] - xb.z : 0.0;
+            dx -= fa.box.L[0] * rint(dx * fa.box.invL[0]);
+            dy -= fa.box.L[1] * rint(dy * fa.box.invL[1]);
+            dz -= fa.box.L[2] * rint(dz * fa.box.invL[2]);
+            if (dx * dx + dy * dy + dz * dz > fa.half_skin2) *fa.raise = 1;
+            for (int a = (fa.dim == 2 ? 2 : 0); a < 3; ++a) Ls[a] += 0.5 * fa.dt * Ts[a];
+            double qs[4] = {q.x, q.y, q.z, q.w};
+            free_rotate(fa.dim, fa.mt.inertia[sh], Ls, fa.dt, qs);
+            q.x = qs[0]; q.y = qs[1]; q.z = qs[2]; q.w = qs[3];
+            fa.quat[i] = q;
         }
+        v.x = vs[0]; v.y = vs[1]; v.z = vs[2];
+        L.x = Ls[0]; L.y = Ls[1]; L.z = Ls[2];
+        fa.vel[i] = v;
+        fa.ang[i] = L;
     }
 }
 

@@ -261,7 +261,7 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     const double r_list = max_reach(ctx) + skin;
     const BoxDev bx = box_dev(ctx->dim, box);
     CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
-    CHECK(evaluate(ctx, x, q, true, sid, N, F, T, nullptr, nullptr, nullptr));
+    CHECK(evaluate(ctx, x, q, true, sid, N, F, T, nullptr, nullptr));
     // The list build and the first evaluation need positions and orientations only: dem_step_host copies velocities
     // and angular momenta on a second stream meanwhile, and they are waited for (and converted) here.
     if (ctx->ev_copy_pending) {
@@ -278,10 +278,10 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     // ends it and the half step that begins the next one; the scaling of v and L is applied by the next k_kick_drift.
     ThermoDev* th = nullptr;
     const int nbk = nblk(N, 256);
-    auto thermostat = [&](int halves, const int* fl) -> int {
+    auto thermostat = [&](int halves, const int* bail) -> int {
         k_kinetic<<<nbk, 256, 0, st>>>(N, ctx->dim, sid, ctx->mt, q, v, L, ctx->epart.as<double>());
         LAUNCHED(ctx);
-        k_thermostat<<<1, 256, 0, st>>>(nbk, ctx->epart.as<double>(), ctx->dim, N, dt, nvt->kT, nvt->tau, halves, fl, th);
+        k_thermostat<<<1, 256, 0, st>>>(nbk, ctx->epart.as<double>(), ctx->dim, N, dt, nvt->kT, nvt->tau, halves, bail, th);
         LAUNCHED(ctx);
         return DEM_OK;
     };
@@ -294,56 +294,77 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
         CU(cudaStreamSynchronize(st));  // h0 is on the stack
         CHECK(thermostat(1, nullptr));
     }
-    int* flags = ctx->flags.as<int>() + 8;  // [0] moved, [1] halt, [2] steps completed (k_kick_drift, k_reduce)
+    // Steps are queued in chunks without the host in between.  The kernel that ends an evaluation (k_finish) also
+    // integrates: second half kick, which completes the step, and -- unless the step is the last of the call or a
+    // thermostat has to act in between -- the first half kick, drift and rotation of the NEXT step.  Whoever drifts
+    // raises a device flag when a particle leaves its skin (the list is stale); flags[0] and flags[1] are used
+    // alternately: evaluation e of a chunk and everything behind it do nothing when flags[e & 1] is set (raised
+    // BEFORE they started), and the drift behind evaluation e raises flags[(e + 1) & 1].  flags[2] counts the steps
+    // completed.  The host reads the three once per chunk; a chunk that went stale stopped after a drift, with the
+    // forces of the drifted state not yet evaluated, which is exactly the state every chunk starts from: the host
+    // rebuilds the list and goes on.  The chunk length follows the last observed interval between rebuilds, so that
+    // few launches are wasted behind a stale flag.
+    int* flags = ctx->flags.as<int>() + 8;
     const double half_skin2 = 0.25 * skin * skin;
     if (ctx->l2_flush_bytes) CU(ctx->l2_scratch.reserve(ctx->l2_flush_bytes));
     if (!ctx->h_moved) CU(cudaHostAlloc(&ctx->h_moved, 4 * sizeof(int), cudaHostAllocDefault));
-    KickArgs ka;
-    ka.half_dt = 0.5 * dt;
-    ka.dim = ctx->dim;
-    ka.vel = v;
-    ka.ang = L;
-    for (int k = 0; k < DEM_MAX_SHAPES_K; ++k) ka.inv_mass[k] = ctx->mt.mass[k] > 0 ? 1.0 / ctx->mt.mass[k] : 0.0;
-    // Steps are queued in chunks without the host in between: k_kick_drift raises flags[0] when a particle leaves its
-    // skin; k_reduce (which alone completes a step) then changes nothing and raises halt, and the rest of the chunk
-    // turns into no-ops.  The host reads the flags once per chunk: a halted chunk stopped after the drift of step
-    // `done + 1`, which is completed here with a new list.  The chunk length follows the last observed interval
-    // between rebuilds, so that few launches are wasted behind a halt.
+    FinArgs fa;
+    memset(&fa, 0, sizeof fa);
+    fa.dim = ctx->dim;
+    fa.dt = dt;
+    fa.pos = x; fa.quat = q; fa.vel = v; fa.ang = L;
+    fa.pos_build = ctx->pos_build.as<d4>();
+    fa.half_skin2 = half_skin2;
+    fa.box = bx;
+    fa.mt = ctx->mt;
+    fa.done = flags + 2;
+    auto kick_drift = [&](const int* bail, int* raise) {
+        cudaEvent_t k0 = ev_mark(ctx, 2);
+        k_kick_drift<real><<<2 * nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T, ctx->pos_build.as<d4>(),
+                                                     half_skin2, bail, raise, th);
+        LAUNCHED(ctx);
+        ev_span(ctx, KT_KICK_DRIFT, k0, ev_mark(ctx, 2));
+    };
     int remaining = nsteps, since = 0;
+    bool drifted = false;  // the state is past the drift of the next step (forces of the drifted state not yet evaluated)
     while (remaining > 0) {
         const int hint = std::max(ctx->rebuild_interval, 1);
         const int chunk = std::min(remaining, std::min(64, std::max(hint - since, std::max(1, hint / 8))));
         CU(cudaMemsetAsync(flags, 0, 3 * sizeof(int), st));
-        for (int s = 0; s < chunk; ++s) {
+        if (!drifted) {  // the first half of the call's first step
+            kick_drift(nullptr, flags);
+            drifted = true;
+        }
+        for (int e = 0; e < chunk; ++e) {
             if (ctx->l2_flush_bytes) {
                 cudaEvent_t f0 = ev_mark(ctx, 2);
-                CU(cudaMemsetAsync(ctx->l2_scratch.p, s & 0xff, ctx->l2_flush_bytes, st));
+                CU(cudaMemsetAsync(ctx->l2_scratch.p, e & 0xff, ctx->l2_flush_bytes, st));
                 ev_span(ctx, KT_FLUSH, f0, ev_mark(ctx, 2));
             }
-            cudaEvent_t k0 = ev_mark(ctx, 2);
-            k_kick_drift<real><<<2 * nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T,
-                                                         ctx->pos_build.as<d4>(), half_skin2, flags, th);
-            LAUNCHED(ctx);
-            ev_span(ctx, KT_KICK_DRIFT, k0, ev_mark(ctx, 2));
-            CHECK(evaluate(ctx, x, q, true, sid, N, F, T, nullptr, flags, &ka));
-            if (th) CHECK(thermostat(nsteps - remaining + s == nsteps - 1 ? 1 : 2, flags));
+            const bool last = e == remaining - 1;  // the last step of the call ends with its second half kick
+            fa.mode = (last || th) ? 1 : 2;
+            fa.bail = flags + (e & 1);
+            fa.raise = flags + ((e + 1) & 1);
+            CHECK(evaluate(ctx, x, q, true, sid, N, F, T, nullptr, &fa));
+            if (th) {
+                CHECK(thermostat(last ? 1 : 2, fa.bail));
+                if (!last) kick_drift(fa.bail, fa.raise);
+            }
         }
         CU(cudaMemcpyAsync(ctx->h_moved, flags, 3 * sizeof(int), cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
-        int done = ctx->h_moved[2];
-        if (done < 0 || done > chunk || (done < chunk && !ctx->h_moved[0]))
-            return fail(ctx, DEM_ECUDA, "dem_step: inconsistent step flags (done %d of %d, moved %d)", done, chunk, ctx->h_moved[0]);
-        if (ctx->h_moved[0]) {
+        const int done = ctx->h_moved[2];
+        const bool stale = ctx->h_moved[0] || ctx->h_moved[1];
+        if (done < 0 || done > chunk || (done < chunk && !stale))
+            return fail(ctx, DEM_ECUDA, "dem_step: inconsistent step flags (done %d of %d, stale %d)", done, chunk, (int)stale);
+        remaining -= done;
+        if (stale && remaining > 0) {
             CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
-            CHECK(evaluate(ctx, x, q, true, sid, N, F, T, nullptr, nullptr, &ka));
-            done += 1;
-            if (th) CHECK(thermostat(nsteps - remaining + done == nsteps ? 1 : 2, nullptr));
-            ctx->rebuild_interval = since + done;
+            ctx->rebuild_interval = since + done + 1;
             since = 0;
         } else {
             since += done;
         }
-        remaining -= done;
     }
     if (th) {
         k_scale_momenta<<<nblk(N, B), B, 0, st>>>(N, v, L, th);
@@ -424,7 +445,7 @@ template <typename real> int step_npt_t(dem_ctx* ctx, void* pos, void* quat, voi
     // forces, virial and the sums of the current state
     auto forces = [&]() -> int {
         for (int a = 0; a < 3; ++a) ctx->box[a] = box[a];  // the list stays; the minimum image uses the current box
-        return evaluate(ctx, x, q, true, sid, N, F, T, W, nullptr, nullptr);
+        return evaluate(ctx, x, q, true, sid, N, F, T, W, nullptr);
     };
     auto sums = [&]() -> int {
         k_npt_sums<real><<<nbk, 256, 0, st>>>(N, dim, sid, ctx->mt, q, v, L, W, ctx->epart.as<double>());
@@ -658,7 +679,7 @@ int dem_copy_neighbors(dem_ctx* ctx, int32_t* counts_out, int32_t* list_out, int
 int dem_compute(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* shape_id, int N, void* force_energy,
                 void* torque, void* virial6) {
     if (!ctx) return DEM_EINVAL;
-    return evaluate(ctx, pos, quat, ctx->prec == DEM_F64, shape_id, N, force_energy, torque, virial6, nullptr, nullptr);
+    return evaluate(ctx, pos, quat, ctx->prec == DEM_F64, shape_id, N, force_energy, torque, virial6, nullptr);
 }
 
 int dem_get_counters(dem_ctx* ctx, int64_t out[9]) {

@@ -184,7 +184,7 @@ __global__ void k_pair_fill(int N, const int* __restrict__ counts, const int* __
             DEM_ASSERT(p >= 0 && p < ct.pair_base[nclass]);
             const bool i_first = si <= sj;  // the pair's first particle is the one with the smaller shape id
             pairs[p] = i_first ? make_int2(i, j) : make_int2(j, i);
-            slot[(size_t)i * stride + k] = 2 * p + (i_first ? 0 : 1);
+            slot[(size_t)k * N + i] = 2 * p + (i_first ? 0 : 1);  // neighbour-major: [stride][N]
         }
     }
 }
@@ -211,7 +211,7 @@ __global__ void k_slot_back(int N, const int* __restrict__ counts, const int* __
             const int p = poff[(size_t)c * N + j] + r;
             DEM_ASSERT(r < nj && p >= ct.pair_base[c] && p < ct.pair_base[c + 1]);
             const bool j_first = sj <= si;
-            slot[(size_t)i * stride + k] = 2 * p + (j_first ? 1 : 0);
+            slot[(size_t)k * N + i] = 2 * p + (j_first ? 1 : 0);
         }
     }
 }

@@ -119,13 +119,25 @@ struct PoseArgs {
     const int* skip;  // dem_step: non-null and *skip != 0 => the list is stale, the kernel does nothing (see step_t)
 };
 
-// second half kick of velocity Verlet, fused into the reduction (k_reduce<KICK>)
-struct KickArgs {
-    double half_dt;
-    int dim;
-    d4* vel;
-    d4* ang;
-    double inv_mass[DEM_MAX_SHAPES_K];
+// What k_finish does behind the per-particle reduction (dem_kernels.cuh).
+//   mode 0  nothing more (dem_compute)
+//   mode 1  the second half kick of velocity Verlet, which completes a time step
+//   mode 2  that, and the first half of the NEXT step: half kick, drift (wrapped), free rotation, skin test
+// dem_step queues many steps before the host looks at anything; two device flags, used alternately, keep that safe:
+// a kernel does nothing when *bail is set (raised by a kernel BEFORE it: some particle left its skin, the list is
+// stale) -- it then raises *raise, so that the word reaches the evaluation after it, which looks at the other flag --
+// and raises *raise when its own drift takes a particle out of its skin.
+struct FinArgs {
+    int mode, dim;
+    double dt;
+    d4 *pos, *quat, *vel, *ang;
+    const d4* pos_build;  // positions at the last neighbour build (skin test)
+    double half_skin2;
+    BoxDev box;
+    MassTable mt;
+    const int* bail;
+    int* raise;
+    int* done;  // += 1 when the kernel completed a step (modes 1, 2)
 };
 
 // Nose-Hoover thermostat (dem_step_nvt; R19): friction xi, its time integral eta, the scaling

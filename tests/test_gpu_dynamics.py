@@ -214,19 +214,20 @@ def test_config3_drift_is_truncation_not_precision(pkg):
     """Config 3 (FP32, dt = 5e-4) shows max |E(t) - E(0)|/N = 2.3e-4, above north_star's 1e-4.  What that number is:
     (i) the same run in a DEM_F64 context reads the same value, so it is not single precision; (ii) at dt/2 it drops by
     ~4: the O(dt^2) offset of a second-order integrator started from a lattice, reached within the first
-    few hundred steps; (iii) it does not grow: the least-squares drift over 10^4 steps -- the measure PAPER.md:85
-    reports -- is below 1e-4 per particle (R18)."""
+    200 steps; (iii) behind that offset the energy creeps at (5-7)e-5 per particle per 10^4 steps in BOTH precisions
+    (1.2e-5 epsilon/tau per particle; PAPER.md:85 reports 1.4e-5 for its squares): the least-squares rate over steps
+    1,000 ... 20,000 -- the measure PAPER.md:85 uses -- is below north_star's 1e-4 per 10^4 steps (R18)."""
     st = di.make_config(3)
-    steps = np.arange(1, 51) * 200
-    r32 = _run(pkg, st, "f32", st["dt"], 10000, skin=0.2, chunks=50)
-    r64 = _run(pkg, st, "f64", st["dt"], 10000, skin=0.2, chunks=50)
+    steps = np.arange(1, 101) * 200
+    r32 = _run(pkg, st, "f32", st["dt"], 20000, skin=0.2, chunks=100)
+    r64 = _run(pkg, st, "f64", st["dt"], 20000, skin=0.2, chunks=100)
     e32, e64 = r32["energies"].sum(1) / st["N"], r64["energies"].sum(1) / st["N"]
     d32, d64 = np.abs(e32 - r32["e0"] / st["N"]).max(), np.abs(e64 - r64["e0"] / st["N"]).max()
-    s32, s64 = _lsq_drift(steps, e32), _lsq_drift(steps, e64)
+    s32, s64 = _lsq_drift(steps[4:], e32[4:]), _lsq_drift(steps[4:], e64[4:])
     half = _run(pkg, st, "f64", st["dt"] / 2, 4000, skin=0.2, chunks=20)
     dh = np.abs(half["energies"].sum(1) - half["e0"]).max() / st["N"]
-    print("config 3, 10^4 steps: max dev f32 %.3e f64 %.3e; lsq drift per 10^4 steps f32 %.3e f64 %.3e; f64 at dt/2 "
-          "(2000 tau-equivalent steps) max dev %.3e" % (d32, d64, s32, s64, dh))
+    print("config 3, 2 x 10^4 steps: max dev f32 %.3e f64 %.3e; lsq drift per 10^4 steps f32 %.3e f64 %.3e; f64 at dt/2 "
+          "(4000 steps) max dev %.3e" % (d32, d64, s32, s64, dh))
     assert abs(d32 - d64) < 0.1 * d64, (d32, d64)
     assert 2.8 < d64 / dh < 5.5, (d64, dh)
     assert abs(s32) < 1e-4 and abs(s64) < 1e-4, (s32, s64)
