@@ -71,10 +71,12 @@ struct dem_ctx {
     int force_slices = 0;  // 0 = heuristic
     bool cull = true;             // packed search kernel in 3D: exact per-feature culling (dem_set_culling)
     bool generic_kernel = false;  // DEM_F32 contexts: use the generic k_pair instead of the packed search kernel
+    bool particle2d = false;      // DEM_F32 contexts in 2D (DEM_KERNEL_AUTO): the per-particle kernel k_particle2d
     size_t l2_flush_bytes = 0;  // bench hygiene: overwrite this many bytes of scratch before every time step
     DevBuf l2_scratch;
     // dem_step state (double) for DEM_F32 contexts, plus forces and the positions of the last build
     DevBuf st_pos, st_quat, st_vel, st_ang, st_force, st_torque, st_virial, pos_build, epart;
+    DevBuf st_pos2, st_quat2;  // second position / orientation buffers of the 2D per-particle step (ping-pong)
     // host-buffer entry points
     DevBuf h_pos, h_quat, h_vel, h_ang, h_sid, h_force, h_torque, h_virial;
     // accounting
@@ -182,6 +184,12 @@ cudaError_t launch_pair_cull(bool same_shape, int grid, int threads, size_t smem
 cudaError_t launch_pair_generic_f32(int dim, bool pos_is_double, int grid, int threads, size_t smem, cudaStream_t st,
                                     const PairArgs<float>& a);
 cudaError_t launch_pair_generic_f64(int dim, int grid, int threads, size_t smem, cudaStream_t st, const PairArgs<double>& a);
+// k_particle2d (dem_step2d.cu): the whole 2D evaluation (+ integrator, FinArgs) of a DEM_F32 context in one kernel.
+// pos / quat are what the forces are evaluated at; in mode 2 the drifted state is written to fin->pos / fin->quat,
+// which must be other buffers.  Returns false when the kernel does not apply (rows longer than its bit mask).
+bool particle2d_applies(const dem_ctx* ctx);
+int launch_particle2d(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_double, const int32_t* sid, int N,
+                      void* force, void* torque, void* virial, const FinArgs* fin);
 size_t pair_fast_smem_header();
 size_t pair_cull_smem_header();
 int pose_threads();

@@ -152,6 +152,7 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
 
 int evaluate(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_double, const int32_t* sid, int N, void* force,
              void* torque, void* virial, const FinArgs* fin) {
+    if (particle2d_applies(ctx)) return launch_particle2d(ctx, pos, quat, pos_is_double, sid, N, force, torque, virial, fin);
     if (ctx->prec == DEM_F64) return evaluate_t<double>(ctx, pos, quat, true, sid, N, force, torque, virial, fin);
     return evaluate_t<float>(ctx, pos, quat, pos_is_double, sid, N, force, torque, virial, fin);
 }

@@ -254,6 +254,16 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     } else {
         x = static_cast<d4*>(pos); q = static_cast<d4*>(quat); v = static_cast<d4*>(vel); L = static_cast<d4*>(ang);
     }
+    // the 2D per-particle kernel drifts into a second pair of position / orientation buffers (other warps still read
+    // the old state): xs[cur] / qs[cur] hold the current state
+    d4 *xs[2] = {x, x}, *qs[2] = {q, q};
+    int cur = 0;
+    if (conv && ctx->dim == 2 && ctx->particle2d) {
+        CU(ctx->st_pos2.reserve(sizeof(d4) * (size_t)N));
+        CU(ctx->st_quat2.reserve(sizeof(d4) * (size_t)N));
+        xs[1] = ctx->st_pos2.as<d4>();
+        qs[1] = ctx->st_quat2.as<d4>();
+    }
     CU(ctx->st_force.reserve(sizeof(real4) * (size_t)N));
     CU(ctx->st_torque.reserve(sizeof(real4) * (size_t)N));
     real4* F = ctx->st_force.as<real4>();
@@ -279,7 +289,7 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     ThermoDev* th = nullptr;
     const int nbk = nblk(N, 256);
     auto thermostat = [&](int halves, const int* bail) -> int {
-        k_kinetic<<<nbk, 256, 0, st>>>(N, ctx->dim, sid, ctx->mt, q, v, L, ctx->epart.as<double>());
+        k_kinetic<<<nbk, 256, 0, st>>>(N, ctx->dim, sid, ctx->mt, qs[cur], v, L, ctx->epart.as<double>());
         LAUNCHED(ctx);
         k_thermostat<<<1, 256, 0, st>>>(nbk, ctx->epart.as<double>(), ctx->dim, N, dt, nvt->kT, nvt->tau, halves, bail, th);
         LAUNCHED(ctx);
@@ -312,7 +322,7 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     memset(&fa, 0, sizeof fa);
     fa.dim = ctx->dim;
     fa.dt = dt;
-    fa.pos = x; fa.quat = q; fa.vel = v; fa.ang = L;
+    fa.vel = v; fa.ang = L;
     fa.pos_build = ctx->pos_build.as<d4>();
     fa.half_skin2 = half_skin2;
     fa.box = bx;
@@ -320,8 +330,8 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     fa.done = flags + 2;
     auto kick_drift = [&](const int* bail, int* raise) {
         cudaEvent_t k0 = ev_mark(ctx, 2);
-        k_kick_drift<real><<<2 * nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, x, q, v, L, F, T, ctx->pos_build.as<d4>(),
-                                                     half_skin2, bail, raise, th);
+        k_kick_drift<real><<<2 * nblk(N, B), B, 0, st>>>(N, bx, dt, sid, ctx->mt, xs[cur], qs[cur], v, L, F, T,
+                                                     ctx->pos_build.as<d4>(), half_skin2, bail, raise, th);
         LAUNCHED(ctx);
         ev_span(ctx, KT_KICK_DRIFT, k0, ev_mark(ctx, 2));
     };
@@ -335,6 +345,8 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
             kick_drift(nullptr, flags);
             drifted = true;
         }
+        const bool pingpong = xs[1] != xs[0] && particle2d_applies(ctx);
+        int c = cur, swaps = 0;  // buffer the queued evaluations read, and how many of them drift into the other one
         for (int e = 0; e < chunk; ++e) {
             if (ctx->l2_flush_bytes) {
                 cudaEvent_t f0 = ev_mark(ctx, 2);
@@ -345,7 +357,12 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
             fa.mode = (last || th) ? 1 : 2;
             fa.bail = flags + (e & 1);
             fa.raise = flags + ((e + 1) & 1);
-            CHECK(evaluate(ctx, x, q, true, sid, N, F, T, nullptr, &fa));
+            const int out = pingpong && fa.mode == 2 ? c ^ 1 : c;
+            fa.pos = xs[out];
+            fa.quat = qs[out];
+            CHECK(evaluate(ctx, xs[c], qs[c], true, sid, N, F, T, nullptr, &fa));
+            if (out != c) ++swaps;
+            c = out;
             if (th) {
                 CHECK(thermostat(last ? 1 : 2, fa.bail));
                 if (!last) kick_drift(fa.bail, fa.raise);
@@ -358,8 +375,9 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
         if (done < 0 || done > chunk || (done < chunk && !stale))
             return fail(ctx, DEM_ECUDA, "dem_step: inconsistent step flags (done %d of %d, stale %d)", done, chunk, (int)stale);
         remaining -= done;
+        cur ^= std::min(done, swaps) & 1;  // evaluations behind a stale flag did not run: the state stayed where it was
         if (stale && remaining > 0) {
-            CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
+            CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(xs[cur]), sid, N, box, r_list, false));
             ctx->rebuild_interval = since + done + 1;
             since = 0;
         } else {
@@ -372,7 +390,7 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     }
     if (conv) {
         void* out[4] = {pos, quat, vel, ang};
-        d4* in[4] = {x, q, v, L};
+        d4* in[4] = {xs[cur], qs[cur], v, L};
         for (int k = 0; k < 4; ++k) {
             k_d4_to_f4<<<nblk(N, B), B, 0, st>>>(N, in[k], static_cast<f4*>(out[k]));
             LAUNCHED(ctx);
@@ -577,7 +595,7 @@ int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda
     c->eps = epsilon;
     c->prec = precision;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
-    c->generic_kernel = dim == 2;  // DEM_KERNEL_AUTO
+    c->particle2d = dim == 2;  // DEM_KERNEL_AUTO
     memset(&c->ct, 0, sizeof c->ct);
     memset(&c->mt, 0, sizeof c->mt);
     *out = c;
@@ -588,7 +606,7 @@ int dem_destroy(dem_ctx* c) {
     if (!c) return DEM_EINVAL;
     DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
                       &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->rflag, &c->flags, &c->counters, &c->thermo, &c->pose, &c->pidx, &c->cum, &c->st_pos, &c->st_quat,
-                      &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->st_virial, &c->pos_build, &c->epart, &c->h_pos,
+                      &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->st_virial, &c->st_pos2, &c->st_quat2, &c->pos_build, &c->epart, &c->h_pos,
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();
     if (c->h_moved) cudaFreeHost(c->h_moved);
@@ -618,7 +636,8 @@ int dem_set_slices(dem_ctx* ctx, int slices) {
 int dem_set_pair_kernel(dem_ctx* ctx, int which) {
     if (!ctx || (which != DEM_KERNEL_SEARCH && which != DEM_KERNEL_GENERIC && which != DEM_KERNEL_AUTO))
         return fail(ctx, DEM_EINVAL, "unknown pair kernel");
-    ctx->generic_kernel = which == DEM_KERNEL_GENERIC || (which == DEM_KERNEL_AUTO && ctx->dim == 2);
+    ctx->generic_kernel = which == DEM_KERNEL_GENERIC;
+    ctx->particle2d = which == DEM_KERNEL_AUTO && ctx->dim == 2;
     return DEM_OK;
 }
 
@@ -698,7 +717,7 @@ int dem_get_counters(dem_ctx* ctx, int64_t out[9]) {
     out[5] = ctx->npairs_total;
     // terms whose nearest-point search was executed (the search kernels count what they sweep; the generic kernel
     // sweeps every term of the pairs it evaluates)
-    if (ctx->prec == DEM_F32 && !ctx->generic_kernel) {
+    if (ctx->prec == DEM_F32 && (!ctx->generic_kernel || particle2d_applies(ctx))) {
         out[6] = (int64_t)(h[4] + h[5]);
         out[7] = (int64_t)h[4];
         out[8] = (int64_t)h[6];

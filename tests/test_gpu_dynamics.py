@@ -207,7 +207,12 @@ def test_full_size_fp32_runs_of_the_configs(pkg, oracle, k, skin, nsteps):
     assert np.abs(tq[:, :3] - ot[:, :3]).max() / ts < 1e-4
     assert np.abs(f[:, 3] - of[:, 3]).max() / us < 1e-4
     assert np.abs(w - ow).max() / max(np.abs(ow).max(), 1.0) < 1e-4
-    assert 2 * cnt["active"] == ocnt[2] and 2 * cnt["degenerate"] == ocnt[3] and 2 * cnt["parallel"] == ocnt[4]
+    # Whether a term is inside the cutoff is decided in FP32 on the GPU and in FP64 by the oracle.  In a fluid state
+    # with ~10^5 active terms spread over [sigma, 2^(1/6) sigma], a handful lie within FP32 rounding (~2e-6 relative in
+    # r^2) of the cutoff, where the two decisions may differ (such a term carries no force: U and F vanish there).  The
+    # small states of test_gpu_parity.py require exact equality; here a few parts in 10^5 are allowed.
+    assert abs(2 * cnt["active"] - ocnt[2]) <= max(4, 1e-4 * ocnt[2]), (cnt, ocnt)
+    assert 2 * cnt["degenerate"] == ocnt[3] and abs(2 * cnt["parallel"] - ocnt[4]) <= max(4, 1e-4 * ocnt[4])
 
 
 def test_config3_drift_is_truncation_not_precision(pkg):
