@@ -123,7 +123,7 @@ int dem_copy_neighbors(dem_ctx* ctx, int32_t* counts_out, int32_t* list_out, int
 int dem_compute(dem_ctx* ctx, const void* pos, const void* quat, const int32_t* shape_id, int N, void* force_energy,
                 void* torque, void* virial6);
 
-/* Counters of the last dem_compute (synchronises): out[0] unique particle pairs evaluated, out[1] Eq. 1/2 terms
+/* Counters of the last dem_compute (not of dem_step, whose kernels keep none) (synchronises): out[0] unique particle pairs evaluated, out[1] Eq. 1/2 terms
  * of those pairs (polygon faces, each unique pair once), out[2] terms inside the WCA cutoff, out[3] degenerate terms
  * skipped, out[4] terms that took the parallel-edge branch, out[5] unique pairs in the work list, out[6] terms whose
  * nearest-point search was actually executed (= out[1] unless exact culling proved features out of reach: see

@@ -77,6 +77,16 @@ struct dem_ctx {
     // dem_step state (double) for DEM_F32 contexts, plus forces and the positions of the last build
     DevBuf st_pos, st_quat, st_vel, st_ang, st_force, st_torque, st_virial, pos_build, epart;
     DevBuf st_pos2, st_quat2;  // second position / orientation buffers of the 2D per-particle step (ping-pong)
+    // A DEM_F32 context that is handed back, unchanged, the arrays its last dem_step returned continues from its internal
+    // double state, neighbour list and forces instead of converting, rebuilding and re-evaluating (dem_lib.cu: step_t)
+    struct Resume {
+        bool valid = false;
+        const void *pos = nullptr, *quat = nullptr, *vel = nullptr, *ang = nullptr;
+        const int32_t* sid = nullptr;
+        int N = 0, cur = 0;
+        double box[3] = {0, 0, 0}, skin = 0;
+    } resume;
+    DevBuf sid_copy;
     // host-buffer entry points
     DevBuf h_pos, h_quat, h_vel, h_ang, h_sid, h_force, h_torque, h_virial;
     // accounting
@@ -94,6 +104,7 @@ struct dem_ctx {
     cudaEvent_t ev_copy = nullptr;
     bool ev_copy_pending = false;
     double nvt_dof = 0;            // degrees of freedom counted by the last dem_step_nvt
+    int steps_since_build = 0;     // age of the list when the last dem_step returned (carried into a resumed call)
     int rebuild_interval = 8;      // steps between the last two neighbour rebuilds of dem_step (sizes its chunks)
 };
 

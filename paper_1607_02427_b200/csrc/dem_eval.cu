@@ -60,7 +60,7 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
         a.pc.eps = (real)ctx->eps;
         a.pc.eps_par = (real)ctx->eps_par;
         a.pc.degen2 = (real)((1e-6 * sigma) * (1e-6 * sigma));
-        a.counters = ctx->counters.as<unsigned long long>();
+        a.counters = fin ? nullptr : ctx->counters.as<unsigned long long>();  // kept for dem_compute only
         a.cum = (ctx->timing && ctx->cum.p) ? ctx->cum.as<unsigned long long>() : nullptr;
         // candidate cutoff of the FP32 search kernel: FP32 rounding of the packed formulation (1e-3 relative) plus
         // its error on near-parallel edges, at most sin(angle) x edge length with the angle below ~1e-3 where the

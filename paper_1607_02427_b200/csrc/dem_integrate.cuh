@@ -303,6 +303,26 @@ __global__ void k_energy(int N, int dim, const int* __restrict__ sid, MassTable 
         for (int a = 0; a < 3; ++a) partial[3 * blockIdx.x + a] = sh[a][0];
 }
 
+// Are the caller's float arrays still what the last dem_step returned, i.e. the internal double state rounded to float
+// (and the shape ids the ones the list was built with)?  Raises *differ otherwise.
+static __global__ void k_same_state(int n, const f4* __restrict__ pos, const f4* __restrict__ quat, const f4* __restrict__ vel,
+                                    const f4* __restrict__ ang, const int* __restrict__ sid, const d4* __restrict__ x,
+                                    const d4* __restrict__ q, const d4* __restrict__ v, const d4* __restrict__ L,
+                                    const int* __restrict__ sid_copy, int* __restrict__ differ) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const f4* f[4] = {pos, quat, vel, ang};
+    const d4* d[4] = {x, q, v, L};
+    bool same = sid[i] == sid_copy[i];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const f4 a = f[k][i];
+        const d4 b = d[k][i];
+        same = same && a.x == (float)b.x && a.y == (float)b.y && a.z == (float)b.z && a.w == (float)b.w;
+    }
+    if (!same) *differ = 1;
+}
+
 // ---- precision conversion of state arrays (DEM_F32 contexts integrate in double, R15b) --------------------------------
 __global__ void k_f4_to_d4(int n, const f4* __restrict__ in, d4* __restrict__ out) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;

@@ -114,7 +114,7 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
         c_deg += __shfl_xor_sync(0xffffffffu, c_deg, o);
         c_par += __shfl_xor_sync(0xffffffffu, c_par, o);
     }
-    if ((threadIdx.x & 31) == 0) {
+    if ((threadIdx.x & 31) == 0 && a.counters) {  // null inside dem_step: counters belong to dem_compute
         if (c_eval) atomicAdd(a.counters + 0, (unsigned long long)c_eval);
         if (c_act) atomicAdd(a.counters + 1, (unsigned long long)c_act);
         if (c_deg) atomicAdd(a.counters + 2, (unsigned long long)c_deg);

@@ -239,7 +239,28 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     const int B = 256;
     const bool conv = ctx->prec == DEM_F32;
     d4 *x, *q, *v, *L;
+    bool resumed = false;
     if (conv) {  // R15b: a DEM_F32 context integrates its state in double
+        // Handed back the very arrays the last call returned (same pointers, same contents)?  Then the internal double
+        // state, the neighbour list and the forces are still those of that state: go on from them.
+        dem_ctx::Resume& rs = ctx->resume;
+        if (rs.valid && !ctx->ev_copy_pending && rs.pos == pos && rs.quat == quat && rs.vel == vel && rs.ang == ang &&
+            rs.sid == sid && rs.N == N && rs.skin == skin && rs.box[0] == box[0] && rs.box[1] == box[1] &&
+            rs.box[2] == box[2] && ctx->have_list && ctx->N == N) {
+            int* differ = ctx->flags.as<int>() + 12;
+            CU(cudaMemsetAsync(differ, 0, sizeof(int), st));
+            k_same_state<<<nblk(N, B), B, 0, st>>>(N, static_cast<const f4*>(pos), static_cast<const f4*>(quat),
+                                                   static_cast<const f4*>(vel), static_cast<const f4*>(ang), sid,
+                                                   (rs.cur ? ctx->st_pos2 : ctx->st_pos).as<d4>(),
+                                                   (rs.cur ? ctx->st_quat2 : ctx->st_quat).as<d4>(), ctx->st_vel.as<d4>(),
+                                                   ctx->st_ang.as<d4>(), ctx->sid_copy.as<int>(), differ);
+            LAUNCHED(ctx);
+            int h = 1;
+            CU(cudaMemcpyAsync(&h, differ, sizeof(int), cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+            resumed = h == 0;
+        }
+        rs.valid = false;  // until this call returns
         CU(ctx->st_pos.reserve(sizeof(d4) * (size_t)N));
         CU(ctx->st_quat.reserve(sizeof(d4) * (size_t)N));
         CU(ctx->st_vel.reserve(sizeof(d4) * (size_t)N));
@@ -247,7 +268,7 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
         x = ctx->st_pos.as<d4>(); q = ctx->st_quat.as<d4>(); v = ctx->st_vel.as<d4>(); L = ctx->st_ang.as<d4>();
         const void* in[4] = {pos, quat, vel, ang};
         d4* out[4] = {x, q, v, L};
-        for (int k = 0; k < 2; ++k) {  // velocities and angular momenta follow the first evaluation (see below)
+        for (int k = 0; k < 2 && !resumed; ++k) {  // velocities and angular momenta follow the first evaluation (see below)
             k_f4_to_d4<<<nblk(N, B), B, 0, st>>>(N, static_cast<const f4*>(in[k]), out[k]);
             LAUNCHED(ctx);
         }
@@ -263,6 +284,7 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
         CU(ctx->st_quat2.reserve(sizeof(d4) * (size_t)N));
         xs[1] = ctx->st_pos2.as<d4>();
         qs[1] = ctx->st_quat2.as<d4>();
+        if (resumed) cur = ctx->resume.cur;
     }
     CU(ctx->st_force.reserve(sizeof(real4) * (size_t)N));
     CU(ctx->st_torque.reserve(sizeof(real4) * (size_t)N));
@@ -270,15 +292,17 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     real4* T = ctx->st_torque.as<real4>();
     const double r_list = max_reach(ctx) + skin;
     const BoxDev bx = box_dev(ctx->dim, box);
-    CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
-    CHECK(evaluate(ctx, x, q, true, sid, N, F, T, nullptr, nullptr));
+    if (!resumed) {
+        CHECK(build_neighbors_t<double>(ctx, reinterpret_cast<const double*>(x), sid, N, box, r_list, false));
+        CHECK(evaluate(ctx, x, q, true, sid, N, F, T, nullptr, nullptr));
+    }
     // The list build and the first evaluation need positions and orientations only: dem_step_host copies velocities
     // and angular momenta on a second stream meanwhile, and they are waited for (and converted) here.
     if (ctx->ev_copy_pending) {
         CU(cudaStreamWaitEvent(st, ctx->ev_copy, 0));
         ctx->ev_copy_pending = false;
     }
-    if (conv) {
+    if (conv && !resumed) {
         k_f4_to_d4<<<nblk(N, B), B, 0, st>>>(N, static_cast<const f4*>(vel), v);
         LAUNCHED(ctx);
         k_f4_to_d4<<<nblk(N, B), B, 0, st>>>(N, static_cast<const f4*>(ang), L);
@@ -335,11 +359,13 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
         LAUNCHED(ctx);
         ev_span(ctx, KT_KICK_DRIFT, k0, ev_mark(ctx, 2));
     };
-    int remaining = nsteps, since = 0;
+    int remaining = nsteps, since = resumed ? ctx->steps_since_build : 0;
     bool drifted = false;  // the state is past the drift of the next step (forces of the drifted state not yet evaluated)
     while (remaining > 0) {
-        const int hint = std::max(ctx->rebuild_interval, 1);
-        const int chunk = std::min(remaining, std::min(64, std::max(hint - since, std::max(1, hint / 8))));
+        // up to the predicted number of steps until the next rebuild (at least 8); past the prediction, 16 at a time: a step
+        // queued behind a stale flag costs three empty launches, a chunk boundary a host round trip
+        const int predicted = std::max(ctx->rebuild_interval, 1) - since;
+        const int chunk = std::min(remaining, predicted > 0 ? std::min(64, std::max(predicted, 8)) : 16);
         CU(cudaMemsetAsync(flags, 0, 3 * sizeof(int), st));
         if (!drifted) {  // the first half of the call's first step
             kick_drift(nullptr, flags);
@@ -407,6 +433,16 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
         nvt->thermo[1] = h1.eta;
         ctx->nvt_dof = h1.dof;
     }
+    ctx->steps_since_build = since;
+    if (conv) {  // what a next call must find unchanged to go on from here
+        CU(ctx->sid_copy.reserve(sizeof(int) * (size_t)N));
+        CU(cudaMemcpyAsync(ctx->sid_copy.p, sid, sizeof(int) * (size_t)N, cudaMemcpyDeviceToDevice, st));
+        dem_ctx::Resume& rs = ctx->resume;
+        rs.pos = pos; rs.quat = quat; rs.vel = vel; rs.ang = ang; rs.sid = sid;
+        rs.N = N; rs.cur = cur; rs.skin = skin;
+        for (int a = 0; a < 3; ++a) rs.box[a] = box[a];
+        rs.valid = true;
+    }
     // the internal list was built from internal (double) positions; a later dem_compute on caller arrays is still valid
     return DEM_OK;
 }
@@ -427,6 +463,7 @@ template <typename real> int step_npt_t(dem_ctx* ctx, void* pos, void* quat, voi
     typedef typename vec4<real>::type real4;
     if (N < 2 || !pos || !quat || !vel || !ang || !sid) return fail(ctx, DEM_EINVAL, "bad particle arrays");
     if (nsteps < 0 || !(skin >= 0)) return fail(ctx, DEM_EINVAL, "bad nsteps / skin");
+    ctx->resume.valid = false;  // this path shares dem_step's internal state and moves the box
     CHECK(sync_tables(ctx));
     cudaStream_t st = ctx->stream;
     const int B = 256, dim = ctx->dim;
@@ -606,7 +643,7 @@ int dem_destroy(dem_ctx* c) {
     if (!c) return DEM_EINVAL;
     DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
                       &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->rflag, &c->flags, &c->counters, &c->thermo, &c->pose, &c->pidx, &c->cum, &c->st_pos, &c->st_quat,
-                      &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->st_virial, &c->st_pos2, &c->st_quat2, &c->pos_build, &c->epart, &c->h_pos,
+                      &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->st_virial, &c->st_pos2, &c->st_quat2, &c->sid_copy, &c->pos_build, &c->epart, &c->h_pos,
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();
     if (c->h_moved) cudaFreeHost(c->h_moved);
@@ -622,6 +659,7 @@ const char* dem_last_error(const dem_ctx* c) { return c ? c->err.c_str() : "null
 int dem_set_eps_par(dem_ctx* ctx, double eps_par) {
     if (!ctx || !(eps_par >= 0)) return fail(ctx, DEM_EINVAL, "eps_par must be >= 0");
     ctx->eps_par = eps_par;
+    ctx->resume.valid = false;  // the stored forces were evaluated with the old threshold
     return DEM_OK;
 }
 
@@ -630,6 +668,7 @@ int dem_set_slices(dem_ctx* ctx, int slices) {
     if (!ctx || slices < 0) return fail(ctx, DEM_EINVAL, "slices must be >= 0");
     ctx->force_slices = slices;
     ctx->have_list = false;
+    ctx->resume.valid = false;
     return DEM_OK;
 }
 
@@ -669,6 +708,7 @@ int dem_create_shape(dem_ctx* ctx, const double* verts, int nv, const int* face_
 int dem_build_neighbors(dem_ctx* ctx, const void* pos, const int32_t* shape_id, int N, const double box[3], double r_cut) {
     if (!ctx) return DEM_EINVAL;
     if (!box) return fail(ctx, DEM_EINVAL, "null box");
+    ctx->resume.valid = false;  // the caller's list replaces dem_step's
     if (ctx->prec == DEM_F64) return build_neighbors_t<double>(ctx, static_cast<const double*>(pos), shape_id, N, box, r_cut, true);
     return build_neighbors_t<float>(ctx, static_cast<const float*>(pos), shape_id, N, box, r_cut, true);
 }
