@@ -64,6 +64,7 @@ struct dem_ctx {
     DevBuf cell_of, rank, cell_start, order, xs, counts, list, slot, scratch_scan, pcnt, pairs, rec, rflag, flags, counters, thermo;
     DevBuf cum;         // running totals of the swept-term counters while timing is on
     DevBuf pose, pidx;  // FP32 search kernel: compacted pose records per class (k_pose)
+    DevBuf cmask;       // culling kernel: survivor masks per compacted pair (k_pose_cull)
     ClassTable ct;
     int nclass = 0;
     int class_sa[DEM_MAX_CLASSES], class_sb[DEM_MAX_CLASSES], class_np[DEM_MAX_CLASSES];
@@ -190,6 +191,8 @@ int evaluate(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_double
 
 // ---- kernel launchers (one translation unit per kernel family) ------------------------------------------------------------
 void launch_pose(int dim, bool pos_is_double, int grid, cudaStream_t st, const PoseArgs& pa);
+void launch_pose_cull(bool pos_is_double, int grid, size_t smem, cudaStream_t st, const PoseArgs& pa);
+int pose_cull_max_words();
 cudaError_t launch_pair_fast(int dim, bool tv3, int grid, int threads, size_t smem, cudaStream_t st, const PairArgs<float>& a);
 cudaError_t launch_pair_cull(bool same_shape, int grid, int threads, size_t smem, cudaStream_t st, const PairArgs<float>& a);
 cudaError_t launch_pair_generic_f32(int dim, bool pos_is_double, int grid, int threads, size_t smem, cudaStream_t st,

@@ -33,6 +33,7 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
     if (search) {
         CU(ctx->pose.reserve(sizeof(f4) * 6 * std::max<size_t>(list_base[ctx->nclass], 1)));
         CU(ctx->pidx.reserve(sizeof(int) * std::max<size_t>(list_base[ctx->nclass], 1)));
+        if (cull) CU(ctx->cmask.reserve(sizeof(unsigned) * pose_cull_max_words() * std::max<size_t>(list_base[ctx->nclass], 1)));
     }
     const BoxDev bx = box_dev(ctx->dim, ctx->box);
     for (int c = 0; c < ctx->nclass; ++c) {
@@ -92,7 +93,23 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
                 pa.counters = a.counters;
                 pa.rflag = a.rflag;
                 pa.skip = skip;
-                launch_pose(ctx->dim, pos_is_double, nblk(np, pose_block), st, pa);
+                // culling: the cull tests run in the pose kernel (k_pose_cull), which hands per-pair survivor masks to the
+                // search kernel and lists only pairs with a surviving feature -- unless the masks would not fit its
+                // registers or the pairs are sliced (then k_pair_cull tests for itself)
+                const int mw_e = (HB.ne + 31) / 32, mw_vj = (HB.nv + 31) / 32, mw_vi = (HA.nv + 31) / 32;
+                const double ra = HA.circumradius + rcs, rb = HB.circumradius + rcs;
+                const bool premask = cull && a.slices == 1 && mw_e + mw_vj + mw_vi <= pose_cull_max_words();
+                if (premask) {
+                    pa.table = a.table; pa.sa = a.sa; pa.sb = a.sb;
+                    pa.cull_a2 = (float)(ra * ra);
+                    pa.cull_b2 = (float)(rb * rb);
+                    pa.cmask = ctx->cmask.as<unsigned>() + (size_t)pose_cull_max_words() * list_base[c];
+                    pa.mw_e = mw_e; pa.mw_vj = mw_vj; pa.mw_vi = mw_vi;
+                    a.cmask = pa.cmask; a.mw_e = mw_e; a.mw_vj = mw_vj; a.mw_vi = mw_vi;
+                    launch_pose_cull(pos_is_double, nblk(np, pose_block), smem, st, pa);
+                } else {
+                    launch_pose(ctx->dim, pos_is_double, nblk(np, pose_block), st, pa);
+                }
                 LAUNCHED(ctx);
                 em = ev_mark(ctx);
                 // the padded work list bounds the tiles; grid cap in blocks per SM measured on cfg4 (one tile per warp
@@ -101,7 +118,6 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
                 grid = (int)std::min<long long>(nblk(list_items, threads), (long long)ctx->sm_count * 64);
                 if (cull) {
                     smem += pair_cull_smem_header();
-                    const double ra = HA.circumradius + rcs, rb = HB.circumradius + rcs;
                     a.cull_a2 = (real)(ra * ra);
                     a.cull_b2 = (real)(rb * rb);
                     CU(launch_pair_cull(same, grid, threads, smem, st, a));

@@ -464,6 +464,127 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THR
     }
 }
 
+// ---- a3 with exact per-feature culling (3D, the library default) ----------------------------------------------------------
+// k_pose plus the cull tests of k_pair_cull, done here because this kernel has the pose in registers and idle issue slots
+// (it is bound by the latency of its gathers), while the search kernel behind it runs at 10 warps per SM: every feature
+// of a particle lies within its circumradius R of its centre, so an outer feature of the other particle at R + rc_search or
+// more from that centre cannot be a candidate against any of its features.  Per pair three bit masks come out (edges of
+// j near i, vertices of j near i, vertices of i near j; at most DEM_CM_WORDS words), and only pairs with a surviving
+// feature enter the work list at all.
+#define DEM_CM_WORDS 8
+template <typename PosT> __global__ void __launch_bounds__(DEM_POSE_THREADS) k_pose_cull(const PoseArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ int wcount[DEM_POSE_THREADS / 32], s_prefix;
+    if (a.skip && *a.skip) return;  // the work-list count stays 0: the search kernel behind finds no tile
+    f4* sm = reinterpret_cast<f4*>(smem_raw);
+    const bool same = a.sa.off == a.sb.off;
+    for (int k = threadIdx.x; k < a.sa.len; k += blockDim.x) sm[k] = a.table[a.sa.off + k];
+    if (!same)
+        for (int k = threadIdx.x; k < a.sb.len; k += blockDim.x) sm[a.sa.len + k] = a.table[a.sb.off + k];
+    const f4* AV = sm;
+    const f4* BV = same ? sm : sm + a.sa.len;
+    const f4* BOE = BV + a.sb.nv + 2 * a.sb.ne + 4 * a.sb.nf + 2 * a.sb.nfe;
+    const unsigned full = 0xffffffffu;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    bool valid = false;
+    double d[3] = {0.0, 0.0, 0.0};
+    d4 qi, qj;
+    qi.x = qj.x = 1.0; qi.y = qi.z = qi.w = qj.y = qj.z = qj.w = 0.0;
+    if (p < a.npairs) {
+        const int2 ij = a.pairs[p];
+        const d4 xi = load4d(static_cast<const PosT*>(a.pos), ij.x), xj = load4d(static_cast<const PosT*>(a.pos), ij.y);
+        qi = load4d(static_cast<const PosT*>(a.quat), ij.x);
+        qj = load4d(static_cast<const PosT*>(a.quat), ij.y);
+        d[0] = xj.x - xi.x; d[1] = xj.y - xi.y; d[2] = xj.z - xi.z;
+        d[0] -= a.box.L[0] * rint(d[0] * a.box.invL[0]);
+        d[1] -= a.box.L[1] * rint(d[1] * a.box.invL[1]);
+        d[2] -= a.box.L[2] * rint(d[2] * a.box.invL[2]);
+        valid = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] < a.reach2;
+    }
+    __syncthreads();  // the staged tables
+    float Mi[9], R[9], t[3];
+    unsigned cm[DEM_CM_WORDS];
+#pragma unroll
+    for (int w = 0; w < DEM_CM_WORDS; ++w) cm[w] = 0u;
+    unsigned anybit = 0u;
+    if (valid) {
+        const double qa[4] = {qi.x, qi.y, qi.z, qi.w}, qb[4] = {qj.x, qj.y, qj.z, qj.w};
+        pair_pose<float>(qa, qb, d, Mi, R, t);
+        // in j's frame the centre of i is -R^T t: |R v + t| = |v + R^T t|, no rotation of the features is needed
+        float tp[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) tp[k] = R[k] * t[0] + R[3 + k] * t[1] + R[6 + k] * t[2];
+#pragma unroll
+        for (int w = 0; w < DEM_CM_WORDS; ++w) {
+            unsigned m = 0u;
+            if (w < a.mw_e) {  // edges of j: nearest point of the segment to the centre of i
+                const int l0 = 32 * w, n = min(32, a.sb.ne - l0);
+                for (int k = 0; k < n; ++k) {
+                    const f4 a0 = BOE[2 * (l0 + k)], a1 = BOE[2 * (l0 + k) + 1];
+                    const float qx = a0.x + tp[0], qy = a0.y + tp[1], qz = a0.z + tp[2];
+                    const float s = fminf(fmaxf(-(qx * a1.x + qy * a1.y + qz * a1.z), 0.f), a0.w);
+                    const float cx = qx + s * a1.x, cy = qy + s * a1.y, cz = qz + s * a1.z;
+                    m |= (cx * cx + cy * cy + cz * cz < a.cull_a2 ? 1u : 0u) << k;
+                }
+            } else if (w < a.mw_e + a.mw_vj) {  // vertices of j near i
+                const int o0 = 32 * (w - a.mw_e), n = min(32, a.sb.nv - o0);
+                for (int k = 0; k < n; ++k) {
+                    const f4 v = BV[o0 + k];
+                    const float qx = v.x + tp[0], qy = v.y + tp[1], qz = v.z + tp[2];
+                    m |= (qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
+                }
+            } else if (w < a.mw_e + a.mw_vj + a.mw_vi) {  // vertices of i near j: |R^T (v - t)| = |v - t|
+                const int o0 = 32 * (w - a.mw_e - a.mw_vj), n = min(32, a.sa.nv - o0);
+                for (int k = 0; k < n; ++k) {
+                    const f4 v = AV[o0 + k];
+                    const float qx = v.x - t[0], qy = v.y - t[1], qz = v.z - t[2];
+                    m |= (qx * qx + qy * qy + qz * qz < a.cull_b2 ? 1u : 0u) << k;
+                }
+            }
+            cm[w] = m;
+            anybit |= m;
+        }
+    }
+    const bool keep = valid && anybit != 0u;
+    if (p < a.npairs && !keep)  // beyond the reach, or no feature within reach of the other particle: contributes nothing
+        for (int sl = 0; sl < a.slices; ++sl) a.rflag[(size_t)p * a.slices + sl] = 0;
+    // compaction as in k_pose
+    const unsigned m = __ballot_sync(full, keep);
+    if (lane == 0) wcount[warp] = __popc(m);
+    __syncthreads();
+    int tot = 0;
+#pragma unroll
+    for (int k = 0; k < DEM_POSE_THREADS / 32; ++k) tot += wcount[k];
+    const int tot_pad = (tot + a.pad - 1) & ~(a.pad - 1);
+    if (threadIdx.x == 0) {
+        s_prefix = tot_pad ? atomicAdd(a.count, tot_pad) : 0;
+    }
+    if (a.counters) {  // pairs inside the reach (dem_get_counters out[0]), whether or not a feature survives
+        const unsigned mv = __ballot_sync(full, valid);
+        if (lane == 0 && mv) atomicAdd(a.counters, (unsigned long long)__popc(mv));
+    }
+    __syncthreads();
+    if ((int)threadIdx.x < tot_pad - tot) a.pidx[s_prefix + tot + threadIdx.x] = -1;
+    if (keep) {
+        int wb = s_prefix;
+        for (int k = 0; k < warp; ++k) wb += wcount[k];
+        const int c = wb + __popc(m & ((1u << lane) - 1u));
+        const size_t n = a.plane;
+        DEM_ASSERT(c >= 0 && (size_t)c < n && s_prefix + tot_pad <= (int)n);
+        f4 v;
+        v.x = R[0]; v.y = R[1]; v.z = R[2]; v.w = R[3]; a.pose[c] = v;
+        v.x = R[4]; v.y = R[5]; v.z = R[6]; v.w = R[7]; a.pose[n + c] = v;
+        v.x = R[8]; v.y = t[0]; v.z = t[1]; v.w = t[2]; a.pose[2 * n + c] = v;
+        v.x = Mi[0]; v.y = Mi[1]; v.z = Mi[2]; v.w = Mi[3]; a.pose[3 * n + c] = v;
+        v.x = Mi[4]; v.y = Mi[5]; v.z = Mi[6]; v.w = Mi[7]; a.pose[4 * n + c] = v;
+        v.x = Mi[8]; v.y = (float)d[0]; v.z = (float)d[1]; v.w = (float)d[2]; a.pose[5 * n + c] = v;
+        a.pidx[c] = p;
+#pragma unroll
+        for (int w = 0; w < DEM_CM_WORDS; ++w)
+            if (w < a.mw_e + a.mw_vj + a.mw_vi) a.cmask[(size_t)w * n + c] = cm[w];
+    }
+}
+
 // ---- the kernel ---------------------------------------------------------------------------------------------------------
 // One warp = 32 consecutive (pair, slice) items of one pair class (same shapes, same loop bounds).  TE / TV = packed
 // outer pairs per sweep for edges / vertices (2 TE outer edges, 2 TV outer vertices share every inner-feature load).
@@ -1000,73 +1121,111 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
 #pragma unroll
             for (int k = 0; k < 3; ++k) tp[h][k] = R[k] * tq[h][0] + R[3 + k] * tq[h][1] + R[6 + k] * tq[h][2];
         }
-        // (1) edges of j whose distance from i's centre is below R_i + rc_search
-        for (int l0 = ob, le = min(oe, oE); l0 < le; l0 += 32) {
-            const int n = min(32, le - l0);
+        if (a.cmask) {
+            // the cull tests were done by k_pose_cull: one mask word per 32 outer features (slices == 1 on this path)
+            const unsigned* cm = a.cmask + cbase + lane;
+            for (int wd = 0; wd < a.mw_e; ++wd) {
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                unsigned mask = 0u;
-                for (int k = 0; k < n; ++k) {
-                    const f4 a0 = B.OE[2 * (l0 + k)], a1 = B.OE[2 * (l0 + k) + 1];
-                    const float qx = a0.x + tp[h][0], qy = a0.y + tp[h][1], qz = a0.z + tp[h][2];
-                    const float s = fminf(fmaxf(-(qx * a1.x + qy * a1.y + qz * a1.z), 0.f), a0.w);
-                    const float cx = qx + s * a1.x, cy = qy + s * a1.y, cz = qz + s * a1.z;
-                    mask |= (cx * cx + cy * cy + cz * cz < a.cull_a2 ? 1u : 0u) << k;
-                }
-                DEM_EMIT(PH_EE, valid[h] ? mask : 0u, lane + 32 * h, l0, 0u);
+                for (int h = 0; h < 2; ++h)
+                    DEM_EMIT(PH_EE, valid[h] ? __ldg(cm + (size_t)wd * plane + 32 * h) : 0u, lane + 32 * h, 32 * wd, 0u);
             }
-        }
-        sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
-        // (2) vertices of j near i: |R v + t| = |v + R^T t|;  (3) vertices of i near j: |R^T (v - t)| = |v - t|
-        const int o2 = max(ob, oE) - oE, n2 = min(oe, oV) - oE, o3 = max(ob, oV) - oV, n3 = min(oe, oV + A.nv) - oV;
-        if constexpr (SAME) {  // one shape: both sums sweep the same face table, so their survivors share the passes
-            for (int c0 = 0; c0 < A.nv; c0 += 32) {
+            sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
+            if constexpr (SAME) {
+                for (int wd = 0; wd < a.mw_vj; ++wd) {
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    unsigned m2 = 0u, m3 = 0u;
-                    for (int k = 0; k < 32; ++k) {
-                        const int o = c0 + k;
-                        if (o >= A.nv) break;
-                        const f4 v = A.V[o];
-                        const float qx = v.x + tp[h][0], qy = v.y + tp[h][1], qz = v.z + tp[h][2];
-                        const float rx = v.x - tq[h][0], ry = v.y - tq[h][1], rz = v.z - tq[h][2];
-                        m2 |= (o >= o2 && o < n2 && qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
-                        m3 |= (o >= o3 && o < n3 && rx * rx + ry * ry + rz * rz < a.cull_b2 ? 1u : 0u) << k;
+                    for (int h = 0; h < 2; ++h) {
+                        const unsigned m2 = valid[h] ? __ldg(cm + (size_t)(a.mw_e + wd) * plane + 32 * h) : 0u;
+                        const unsigned m3 = valid[h] ? __ldg(cm + (size_t)(a.mw_e + a.mw_vj + wd) * plane + 32 * h) : 0u;
+                        DEM_EMIT(PH_VF_BOTH, m2, lane + 32 * h, 32 * wd, 0u);
+                        DEM_EMIT(PH_VF_BOTH, m3, lane + 32 * h, 32 * wd, 0x8000u);
                     }
-                    DEM_EMIT(PH_VF_BOTH, valid[h] ? m2 : 0u, lane + 32 * h, c0, 0u);
-                    DEM_EMIT(PH_VF_BOTH, valid[h] ? m3 : 0u, lane + 32 * h, c0, 0x8000u);
                 }
+                sweep_items<PH_VF_BOTH>(w, cc, A, B, a.sa, a.sb, nrc2);
+            } else {
+                for (int wd = 0; wd < a.mw_vj; ++wd) {
+#pragma unroll
+                    for (int h = 0; h < 2; ++h)
+                        DEM_EMIT(PH_VF_OWN, valid[h] ? __ldg(cm + (size_t)(a.mw_e + wd) * plane + 32 * h) : 0u, lane + 32 * h,
+                                 32 * wd, 0u);
+                }
+                sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
+                for (int wd = 0; wd < a.mw_vi; ++wd) {
+#pragma unroll
+                    for (int h = 0; h < 2; ++h)
+                        DEM_EMIT(PH_VF_OTHER, valid[h] ? __ldg(cm + (size_t)(a.mw_e + a.mw_vj + wd) * plane + 32 * h) : 0u,
+                                 lane + 32 * h, 32 * wd, 0u);
+                }
+                sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
             }
-            sweep_items<PH_VF_BOTH>(w, cc, A, B, a.sa, a.sb, nrc2);
         } else {
-            for (int o0 = o2; o0 < n2; o0 += 32) {
-                const int n = min(32, n2 - o0);
-#pragma unroll
+            // (1) edges of j whose distance from i's centre is below R_i + rc_search
+            for (int l0 = ob, le = min(oe, oE); l0 < le; l0 += 32) {
+                const int n = min(32, le - l0);
+    #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     unsigned mask = 0u;
                     for (int k = 0; k < n; ++k) {
-                        const f4 v = B.V[o0 + k];
-                        const float qx = v.x + tp[h][0], qy = v.y + tp[h][1], qz = v.z + tp[h][2];
-                        mask |= (qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
+                        const f4 a0 = B.OE[2 * (l0 + k)], a1 = B.OE[2 * (l0 + k) + 1];
+                        const float qx = a0.x + tp[h][0], qy = a0.y + tp[h][1], qz = a0.z + tp[h][2];
+                        const float s = fminf(fmaxf(-(qx * a1.x + qy * a1.y + qz * a1.z), 0.f), a0.w);
+                        const float cx = qx + s * a1.x, cy = qy + s * a1.y, cz = qz + s * a1.z;
+                        mask |= (cx * cx + cy * cy + cz * cz < a.cull_a2 ? 1u : 0u) << k;
                     }
-                    DEM_EMIT(PH_VF_OWN, valid[h] ? mask : 0u, lane + 32 * h, o0, 0u);
+                    DEM_EMIT(PH_EE, valid[h] ? mask : 0u, lane + 32 * h, l0, 0u);
                 }
             }
-            sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
-            for (int o0 = o3; o0 < n3; o0 += 32) {
-                const int n = min(32, n3 - o0);
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    unsigned mask = 0u;
-                    for (int k = 0; k < n; ++k) {
-                        const f4 v = A.V[o0 + k];
-                        const float qx = v.x - tq[h][0], qy = v.y - tq[h][1], qz = v.z - tq[h][2];
-                        mask |= (qx * qx + qy * qy + qz * qz < a.cull_b2 ? 1u : 0u) << k;
+            sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
+            // (2) vertices of j near i: |R v + t| = |v + R^T t|;  (3) vertices of i near j: |R^T (v - t)| = |v - t|
+            const int o2 = max(ob, oE) - oE, n2 = min(oe, oV) - oE, o3 = max(ob, oV) - oV, n3 = min(oe, oV + A.nv) - oV;
+            if constexpr (SAME) {  // one shape: both sums sweep the same face table, so their survivors share the passes
+                for (int c0 = 0; c0 < A.nv; c0 += 32) {
+    #pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        unsigned m2 = 0u, m3 = 0u;
+                        for (int k = 0; k < 32; ++k) {
+                            const int o = c0 + k;
+                            if (o >= A.nv) break;
+                            const f4 v = A.V[o];
+                            const float qx = v.x + tp[h][0], qy = v.y + tp[h][1], qz = v.z + tp[h][2];
+                            const float rx = v.x - tq[h][0], ry = v.y - tq[h][1], rz = v.z - tq[h][2];
+                            m2 |= (o >= o2 && o < n2 && qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
+                            m3 |= (o >= o3 && o < n3 && rx * rx + ry * ry + rz * rz < a.cull_b2 ? 1u : 0u) << k;
+                        }
+                        DEM_EMIT(PH_VF_BOTH, valid[h] ? m2 : 0u, lane + 32 * h, c0, 0u);
+                        DEM_EMIT(PH_VF_BOTH, valid[h] ? m3 : 0u, lane + 32 * h, c0, 0x8000u);
                     }
-                    DEM_EMIT(PH_VF_OTHER, valid[h] ? mask : 0u, lane + 32 * h, o0, 0u);
                 }
+                sweep_items<PH_VF_BOTH>(w, cc, A, B, a.sa, a.sb, nrc2);
+            } else {
+                for (int o0 = o2; o0 < n2; o0 += 32) {
+                    const int n = min(32, n2 - o0);
+    #pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        unsigned mask = 0u;
+                        for (int k = 0; k < n; ++k) {
+                            const f4 v = B.V[o0 + k];
+                            const float qx = v.x + tp[h][0], qy = v.y + tp[h][1], qz = v.z + tp[h][2];
+                            mask |= (qx * qx + qy * qy + qz * qz < a.cull_a2 ? 1u : 0u) << k;
+                        }
+                        DEM_EMIT(PH_VF_OWN, valid[h] ? mask : 0u, lane + 32 * h, o0, 0u);
+                    }
+                }
+                sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
+                for (int o0 = o3; o0 < n3; o0 += 32) {
+                    const int n = min(32, n3 - o0);
+    #pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        unsigned mask = 0u;
+                        for (int k = 0; k < n; ++k) {
+                            const f4 v = A.V[o0 + k];
+                            const float qx = v.x - tq[h][0], qy = v.y - tq[h][1], qz = v.z - tq[h][2];
+                            mask |= (qx * qx + qy * qy + qz * qz < a.cull_b2 ? 1u : 0u) << k;
+                        }
+                        DEM_EMIT(PH_VF_OTHER, valid[h] ? mask : 0u, lane + 32 * h, o0, 0u);
+                    }
+                }
+                sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
             }
-            sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
         }
         if (w.qn > 0) {
             w.touched |= drain_terms(w.fs, w.q, w.sacc, w.scnt, w.qn, w.qn, w.sp, w.nown);

@@ -642,7 +642,7 @@ int dem_create(dem_ctx** out, int dim, double epsilon, int precision, void* cuda
 int dem_destroy(dem_ctx* c) {
     if (!c) return DEM_EINVAL;
     DevBuf* bufs[] = {&c->table, &c->cell_of, &c->rank, &c->cell_start, &c->order, &c->xs, &c->counts, &c->list, &c->slot,
-                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->rflag, &c->flags, &c->counters, &c->thermo, &c->pose, &c->pidx, &c->cum, &c->st_pos, &c->st_quat,
+                      &c->scratch_scan, &c->pcnt, &c->pairs, &c->rec, &c->rflag, &c->flags, &c->counters, &c->thermo, &c->pose, &c->pidx, &c->cmask, &c->cum, &c->st_pos, &c->st_quat,
                       &c->st_vel, &c->st_ang, &c->st_force, &c->st_torque, &c->st_virial, &c->st_pos2, &c->st_quat2, &c->sid_copy, &c->pos_build, &c->epart, &c->h_pos,
                       &c->h_quat, &c->h_vel, &c->h_ang, &c->h_sid, &c->h_force, &c->h_torque, &c->h_virial, &c->l2_scratch};
     for (DevBuf* b : bufs) b->release();

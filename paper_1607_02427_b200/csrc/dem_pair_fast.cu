@@ -17,6 +17,18 @@ void launch_pose(int dim, bool pos_is_double, int grid, cudaStream_t st, const P
     }
 }
 
+// a3 with the cull tests of the 3D search kernel (the library default path); smem = the staged shape tables
+void launch_pose_cull(bool pos_is_double, int grid, size_t smem, cudaStream_t st, const PoseArgs& pa) {
+    if (pos_is_double) {
+        if (smem > 48 * 1024) cudaFuncSetAttribute(k_pose_cull<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        k_pose_cull<double><<<grid, DEM_POSE_THREADS, smem, st>>>(pa);
+    } else {
+        if (smem > 48 * 1024) cudaFuncSetAttribute(k_pose_cull<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        k_pose_cull<float><<<grid, DEM_POSE_THREADS, smem, st>>>(pa);
+    }
+}
+int pose_cull_max_words() { return DEM_CM_WORDS; }
+
 // tv3: 3 packed outer vertex pairs per sweep (tiles of 6 vertices) instead of 2 (tiles of 4)
 cudaError_t launch_pair_fast(int dim, bool tv3, int grid, int threads, size_t smem, cudaStream_t st,
                              const PairArgs<float>& a) {

@@ -97,6 +97,8 @@ template <typename real> struct PairArgs {
     const int* pidx;      //   (written by k_pose)
     const int* count;
     size_t plane;         //   stride of the pose planes
+    const unsigned* cmask;  // culling kernel: per-pair survivor masks written by k_pose_cull, [words][plane] (null: the
+    int mw_e, mw_vj, mw_vi; //   kernel runs the cull tests itself); words for edges of j, vertices of j, vertices of i
     unsigned long long* counters;  // [0] pairs evaluated, [1] active, [2] degenerate, [3] parallel, [4..6] swept terms
     unsigned long long* cum;       // running totals of [4..6] while bench's timing is on (else null)
 };
@@ -116,6 +118,12 @@ struct PoseArgs {
     int pad;       // entries per warp tile of the kernel that follows: 32 (k_pair_fast) or 64 (k_pair_cull)
     unsigned long long* counters;  // [0] += pairs inside the reach
     unsigned char* rflag;  // result-record flags of the class: pairs beyond the reach get 0 here (no record is written)
+    // k_pose_cull only: the class's shapes and cull radii; survivor masks out ([mw_e + mw_vj + mw_vi][plane])
+    const f4* table;
+    ShapeDev sa, sb;
+    float cull_a2, cull_b2;
+    unsigned* cmask;
+    int mw_e, mw_vj, mw_vi;
     const int* skip;  // dem_step: non-null and *skip != 0 => the list is stale, the kernel does nothing (see step_t)
 };
 
