@@ -370,7 +370,8 @@ def main():
                     "note": "the Eq. 2 terms swept after exact per-vertex culling cost %.2f Gflop per launch: not the bound" % (
                         swept_flops(tot) / evals / 1e9)}
     else:
-        evals = max(n_pair_launches // max(n_classes, 1), 1)          # force evaluations timed
+        # force evaluations timed (several classes: one fork-to-join span per evaluation, pose kernels included)
+        evals = max(n_pair_launches if n_classes > 1 else n_pair_launches, 1)
         kern_ms_per_eval = pair_ms / evals
         # per evaluation: summed over the timed evaluations by the search kernels themselves; the generic kernel sweeps
         # every term of every listed pair in reach (nominal count)
@@ -399,7 +400,7 @@ def main():
         if st["dim"] == 3 and us.get("pose"):
             # k_pose: pair list (8 B), positions and orientations of N particles in double (64 B each, gathered), pose
             # records of the pairs inside the reach (96 B + 4 B index), one flag byte per pair
-            out["k_pose"] = hbm_line(us["pose"] * max(n_classes, 1), npairs_listed * 9 + n * 64 + npairs_eval * 100)
+            out["k_pose"] = hbm_line(us["pose"], npairs_listed * 9 + n * 64 + npairs_eval * 100)
         if us.get("reduce"):
             # k_finish: slots (4 B per listed neighbour), flags (1 B per listed neighbour), x q v L read + written, build positions
             out["k_finish"] = hbm_line(us["reduce"], nsum * 5 + n * (8 * 32 + 32 + 4))
@@ -422,7 +423,7 @@ def main():
     if searched and not args.cull and not particle2d:
         dem.set_culling(True)
         cms, _, _, ckt, ctot = timed(3, args.steps, False)
-        cev = max(ckt["pair"][0] // max(n_classes, 1), 1)
+        cev = max(ckt["pair"][0], 1)
         ckern = ckt["pair"][1] / cev
         ctf = swept_flops(ctot) / cev / (ckern * 1e-3) / 1e12
         culled = {"value": n * world * args.steps / (cms * 1e-3), "unit": "particle-timesteps/s",
@@ -448,7 +449,7 @@ def main():
             if cull is not None:
                 dem.set_culling(cull)
             tms, _, _, tkt, ttot = timed(3, min(args.steps, 100), False)
-            tev = max(tkt["pair"][0] // max(n_classes, 1), 1) if not particle2d else max(tkt["pair"][0], 1)
+            tev = max(tkt["pair"][0], 1)
             arms[name] = {"value": n * world * min(args.steps, 100) / (tms * 1e-3), "ms_per_step": tms / min(args.steps, 100),
                           "kernel_ms": tkt["pair"][1] / tev, "pose_kernel_ms": tkt["pose"][1] / tev}
             if st["dim"] == 3 and searched:

@@ -20,7 +20,9 @@ int dem_set_l2_flush(dem_ctx* ctx, int64_t bytes);
  * 1 = the pose kernel and the pair-feature kernel of every evaluation; 2 = also the reduction, the integrator kernel,
  * the L2 flush and the neighbour build (k_neigh alone, and the whole build).  dem_kernel_times returns, per kernel
  * kind, the number of bracketed launches and their summed duration in milliseconds since the last call, and resets
- * them (synchronises). */
+ * them (synchronises).  A system with several pair classes (several shapes) runs its classes' pose and pair kernels on
+ * side streams at the same time: it then reports ONE DEM_KT_PAIR span per evaluation, from the fork to the join (all pose
+ * and pair kernels of the evaluation), and no DEM_KT_POSE spans. */
 enum { DEM_KT_POSE = 0, DEM_KT_PAIR = 1, DEM_KT_REDUCE = 2, DEM_KT_KICK_DRIFT = 3, DEM_KT_NEIGH = 4, DEM_KT_BUILD = 5,
        DEM_KT_FLUSH = 6, DEM_KT_OTHER = 7, DEM_KT_COUNT = 8 };
 int dem_set_timing(dem_ctx* ctx, int level);

@@ -104,6 +104,10 @@ struct dem_ctx {
     cudaStream_t copy_stream = nullptr;  // dem_step_host: second H2D stream (velocities, angular momenta)
     cudaEvent_t ev_copy = nullptr;
     bool ev_copy_pending = false;
+    // pair classes beyond the first run their pose + pair kernels on side streams, so that the tails of the per-class
+    // launches overlap (mixed-shape systems: config 5 has three classes); forked from and joined to `stream` with events
+    cudaStream_t class_stream[3] = {nullptr, nullptr, nullptr};
+    cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
     double nvt_dof = 0;            // degrees of freedom counted by the last dem_step_nvt
     int steps_since_build = 0;     // age of the list when the last dem_step returned (carried into a resumed call)
     int rebuild_interval = 8;      // steps between the last two neighbour rebuilds of dem_step (sizes its chunks)
@@ -140,7 +144,7 @@ inline int nblk(long long n, int b) { return (int)((n + b - 1) / b); }
 // kernel kinds of the time accounting (dem_kernel_times of include/dem_bench.h)
 enum { KT_POSE = 0, KT_PAIR = 1, KT_REDUCE = 2, KT_KICK_DRIFT = 3, KT_NEIGH = 4, KT_BUILD = 5, KT_FLUSH = 6, KT_OTHER = 7, KT_COUNT = 8 };
 // record an event on the context's stream (null when timing is below `level` or an event cannot be created)
-inline cudaEvent_t ev_mark(dem_ctx* c, int level = 1) {
+inline cudaEvent_t ev_mark(dem_ctx* c, int level = 1, cudaStream_t on = nullptr, bool on_given = false) {
     if (c->timing < level) return nullptr;
     if (c->ev_used == c->ev_pool.size()) {
         cudaEvent_t e;
@@ -148,7 +152,7 @@ inline cudaEvent_t ev_mark(dem_ctx* c, int level = 1) {
         c->ev_pool.push_back(e);
     }
     cudaEvent_t e = c->ev_pool[c->ev_used++];
-    cudaEventRecord(e, c->stream);
+    cudaEventRecord(e, on_given ? on : c->stream);
     return e;
 }
 inline void ev_span(dem_ctx* c, int kind, cudaEvent_t a, cudaEvent_t b) {

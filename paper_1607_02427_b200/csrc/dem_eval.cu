@@ -17,10 +17,9 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
     if (!ctx->have_list) return fail(ctx, DEM_ESTALE, "no neighbour list: call dem_build_neighbors first");
     if (N != ctx->N) return fail(ctx, DEM_ESTALE, "N = %d differs from the last build (%d)", N, ctx->N);
     if (!pos || !quat || !sid || !force || !torque) return fail(ctx, DEM_EINVAL, "null particle array");
-    cudaStream_t st = ctx->stream;
     const int* skip = fin ? fin->bail : nullptr;
     // counters[0..7] (unsigned long long) followed by the per-class lengths of the k_pose work lists (int): one memset
-    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES, st));
+    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES, ctx->stream));
     int* ccount = reinterpret_cast<int*>(ctx->counters.as<unsigned long long>() + 8);
     // capacity of a class's work list: its pairs plus the padding of every k_pose block to a whole warp tile
     const int pose_block = pose_threads();
@@ -36,9 +35,34 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
         if (cull) CU(ctx->cmask.reserve(sizeof(unsigned) * pose_cull_max_words() * std::max<size_t>(list_base[ctx->nclass], 1)));
     }
     const BoxDev bx = box_dev(ctx->dim, ctx->box);
+    // classes beyond the first populated one go to side streams (their kernels write disjoint records)
+    int populated = 0, side_used = 0;
+    for (int c = 0; c < ctx->nclass; ++c) populated += ctx->class_np[c] > 0;
+    if (populated > 1) {
+        if (!ctx->ev_fork) {
+            CU(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
+            for (int k = 0; k < 3; ++k) {
+                CU(cudaStreamCreateWithFlags(&ctx->class_stream[k], cudaStreamNonBlocking));
+                CU(cudaEventCreateWithFlags(&ctx->ev_join[k], cudaEventDisableTiming));
+            }
+        }
+        CU(cudaEventRecord(ctx->ev_fork, ctx->stream));
+    }
+    // with several classes in flight at once the kernels' own durations overlap: one span from fork to join is timed
+    // instead (pose + pair kernels of all classes; include/dem_bench.h)
+    cudaEvent_t span0 = populated > 1 ? ev_mark(ctx) : nullptr;
+    int seen = 0;
     for (int c = 0; c < ctx->nclass; ++c) {
         const int np = ctx->class_np[c];
         if (np == 0) continue;
+        cudaStream_t st = ctx->stream;
+        const int side = seen == 0 ? -1 : (seen - 1) % 3;
+        if (side >= 0) {
+            st = ctx->class_stream[side];
+            if (side_used < 3 && seen - 1 < 3) CU(cudaStreamWaitEvent(st, ctx->ev_fork, 0));
+            side_used = std::max(side_used, side + 1);
+        }
+        ++seen;
         const HostShape &HA = ctx->shapes[ctx->class_sa[c]], &HB = ctx->shapes[ctx->class_sb[c]];
         PairArgs<real> a;
         memset(&a, 0, sizeof a);
@@ -74,7 +98,7 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
         const long long items = (long long)((np + 31) & ~31) * a.slices;
         const int threads = 128;
         int grid = (int)std::min<long long>(nblk(items, threads), (long long)ctx->sm_count * 64);
-        cudaEvent_t e0 = ev_mark(ctx), em = e0;
+        cudaEvent_t e0 = populated > 1 ? nullptr : ev_mark(ctx, 1, st, true), em = e0;
         if constexpr (std::is_same<real, float>::value) {
             if (search) {
                 // a3 (relative poses, reach test, compaction) runs as its own kernel in front of the search kernel
@@ -111,7 +135,7 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
                     launch_pose(ctx->dim, pos_is_double, nblk(np, pose_block), st, pa);
                 }
                 LAUNCHED(ctx);
-                em = ev_mark(ctx);
+                if (populated == 1) em = ev_mark(ctx, 1, st, true);
                 // the padded work list bounds the tiles; grid cap in blocks per SM measured on cfg4 (one tile per warp
                 // beats one persistent wave)
                 const long long list_items = (long long)list_cap(c) * a.slices / (cull ? 2 : 1);
@@ -135,10 +159,16 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
             CU(launch_pair_generic_f64(ctx->dim, grid, threads, smem, st, a));
         }
         LAUNCHED(ctx);
-        cudaEvent_t e1 = ev_mark(ctx);
+        cudaEvent_t e1 = populated > 1 ? nullptr : ev_mark(ctx, 1, st, true);
         if (em != e0) ev_span(ctx, KT_POSE, e0, em);
         ev_span(ctx, KT_PAIR, em, e1);
     }
+    for (int k = 0; k < side_used; ++k) {  // join the side streams
+        CU(cudaEventRecord(ctx->ev_join[k], ctx->class_stream[k]));
+        CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_join[k], 0));
+    }
+    if (populated > 1) ev_span(ctx, KT_PAIR, span0, ev_mark(ctx));
+    cudaStream_t st = ctx->stream;
     cudaEvent_t r0 = ev_mark(ctx, 2);
     {
         FinArgs fa;

@@ -649,6 +649,11 @@ int dem_destroy(dem_ctx* c) {
     if (c->h_moved) cudaFreeHost(c->h_moved);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->ev_copy) cudaEventDestroy(c->ev_copy);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    for (int k = 0; k < 3; ++k) {
+        if (c->class_stream[k]) cudaStreamDestroy(c->class_stream[k]);
+        if (c->ev_join[k]) cudaEventDestroy(c->ev_join[k]);
+    }
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return DEM_OK;

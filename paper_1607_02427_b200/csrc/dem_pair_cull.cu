@@ -8,8 +8,12 @@ size_t pair_cull_smem_header() { return cull_smem_header(); }
 
 cudaError_t launch_pair_cull(bool same_shape, int grid, int threads, size_t smem, cudaStream_t st,
                              const PairArgs<float>& a) {
-    // measured on cfg4: 167 registers without spills beat 128 / 96 / 80 with
-    void (*kern)(const PairArgs<float>) = same_shape ? k_pair_cull<3, true> : k_pair_cull<3, false>;
+    // Blocks per SM, measured with the cull tests in k_pose_cull: small shapes (octahedra, cfg4) run best at 4 (128
+    // registers, some spills: 58.6 us from the lattice, 128.8 us thermalised) against 3 (168 registers, none: 63.1 / 148.0)
+    // and 5 (96: 67.9 / 155.6); large tables (truncated icosahedra, cfg5) at 3 (51.0 against 55.0 us per class launch)
+    const bool small = a.sa.len + a.sb.len <= 512;
+    void (*kern)(const PairArgs<float>) =
+        small ? (same_shape ? k_pair_cull<4, true> : k_pair_cull<4, false>) : (same_shape ? k_pair_cull<3, true> : k_pair_cull<3, false>);
     if (smem > 48 * 1024) {
         const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
