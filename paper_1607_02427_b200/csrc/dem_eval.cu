@@ -174,7 +174,12 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
         FinArgs fa;
         if (fin) fa = *fin;
         else memset(&fa, 0, sizeof fa);
-        const int grid = nblk(N, 256);
+        // lanes per particle: one for large systems, several where there are too few particles to hide the latency of a
+        // serial walk over a particle's slots (N = 256: 32 lanes)
+        int lanes = 1;
+        while (lanes < 32 && (long long)N * lanes < 65536) lanes <<= 1;
+        fa.lanes = lanes;
+        const int grid = nblk((long long)N * lanes, 256);
         const int* counts = ctx->counts.as<int>();
         const int* slot = ctx->slot.as<int>();
         const real4* rec = ctx->rec.as<real4>();

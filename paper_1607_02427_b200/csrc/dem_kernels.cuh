@@ -141,31 +141,34 @@ __global__ void __launch_bounds__(256) k_finish(int N, const int* __restrict__ c
                                                 typename vec4<real>::type* __restrict__ torque, real* __restrict__ virial,
                                                 FinArgs fa) {
     typedef typename vec4<real>::type real4;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    // fa.lanes lanes share a particle (1 for large systems; small ones are bound by the latency of the serial walk over
+    // a particle's slots, so several lanes split it and combine with shuffles: still a fixed order for a given N)
+    const int lpp = fa.lanes, gid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = gid / lpp, sub = gid - i * lpp;
     if (MODE != 0) {
         if (fa.bail && *fa.bail) {               // the list went stale before this step: change nothing, and pass
-            if (i == 0 && fa.raise) *fa.raise = 1;  // the word on (the next evaluation looks at the other flag)
+            if (gid == 0 && fa.raise) *fa.raise = 1;  // the word on (the next evaluation looks at the other flag)
             return;
         }
-        if (i == 0 && fa.done) *fa.done += 1;    // nothing in this kernel reads it
+        if (gid == 0 && fa.done) *fa.done += 1;  // nothing in this kernel reads it
     }
-    if (i >= N) return;
+    const bool live = i < N, lead = live && sub == 0;
     // state loads first: they do not depend on the reduction
     d4 v, L, x, q, xb;
     int sh = 0;
-    if (MODE >= 1) {
+    if (MODE >= 1 && lead) {
         v = fa.vel[i];
         L = fa.ang[i];
         sh = sid[i];
     }
-    if (MODE == 2) {
+    if (MODE == 2 && lead) {
         x = fa.pos[i];
         q = fa.quat[i];
         xb = fa.pos_build[i];
     }
     real F[3] = {0, 0, 0}, T[3] = {0, 0, 0}, U = 0, W[6] = {0, 0, 0, 0, 0, 0};
-    const int n = counts[i];
-    for (int k0 = 0; k0 < n; k0 += 4) {
+    const int n = live ? counts[i] : 0;
+    for (int k0 = 4 * sub; k0 < n; k0 += 4 * lpp) {
         int sl[4];
         size_t ri[4];
         int S[4];
@@ -216,6 +219,19 @@ __global__ void __launch_bounds__(256) k_finish(int N, const int* __restrict__ c
             }
         }
     }
+    for (int o = 1; o < lpp; o <<= 1) {  // combine the lanes of a particle (lpp divides 32: no particle straddles a warp)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            F[a] += __shfl_xor_sync(0xffffffffu, F[a], o);
+            T[a] += __shfl_xor_sync(0xffffffffu, T[a], o);
+        }
+        U += __shfl_xor_sync(0xffffffffu, U, o);
+        if (virial) {
+#pragma unroll
+            for (int a = 0; a < 6; ++a) W[a] += __shfl_xor_sync(0xffffffffu, W[a], o);
+        }
+    }
+    if (!lead) return;
     if (MODE != 2) {
         real4 f, t;
         f.x = F[0]; f.y = F[1]; f.z = F[2]; f.w = U;

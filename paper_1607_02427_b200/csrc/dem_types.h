@@ -137,6 +137,7 @@ struct PoseArgs {
 // and raises *raise when its own drift takes a particle out of its skin.
 struct FinArgs {
     int mode, dim;
+    int lanes;  // lanes per particle in k_finish's reduction (power of two <= 32; small systems use several: latency)
     double dt;
     d4 *pos, *quat, *vel, *ang;
     const d4* pos_build;  // positions at the last neighbour build (skin test)
