@@ -37,8 +37,10 @@ def gpu_compute(st, precision, slices=0, r_cut=None, virial=True, kernel=None, c
     return out
 
 
-def assert_parity(st, precision, oracle, slices=0, subset=None, r_cut=None, tol=None, kernel=None, cull=None):
-    """Element-by-element comparison of force, torque, energy, virial and of the term counters."""
+def assert_parity(st, precision, oracle, slices=0, subset=None, r_cut=None, tol=None, kernel=None, cull=None, wlever=None):
+    """Element-by-element comparison of force, torque, energy, virial and of the term counters.  wlever: a length; the
+    virial W = -1/2 d x F is then compared relative to at least wlever x (force scale) -- for states whose centre
+    separations |d| are much longer than the contact gaps, where |d| times the force tolerance exceeds max |W|."""
     st = round_state(st, precision)
     f, tq, w, cnt = gpu_compute(st, precision, slices, r_cut, kernel=kernel, cull=cull)
     of, ot, ow, ocnt = oracle.compute(st, subset=subset)
@@ -49,7 +51,7 @@ def assert_parity(st, precision, oracle, slices=0, subset=None, r_cut=None, tol=
     ef = np.abs(f[:, :3] - of[:, :3]).max() / fs
     et = np.abs(tq[:, :3] - ot[:, :3]).max() / ts
     eu = np.abs(f[:, 3] - of[:, 3]).max() / us
-    ws = max(np.abs(ow).max(), 1.0)
+    ws = max(np.abs(ow).max(), 1.0, (wlever or 0.0) * fs)
     ew = np.abs(w - ow).max() / ws
     assert ef < tol, "force error %.3e (scale %.3g)" % (ef, fs)
     assert et < tol, "torque error %.3e (scale %.3g)" % (et, ts)

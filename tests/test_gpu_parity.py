@@ -346,3 +346,48 @@ def test_host_buffer_entry_point_matches_device_path(pkg):
     assert np.array_equal(fo.numpy().astype(np.float64), f) and np.array_equal(to.numpy().astype(np.float64), tq)
     assert np.array_equal(wo.numpy().astype(np.float64), w)
     dem.close()
+
+
+@pytest.mark.parametrize("length", [5.0, 20.0, 100.0])
+def test_long_thin_near_parallel_edges(pkg, oracle, length):
+    """The packed FP32 search only has to FLAG every term the exact routine would accept; its line-line solve loses its
+    digits on near-parallel edges and the candidate cutoff carries a slack for that (4e-3 x longest edge, DESIGN.md
+    section 5).  Rods 50, 200 and 1000 sigma long (one edge each), in pairs at angles 1e-5 ... 1e-2 and gaps around
+    sigma, overlapping fully, partly and end to end: the search kernel (culling on and off) must find exactly the active,
+    degenerate and parallel-branch terms of the generic FP32 kernel, and both must match the oracle."""
+    sig = 0.1
+    shapes = [di.rod(length, sig / 2)]
+    reach = di.default_rcut(shapes)
+    rng = np.random.default_rng(int(length))
+    angles = [0.0, 1e-5, 1e-4, 5e-4, 9e-4, 1.1e-3, 3e-3, 1e-2]
+    m = 4 * len(angles)
+    spacing = 3.0 * reach
+    side = int(math.ceil(m ** (1.0 / 3.0)))
+    n = 2 * m
+    pos, quat = np.zeros((n, 4)), np.zeros((n, 4))
+    for k in range(m):
+        ang = angles[k % len(angles)]
+        cell = np.array([k % side, (k // side) % side, k // (side * side)], dtype=np.float64)
+        c = (cell - side / 2 + 0.5) * spacing
+        gap = sig * rng.uniform(0.85, 1.1)
+        shift = (0.0, 0.3, 0.9, 0.999)[k // len(angles)] * length      # overlap: full, most, a tenth, end to end
+        g = rng.standard_normal(3)
+        g[2] = 0.0
+        g /= np.linalg.norm(g)                                          # gap direction, perpendicular to the rods (z)
+        pos[2 * k, :3] = c
+        pos[2 * k + 1, :3] = c + gap * g + [0, 0, shift]
+        quat[2 * k] = [1, 0, 0, 0]
+        quat[2 * k + 1] = [math.cos(ang / 2), *(math.sin(ang / 2) * g)]  # tilt ABOUT the gap direction: the lines stay `gap` apart
+    st = dict(dim=3, shapes=shapes, box=np.array([side * spacing] * 3), pos=pos, quat=quat, vel=np.zeros((n, 4)),
+              angmom=np.zeros((n, 4)), shape_id=np.zeros(n, dtype=np.int32), N=n, r_cut=reach, epsilon=1.0)
+    # FP32 holds the end points of an edge of length L to ulp(L): r* is then good to ~2^-23 L / sigma relative and the
+    # force to 13 times that (F ~ r^-13), whichever kernel runs: the north_star tolerance is meant for the paper's
+    # shapes (edge / sigma <= 8.5); here it is widened to that bound.  The point of this test is the candidate SET.
+    tol = max(TOL["f32"], 4 * 13 * 2.0 ** -23 * length / sig)
+    ref = assert_parity(st, "f32", oracle, kernel=1, tol=tol, wlever=0.5 * length)
+    assert ref["counters"]["active"] >= m // 2 and ref["counters"]["parallel"] > 0
+    for cull in (False, True):
+        r = assert_parity(st, "f32", oracle, kernel=0, cull=cull, tol=tol, wlever=0.5 * length)
+        for key in ("active", "degenerate", "parallel", "pairs_evaluated"):
+            assert r["counters"][key] == ref["counters"][key], (key, cull)
+    assert_parity(st, "f64", oracle)
