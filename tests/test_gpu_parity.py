@@ -307,6 +307,17 @@ def test_error_codes(pkg):
     assert e.value.code == -7
     with pytest.raises(TypeError):
         dem.compute(t["pos"].cpu(), t["quat"], t["shape_id"])  # no CPU path
+    # a shape id outside the registered shapes is caught on the device during the build, not used as an index
+    bad = t["shape_id"].clone()
+    bad[7] = 5
+    with pytest.raises(pkg.DemError) as e:
+        dem.build_neighbors(t["pos"], bad, st["box"], st["r_cut"])
+    assert e.value.code == -1  # DEM_EINVAL
+    bad[7] = -1
+    with pytest.raises(pkg.DemError) as e:
+        dem.build_neighbors(t["pos"], bad, st["box"], st["r_cut"])
+    assert e.value.code == -1
+    dem.build_neighbors(t["pos"], t["shape_id"], st["box"], st["r_cut"])
     # a list built with a larger cutoff (skin) gives identical forces: the extra pairs contribute exactly zero
     f0, t0, _ = dem.compute(t["pos"], t["quat"], t["shape_id"])
     dem.build_neighbors(t["pos"], t["shape_id"], st["box"], 1.4 * st["r_cut"])
