@@ -230,6 +230,25 @@ __global__ void __launch_bounds__(DEM_P2D_THREADS, 5) k_particle2d(const Particl
                     surv |= (unsigned long long)(x * x + y * y < c2) << o;
                 }
                 c_swept += (unsigned)(__popcll(surv) * In.ne);
+                // With culling one or two vertices survive per side: a packed pair of them would mostly carry a
+                // duplicate, so the survivors are swept one at a time with scalar arithmetic (without culling the packed
+                // sweep below takes them two at a time)
+                if (a.cull) {
+                    while (surv) {
+                        const int o0 = __ffsll((long long)surv) - 1;
+                        surv &= surv - 1ull;
+                        const f4 va = Out.V[o0];
+                        float pa[3];
+                        if (side == 0) vertex_to_i<float>(va.x, va.y, 0.f, R, t, pa);
+                        else vertex_to_j<float>(va.x, va.y, 0.f, R, t, pa);
+                        for (int kk = 0; kk < In.ne; ++kk) {
+                            const f4 e0 = In.E[2 * kk], e1 = In.E[2 * kk + 1];
+                            const float sd = e0.z * pa[1] - e0.w * pa[0] + e1.y, am = e0.z * pa[0] + e0.w * pa[1] + e1.z;
+                            const float ex = fmaxf(fabsf(am) - e1.w, 0.f);
+                            if (sd * sd + ex * ex + nrc2 < 0.f) note(side, o0, kk);
+                        }
+                    }
+                }
                 while (surv) {  // two surviving vertices per packed sweep
                     const int o0 = __ffsll((long long)surv) - 1;
                     surv &= surv - 1ull;
