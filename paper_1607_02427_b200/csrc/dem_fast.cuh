@@ -1034,7 +1034,9 @@ __device__ __forceinline__ void write_items(CullCtx& cc, unsigned mask, int owne
         write_items(cc, m_, (OWNER), (O0), (FLAG), off_, tot_);                           \
     } while (0)
 
-template <int MINB, bool SAME>  // SAME: both particles of the class have the same shape
+// SAME: both particles of the class have the same shape.  ONESITE: one sweep site per phase (small code, for large shape
+// tables) instead of one behind every emit site (the two owner slots' emits interleave: faster for small shapes).
+template <int MINB, bool SAME, bool ONESITE>
 __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a) {
     // a warp tile is 64 pairs (two per lane: owner slots lane and lane + 32), so that the item passes run fuller
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -1121,6 +1123,100 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
 #pragma unroll
             for (int k = 0; k < 3; ++k) tp[h][k] = R[k] * tq[h][0] + R[3 + k] * tq[h][1] + R[6 + k] * tq[h][2];
         }
+        if constexpr (ONESITE) {
+            // Large shape tables (truncated icosahedra: 7 mask words per pair, faces of two sizes).  Every phase is ONE loop
+            // over its (mask word, owner slot) units with ONE sweep site -- the item list is swept when the next batch
+            // would overflow it and once when the phase ends.  The sweeps are big unrolled bodies; with a copy behind every
+            // emit site the kernel has 28 k instructions, and a third of its stall samples are instruction fetches.
+            // Survivor masks come from k_pose_cull (a.cmask) or are tested here (sliced pairs, masks that do not fit).
+            const bool pre = a.cmask != nullptr;
+            const unsigned* cm = a.cmask + (pre ? cbase + lane : 0);
+            auto edge_word = [&](int l0, int n, float px_, float py_, float pz_) -> unsigned {
+                unsigned m = 0u;
+                for (int k = 0; k < n; ++k) {
+                    const f4 a0 = B.OE[2 * (l0 + k)], a1 = B.OE[2 * (l0 + k) + 1];
+                    const float qx = a0.x + px_, qy = a0.y + py_, qz = a0.z + pz_;
+                    const float s = fminf(fmaxf(-(qx * a1.x + qy * a1.y + qz * a1.z), 0.f), a0.w);
+                    const float cx = qx + s * a1.x, cy = qy + s * a1.y, cz = qz + s * a1.z;
+                    m |= (cx * cx + cy * cy + cz * cz < a.cull_a2 ? 1u : 0u) << k;
+                }
+                return m;
+            };
+            auto vert_word = [&](const f4* V, int o0, int n, float sx, float sy, float sz, float lim2) -> unsigned {
+                unsigned m = 0u;  // |v + s|^2 < lim2
+                for (int k = 0; k < n; ++k) {
+                    const f4 v = V[o0 + k];
+                    const float qx = v.x + sx, qy = v.y + sy, qz = v.z + sz;
+                    m |= (qx * qx + qy * qy + qz * qz < lim2 ? 1u : 0u) << k;
+                }
+                return m;
+            };
+            const int e_lo = pre ? 0 : ob, e_hi = pre ? B.ne : min(oe, oE);
+            const int vj_lo = pre ? 0 : max(ob, oE) - oE, vj_hi = pre ? B.nv : min(oe, oV) - oE;
+            const int vi_lo = pre ? 0 : max(ob, oV) - oV, vi_hi = pre ? A.nv : min(oe, oV + A.nv) - oV;
+            const int nw_e = (max(e_hi - e_lo, 0) + 31) >> 5, nw_vj = (max(vj_hi - vj_lo, 0) + 31) >> 5,
+                      nw_vi = (max(vi_hi - vi_lo, 0) + 31) >> 5;
+            // phase 0: edges of j; then the two vertex-face sums, sharing their passes in one-shape classes
+            for (int u = 0; u <= 2 * nw_e; ++u) {
+                const bool last = u == 2 * nw_e;
+                const int h = u & 1, wd = u >> 1, l0 = e_lo + 32 * wd;
+                unsigned m = 0u;
+                if (!last && (h ? valid[1] : valid[0]))
+                    m = pre ? __ldg(cm + (size_t)wd * plane + 32 * h)
+                            : edge_word(l0, min(32, e_hi - l0), h ? tp[1][0] : tp[0][0], h ? tp[1][1] : tp[0][1], h ? tp[1][2] : tp[0][2]);
+                int off_;
+                const int tot_ = count_items(w, m, off_);
+                if (last || cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
+                if (!last) write_items(cc, m, lane + 32 * h, l0, 0u, off_, tot_);
+            }
+            auto vf_mask = [&](bool other, int wd, int h) -> unsigned {
+                if (!(h ? valid[1] : valid[0])) return 0u;
+                if (!other) {
+                    if (wd >= nw_vj) return 0u;
+                    const int o0 = vj_lo + 32 * wd;
+                    return pre ? __ldg(cm + (size_t)(a.mw_e + wd) * plane + 32 * h)
+                               : vert_word(B.V, o0, min(32, vj_hi - o0), h ? tp[1][0] : tp[0][0], h ? tp[1][1] : tp[0][1],
+                                           h ? tp[1][2] : tp[0][2], a.cull_a2);
+                }
+                if (wd >= nw_vi) return 0u;
+                const int o0 = vi_lo + 32 * wd;
+                return pre ? __ldg(cm + (size_t)(a.mw_e + a.mw_vj + wd) * plane + 32 * h)
+                           : vert_word(A.V, o0, min(32, vi_hi - o0), -(h ? tq[1][0] : tq[0][0]), -(h ? tq[1][1] : tq[0][1]),
+                                       -(h ? tq[1][2] : tq[0][2]), a.cull_b2);
+            };
+            if constexpr (SAME) {
+                const int nw = max(nw_vj, nw_vi);
+                for (int u = 0; u <= 4 * nw; ++u) {
+                    const bool last = u == 4 * nw;
+                    const int h = u & 1, wd = u >> 2;
+                    const bool other = (u >> 1) & 1;
+                    const unsigned m = last ? 0u : vf_mask(other, wd, h);
+                    int off_;
+                    const int tot_ = count_items(w, m, off_);
+                    if (last || cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH_VF_BOTH>(w, cc, A, B, a.sa, a.sb, nrc2);
+                    if (!last) write_items(cc, m, lane + 32 * h, (other ? vi_lo : vj_lo) + 32 * wd, other ? 0x8000u : 0u, off_, tot_);
+                }
+            } else {
+                for (int u = 0; u <= 2 * nw_vj; ++u) {
+                    const bool last = u == 2 * nw_vj;
+                    const int h = u & 1, wd = u >> 1;
+                    const unsigned m = last ? 0u : vf_mask(false, wd, h);
+                    int off_;
+                    const int tot_ = count_items(w, m, off_);
+                    if (last || cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
+                    if (!last) write_items(cc, m, lane + 32 * h, vj_lo + 32 * wd, 0u, off_, tot_);
+                }
+                for (int u = 0; u <= 2 * nw_vi; ++u) {
+                    const bool last = u == 2 * nw_vi;
+                    const int h = u & 1, wd = u >> 1;
+                    const unsigned m = last ? 0u : vf_mask(true, wd, h);
+                    int off_;
+                    const int tot_ = count_items(w, m, off_);
+                    if (last || cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
+                    if (!last) write_items(cc, m, lane + 32 * h, vi_lo + 32 * wd, 0u, off_, tot_);
+                }
+            }
+        } else
         if (a.cmask) {
             // the cull tests were done by k_pose_cull: one mask word per 32 outer features (slices == 1 on this path)
             const unsigned* cm = a.cmask + cbase + lane;
