@@ -60,6 +60,7 @@ struct dem_ctx {
     MassTable mt;
     // neighbour list state
     bool have_list = false;
+    bool list_from_step = false;  // the list was built by dem_step (cutoff = reach + skin, pos_build and sid_copy valid)
     int N = 0, stride = 16, max_count = 0;
     double box[3] = {0, 0, 0}, r_cut = 0;
     GridDev grid;

@@ -323,6 +323,21 @@ static __global__ void k_same_state(int n, const f4* __restrict__ pos, const f4*
     if (!same) *differ = 1;
 }
 
+// Is the neighbour list of an earlier dem_step call still good for these positions and shape ids?  Raises *stale when a
+// particle is farther than skin/2 from where it was at the build (the criterion of the step loop) or a shape id changed.
+static __global__ void k_list_valid(int n, BoxDev box, const d4* __restrict__ pos, const d4* __restrict__ pos_build,
+                                    const int* __restrict__ sid, const int* __restrict__ sid_build, double half_skin2,
+                                    int* __restrict__ stale) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const d4 x = pos[i], xb = pos_build[i];
+    double dx = x.x - xb.x, dy = x.y - xb.y, dz = box.dim == 3 ? x.z - xb.z : 0.0;
+    dx -= box.L[0] * rint(dx * box.invL[0]);
+    dy -= box.L[1] * rint(dy * box.invL[1]);
+    dz -= box.L[2] * rint(dz * box.invL[2]);
+    if (!(dx * dx + dy * dy + dz * dz <= half_skin2) || sid[i] != sid_build[i]) *stale = 1;
+}
+
 // ---- precision conversion of state arrays (DEM_F32 contexts integrate in double, R15b) --------------------------------
 __global__ void k_f4_to_d4(int n, const f4* __restrict__ in, d4* __restrict__ out) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;

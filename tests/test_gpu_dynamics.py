@@ -85,6 +85,53 @@ def test_rebuilds_do_not_change_the_trajectory(pkg):
     assert np.abs(a["pos"] - b["pos"]).max() < 1e-9
 
 
+@pytest.mark.parametrize("kind,cells", [("squares", 8), ("mixed", 4)])
+def test_state_edited_between_calls(pkg, oracle, kind, cells):
+    """Between two dem_step calls the caller rescales the velocities (the list of the first call is still valid and is
+    kept), then exchanges the places of two distant particles and changes one shape id (the list is stale: it must be rebuilt).
+    Each leg is compared with the oracle run on the same edited state."""
+    import torch
+
+    st = di.dense_state(kind, cells)
+    dt, n = 5e-4, st["N"]
+    dem, t = pkg.from_state(st, "f64")
+    f = torch.empty((n, 4), dtype=dem.dtype, device="cuda")
+    tq = torch.empty((n, 4), dtype=dem.dtype, device="cuda")
+
+    def leg(nsteps):
+        dem.step(t["pos"], t["quat"], t["vel"], t["angmom"], t["shape_id"], st["box"], dt, nsteps, 0.4, f, tq)
+        ref = oracle.step(cur, dt, nsteps)
+        for k in ("pos", "quat", "vel", "angmom"):
+            assert np.abs(t[k].cpu().numpy() - ref[k]).max() < 1e-8, k
+            cur[k] = ref[k]
+        assert np.abs(f.cpu().numpy() - ref["force"]).max() < 1e-7 * max(1.0, np.abs(ref["force"]).max())
+
+    cur = dict(st)
+    leg(40)
+    builds = dem.launch_count()
+    t["vel"].mul_(0.5)
+    cur["vel"] = cur["vel"] * 0.5
+    before = dem.launch_count()
+    leg(40)
+    kept = dem.launch_count() - before
+    # two particles far apart exchange their places; one truncated icosahedron becomes a tetrahedron of the same
+    # circumsphere (the other way round would overlap its neighbours)
+    pos = t["pos"].cpu().numpy()
+    pos[[0, n // 2]] = pos[[n // 2, 0]]
+    sid = np.array(cur["shape_id"]).copy()
+    if kind == "mixed":
+        sid[np.nonzero(sid == 0)[0][1]] = 1
+    t["pos"].copy_(torch.from_numpy(pos))
+    t["shape_id"].copy_(torch.from_numpy(sid))
+    cur["pos"], cur["shape_id"] = pos, sid
+    before = dem.launch_count()
+    leg(5)
+    rebuilt = dem.launch_count() - before
+    assert rebuilt - 5 * (kept // 40) > 3          # the list kernels ran again in the last leg
+    assert builds > 0
+    dem.close()
+
+
 def test_config1_energy_parity_and_drift_gate(pkg, oracle):
     """Config 1 in FP64: 1000 steps at dt = 1e-4 against the oracle's energies, then the north_star gate:
     max_t |E(t) - E(0)| / N < 1e-4 over 10^4 steps (sampled every 500 steps)."""
