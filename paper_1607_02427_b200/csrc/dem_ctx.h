@@ -8,6 +8,7 @@
 // The pair kernels are template-heavy; one translation unit each lets nvcc compile them in parallel.
 #pragma once
 #include <cuda_runtime.h>
+#include <cstdlib>
 
 #include <cstdarg>
 #include <cstdio>

@@ -18,8 +18,9 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
     if (N != ctx->N) return fail(ctx, DEM_ESTALE, "N = %d differs from the last build (%d)", N, ctx->N);
     if (!pos || !quat || !sid || !force || !torque) return fail(ctx, DEM_EINVAL, "null particle array");
     const int* skip = fin ? fin->bail : nullptr;
-    // counters[0..7] (unsigned long long) followed by the per-class lengths of the k_pose work lists (int): one memset
-    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES, ctx->stream));
+    // counters[0..7] (unsigned long long) followed by the per-class lengths of the k_pose work lists and the per-class
+    // tile counters of the search kernel (int): one memset
+    CU(cudaMemsetAsync(ctx->counters.p, 0, sizeof(unsigned long long) * 8 + sizeof(int) * 2 * DEM_MAX_CLASSES, ctx->stream));
     int* ccount = reinterpret_cast<int*>(ctx->counters.as<unsigned long long>() + 8);
     // capacity of a class's work list: its pairs plus the padding of every k_pose block to a whole warp tile
     const int pose_block = pose_threads();
@@ -136,10 +137,14 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
                 }
                 LAUNCHED(ctx);
                 if (populated == 1) em = ev_mark(ctx, 1, st, true);
-                // the padded work list bounds the tiles; grid cap in blocks per SM measured on cfg4 (one tile per warp
-                // beats one persistent wave)
+                // the padded work list bounds the tiles; grid cap in blocks per SM measured on cfg4 for k_pair_cull (one
+                // tile per warp beats one persistent wave of statically dealt tiles)
                 const long long list_items = (long long)list_cap(c) * a.slices / (cull ? 2 : 1);
                 grid = (int)std::min<long long>(nblk(list_items, threads), (long long)ctx->sm_count * 64);
+                if (!cull) {  // k_pair_fast deals its tiles out through a counter (267.7 against 270.4 us on cfg4)
+                    a.tile = ccount + DEM_MAX_CLASSES + c;
+                    grid = (int)std::min<long long>(grid, (long long)ctx->sm_count * 4);  // one resident wave
+                }
                 if (cull) {
                     smem += pair_cull_smem_header();
                     a.cull_a2 = (real)(ra * ra);
@@ -180,18 +185,17 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
         while (lanes < 32 && (long long)N * lanes < 65536) lanes <<= 1;
         fa.lanes = lanes;
         const int grid = nblk((long long)N * lanes, 256);
-        const int* counts = ctx->counts.as<int>();
         const int* slot = ctx->slot.as<int>();
         const real4* rec = ctx->rec.as<real4>();
         const unsigned char* rf = ctx->rflag.as<unsigned char>();
         real4 *F = static_cast<real4*>(force), *T = static_cast<real4*>(torque);
         real* W = static_cast<real*>(virial);
         if (fa.mode == 2)
-            k_finish<real, 2><<<grid, 256, 0, st>>>(N, counts, slot, sid, ctx->ct, ctx->nclass, rec, rf, F, T, W, fa);
+            k_finish<real, 2><<<grid, 256, 0, st>>>(N, ctx->stride, slot, sid, ctx->ct, ctx->nclass, rec, rf, F, T, W, fa);
         else if (fa.mode == 1)
-            k_finish<real, 1><<<grid, 256, 0, st>>>(N, counts, slot, sid, ctx->ct, ctx->nclass, rec, rf, F, T, W, fa);
+            k_finish<real, 1><<<grid, 256, 0, st>>>(N, ctx->stride, slot, sid, ctx->ct, ctx->nclass, rec, rf, F, T, W, fa);
         else
-            k_finish<real, 0><<<grid, 256, 0, st>>>(N, counts, slot, sid, ctx->ct, ctx->nclass, rec, rf, F, T, W, fa);
+            k_finish<real, 0><<<grid, 256, 0, st>>>(N, ctx->stride, slot, sid, ctx->ct, ctx->nclass, rec, rf, F, T, W, fa);
     }
     LAUNCHED(ctx);
     ev_span(ctx, KT_REDUCE, r0, ev_mark(ctx, 2));

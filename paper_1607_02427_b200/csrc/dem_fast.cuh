@@ -631,18 +631,40 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
     const float nrc2 = -a.rc2_search;
     const int count = *a.count;                // pairs inside the reach, compacted by k_pose
     const int np_pad = (count + 31) & ~31;     // slices are warp-uniform
-    const long long n_wtiles = (long long)(np_pad >> 5) * a.slices;
+    const int tps = np_pad >> 5;               // tiles per slice
+    const int n_wtiles = tps * a.slices;       // (a work list holds far fewer than 2^31 / 32 tiles: 96 bytes per pair)
     const size_t plane = a.plane;
     unsigned n_ee = 0u, n_vf = 0u, n_vfe = 0u;
+    auto slice_terms = [&](int ob, int oe, unsigned& e_, unsigned& v_, unsigned& ve_) {
+        if (DIM == 3) {
+            const int oE_ = B.ne, oV_ = B.ne + B.nv;
+            const int r1 = max(min(oe, oE_) - ob, 0), r2 = max(min(oe, oV_) - max(ob, oE_), 0),
+                      r3 = max(min(oe, oV_ + A.nv) - max(ob, oV_), 0);
+            e_ = (unsigned)(r1 * A.ne);
+            v_ = (unsigned)(r2 * A.nf + r3 * B.nf);
+            ve_ = (unsigned)(r2 * a.sa.nfe + r3 * a.sb.nfe);
+        } else {
+            const int r1 = max(min(oe, B.nv) - ob, 0), r2 = max(min(oe, B.nv + A.nv) - max(ob, B.nv), 0);
+            e_ = (unsigned)(r1 * A.ne + r2 * B.ne);  // 2D: vertex-edge terms
+            v_ = ve_ = 0u;
+        }
+    };
+    unsigned t_ee = 0u, t_vf = 0u, t_vfe = 0u;  // per pair of an unsliced class: the same for every tile
+    if (a.slices == 1) slice_terms(0, a.n_outer, t_ee, t_vf, t_vfe);
     // Each warp takes every (gridDim.x * 4)-th tile (one tile per warp unless the class has more tiles than the grid
     // cap).  The pose records of a warp's next tile are copied global -> shared with cp.async while the current tile is
     // being swept; each lane copies and later reads only its own records.
-    const long long wt_stride = (long long)gridDim.x * 4;
+    const int wt_stride = (int)gridDim.x * 4;
     f4* spose = stage_pose + warp * (2 * 3 * 32);   // [2][3][32]
     int* spidx = stage_pidx + warp * (2 * 32);      // [2][32]
-    auto stage = [&](int buf, long long wt_) {
+    // tile -> (slice, first entry of the work list): no division for unsliced classes
+    auto locate = [&](int wt_, int& slice_, int& c0_) {
+        slice_ = a.slices == 1 ? 0 : wt_ / tps;
+        c0_ = (wt_ - slice_ * tps) * 32;
+    };
+    auto stage = [&](int buf, int wt_, int c0_) {
         if (wt_ < n_wtiles) {
-            const int c_ = (int)((wt_ * 32 + lane) % np_pad);
+            const int c_ = c0_ + lane;
             DEM_ASSERT(c_ >= 0 && (size_t)count <= plane);
             if (c_ < count) {
 #pragma unroll
@@ -655,13 +677,26 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
         }
         asm volatile("cp.async.commit_group;");
     };
+    // With a tile counter (a.tile, zeroed per evaluation) the grid is one resident wave and every warp takes its next
+    // tile from the counter, one tile ahead of the one it sweeps: no warp waits for the slowest warp of its block and
+    // the tables are staged once per block.
+    auto next_tile = [&](int wt_) -> int {
+        if (!a.tile) return wt_ + wt_stride;
+        int v = 0;
+        if (lane == 0) v = atomicAdd(a.tile, 1);
+        return __shfl_sync(full, v, 0);
+    };
     int buf = 0;
-    stage(0, (long long)blockIdx.x * 4 + warp);
-    for (long long wt = (long long)blockIdx.x * 4 + warp; wt < n_wtiles; wt += wt_stride, buf ^= 1) {
-        const long long item = wt * 32 + lane;
-        const int slice = (int)(item / np_pad), c = (int)(item - (long long)slice * np_pad);
+    int wt = a.tile ? next_tile(0) : (int)blockIdx.x * 4 + warp, slice = 0, c0 = 0;
+    if (wt < n_wtiles) locate(wt, slice, c0);
+    stage(0, wt, c0);
+    for (int wt_next, slice_next, c0_next; wt < n_wtiles; wt = wt_next, slice = slice_next, c0 = c0_next, buf ^= 1) {
+        const int c = c0 + lane;
         const bool in_list = c < count;
-        stage(buf ^ 1, wt + wt_stride);
+        wt_next = next_tile(wt);
+        slice_next = c0_next = 0;
+        if (wt_next < n_wtiles) locate(wt_next, slice_next, c0_next);
+        stage(buf ^ 1, wt_next, c0_next);
         asm volatile("cp.async.wait_group 1;" ::: "memory");
         __syncwarp();  // the cooperative evaluation reads other lanes' staged poses
         w.sp = spose + buf * 3 * 32;
@@ -684,20 +719,13 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
 
 #pragma unroll
             for (int k = 0; k < 7; ++k) w.sacc[k * 32 + lane] = 0.f;
-            const int ob = (int)((long long)slice * a.n_outer / a.slices);
-            const int oe = (int)((long long)(slice + 1) * a.n_outer / a.slices);
+            const int ob = a.slices == 1 ? 0 : slice * a.n_outer / a.slices;   // (n_outer <= 3 x 2^15: no overflow)
+            const int oe = a.slices == 1 ? a.n_outer : (slice + 1) * a.n_outer / a.slices;
             if (valid) {  // terms this lane sweeps (for the flop count; the kernel sweeps every term of its pairs)
-                if (DIM == 3) {
-                    const int oE_ = B.ne, oV_ = B.ne + B.nv;
-                    const int r1 = max(min(oe, oE_) - ob, 0), r2 = max(min(oe, oV_) - max(ob, oE_), 0),
-                              r3 = max(min(oe, oV_ + A.nv) - max(ob, oV_), 0);
-                    n_ee += (unsigned)(r1 * A.ne);
-                    n_vf += (unsigned)(r2 * A.nf + r3 * B.nf);
-                    n_vfe += (unsigned)(r2 * a.sa.nfe + r3 * a.sb.nfe);
-                } else {
-                    const int r1 = max(min(oe, B.nv) - ob, 0), r2 = max(min(oe, B.nv + A.nv) - max(ob, B.nv), 0);
-                    n_ee += (unsigned)(r1 * A.ne + r2 * B.ne);  // 2D: vertex-edge terms
-                }
+                if (a.slices != 1) slice_terms(ob, oe, t_ee, t_vf, t_vfe);
+                n_ee += t_ee;
+                n_vf += t_vf;
+                n_vfe += t_vfe;
             }
             if (DIM == 3) {
                 const int oE = B.ne, oV = B.ne + B.nv;
@@ -856,7 +884,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
                         F[k] = w.sacc[k * 32 + lane];
                         T[k] = w.sacc[(3 + k) * 32 + lane];
                     }
-                    const int c_ = (int)((wt * 32 + lane) % np_pad);
+                    const int c_ = c;
                     const f4 p3 = a.pose[3 * plane + c_], p4 = a.pose[4 * plane + c_],
                              p5 = a.pose[5 * plane + c_];
                     const float Mi[9] = {p3.x, p3.y, p3.z, p3.w, p4.x, p4.y, p4.z, p4.w, p5.x};
@@ -1030,13 +1058,16 @@ __device__ __forceinline__ void write_items(CullCtx& cc, unsigned mask, int owne
         int off_;                                                                         \
         const unsigned m_ = (MASK);                                                       \
         const int tot_ = count_items(w, m_, off_);                                        \
-        if (cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH>(w, cc, A, B, a.sa, a.sb, nrc2);    \
+        if constexpr (!NOOVF)                                                             \
+            if (cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH>(w, cc, A, B, a.sa, a.sb, nrc2); \
         write_items(cc, m_, (OWNER), (O0), (FLAG), off_, tot_);                           \
     } while (0)
 
 // SAME: both particles of the class have the same shape.  ONESITE: one sweep site per phase (small code, for large shape
 // tables) instead of one behind every emit site (the two owner slots' emits interleave: faster for small shapes).
-template <int MINB, bool SAME, bool ONESITE>
+// NOOVF: every item of a tile's phase fits the list (64 pairs x outer features <= DEM_IQCAP), so that the emit sites
+// need no sweep of their own: three sweep sites in all (the instruction cache holds them).
+template <int MINB, bool SAME, bool ONESITE, bool NOOVF>
 __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a) {
     // a warp tile is 64 pairs (two per lane: owner slots lane and lane + 32), so that the item passes run fuller
     extern __shared__ __align__(16) unsigned char smem_raw[];

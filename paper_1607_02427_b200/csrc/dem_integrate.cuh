@@ -35,11 +35,13 @@ __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict
         const d4 xb = pos_build[i];
         double xs[3] = {x.x, x.y, x.z}, vs[3] = {v.x * sc, v.y * sc, v.z * sc};
         const double Fs[3] = {(double)F.x, (double)F.y, (double)F.z};
-        for (int a = 0; a < box.dim; ++a) {
-            vs[a] += hm * Fs[a];
-            xs[a] += dt * vs[a];
-            xs[a] -= box.L[a] * rint(xs[a] * box.invL[a]);
-        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a)  // (static indices: the state stays in registers)
+            if (a < box.dim) {
+                vs[a] += hm * Fs[a];
+                xs[a] += dt * vs[a];
+                xs[a] -= box.L[a] * rint(xs[a] * box.invL[a]);
+            }
         x.x = xs[0]; x.y = xs[1]; x.z = xs[2];
         v.x = vs[0]; v.y = vs[1]; v.z = vs[2];
         pos[i] = x;
@@ -54,7 +56,9 @@ __global__ void k_kick_drift(int N, BoxDev box, double dt, const int* __restrict
         const typename vec4<real>::type T = torque[i];
         double Ls[3] = {L.x * sc, L.y * sc, L.z * sc};
         const double Ts[3] = {(double)T.x, (double)T.y, (double)T.z};
-        for (int a = (box.dim == 2 ? 2 : 0); a < 3; ++a) Ls[a] += 0.5 * dt * Ts[a];
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            if (box.dim == 3 || a == 2) Ls[a] += 0.5 * dt * Ts[a];
         double qs[4] = {q.x, q.y, q.z, q.w};
         free_rotate(box.dim, mt.inertia[s], Ls, dt, qs);
         L.x = Ls[0]; L.y = Ls[1]; L.z = Ls[2];

@@ -132,8 +132,9 @@ __global__ void __launch_bounds__(128) k_pair(const PairArgs<real> a) {
 // half kick of the next step, the drift, the free rotation and the skin test), which saves the passes over F, tau, v
 // and L that separate kernels would need.  Forces and torques are stored only in modes 0 and 1 (mode 2 consumes them
 // in registers; the step that ends a dem_step call runs in mode 1).
+#define DEM_FIN_W 8
 template <typename real, int MODE>
-__global__ void __launch_bounds__(256) k_finish(int N, const int* __restrict__ counts, const int* __restrict__ slot,
+__global__ void __launch_bounds__(256) k_finish(int N, int stride, const int* __restrict__ slot,
                                                 const int* __restrict__ sid, ClassTable ct, int nclass,
                                                 const typename vec4<real>::type* __restrict__ rec,
                                                 const unsigned char* __restrict__ rflag,
@@ -145,6 +146,23 @@ __global__ void __launch_bounds__(256) k_finish(int N, const int* __restrict__ c
     // a particle's slots, so several lanes split it and combine with shuffles: still a fixed order for a given N)
     const int lpp = fa.lanes, gid = blockIdx.x * blockDim.x + threadIdx.x;
     const int i = gid / lpp, sub = gid - i * lpp;
+    // The kernel is a chain of dependent loads (stale flag -> slots -> record flags -> state): ask the L2 for everything
+    // whose address is known now, so that the chain runs on L2 hits
+    if (i < N) {
+#pragma unroll
+        for (int u = 0; u < DEM_FIN_W; ++u)
+            if (DEM_FIN_W * sub + u < stride)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(slot + (size_t)(DEM_FIN_W * sub + u) * N + i));
+        if (MODE >= 1 && sub == 0) {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(fa.vel + i));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(fa.ang + i));
+            if (MODE == 2) {
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(fa.pos + i));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(fa.quat + i));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(fa.pos_build + i));
+            }
+        }
+    }
     if (MODE != 0) {
         if (fa.bail && *fa.bail) {               // the list went stale before this step: change nothing, and pass
             if (gid == 0 && fa.raise) *fa.raise = 1;  // the word on (the next evaluation looks at the other flag)
@@ -153,30 +171,19 @@ __global__ void __launch_bounds__(256) k_finish(int N, const int* __restrict__ c
         if (gid == 0 && fa.done) *fa.done += 1;  // nothing in this kernel reads it
     }
     const bool live = i < N, lead = live && sub == 0;
-    // state loads first: they do not depend on the reduction
-    d4 v, L, x, q, xb;
-    int sh = 0;
-    if (MODE >= 1 && lead) {
-        v = fa.vel[i];
-        L = fa.ang[i];
-        sh = sid[i];
-    }
-    if (MODE == 2 && lead) {
-        x = fa.pos[i];
-        q = fa.quat[i];
-        xb = fa.pos_build[i];
-    }
     real F[3] = {0, 0, 0}, T[3] = {0, 0, 0}, U = 0, W[6] = {0, 0, 0, 0, 0, 0};
-    const int n = live ? counts[i] : 0;
-    for (int k0 = 4 * sub; k0 < n; k0 += 4 * lpp) {
-        int sl[4];
-        size_t ri[4];
-        int S[4];
-        unsigned any[4];
+    // A particle's slots are walked DEM_FIN_W at a time: the slot loads of a batch are in flight together, then its flag
+    // loads.  Rows end with -1 (k_slot_back pads them), so the walk does not wait for the particle's neighbour count.
+    for (int k0 = DEM_FIN_W * sub; live && k0 < stride; k0 += DEM_FIN_W * lpp) {
+        int sl[DEM_FIN_W];
+        int ri[DEM_FIN_W];   // (record indices fit an int: checked at the build)
+        int S[DEM_FIN_W];
+        unsigned any[DEM_FIN_W];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) sl[u] = k0 + u < n ? slot[(size_t)(k0 + u) * N + i] : -1;
+        for (int u = 0; u < DEM_FIN_W; ++u) sl[u] = k0 + u < stride ? slot[(size_t)(k0 + u) * N + i] : -1;
+        if (sl[0] < 0) break;
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < DEM_FIN_W; ++u) {
             any[u] = 0u;
             S[u] = 0;
             ri[u] = 0;
@@ -186,19 +193,19 @@ __global__ void __launch_bounds__(256) k_finish(int N, const int* __restrict__ c
                 while (c + 1 < nclass && p >= ct.pair_base[c + 1]) ++c;
                 DEM_ASSERT(p < ct.pair_base[nclass] && p >= ct.pair_base[c]);
                 S[u] = ct.slices[c];
-                ri[u] = (size_t)ct.rec_base[c] + (size_t)(p - ct.pair_base[c]) * S[u];
+                ri[u] = ct.rec_base[c] + (p - ct.pair_base[c]) * S[u];
                 // bit s: slice s of the pair has a record (more than 32 slices: every flag is looked at below)
                 for (int s = 0; s < S[u] && s < 32; ++s) any[u] |= (unsigned)(rflag[ri[u] + s] != 0) << s;
                 if (S[u] > 32) any[u] |= 0x80000000u;
             }
         }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < DEM_FIN_W; ++u) {
             if (!any[u]) continue;  // this pair contributes nothing: no record was written
             const int side = sl[u] & 1;
             for (int s = 0; s < S[u]; ++s) {
                 if (S[u] <= 32 ? !((any[u] >> s) & 1u) : !rflag[ri[u] + s]) continue;
-                const real4* r = rec + DEM_REC * (ri[u] + s);
+                const real4* r = rec + DEM_REC * (size_t)(ri[u] + s);
                 const real4 r0 = r[0], r1 = r[1], r2 = r[2];
                 const real dx = r1.w, dy = r2.x, dz = r2.y;
                 if (side) {  // this particle is the pair's second one: F_j = -F_i, tau_j = -tau_i + d x F_i
@@ -244,18 +251,33 @@ __global__ void __launch_bounds__(256) k_finish(int N, const int* __restrict__ c
         }
     }
     if (MODE >= 1) {
+        // the state was asked for at the top (L2 prefetch): loading it only now keeps it out of the walk's registers
+        d4 v = fa.vel[i], L = fa.ang[i], x, q, xb;
+        const int sh = sid[i];
+        if (MODE == 2) {
+            x = fa.pos[i];
+            q = fa.quat[i];
+            xb = fa.pos_build[i];
+        }
         const double hm = 0.5 * fa.dt / fa.mt.mass[sh];
         double vs[3] = {v.x, v.y, v.z}, Ls[3] = {L.x, L.y, L.z};
         const double Fs[3] = {(double)F[0], (double)F[1], (double)F[2]}, Ts[3] = {(double)T[0], (double)T[1], (double)T[2]};
-        for (int a = 0; a < fa.dim; ++a) vs[a] += hm * Fs[a];                       // second half kick: the step is done
-        for (int a = (fa.dim == 2 ? 2 : 0); a < 3; ++a) Ls[a] += 0.5 * fa.dt * Ts[a];
+        // (loops unrolled with predicates: static indices keep the state in registers)
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            if (a < fa.dim) vs[a] += hm * Fs[a];                                    // second half kick: the step is done
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            if (fa.dim == 3 || a == 2) Ls[a] += 0.5 * fa.dt * Ts[a];
         if (MODE == 2) {  // first half of the next step (the same arithmetic as k_kick_drift)
             double xs[3] = {x.x, x.y, x.z};
-            for (int a = 0; a < fa.dim; ++a) {
-                vs[a] += hm * Fs[a];
-                xs[a] += fa.dt * vs[a];
-                xs[a] -= fa.box.L[a] * rint(xs[a] * fa.box.invL[a]);
-            }
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                if (a < fa.dim) {
+                    vs[a] += hm * Fs[a];
+                    xs[a] += fa.dt * vs[a];
+                    xs[a] -= fa.box.L[a] * rint(xs[a] * fa.box.invL[a]);
+                }
             x.x = xs[0]; x.y = xs[1]; x.z = xs[2];
             fa.pos[i] = x;
             double dx = xs[0] - xb.x, dy = xs[1] - xb.y, dz = fa.dim == 3 ? xs[2] - xb.z : 0.0;
@@ -263,7 +285,9 @@ __global__ void __launch_bounds__(256) k_finish(int N, const int* __restrict__ c
             dy -= fa.box.L[1] * rint(dy * fa.box.invL[1]);
             dz -= fa.box.L[2] * rint(dz * fa.box.invL[2]);
             if (dx * dx + dy * dy + dz * dz > fa.half_skin2) *fa.raise = 1;
-            for (int a = (fa.dim == 2 ? 2 : 0); a < 3; ++a) Ls[a] += 0.5 * fa.dt * Ts[a];
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                if (fa.dim == 3 || a == 2) Ls[a] += 0.5 * fa.dt * Ts[a];
             double qs[4] = {q.x, q.y, q.z, q.w};
             free_rotate(fa.dim, fa.mt.inertia[sh], Ls, fa.dt, qs);
             q.x = qs[0]; q.y = qs[1]; q.z = qs[2]; q.w = qs[3];

@@ -124,7 +124,7 @@ int build_neighbors_t(dem_ctx* ctx, const PosT* pos, const int32_t* sid, int N, 
     CU(ctx->counts.reserve(sizeof(int) * (size_t)N));
     CU(ctx->scratch_scan.reserve(sizeof(int) * scan_ints));
     CU(ctx->flags.reserve(sizeof(int) * 16));
-    CU(ctx->counters.reserve(sizeof(unsigned long long) * 8 + sizeof(int) * DEM_MAX_CLASSES));
+    CU(ctx->counters.reserve(sizeof(unsigned long long) * 8 + sizeof(int) * 2 * DEM_MAX_CLASSES));
     CU(ctx->pos_build.reserve(sizeof(d4) * (size_t)N));
     int* cell_start = ctx->cell_start.as<int>();
     CU(cudaMemsetAsync(cell_start, 0, sizeof(int) * ((size_t)g.ncell + 1), st));

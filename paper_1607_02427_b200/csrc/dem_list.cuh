@@ -214,6 +214,7 @@ __global__ void k_slot_back(int N, const int* __restrict__ counts, const int* __
             slot[(size_t)k * N + i] = 2 * p + (j_first ? 1 : 0);
         }
     }
+    for (int k = n; k < stride; ++k) slot[(size_t)k * N + i] = -1;  // end of the row (k_finish stops there)
 }
 
 }  // namespace dem

@@ -15,7 +15,7 @@ __device__ __forceinline__ void quat_mul_d(const double* a, const double* b, dou
 // Torque-free rotation over dt with the lab-frame angular momentum L held fixed.  Spherical tops (and 2D): exact,
 // q <- exp(dt/2 L/I0) q.  Otherwise the symmetric splitting of the free-rotor Hamiltonian into rotations about the
 // body axes x(dt/2) y(dt/2) z(dt) y(dt/2) x(dt/2) (the family of PAPER.md ref. 23).
-__device__ inline void free_rotate(int dim, const double* I, const double* L, double dt, double* q) {
+__device__ __forceinline__ void free_rotate(int dim, const double* I, const double* L, double dt, double* q) {
     const bool spherical = dim == 2 || (I[0] == I[1] && I[1] == I[2]);
     if (spherical) {
         const double I0 = I[2];
@@ -42,18 +42,21 @@ __device__ inline void free_rotate(int dim, const double* I, const double* L, do
         double inv = 1.5 - 0.5 * n2;
         inv = inv * (1.5 - 0.5 * n2 * inv * inv);
         inv = inv * (1.5 - 0.5 * n2 * inv * inv);
+#pragma unroll
         for (int k = 0; k < 4; ++k) q[k] = o[k] * inv;
         return;
     }
     double M[9], Lb[3];
     quat_to_mat<double>(q[0], q[1], q[2], q[3], M);
+#pragma unroll
     for (int a = 0; a < 3; ++a) Lb[a] = M[a] * L[0] + M[3 + a] * L[1] + M[6 + a] * L[2];  // R^T L
-    const int axis_seq[5] = {0, 1, 2, 1, 0};
-    const double frac[5] = {0.5, 0.5, 1.0, 0.5, 0.5};
+    // (unrolled with compile-time axes: every array index is static, so that L_b and q stay in registers)
+#pragma unroll
     for (int s = 0; s < 5; ++s) {
-        const int a = axis_seq[s];
+        const int a = s < 3 ? s : 4 - s;  // x y z y x
+        const double fr = s == 2 ? 1.0 : 0.5;
         if (!(I[a] > 0.0)) continue;
-        const double phi = frac[s] * dt * Lb[a] / I[a];
+        const double phi = fr * dt * Lb[a] / I[a];
         double sn, cs;
         sincos(phi, &sn, &cs);
         const int b = (a + 1) % 3, c = (a + 2) % 3;
@@ -65,9 +68,11 @@ __device__ inline void free_rotate(int dim, const double* I, const double* L, do
         double rq[4] = {ch, 0, 0, 0}, o[4];
         rq[1 + a] = sh;
         quat_mul_d(q, rq, o);  // body-axis rotation composes on the right
+#pragma unroll
         for (int k = 0; k < 4; ++k) q[k] = o[k];
     }
     const double n = sqrt(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
+#pragma unroll
     for (int k = 0; k < 4; ++k) q[k] /= n;
 }
 

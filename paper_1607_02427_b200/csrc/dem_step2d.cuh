@@ -192,27 +192,36 @@ __global__ void __launch_bounds__(DEM_P2D_THREADS, 5) k_particle2d(const Particl
             acc.nactive = acc.ndegen = acc.npar = 0u;
             // The sweeps only note candidates (side, vertex, edge: one per term inside the candidate cutoff) in a small
             // per-lane list; the exact scalar routines run on them afterwards, in one place.
-            unsigned cand[4] = {0u, 0u, 0u, 0u};
+            // (four named registers, filled and emptied with static moves: an indexed array would live in local memory)
+            unsigned cand0 = 0u, cand1 = 0u, cand2 = 0u, cand3 = 0u;
             int ncand = 0;
+            auto eval_cand = [&](unsigned c0) {
+                const int sd_ = (int)(c0 >> 31), o_ = (int)((c0 >> 12) & 0x7ffffu), k_ = (int)(c0 & 0xfffu);
+                if (sd_ == 0) {
+                    const f4 v = B.V[o_];
+                    float p[3];
+                    vertex_to_i<float>(v.x, v.y, 0.f, R, t, p);
+                    term_ve_own<float>(A, k_, p[0], p[1], pc, acc);
+                } else {
+                    const f4 v = A.V[o_];
+                    float p[3];
+                    vertex_to_j<float>(v.x, v.y, 0.f, R, t, p);
+                    term_ve_other<float>(B, k_, v.x, v.y, p[0], p[1], R, pc, acc);
+                }
+            };
             auto note = [&](int side, int o, int kk) {
                 if (ncand == 4) {  // list full (rare): evaluate the oldest entry now
-                    const unsigned c0 = cand[0];
-                    cand[0] = cand[1]; cand[1] = cand[2]; cand[2] = cand[3];
+                    const unsigned c0 = cand0;
+                    cand0 = cand1; cand1 = cand2; cand2 = cand3;
                     ncand = 3;
-                    const int sd_ = (int)(c0 >> 31), o_ = (int)((c0 >> 12) & 0x7ffffu), k_ = (int)(c0 & 0xfffu);
-                    if (sd_ == 0) {
-                        const f4 v = B.V[o_];
-                        float p[3];
-                        vertex_to_i<float>(v.x, v.y, 0.f, R, t, p);
-                        term_ve_own<float>(A, k_, p[0], p[1], pc, acc);
-                    } else {
-                        const f4 v = A.V[o_];
-                        float p[3];
-                        vertex_to_j<float>(v.x, v.y, 0.f, R, t, p);
-                        term_ve_other<float>(B, k_, v.x, v.y, p[0], p[1], R, pc, acc);
-                    }
+                    eval_cand(c0);
                 }
-                cand[ncand++] = ((unsigned)side << 31) | ((unsigned)o << 12) | (unsigned)kk;
+                const unsigned v = ((unsigned)side << 31) | ((unsigned)o << 12) | (unsigned)kk;
+                if (ncand == 0) cand0 = v;
+                else if (ncand == 1) cand1 = v;
+                else if (ncand == 2) cand2 = v;
+                else cand3 = v;
+                ++ncand;
             };
 #pragma unroll 1
             for (int side = 0; side < 2; ++side) {
@@ -277,20 +286,10 @@ __global__ void __launch_bounds__(DEM_P2D_THREADS, 5) k_particle2d(const Particl
                 }
             }
 #pragma unroll 1
-            for (int c = 0; c < ncand; ++c) {
-                const unsigned c0 = cand[c];
-                const int sd_ = (int)(c0 >> 31), o_ = (int)((c0 >> 12) & 0x7ffffu), k_ = (int)(c0 & 0xfffu);
-                if (sd_ == 0) {
-                    const f4 v = B.V[o_];
-                    float p[3];
-                    vertex_to_i<float>(v.x, v.y, 0.f, R, t, p);
-                    term_ve_own<float>(A, k_, p[0], p[1], pc, acc);
-                } else {
-                    const f4 v = A.V[o_];
-                    float p[3];
-                    vertex_to_j<float>(v.x, v.y, 0.f, R, t, p);
-                    term_ve_other<float>(B, k_, v.x, v.y, p[0], p[1], R, pc, acc);
-                }
+            for (int c = 0; c < ncand; ++c) {  // oldest first
+                const unsigned c0 = cand0;
+                cand0 = cand1; cand1 = cand2; cand2 = cand3;
+                eval_cand(c0);
             }
             if (acc.nactive) {
                 float o10[10];

@@ -96,6 +96,7 @@ template <typename real> struct PairArgs {
     const f4* pose;       // FP32 search kernel: this class's compacted pose records, pair indices and their number
     const int* pidx;      //   (written by k_pose)
     const int* count;
+    int* tile;            //   next tile to take (zero at launch), or null: tiles are dealt out by block and warp index
     size_t plane;         //   stride of the pose planes
     const unsigned* cmask;  // culling kernel: per-pair survivor masks written by k_pose_cull, [words][plane] (null: the
     int mw_e, mw_vj, mw_vi; //   kernel runs the cull tests itself); words for edges of j, vertices of j, vertices of i
