@@ -82,7 +82,7 @@ def build(force=False, verbose=False):
         obj = os.path.join(OBJDIR, "%s.%s.o" % (base, key))
         if force or not os.path.exists(obj):
             for old in glob.glob(os.path.join(OBJDIR, base + ".*.o")):
-                if time.time() - os.path.getmtime(old) > 3600:  # objects of abandoned source states
+                if time.time() - os.path.getmtime(old) > 600:  # objects of abandoned source states
                     os.remove(old)
             jobs.append((src, obj))
         else:
