@@ -193,6 +193,22 @@ int dem_energy(dem_ctx* ctx, const void* quat, const void* vel, const void* angm
                const void* force_energy, int N, double out[3]);
 
 /*
+ * The same three sums without any device allocation, for callers that cannot call cudaMalloc (CUDA graph capture, tight
+ * serving loops): the per-block partial sums go to a fixed device array inside the library (96 KiB, held by every GPU
+ * that loads the library until exit) instead of a buffer the context allocates.
+ *   quat, vel, angmom, force_energy  DEVICE real[N][4]   shape_id  DEVICE int32[N]   (as dem_energy)
+ *   out_dev    DEVICE double[3]: U, K_trans, K_rot; written by the context's stream, NOT synchronised
+ * N <= DEM_ENERGY_STATIC_MAX_N, else DEM_EINVAL (use dem_energy).  Calls no cudaMalloc / cudaFree, copies nothing to
+ * the host and does not touch the context's own buffers.  All calls (of every context on a GPU) share the one array:
+ * calls issued to one stream are safe, calls that overlap on the GPU race.  The array needs no clearing: a call reads
+ * only what it has just written.  The first call on a device looks the array's address up (cudaGetSymbolAddress): make
+ * it outside a graph capture.  Sums are in double in a fixed order; they differ from dem_energy's by summation order only.
+ */
+#define DEM_ENERGY_STATIC_MAX_N (1 << 20)
+int dem_energy_static(dem_ctx* ctx, const void* quat, const void* vel, const void* angmom, const int32_t* shape_id,
+                      const void* force_energy, int N, double* out_dev);
+
+/*
  * Host-buffer forms (the end-to-end path): same semantics, every particle array is a HOST pointer (pinned memory
  * gives the best copy rate); the library copies inputs to device scratch it owns, runs dem_build_neighbors +
  * dem_compute (or dem_step), copies the results back and synchronises.

@@ -21,7 +21,7 @@ STATUS_NAMES = {0: "DEM_OK", -1: "DEM_EINVAL", -2: "DEM_ENOMEM", -3: "DEM_ECUDA"
 # every symbol include/dem.h declares (tests check that the built library exports all of them)
 EXPORTS = ["dem_create", "dem_destroy", "dem_last_error", "dem_set_eps_par", "dem_create_shape", "dem_build_neighbors",
            "dem_get_neighbors", "dem_copy_neighbors", "dem_compute", "dem_get_counters", "dem_step", "dem_step_nvt", "dem_step_npt",
-           "dem_energy",
+           "dem_energy", "dem_energy_static",
            "dem_compute_host", "dem_step_host", "dem_set_slices", "dem_set_pair_kernel", "dem_set_culling", "dem_version"]
 # include/dem_bench.h (measurement hooks)
 EXPORTS_BENCH = ["dem_set_l2_flush", "dem_set_timing", "dem_kernel_times", "dem_swept_totals", "dem_launch_count",
@@ -267,6 +267,14 @@ class Dem:
                               _dev(shape_id, torch.int32), _dev(force, self.dtype), C.c_int(quat.shape[0]), out)
         _check(self._ctx, rc)
         return np.array(out[:])
+
+    def energy_static(self, quat, vel, angmom, shape_id, force, out):
+        """dem_energy_static: `out` is a DEVICE float64 tensor of 3 entries; asynchronous, allocates nothing."""
+        torch = self.torch
+        rc = lib().dem_energy_static(self._ctx, _dev(quat, self.dtype), _dev(vel, self.dtype), _dev(angmom, self.dtype),
+                                     _dev(shape_id, torch.int32), _dev(force, self.dtype), C.c_int(quat.shape[0]),
+                                     _dev(out, torch.float64))
+        _check(self._ctx, rc)
 
     # ---- host-buffer forms ---------------------------------------------------------------------------------------------
     def _hostarr(self, a, name, width=4):
