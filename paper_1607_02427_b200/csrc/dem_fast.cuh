@@ -148,23 +148,26 @@ static __device__ __noinline__ unsigned drain_terms(const FastShared* fs, unsign
         scnt[1] += nd;
         scnt[2] += np;
     }
-    unsigned act = __ballot_sync(full, loc.nactive != 0u);
-    unsigned touched = 0u;  // bit h: this lane's owner slot lane + 32 h received a contribution
-    while (act) {
-        const int s = __ffs(act) - 1;
-        act &= act - 1;
-        const int ow = __shfl_sync(full, owner, s);
-        const float fx = __shfl_sync(full, loc.F[0], s), fy = __shfl_sync(full, loc.F[1], s),
-                    fz = __shfl_sync(full, loc.F[2], s), tx = __shfl_sync(full, loc.T[0], s),
-                    ty = __shfl_sync(full, loc.T[1], s), tz = __shfl_sync(full, loc.T[2], s),
-                    uu = __shfl_sync(full, loc.u, s);
-        if (lane == (ow & 31)) {  // owner slots ow and ow + 32 (64-pair tiles) belong to the same lane
-            sacc[0 * nown + ow] += fx; sacc[1 * nown + ow] += fy; sacc[2 * nown + ow] += fz;
-            sacc[3 * nown + ow] += tx; sacc[4 * nown + ow] += ty; sacc[5 * nown + ow] += tz;
-            sacc[6 * nown + ow] += uu;
-            touched |= 1u << (ow >> 5);
+    // Add the lanes' results to their owners' accumulators.  Lanes with different owners write different shared-memory
+    // words, so they go together; lanes with the same owner take turns in lane order (round r: the lane that is the
+    // r-th of its owner's lanes), which is the order a serial walk over the lanes would give: the sums do not depend on
+    // scheduling, bit for bit.
+    const bool actl = loc.nactive != 0u;
+    const unsigned peers = __match_any_sync(full, actl ? owner : 64 + lane);
+    const int rank = __popc(peers & ((1u << lane) - 1u));
+    const int rounds = (int)__reduce_max_sync(full, actl ? (unsigned)rank + 1u : 0u);
+    for (int r = 0; r < rounds; ++r) {
+        if (actl && rank == r) {
+            sacc[0 * nown + owner] += loc.F[0]; sacc[1 * nown + owner] += loc.F[1]; sacc[2 * nown + owner] += loc.F[2];
+            sacc[3 * nown + owner] += loc.T[0]; sacc[4 * nown + owner] += loc.T[1]; sacc[5 * nown + owner] += loc.T[2];
+            sacc[6 * nown + owner] += loc.u;
         }
+        __syncwarp();
     }
+    // bit h of the result: this lane's owner slot lane + 32 h received a contribution
+    const unsigned w0 = __reduce_or_sync(full, actl && owner < 32 ? 1u << owner : 0u);
+    const unsigned w1 = nown > 32 ? __reduce_or_sync(full, actl && owner >= 32 ? 1u << (owner - 32) : 0u) : 0u;
+    const unsigned touched = ((w0 >> lane) & 1u) | (((w1 >> lane) & 1u) << 1);
     __syncwarp();
     return touched;
 }
@@ -984,6 +987,7 @@ __device__ __forceinline__ void sweep_items(WarpCtx& w, CullCtx& cc, const Shape
             for (int k0 = 0; k0 < A.ne; k0 += 32) {
                 const int k1 = min(k0 + 32, A.ne);
                 unsigned mask = 0u;
+#pragma unroll 1
                 for (int k = k0; k < k1; ++k)
                     mask = push_sign(mask, ee_eval(A.E[2 * k], A.E[2 * k + 1], np2x, np2y, np2z, d2x, d2y, d2z, g, a0.w,
                                                    b0.w, nrc2));
@@ -1067,7 +1071,10 @@ __device__ __forceinline__ void write_items(CullCtx& cc, unsigned mask, int owne
 // tables) instead of one behind every emit site (the two owner slots' emits interleave: faster for small shapes).
 // NOOVF: every item of a tile's phase fits the list (64 pairs x outer features <= DEM_IQCAP), so that the emit sites
 // need no sweep of their own: three sweep sites in all (the instruction cache holds them).
-template <int MINB, bool SAME, bool ONESITE, bool NOOVF>
+// PRE (variants with emit sites only): the survivor masks come from k_pose_cull (a.cmask) / are tested here -- one
+// kernel per case, because each case has sweep sites of its own and the thermalised kernel waits for instruction
+// fetches a third of the time when it carries both.
+template <int MINB, bool SAME, bool ONESITE, bool NOOVF, bool PRE>
 __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a) {
     // a warp tile is 64 pairs (two per lane: owner slots lane and lane + 32), so that the item passes run fuller
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -1248,7 +1255,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
                 }
             }
         } else
-        if (a.cmask) {
+        if constexpr (PRE) {
             // the cull tests were done by k_pose_cull: one mask word per 32 outer features (slices == 1 on this path)
             const unsigned* cm = a.cmask + cbase + lane;
             for (int wd = 0; wd < a.mw_e; ++wd) {

@@ -15,13 +15,15 @@ cudaError_t launch_pair_cull(bool same_shape, int grid, int threads, size_t smem
     // ... and large tables also take the variant with one sweep site per phase (6 k instead of 28 k instructions: config 5
     // 0.203 -> 0.178 ms per culled step; config 4 would lose 7 % to it)
     const bool small = a.sa.len + a.sb.len <= 512;
-    void (*kern)(const PairArgs<float>) =
-        small ? (same_shape ? k_pair_cull<4, true, false, false> : k_pair_cull<4, false, false, false>)
-              : (same_shape ? k_pair_cull<3, true, true, false> : k_pair_cull<3, false, true, false>);
-    const bool fits = a.slices == 1 && 64 * std::max(a.sb.ne, a.sa.nv + a.sb.nv) <= 1024;
-    // small shapes whose items always fit the list (octahedra, cubes, tetrahedra): no sweep behind the emit sites,
-    // 12 k instead of 28 k instructions (cfg4: 51.0 -> 50.4 us from the lattice, 127.0 -> 125.9 thermalised)
-    if (small && fits) kern = same_shape ? k_pair_cull<4, true, false, true> : k_pair_cull<4, false, false, true>;
+    const bool pre = a.cmask != nullptr;  // survivor masks from k_pose_cull (never for sliced pairs)
+    // small shapes whose items always fit the list (octahedra, cubes, tetrahedra; their masks always fit k_pose_cull too):
+    // no sweep behind the emit sites
+    const bool fits = pre && a.slices == 1 && 64 * std::max(a.sb.ne, a.sa.nv + a.sb.nv) <= 1024;
+    void (*kern)(const PairArgs<float>);
+    if (!small) kern = same_shape ? k_pair_cull<3, true, true, false, false> : k_pair_cull<3, false, true, false, false>;
+    else if (fits) kern = same_shape ? k_pair_cull<4, true, false, true, true> : k_pair_cull<4, false, false, true, true>;
+    else if (pre) kern = same_shape ? k_pair_cull<4, true, false, false, true> : k_pair_cull<4, false, false, false, true>;
+    else kern = same_shape ? k_pair_cull<4, true, false, false, false> : k_pair_cull<4, false, false, false, false>;
     if (smem > 48 * 1024) {
         const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
