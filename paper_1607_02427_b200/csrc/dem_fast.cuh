@@ -1087,6 +1087,52 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     unsigned* items = reinterpret_cast<unsigned*>(stage_pidx + 4 * 64);     // 4 warps x DEM_IQCAP
     f4* sm = reinterpret_cast<f4*>(items + 4 * DEM_IQCAP);
     const bool same = SAME;
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // The kernel starts with a chain of dependent global loads (work-list length, pose records, masks) beside the staging
+    // of the tables: everything whose address is known is asked for at once.  For unsliced pairs the warp's first tile
+    // sits at a known place of the work list, so its records are fetched before the list's length has arrived (inside
+    // the list's allocation in any case; a tile beyond the length is dropped afterwards).
+    const int count = *a.count;  // a multiple of 64 (k_pose pads its block slices)
+    const size_t plane = a.plane;
+    f4* spose = stage_pose + warp * (3 * 64);
+    int* spidx = stage_pidx + warp * 64;
+    unsigned pm_e[2] = {0u, 0u}, pm_vj[2] = {0u, 0u}, pm_vi[2] = {0u, 0u};
+    auto stage_tile = [&](int cbase_) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int own = lane + 32 * h, c_ = cbase_ + own;
+#pragma unroll
+            for (int k = 0; k < 3; ++k)  // R and t; R_i and d (planes 3-5) are fetched only by pairs that contribute
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
+                                 spose + k * 64 + own)), "l"(a.pose + k * plane + c_));
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(spidx + own)),
+                         "l"(a.pidx + c_));
+        }
+        asm volatile("cp.async.commit_group;");
+    };
+    // small shapes (one mask word per feature kind): the masks of k_pose_cull are asked for while the pose records are
+    // on their way, instead of one dependent load per emit site
+    auto load_masks = [&](int cbase_) {
+        if constexpr (PRE && NOOVF) {
+            const unsigned* cm = a.cmask + cbase_ + lane;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                if (a.mw_e) pm_e[h] = __ldg(cm + 32 * h);
+                if (a.mw_vj) pm_vj[h] = __ldg(cm + (size_t)a.mw_e * plane + 32 * h);
+                if (a.mw_vi) pm_vi[h] = __ldg(cm + (size_t)(a.mw_e + a.mw_vj) * plane + 32 * h);
+            }
+        }
+    };
+    bool spec = false;
+    if constexpr (PRE && NOOVF) {
+        const size_t c0 = ((size_t)blockIdx.x * 4 + warp) * 64;
+        if (c0 + 64 <= plane) {
+            spec = true;
+            stage_tile((int)c0);
+            load_masks((int)c0);
+        }
+    }
     for (int k = threadIdx.x; k < a.sa.len; k += blockDim.x) sm[k] = a.table[a.sa.off + k];
     if (!same)
         for (int k = threadIdx.x; k < a.sb.len; k += blockDim.x) sm[a.sa.len + k] = a.table[a.sb.off + k];
@@ -1104,8 +1150,6 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     if (threadIdx.x < 16) scnt_all[threadIdx.x] = 0u;
     __syncthreads();
 
-    const unsigned full = 0xffffffffu;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpCtx w;
     w.fs = fs;
     w.q = queue + warp * DEM_QCAP;
@@ -1119,27 +1163,16 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     cc.iqn = 0;
     cc.swept_ee = cc.swept_vf = cc.swept_vfe = 0u;
     const float nrc2 = -a.rc2_search;
-    const int count = *a.count;  // a multiple of 64 (k_pose pads its block slices)
     const long long n_wtiles = (long long)(count >> 6) * a.slices;
-    const size_t plane = a.plane;
-    f4* spose = stage_pose + warp * (3 * 64);
-    int* spidx = stage_pidx + warp * 64;
     w.sp = spose;
     for (long long wt = (long long)blockIdx.x * 4 + warp; wt < n_wtiles; wt += (long long)gridDim.x * 4) {
         const int slice = (int)(wt / (count >> 6)), cbase = (int)(wt - (long long)slice * (count >> 6)) * 64;
         __syncwarp();  // the previous tile's readers of the staged poses are done
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int own = lane + 32 * h, c_ = cbase + own;
-            DEM_ASSERT(c_ >= 0 && c_ < count && (size_t)count <= plane);
-#pragma unroll
-            for (int k = 0; k < 3; ++k)  // R and t; R_i and d (planes 3-5) are fetched only by pairs that contribute
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
-                                 spose + k * 64 + own)), "l"(a.pose + k * plane + c_));
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(spidx + own)),
-                         "l"(a.pidx + c_));
+        if (!spec) {
+            stage_tile(cbase);
+            load_masks(cbase);
         }
-        asm volatile("cp.async.commit_group;");
+        spec = false;
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncwarp();
         bool valid[2];
@@ -1255,7 +1288,27 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
                 }
             }
         } else
-        if constexpr (PRE) {
+        if constexpr (PRE && NOOVF) {
+            // masks preloaded above; every item of a phase fits the list
+#pragma unroll
+            for (int h = 0; h < 2; ++h) DEM_EMIT(PH_EE, valid[h] ? pm_e[h] : 0u, lane + 32 * h, 0, 0u);
+            sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
+            if constexpr (SAME) {
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    DEM_EMIT(PH_VF_BOTH, valid[h] ? pm_vj[h] : 0u, lane + 32 * h, 0, 0u);
+                    DEM_EMIT(PH_VF_BOTH, valid[h] ? pm_vi[h] : 0u, lane + 32 * h, 0, 0x8000u);
+                }
+                sweep_items<PH_VF_BOTH>(w, cc, A, B, a.sa, a.sb, nrc2);
+            } else {
+#pragma unroll
+                for (int h = 0; h < 2; ++h) DEM_EMIT(PH_VF_OWN, valid[h] ? pm_vj[h] : 0u, lane + 32 * h, 0, 0u);
+                sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
+#pragma unroll
+                for (int h = 0; h < 2; ++h) DEM_EMIT(PH_VF_OTHER, valid[h] ? pm_vi[h] : 0u, lane + 32 * h, 0, 0u);
+                sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
+            }
+        } else if constexpr (PRE) {
             // the cull tests were done by k_pose_cull: one mask word per 32 outer features (slices == 1 on this path)
             const unsigned* cm = a.cmask + cbase + lane;
             for (int wd = 0; wd < a.mw_e; ++wd) {
@@ -1393,6 +1446,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
             rec[0] = r0; rec[1] = r1; rec[2] = r2;
         }
     }
+    if (spec) asm volatile("cp.async.wait_all;" ::: "memory");  // a first tile fetched ahead that lay beyond the list
     const unsigned s_ee = __reduce_add_sync(0xffffffffu, cc.swept_ee), s_vf = __reduce_add_sync(0xffffffffu, cc.swept_vf),
                    s_vfe = __reduce_add_sync(0xffffffffu, cc.swept_vfe);
     if (lane == 0) {  // inside dem_step a.counters is null: no global atomic at all (see k_pair_fast)

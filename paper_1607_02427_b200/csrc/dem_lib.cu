@@ -244,9 +244,13 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
         // Handed back the very arrays the last call returned (same pointers, same contents)?  Then the internal double
         // state, the neighbour list and the forces are still those of that state: go on from them.
         dem_ctx::Resume& rs = ctx->resume;
-        if (rs.valid && !ctx->ev_copy_pending && rs.pos == pos && rs.quat == quat && rs.vel == vel && rs.ang == ang &&
+        if (rs.valid && rs.pos == pos && rs.quat == quat && rs.vel == vel && rs.ang == ang &&
             rs.sid == sid && rs.N == N && rs.skin == skin && rs.box[0] == box[0] && rs.box[1] == box[1] &&
             rs.box[2] == box[2] && ctx->have_list && ctx->N == N) {
+            if (ctx->ev_copy_pending) {  // dem_step_host: the comparison reads all four arrays, so wait for the side copy
+                CU(cudaStreamWaitEvent(st, ctx->ev_copy, 0));
+                ctx->ev_copy_pending = false;
+            }
             int* differ = ctx->flags.as<int>() + 12;
             CU(cudaMemsetAsync(differ, 0, sizeof(int), st));
             k_same_state<<<nblk(N, B), B, 0, st>>>(N, static_cast<const f4*>(pos), static_cast<const f4*>(quat),

@@ -216,6 +216,43 @@ def test_step_host_matches_device(pkg):
     dem.close()
 
 
+@pytest.mark.parametrize("kind,cells", [("cubes", 4), ("squares", 8)])
+def test_step_host_call_after_call(pkg, kind, cells):
+    """dem_step_host called step after step on the same host arrays goes on from the state the library kept (it checks
+    on the device that the uploaded arrays are the ones it returned) -- the same trajectory as one device-resident run;
+    after the caller edits the velocities in between it must start afresh from the edited state."""
+    import torch
+
+    st = round_state(di.dense_state(kind, cells), "f32")
+    dt = 1e-3
+    dem, _ = pkg.from_state(st, "f32")
+    h = {k: torch.tensor(st[k], dtype=torch.float32).pin_memory() for k in ("pos", "quat", "vel", "angmom")}
+    sid = torch.tensor(st["shape_id"], dtype=torch.int32).pin_memory()
+    hf = torch.empty((st["N"], 4), dtype=torch.float32).pin_memory()
+    l0 = dem.launch_count()
+    dem.step_host(h["pos"], h["quat"], h["vel"], h["angmom"], sid, st["box"], dt, 1, 0.3, hf, None)
+    first = dem.launch_count() - l0
+    for _ in range(11):
+        l0 = dem.launch_count()
+        dem.step_host(h["pos"], h["quat"], h["vel"], h["angmom"], sid, st["box"], dt, 1, 0.3, hf, None)
+        later = dem.launch_count() - l0
+    assert later < first                                   # no list build, no evaluation of the incoming state
+    dev = _run(pkg, st, "f32", dt, 12, skin=0.3)
+    for k in ("pos", "quat", "vel", "angmom"):
+        assert np.array_equal(h[k].numpy().astype(np.float64), dev[k]), k
+    assert np.array_equal(hf.numpy().astype(np.float64), dev["force"])
+    # edited between calls: the next call equals a fresh run from the edited state
+    h["vel"].mul_(0.5)
+    st2 = dict(st)
+    for k in ("pos", "quat", "vel", "angmom"):
+        st2[k] = h[k].numpy().astype(np.float64).copy()
+    dem.step_host(h["pos"], h["quat"], h["vel"], h["angmom"], sid, st["box"], dt, 3, 0.3, hf, None)
+    dem.close()
+    dev2 = _run(pkg, st2, "f32", dt, 3, skin=0.3)
+    for k in ("pos", "quat", "vel", "angmom"):
+        assert np.array_equal(h[k].numpy().astype(np.float64), dev2[k]), k
+
+
 def _lsq_drift(steps, e_per_particle):
     """Least-squares slope of E/N against the step number, times 10^4 steps: PAPER.md:85 reports the long-term drift as
     a rate ((E(t) - E(0))/N per unit time); north_star's bar is that rate over 10^4 steps."""
