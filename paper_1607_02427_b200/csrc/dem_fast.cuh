@@ -213,6 +213,26 @@ __device__ __forceinline__ void push_one(WarpCtx& w, int phase_a, int phase_b, u
     }
 }
 
+// the same for ONE inner feature per lane (k may differ from lane to lane; `have` = this lane flagged a candidate)
+__device__ __forceinline__ void push_lane(WarpCtx& w, int phase_a, int phase_b, bool have, int k, int wa, int oa, bool ok_a,
+                                          int wb, int ob, bool ok_b) {
+    const unsigned full = 0xffffffffu;
+    const unsigned lt = (1u << w.lane) - 1u;
+    const bool ha = have && ok_a, hb = have && ok_b;
+    const unsigned ba = __ballot_sync(full, ha), bb = __ballot_sync(full, hb);
+    if ((ba | bb) == 0u) return;
+    const int na = __popc(ba);
+    DEM_ASSERT(w.qn >= 0 && w.qn + na + __popc(bb) <= DEM_QCAP);
+    if (ha) w.q[w.qn + __popc(ba & lt)] = q_entry(wa, phase_a, oa, k);
+    if (hb) w.q[w.qn + na + __popc(bb & lt)] = q_entry(wb, phase_b, ob, k);
+    w.qn += na + __popc(bb);
+    __syncwarp();
+    while (w.qn >= 32) {
+        w.touched |= drain_terms(w.fs, w.q, w.sacc, w.scnt, 32, w.qn, w.sp, w.nown);
+        w.qn -= 32;
+    }
+}
+
 // tile form: lane-owned outer features o0 + 2 tau and o0 + 2 tau + 1
 template <int T>
 __device__ __forceinline__ void push_and_drain(WarpCtx& w, int phase, const unsigned (&mask)[T], int n, int k0, int o0,
@@ -610,9 +630,11 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
     ShapeView<float> A, B;
     A.nv = a.sa.nv; A.ne = a.sa.ne; A.nf = a.sa.nf;
     A.V = sm; A.E = A.V + A.nv; A.F = A.E + 2 * A.ne; A.FE = A.F + 4 * A.nf; A.OE = A.FE + 2 * a.sa.nfe;
+    A.EB = A.OE + 2 * A.ne; A.FB = A.EB + A.ne;
     B.nv = a.sb.nv; B.ne = a.sb.ne; B.nf = a.sb.nf;
     B.V = same ? sm : sm + a.sa.len; B.E = B.V + B.nv; B.F = B.E + 2 * B.ne; B.FE = B.F + 4 * B.nf;
     B.OE = B.FE + 2 * a.sb.nfe;
+    B.EB = B.OE + 2 * B.ne; B.FB = B.EB + B.ne;
     if (threadIdx.x == 0) {
         fs->A = A;
         fs->B = B;
@@ -956,7 +978,15 @@ __device__ __forceinline__ void load_pose(const f4* sp, int nown, int owner, flo
 }
 
 // sweep the queued items of one phase, 64 per pass (two per lane)
-template <int PHASE>
+// TWOLEVEL (large shapes): an item is first tested against the bounding spheres of the inner features (edges: midpoint
+// and half length; faces: centre and radius; one packed test of ~10 instructions per inner feature for the lane's two
+// items), and only the inner features whose sphere comes within the candidate cutoff of the item's own bounding sphere
+// get the nearest-point search -- lane by lane, since the survivors differ between lanes (shape-local
+// culling).  Measured on config 5 (truncated icosahedra: 90 edges, 32 faces; fork-to-join time of the three classes,
+// from the lattice / thermalised): one level 115 / 83 us; faces two-level 107.6 / 81.6 (the choice); edges too
+// 104.3 / 86.8 -- an edge item's sphere still meets ~9 of the partner's edge spheres, the union over a lane's two items
+// and the maximum over the warp's lanes make 21 searches per pass where the uniform sweep makes 90 cheaper ones.
+template <int PHASE, bool TWOLEVEL = false>
 __device__ __forceinline__ void sweep_items(WarpCtx& w, CullCtx& cc, const ShapeView<float>& A, const ShapeView<float>& B,
                                             const ShapeDev& sda, const ShapeDev& sdb, float nrc2) {
     const unsigned full = 0xffffffffu;
@@ -980,20 +1010,52 @@ __device__ __forceinline__ void sweep_items(WarpCtx& w, CullCtx& cc, const Shape
             vertex_to_i<float>(a0.x, a0.y, a0.z, Ra, ta, pa);
             vertex_to_i<float>(b0.x, b0.y, b0.z, Rb, tb, pb);
             const u64 np2x = pk(-pa[0], -pb[0]), np2y = pk(-pa[1], -pb[1]), np2z = pk(-pa[2], -pb[2]);
-            const u64 d2x = pk(Ra[0] * a1.x + Ra[1] * a1.y + Ra[2] * a1.z, Rb[0] * b1.x + Rb[1] * b1.y + Rb[2] * b1.z);
-            const u64 d2y = pk(Ra[3] * a1.x + Ra[4] * a1.y + Ra[5] * a1.z, Rb[3] * b1.x + Rb[4] * b1.y + Rb[5] * b1.z);
-            const u64 d2z = pk(Ra[6] * a1.x + Ra[7] * a1.y + Ra[8] * a1.z, Rb[6] * b1.x + Rb[7] * b1.y + Rb[8] * b1.z);
+            const float dax = Ra[0] * a1.x + Ra[1] * a1.y + Ra[2] * a1.z, dbx = Rb[0] * b1.x + Rb[1] * b1.y + Rb[2] * b1.z;
+            const float day = Ra[3] * a1.x + Ra[4] * a1.y + Ra[5] * a1.z, dby = Rb[3] * b1.x + Rb[4] * b1.y + Rb[5] * b1.z;
+            const float daz = Ra[6] * a1.x + Ra[7] * a1.y + Ra[8] * a1.z, dbz = Rb[6] * b1.x + Rb[7] * b1.y + Rb[8] * b1.z;
+            const u64 d2x = pk(dax, dbx), d2y = pk(day, dby), d2z = pk(daz, dbz);
             const u64 g = fma2(d2z, np2z, fma2(d2y, np2y, mul2(d2x, np2x)));
-            for (int k0 = 0; k0 < A.ne; k0 += 32) {
-                const int k1 = min(k0 + 32, A.ne);
-                unsigned mask = 0u;
+            if constexpr (TWOLEVEL) {
+                const float rcs = sqrtf(-nrc2), hla = 0.5f * a0.w, hlb = 0.5f * b0.w;
+                // minus the midpoints of the two outer edges; their radii with the candidate cutoff added
+                const u64 nmx = pk(-(pa[0] + hla * dax), -(pb[0] + hlb * dbx)), nmy = pk(-(pa[1] + hla * day), -(pb[1] + hlb * dby)),
+                          nmz = pk(-(pa[2] + hla * daz), -(pb[2] + hlb * dbz));
+                const u64 rho = pk(hla + rcs, hlb + rcs);
+                for (int k0 = 0; k0 < A.ne; k0 += 32) {
+                    const int k1 = min(k0 + 32, A.ne);
+                    unsigned ma = 0u, mb = 0u;
+                    for (int k = k0; k < k1; ++k) {
+                        const f4 eb = A.EB[k];
+                        const u64 dx = add2(bc(eb.x), nmx), dy = add2(bc(eb.y), nmy), dz = add2(bc(eb.z), nmz);
+                        const u64 lim = add2(bc(eb.w), rho);
+                        float lo, hi;
+                        upk(fma2(neg2(lim), lim, fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)))), lo, hi);
+                        ma = push_sign(ma, lo);
+                        mb = push_sign(mb, hi);
+                    }
+                    unsigned mu = ma | mb;  // inner edges that one of the lane's two items has to search
+                    while (__any_sync(full, mu != 0u)) {
+                        const bool have = mu != 0u;
+                        const int bit = have ? 31 - __clz((int)mu) : 0;
+                        const int k = have ? k0 + (k1 - k0 - 1 - bit) : k0;
+                        mu &= ~(1u << bit);
+                        const float v = ee_eval(A.E[2 * k], A.E[2 * k + 1], np2x, np2y, np2z, d2x, d2y, d2z, g, a0.w, b0.w, nrc2);
+                        push_lane(w, PHASE, PHASE, have && v < 0.f, k, wa, oa, ok_a, wb, ob, ok_b);
+                        if (have) cc.swept_ee += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0));
+                    }
+                }
+            } else {
+                for (int k0 = 0; k0 < A.ne; k0 += 32) {
+                    const int k1 = min(k0 + 32, A.ne);
+                    unsigned mask = 0u;
 #pragma unroll 1
-                for (int k = k0; k < k1; ++k)
-                    mask = push_sign(mask, ee_eval(A.E[2 * k], A.E[2 * k + 1], np2x, np2y, np2z, d2x, d2y, d2z, g, a0.w,
-                                                   b0.w, nrc2));
-                if (__any_sync(full, mask != 0u)) push_one(w, PHASE, PHASE, mask, k1 - k0, k0, wa, oa, ok_a, wb, ob, ok_b);
+                    for (int k = k0; k < k1; ++k)
+                        mask = push_sign(mask, ee_eval(A.E[2 * k], A.E[2 * k + 1], np2x, np2y, np2z, d2x, d2y, d2z, g, a0.w,
+                                                       b0.w, nrc2));
+                    if (__any_sync(full, mask != 0u)) push_one(w, PHASE, PHASE, mask, k1 - k0, k0, wa, oa, ok_a, wb, ob, ok_b);
+                }
+                cc.swept_ee += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)A.ne;
             }
-            cc.swept_ee += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)A.ne;
         } else {
             // vertex-face items.  PH_VF_BOTH (one-shape classes: the faces of i and of j are the same table): bit 15 of
             // an item says which sum it belongs to, so both sums share one pass
@@ -1014,16 +1076,51 @@ __device__ __forceinline__ void sweep_items(WarpCtx& w, CullCtx& cc, const Shape
             else
                 vertex_to_i<float>(vb.x, vb.y, vb.z, Rb, tb, pb);
             u64 px[1] = {pk(pa[0], pb[0])}, py[1] = {pk(pa[1], pb[1])}, pz[1] = {pk(pa[2], pb[2])};
-            for (int f0 = 0; f0 < In.nf; f0 += 32) {
-                const int f1 = min(f0 + 32, In.nf);
-                unsigned mask[1] = {0u};
-                sweep_faces<1>(In, sd, f0, f1, px, py, pz, nrc2, mask);
-                if (__any_sync(full, mask[0] != 0u))
-                    push_one(w, oth_a ? PH_VF_OTHER : PH_VF_OWN, oth_b ? PH_VF_OTHER : PH_VF_OWN, mask[0], f1 - f0, f0, wa,
-                             va_i, ok_a, wb, vb_i, ok_b);
+            if constexpr (TWOLEVEL) {
+                const float rcs = sqrtf(-nrc2);
+                const u64 npx = neg2(px[0]), npy = neg2(py[0]), npz = neg2(pz[0]);
+                for (int f0 = 0; f0 < In.nf; f0 += 32) {
+                    const int f1 = min(f0 + 32, In.nf);
+                    unsigned ma = 0u, mb = 0u;
+                    for (int f = f0; f < f1; ++f) {
+                        const f4 fb = In.FB[f];
+                        const u64 dx = add2(bc(fb.x), npx), dy = add2(bc(fb.y), npy), dz = add2(bc(fb.z), npz);
+                        const float l = fb.w + rcs;
+                        float lo, hi;
+                        upk(fma2(dz, dz, fma2(dy, dy, fma2(dx, dx, bc(-l * l)))), lo, hi);
+                        ma = push_sign(ma, lo);
+                        mb = push_sign(mb, hi);
+                    }
+                    unsigned mu = ma | mb;
+                    while (__any_sync(full, mu != 0u)) {
+                        const bool have = mu != 0u;
+                        const int bit = have ? 31 - __clz((int)mu) : 0;
+                        const int f = have ? f0 + (f1 - f0 - 1 - bit) : f0;
+                        mu &= ~(1u << bit);
+                        const f4 f3 = In.F[4 * f + 3];
+                        unsigned m1[1] = {0u};
+                        face_eval_any<1>(In.F + 4 * f, In.FE + 2 * (int)f3.x, (int)f3.y, px, py, pz, nrc2, m1);
+                        push_lane(w, oth_a ? PH_VF_OTHER : PH_VF_OWN, oth_b ? PH_VF_OTHER : PH_VF_OWN, have && (m1[0] & 1u), f,
+                                  wa, va_i, ok_a, wb, vb_i, ok_b);
+                        if (have) {
+                            const unsigned n2 = (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0));
+                            cc.swept_vf += n2;
+                            cc.swept_vfe += n2 * (unsigned)f3.y;
+                        }
+                    }
+                }
+            } else {
+                for (int f0 = 0; f0 < In.nf; f0 += 32) {
+                    const int f1 = min(f0 + 32, In.nf);
+                    unsigned mask[1] = {0u};
+                    sweep_faces<1>(In, sd, f0, f1, px, py, pz, nrc2, mask);
+                    if (__any_sync(full, mask[0] != 0u))
+                        push_one(w, oth_a ? PH_VF_OTHER : PH_VF_OWN, oth_b ? PH_VF_OTHER : PH_VF_OWN, mask[0], f1 - f0, f0, wa,
+                                 va_i, ok_a, wb, vb_i, ok_b);
+                }
+                cc.swept_vf += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)In.nf;
+                cc.swept_vfe += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)sd.nfe;
             }
-            cc.swept_vf += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)In.nf;
-            cc.swept_vfe += (unsigned)((ok_a ? 1 : 0) + (ok_b ? 1 : 0)) * (unsigned)sd.nfe;
         }
     }
     cc.iqn = 0;
@@ -1139,9 +1236,11 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     ShapeView<float> A, B;
     A.nv = a.sa.nv; A.ne = a.sa.ne; A.nf = a.sa.nf;
     A.V = sm; A.E = A.V + A.nv; A.F = A.E + 2 * A.ne; A.FE = A.F + 4 * A.nf; A.OE = A.FE + 2 * a.sa.nfe;
+    A.EB = A.OE + 2 * A.ne; A.FB = A.EB + A.ne;
     B.nv = a.sb.nv; B.ne = a.sb.ne; B.nf = a.sb.nf;
     B.V = same ? sm : sm + a.sa.len; B.E = B.V + B.nv; B.F = B.E + 2 * B.ne; B.FE = B.F + 4 * B.nf;
     B.OE = B.FE + 2 * a.sb.nfe;
+    B.EB = B.OE + 2 * B.ne; B.FB = B.EB + B.ne;
     if (threadIdx.x == 0) {
         fs->A = A;
         fs->B = B;
@@ -1237,7 +1336,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
                             : edge_word(l0, min(32, e_hi - l0), h ? tp[1][0] : tp[0][0], h ? tp[1][1] : tp[0][1], h ? tp[1][2] : tp[0][2]);
                 int off_;
                 const int tot_ = count_items(w, m, off_);
-                if (last || cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH_EE>(w, cc, A, B, a.sa, a.sb, nrc2);
+                if (last || cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH_EE, false>(w, cc, A, B, a.sa, a.sb, nrc2);
                 if (!last) write_items(cc, m, lane + 32 * h, l0, 0u, off_, tot_);
             }
             auto vf_mask = [&](bool other, int wd, int h) -> unsigned {
@@ -1264,7 +1363,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
                     const unsigned m = last ? 0u : vf_mask(other, wd, h);
                     int off_;
                     const int tot_ = count_items(w, m, off_);
-                    if (last || cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH_VF_BOTH>(w, cc, A, B, a.sa, a.sb, nrc2);
+                    if (last || cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH_VF_BOTH, true>(w, cc, A, B, a.sa, a.sb, nrc2);
                     if (!last) write_items(cc, m, lane + 32 * h, (other ? vi_lo : vj_lo) + 32 * wd, other ? 0x8000u : 0u, off_, tot_);
                 }
             } else {
@@ -1274,7 +1373,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
                     const unsigned m = last ? 0u : vf_mask(false, wd, h);
                     int off_;
                     const int tot_ = count_items(w, m, off_);
-                    if (last || cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH_VF_OWN>(w, cc, A, B, a.sa, a.sb, nrc2);
+                    if (last || cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH_VF_OWN, true>(w, cc, A, B, a.sa, a.sb, nrc2);
                     if (!last) write_items(cc, m, lane + 32 * h, vj_lo + 32 * wd, 0u, off_, tot_);
                 }
                 for (int u = 0; u <= 2 * nw_vi; ++u) {
@@ -1283,7 +1382,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
                     const unsigned m = last ? 0u : vf_mask(true, wd, h);
                     int off_;
                     const int tot_ = count_items(w, m, off_);
-                    if (last || cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH_VF_OTHER>(w, cc, A, B, a.sa, a.sb, nrc2);
+                    if (last || cc.iqn + tot_ > DEM_IQCAP) sweep_items<PH_VF_OTHER, true>(w, cc, A, B, a.sa, a.sb, nrc2);
                     if (!last) write_items(cc, m, lane + 32 * h, vi_lo + 32 * wd, 0u, off_, tot_);
                 }
             }

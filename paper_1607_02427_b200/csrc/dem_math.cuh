@@ -64,6 +64,7 @@ DEM_HD double rcp(double x) { return 1.0 / x; }
 //   F [4 nf]    [4f] = (uhat, -uhat.o) [4f+1] = (vhat, -vhat.o) [4f+2] = (nhat, -nhat.o) [4f+3] = (first FE, count, 0, 0)
 //   FE[2 nfe]   face boundary edges in the face's (uhat, vhat) coordinates, CCW about nhat: same layout as 2D edges
 //   OE[2 ne]    3D only: [2k] = (a.xyz, |e|)  [2k+1] = (e/|e|, 0): the edges as the search kernel's outer features
+//   EB[ne]      3D only: (midpoint, half length) of every edge;   FB[nf]  3D only: (centre, radius) of a sphere around every face
 template <typename real> struct ShapeView {
     typedef typename vec4<real>::type real4;
     int nv, ne, nf;
@@ -72,6 +73,8 @@ template <typename real> struct ShapeView {
     const real4* F;
     const real4* FE;
     const real4* OE;
+    const real4* EB;  // 3D: bounding spheres of the edges (midpoint, half length) ...
+    const real4* FB;  // ... and of the faces (centre, radius): OE + 2 ne, EB + ne
 };
 
 template <typename real> struct PairAcc {

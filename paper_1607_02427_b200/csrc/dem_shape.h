@@ -23,11 +23,12 @@ struct HostShape {
     std::vector<int> face_off;   // nf + 1
     std::vector<int> face_verts;
     double rounding = 0, mass = 1, inertia[3] = {1, 1, 1}, circumradius = 0;
-    // flattened table in double, in units of 4 doubles: V (nv) | E (2 ne) | F (4 nf) | FE (2 nfe) | OE (2 ne, 3D only)
+    // flattened table in double, in units of 4 doubles: V (nv) | E (2 ne) | F (4 nf) | FE (2 nfe) | OE (2 ne) | EB (ne) | FB (nf)
+    // (OE, EB, FB in 3D only)
     std::vector<double> table;
     std::vector<std::pair<int, int>> face_groups;  // runs of faces with the same number of boundary edges
     double max_edge = 0;  // longest edge (bounds the search kernel's near-parallel slack)
-    int table_len4() const { return nv + 2 * ne + 4 * nf + 2 * nfe + (dim == 3 ? 2 * ne : 0); }
+    int table_len4() const { return nv + 2 * ne + 4 * nf + 2 * nfe + (dim == 3 ? 2 * ne + ne + nf : 0); }
 };
 
 inline void push4(std::vector<double>& t, double a, double b, double c, double d) {
@@ -227,6 +228,30 @@ inline std::string build_host_shape(HostShape& S, int dim, const double* verts, 
         if (dim == 3) {
             push4(T, a[0], a[1], a[2], len);
             push4(T, len > 0 ? e[0] / len : 0.0, len > 0 ? e[1] / len : 0.0, len > 0 ? e[2] / len : 0.0, 0.0);
+        }
+    }
+    if (dim == 3) {
+        // EB, FB: bounding spheres of the edges (midpoint, half length) and of the faces (centroid of the vertices, largest
+        // vertex distance), for the two-level sweeps of the culling kernel; radii rounded up so that float stays outside
+        const double up = 1.0 + 1e-6;
+        for (int k = 0; k < S.ne; ++k) {
+            const double* a = &S.verts[3 * S.edges[2 * k]];
+            const double* b = &S.verts[3 * S.edges[2 * k + 1]];
+            const double e[3] = {b[0] - a[0], b[1] - a[1], b[2] - a[2]};
+            push4(T, a[0] + 0.5 * e[0], a[1] + 0.5 * e[1], a[2] + 0.5 * e[2],
+                  0.5 * std::sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2]) * up);
+        }
+        for (int f = 0; f < nf; ++f) {
+            const int b = S.face_off[f], n = S.face_off[f + 1] - b;
+            double c[3] = {0, 0, 0}, r = 0;
+            for (int m = 0; m < n; ++m)
+                for (int a = 0; a < 3; ++a) c[a] += S.verts[3 * S.face_verts[b + m] + a] / n;
+            for (int m = 0; m < n; ++m) {
+                const double* p = &S.verts[3 * S.face_verts[b + m]];
+                r = std::max(r, std::sqrt((p[0] - c[0]) * (p[0] - c[0]) + (p[1] - c[1]) * (p[1] - c[1]) +
+                                          (p[2] - c[2]) * (p[2] - c[2])));
+            }
+            push4(T, c[0], c[1], c[2], r * up);
         }
     }
     return "";
