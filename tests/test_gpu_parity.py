@@ -134,10 +134,11 @@ def test_search_kernel_with_and_without_culling(pkg, oracle, kind, cells, slices
     assert b["counters"]["terms_swept"] >= b["counters"]["active"]
 
 
-@pytest.mark.parametrize("n", [7, 9])
+@pytest.mark.parametrize("n", [7, 9, 24])
 def test_faces_with_many_edges(pkg, oracle, n):
     """Prisms over a heptagon / nonagon: faces whose boundary-edge count has no unrolled sweep (run-time edge loop),
-    mixed with quadrilaterals in one shape, against cubes."""
+    mixed with quadrilaterals in one shape, against cubes.  The 24-gon prism's table (48 vertices, 72 edges, two
+    24-edge faces) is a large one: the culling kernel takes its one-sweep-site variant with the two-level face sweep."""
     shapes = [di.prism(n, 0.5, 0.9, 0.06), di.cube(0.8, 0.06)]
     st = di.lattice_state(3, shapes, (5, 5, 5), 1.145, seed=4, jitter=0.01, orient="small", max_angle=0.1,
                           shape_fractions=(0.6, 0.4))
