@@ -119,18 +119,38 @@ static __device__ __noinline__ unsigned drain_terms(const FastShared* fs, unsign
                    : phase == PH_VE_OWN ? (o < B.nv && k < A.ne) : (phase == PH_VE_OTHER && o < A.nv && k < B.ne));
         const PairConst<float> pc = fs->pc;
         float p[3];
-        if (phase == PH_EE) {
-            float d2[3], ee, inv_e;
-            edge_to_i<float>(B, o, R, t, p, d2, ee, inv_e);
-            term_ee<float>(A, k, p[0], p[1], p[2], d2[0], d2[1], d2[2], ee, inv_e, pc, loc);
-        } else if (phase == PH_VF_OWN) {
-            const f4 v = B.V[o];
-            vertex_to_i<float>(v.x, v.y, v.z, R, t, p);
-            term_vf_own<float>(A, k, p[0], p[1], p[2], pc, loc);
-        } else if (phase == PH_VF_OTHER) {
-            const f4 v = A.V[o];
-            vertex_to_j<float>(v.x, v.y, v.z, R, t, p);
-            term_vf_other<float>(B, k, v.x, v.y, v.z, p[0], p[1], p[2], R, pc, loc);
+        // The 3D kinds share one copy of the face routines and one of the WCA code (the kernel's code has to stay small:
+        // DESIGN.md section 10): each kind leaves ci (interaction point on i), del = c_i - c_j, r2; then one accumulate.
+        if (phase <= PH_VF_OTHER) {
+            float ci[3], del[3], r2 = 0.f;
+            bool hit, par = false;
+            if (phase == PH_EE) {
+                float d2[3], ee, inv_e;
+                edge_to_i<float>(B, o, R, t, p, d2, ee, inv_e);
+                hit = term_ee_geom<float>(A, k, p[0], p[1], p[2], d2[0], d2[1], d2[2], ee, inv_e, pc, ci, del, r2, par);
+            } else {
+                const bool own = phase == PH_VF_OWN;  // vertex of j against a face of i (i's frame) / of i against j (j's)
+                const ShapeView<float>& S = own ? A : B;
+                const f4 v = own ? B.V[o] : A.V[o];
+                if (own) vertex_to_i<float>(v.x, v.y, v.z, R, t, p);
+                else vertex_to_j<float>(v.x, v.y, v.z, R, t, p);
+                r2 = point_face_r2<float>(S, k, p[0], p[1], p[2]);
+                hit = r2 < pc.rc2;
+                if (hit) {
+                    float dx, dy, dz;  // p - c with c on the face
+                    point_face_del<float>(S, k, p[0], p[1], p[2], dx, dy, dz);
+                    if (own) {  // c_i = c, c_j = p: del = -(p - c)      (term_vf_own)
+                        ci[0] = p[0] - dx; ci[1] = p[1] - dy; ci[2] = p[2] - dz;
+                        del[0] = -dx; del[1] = -dy; del[2] = -dz;
+                    } else {    // c_i = the vertex, del = R (p' - c')      (term_vf_other)
+                        ci[0] = v.x; ci[1] = v.y; ci[2] = v.z;
+                        del[0] = R[0] * dx + R[1] * dy + R[2] * dz;
+                        del[1] = R[3] * dx + R[4] * dy + R[5] * dz;
+                        del[2] = R[6] * dx + R[7] * dy + R[8] * dz;
+                    }
+                }
+            }
+            if (hit) wca_accumulate<float>(pc, loc, ci[0], ci[1], ci[2], del[0], del[1], del[2], r2, par);
         } else if (phase == PH_VE_OWN) {
             const f4 v = B.V[o];
             vertex_to_i<float>(v.x, v.y, 0.f, R, t, p);

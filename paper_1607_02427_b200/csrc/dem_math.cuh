@@ -229,9 +229,12 @@ DEM_HD_NOINLINE bool segseg_special(real rx, real ry, real rz, real d1x, real d1
 // search flags as candidates, so both paths share the arithmetic of every contributing term.
 
 // edge (p2, d2, e = |d2|^2, inv_e) of j in i's frame against edge k of i (first sum of Eq. 1)
+// (geometry of the term: true when it is inside the cutoff; ci = the interaction point on i, del = c_i - c_j, r2 and the
+// parallel flag then hold what wca_accumulate wants.  term_ee = this + wca_accumulate; the search kernels call the two
+// halves separately so that all term kinds share one copy of the WCA code)
 template <typename real>
-DEM_HD void term_ee(const ShapeView<real>& A, int k, real p2x, real p2y, real p2z, real d2x, real d2y, real d2z, real e,
-                    real inv_e, const PairConst<real>& pc, PairAcc<real>& acc) {
+DEM_HD bool term_ee_geom(const ShapeView<real>& A, int k, real p2x, real p2y, real p2z, real d2x, real d2y, real d2z, real e,
+                         real inv_e, const PairConst<real>& pc, real* ci, real* del, real& r2_out, bool& par_out) {
     typedef typename vec4<real>::type real4;
     const real4 a0 = A.E[2 * k], a1 = A.E[2 * k + 1];
     const real rx = a0.x - p2x, ry = a0.y - p2y, rz = a0.z - p2z;  // r = p1 - p2
@@ -256,8 +259,20 @@ DEM_HD void term_ee(const ShapeView<real>& A, int k, real p2x, real p2y, real p2
     }
     const real dx = rx + s * a1.x - tt * d2x, dy = ry + s * a1.y - tt * d2y, dz = rz + s * a1.z - tt * d2z;
     const real r2 = dx * dx + dy * dy + dz * dz;
-    if (r2 < pc.rc2)
-        wca_accumulate<real>(pc, acc, a0.x + s * a1.x, a0.y + s * a1.y, a0.z + s * a1.z, dx, dy, dz, r2, par);
+    if (!(r2 < pc.rc2)) return false;
+    ci[0] = a0.x + s * a1.x; ci[1] = a0.y + s * a1.y; ci[2] = a0.z + s * a1.z;
+    del[0] = dx; del[1] = dy; del[2] = dz;
+    r2_out = r2;
+    par_out = par;
+    return true;
+}
+template <typename real>
+DEM_HD void term_ee(const ShapeView<real>& A, int k, real p2x, real p2y, real p2z, real d2x, real d2y, real d2z, real e,
+                    real inv_e, const PairConst<real>& pc, PairAcc<real>& acc) {
+    real ci[3], del[3], r2;
+    bool par;
+    if (term_ee_geom<real>(A, k, p2x, p2y, p2z, d2x, d2y, d2z, e, inv_e, pc, ci, del, r2, par))
+        wca_accumulate<real>(pc, acc, ci[0], ci[1], ci[2], del[0], del[1], del[2], r2, par);
 }
 
 // vertex p of j (in i's frame) against face f of i (third sum of Eq. 1)
