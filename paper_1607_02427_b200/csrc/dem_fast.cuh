@@ -257,10 +257,15 @@ __device__ __forceinline__ void push_lane(WarpCtx& w, int phase_a, int phase_b, 
 template <int T>
 __device__ __forceinline__ void push_and_drain(WarpCtx& w, int phase, const unsigned (&mask)[T], int n, int k0, int o0,
                                                int o_end) {
-#pragma unroll
-    for (int tau = 0; tau < T; ++tau)
-        push_one(w, phase, phase, mask[tau], n, k0, w.lane, o0 + 2 * tau, o0 + 2 * tau < o_end, w.lane, o0 + 2 * tau + 1,
+    // one copy of the queue code per call site, not one per packed pair (code size: DESIGN.md section 10); the mask of
+    // the pair is picked with selects so that the array stays in registers
+    static_assert(T <= 3, "mask select below");
+#pragma unroll 1
+    for (int tau = 0; tau < T; ++tau) {
+        const unsigned m = tau == 0 ? mask[0] : (tau == 1 || T < 3) ? mask[T > 1 ? 1 : 0] : mask[T > 2 ? 2 : 0];
+        push_one(w, phase, phase, m, n, k0, w.lane, o0 + 2 * tau, o0 + 2 * tau < o_end, w.lane, o0 + 2 * tau + 1,
                  o0 + 2 * tau + 1 < o_end);
+    }
 }
 
 // ---- search: packed nearest-point distances ---------------------------------------------------------------------------
