@@ -420,8 +420,8 @@ def main():
         nsum = int(counts_h.sum())
         if st["dim"] == 3 and us.get("pose"):
             # k_pose: pair list (8 B), positions and orientations of N particles in double (64 B each, gathered), pose
-            # records of the pairs inside the reach (96 B + 4 B index), one flag byte per pair
-            out["k_pose"] = hbm_line(us["pose"], npairs_listed * 9 + n * 64 + npairs_eval * 100)
+            # records of the pairs inside the reach (48 B R, t + 16 B work-list entry), one flag byte per pair
+            out["k_pose"] = hbm_line(us["pose"], npairs_listed * 9 + n * 64 + npairs_eval * 64)
         if us.get("reduce"):
             # k_finish: slots (4 B per listed neighbour), flags (1 B per listed neighbour), x q v L read + written, build positions
             out["k_finish"] = hbm_line(us["reduce"], nsum * 5 + n * (8 * 32 + 32 + 4))

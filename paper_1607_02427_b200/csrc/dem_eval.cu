@@ -31,8 +31,8 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
     const bool search = std::is_same<real, float>::value && !ctx->generic_kernel;
     const bool cull = search && ctx->dim == 3 && ctx->cull;
     if (search) {
-        CU(ctx->pose.reserve(sizeof(f4) * 6 * std::max<size_t>(list_base[ctx->nclass], 1)));
-        CU(ctx->pidx.reserve(sizeof(int) * std::max<size_t>(list_base[ctx->nclass], 1)));
+        CU(ctx->pose.reserve(sizeof(f4) * 3 * std::max<size_t>(list_base[ctx->nclass], 1)));
+        CU(ctx->pidx.reserve(sizeof(int4) * std::max<size_t>(list_base[ctx->nclass], 1)));
         if (cull) CU(ctx->cmask.reserve(sizeof(unsigned) * pose_cull_max_words() * std::max<size_t>(list_base[ctx->nclass], 1)));
     }
     const BoxDev bx = box_dev(ctx->dim, ctx->box);
@@ -79,6 +79,7 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
         a.pos = pos;
         a.quat = quat;
         a.box = bx;
+        a.pos_double = pos_is_double ? 1 : 0;
         const double reach = reach_of(HA, HB), sigma = HA.rounding + HB.rounding;
         a.reach2 = reach * reach;
         a.pc.rc2 = (real)(std::cbrt(2.0) * sigma * sigma);
@@ -103,15 +104,15 @@ int evaluate_t(dem_ctx* ctx, const void* pos, const void* quat, bool pos_is_doub
         if constexpr (std::is_same<real, float>::value) {
             if (search) {
                 // a3 (relative poses, reach test, compaction) runs as its own kernel in front of the search kernel
-                a.pose = ctx->pose.as<f4>() + 6 * list_base[c];
-                a.pidx = ctx->pidx.as<int>() + list_base[c];
+                a.pose = ctx->pose.as<f4>() + 3 * list_base[c];
+                a.pidx = ctx->pidx.as<int4>() + list_base[c];
                 a.plane = list_cap(c);
                 a.count = ccount + c;
                 PoseArgs pa;
                 pa.pairs = a.pairs; pa.npairs = np; pa.slices = a.slices; pa.pos = pos; pa.quat = quat; pa.box = bx;
                 pa.reach2 = a.reach2;
-                pa.pose = ctx->pose.as<f4>() + 6 * list_base[c];
-                pa.pidx = ctx->pidx.as<int>() + list_base[c];
+                pa.pose = ctx->pose.as<f4>() + 3 * list_base[c];
+                pa.pidx = ctx->pidx.as<int4>() + list_base[c];
                 pa.count = ccount + c;
                 pa.plane = list_cap(c);
                 pa.pad = cull ? 64 : 32;  // a warp of k_pair_cull takes 64 entries, of k_pair_fast 32

@@ -443,13 +443,40 @@ __device__ __forceinline__ void sweep_faces(const ShapeView<float>& S, const Sha
     }
 }
 
+// R_i (rounded once from FP64, as pair_pose does) and the minimum-image separation d of a pair, for the few pairs that
+// contribute: the pose records hold only R and t (48 bytes per pair), and a contributing pair fetches its two particles
+// again instead of every pair carrying another 48 bytes through k_pose.  The arithmetic is that of k_pose, bit for bit.
+static __device__ __forceinline__ void pose_tail(const void* pos, const void* quat, int pos_double, const BoxDev box, int2 ij,
+                                              float* Mi, float* dout) {
+    d4 xi, xj, qi;
+    if (pos_double) {
+        xi = load4d(static_cast<const double*>(pos), ij.x);
+        xj = load4d(static_cast<const double*>(pos), ij.y);
+        qi = load4d(static_cast<const double*>(quat), ij.x);
+    } else {
+        xi = load4d(static_cast<const float*>(pos), ij.x);
+        xj = load4d(static_cast<const float*>(pos), ij.y);
+        qi = load4d(static_cast<const float*>(quat), ij.x);
+    }
+    double d[3] = {xj.x - xi.x, xj.y - xi.y, box.dim == 3 ? xj.z - xi.z : 0.0};
+    d[0] -= box.L[0] * rint(d[0] * box.invL[0]);
+    d[1] -= box.L[1] * rint(d[1] * box.invL[1]);
+    if (box.dim == 3) d[2] -= box.L[2] * rint(d[2] * box.invL[2]);
+    double Di[9];
+    quat_to_mat<double>(qi.x, qi.y, qi.z, qi.w, Di);
+#pragma unroll
+    for (int k = 0; k < 9; ++k) Mi[k] = (float)Di[k];
+    dout[0] = (float)d[0]; dout[1] = (float)d[1]; dout[2] = (float)d[2];
+}
+
 // ---- a3: relative pose of every pair of a class, compacted -----------------------------------------------------------
 // One thread per unique pair: minimum-image separation d, exact reach test (R10), relative pose R = R_i^T R_j,
 // t = R_i^T d and R_i in FP64, rounded once to float.  Pairs inside the reach are compacted into the
 // class's work list (block slices padded to whole warps: see below); pairs beyond it get their result-record flag cleared
 // here (nothing is written for them, the reduction skips them) and never reach the search kernel, so its warps carry 32
-// live pairs each.  Pose record, plane-major for coalesced loads: [6][npairs] float4 =
-// (R0 R1 R2 R3) (R4 R5 R6 R7) (R8 t0 t1 t2) (M0 M1 M2 M3) (M4 M5 M6 M7) (M8 dx dy dz); pidx[c] = the pair's index.
+// live pairs each.  Pose record, plane-major for coalesced loads: [3][npairs] float4 =
+// (R0 R1 R2 R3) (R4 R5 R6 R7) (R8 t0 t1 t2); pidx[c] = the pair's index.  (R_i and d, which only a contributing pair
+// needs, are recomputed by that pair: pose_tail.)
 template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THREADS) k_pose(const PoseArgs a) {
     __shared__ int wcount[DEM_POSE_THREADS / 32], s_prefix;
     if (a.skip && *a.skip) return;  // the work-list count stays 0: the search kernel behind finds no tile
@@ -459,8 +486,9 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THR
     double d[3] = {0.0, 0.0, 0.0};
     d4 qi, qj;
     qi.x = qj.x = 1.0; qi.y = qi.z = qi.w = qj.y = qj.z = qj.w = 0.0;
+    int2 ij = make_int2(0, 0);
     if (p < a.npairs) {
-        const int2 ij = a.pairs[p];
+        ij = a.pairs[p];
         const d4 xi = load4d(static_cast<const PosT*>(a.pos), ij.x), xj = load4d(static_cast<const PosT*>(a.pos), ij.y);
         qi = load4d(static_cast<const PosT*>(a.quat), ij.x);
         qj = load4d(static_cast<const PosT*>(a.quat), ij.y);
@@ -494,7 +522,7 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THR
         for (int sl = 0; sl < a.slices; ++sl) a.rflag[(size_t)p * a.slices + sl] = 0;
     }
     __syncthreads();
-    if ((int)threadIdx.x < tot_pad - tot) a.pidx[s_prefix + tot + threadIdx.x] = -1;
+    if ((int)threadIdx.x < tot_pad - tot) a.pidx[s_prefix + tot + threadIdx.x] = make_int4(-1, 0, 0, 0);
     if (valid) {
         int wb = s_prefix;
         for (int k = 0; k < warp; ++k) wb += wcount[k];
@@ -505,10 +533,7 @@ template <typename PosT, int DIM> __global__ void __launch_bounds__(DEM_POSE_THR
         v.x = R[0]; v.y = R[1]; v.z = R[2]; v.w = R[3]; a.pose[c] = v;
         v.x = R[4]; v.y = R[5]; v.z = R[6]; v.w = R[7]; a.pose[n + c] = v;
         v.x = R[8]; v.y = t[0]; v.z = t[1]; v.w = t[2]; a.pose[2 * n + c] = v;
-        v.x = Mi[0]; v.y = Mi[1]; v.z = Mi[2]; v.w = Mi[3]; a.pose[3 * n + c] = v;
-        v.x = Mi[4]; v.y = Mi[5]; v.z = Mi[6]; v.w = Mi[7]; a.pose[4 * n + c] = v;
-        v.x = Mi[8]; v.y = (float)d[0]; v.z = (float)d[1]; v.w = (float)d[2]; a.pose[5 * n + c] = v;
-        a.pidx[c] = p;
+        a.pidx[c] = make_int4(p, ij.x, ij.y, 0);
     }
 }
 
@@ -538,8 +563,9 @@ template <typename PosT> __global__ void __launch_bounds__(DEM_POSE_THREADS) k_p
     double d[3] = {0.0, 0.0, 0.0};
     d4 qi, qj;
     qi.x = qj.x = 1.0; qi.y = qi.z = qi.w = qj.y = qj.z = qj.w = 0.0;
+    int2 ij = make_int2(0, 0);
     if (p < a.npairs) {
-        const int2 ij = a.pairs[p];
+        ij = a.pairs[p];
         const d4 xi = load4d(static_cast<const PosT*>(a.pos), ij.x), xj = load4d(static_cast<const PosT*>(a.pos), ij.y);
         qi = load4d(static_cast<const PosT*>(a.quat), ij.x);
         qj = load4d(static_cast<const PosT*>(a.quat), ij.y);
@@ -612,7 +638,7 @@ template <typename PosT> __global__ void __launch_bounds__(DEM_POSE_THREADS) k_p
         if (lane == 0 && mv) atomicAdd(a.counters, (unsigned long long)__popc(mv));
     }
     __syncthreads();
-    if ((int)threadIdx.x < tot_pad - tot) a.pidx[s_prefix + tot + threadIdx.x] = -1;
+    if ((int)threadIdx.x < tot_pad - tot) a.pidx[s_prefix + tot + threadIdx.x] = make_int4(-1, 0, 0, 0);
     if (keep) {
         int wb = s_prefix;
         for (int k = 0; k < warp; ++k) wb += wcount[k];
@@ -623,10 +649,7 @@ template <typename PosT> __global__ void __launch_bounds__(DEM_POSE_THREADS) k_p
         v.x = R[0]; v.y = R[1]; v.z = R[2]; v.w = R[3]; a.pose[c] = v;
         v.x = R[4]; v.y = R[5]; v.z = R[6]; v.w = R[7]; a.pose[n + c] = v;
         v.x = R[8]; v.y = t[0]; v.z = t[1]; v.w = t[2]; a.pose[2 * n + c] = v;
-        v.x = Mi[0]; v.y = Mi[1]; v.z = Mi[2]; v.w = Mi[3]; a.pose[3 * n + c] = v;
-        v.x = Mi[4]; v.y = Mi[5]; v.z = Mi[6]; v.w = Mi[7]; a.pose[4 * n + c] = v;
-        v.x = Mi[8]; v.y = (float)d[0]; v.z = (float)d[1]; v.w = (float)d[2]; a.pose[5 * n + c] = v;
-        a.pidx[c] = p;
+        a.pidx[c] = make_int4(p, ij.x, ij.y, 0);
 #pragma unroll
         for (int w = 0; w < DEM_CM_WORDS; ++w)
             if (w < a.mw_e + a.mw_vj + a.mw_vi) a.cmask[(size_t)w * n + c] = cm[w];
@@ -644,7 +667,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
     float* sacc_all = reinterpret_cast<float*>(queue + 4 * DEM_QCAP);  // 4 warps x 7 x 32
     unsigned* scnt_all = reinterpret_cast<unsigned*>(sacc_all + 4 * 7 * 32);  // 4 warps x 4
     f4* stage_pose = reinterpret_cast<f4*>(scnt_all + 16);                 // 4 warps x [2][3][32] float4 (R, t)
-    int* stage_pidx = reinterpret_cast<int*>(stage_pose + 4 * 2 * 3 * 32);  // 4 warps x [2][32]
+    int4* stage_pidx = reinterpret_cast<int4*>(stage_pose + 4 * 2 * 3 * 32);  // 4 warps x [2][32] (pair, i, j, 0)
     f4* sm = reinterpret_cast<f4*>(stage_pidx + 4 * 2 * 32);
     static_assert(sizeof(FastShared) <= 256, "FastShared header");
     // stage the shape-feature tables of the class (a1) into shared memory
@@ -706,7 +729,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
     // being swept; each lane copies and later reads only its own records.
     const int wt_stride = (int)gridDim.x * 4;
     f4* spose = stage_pose + warp * (2 * 3 * 32);   // [2][3][32]
-    int* spidx = stage_pidx + warp * (2 * 32);      // [2][32]
+    int4* spidx = stage_pidx + warp * (2 * 32);     // [2][32]
     // tile -> (slice, first entry of the work list): no division for unsliced classes
     auto locate = [&](int wt_, int& slice_, int& c0_) {
         slice_ = a.slices == 1 ? 0 : wt_ / tps;
@@ -721,7 +744,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
                 for (int k = 0; k < 3; ++k)  // R and t; R_i and d (planes 3-5) are fetched only by pairs that contribute
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
                                      spose + (buf * 3 + k) * 32 + lane)), "l"(a.pose + k * plane + c_));
-                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
                                  spidx + buf * 32 + lane)), "l"(a.pidx + c_));
             }
         }
@@ -751,7 +774,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
         __syncwarp();  // the cooperative evaluation reads other lanes' staged poses
         w.sp = spose + buf * 3 * 32;
         w.touched = 0u;
-        const bool valid = in_list && spidx[buf * 32 + lane] >= 0;  // the work list is padded to whole warps per k_pose block
+        const bool valid = in_list && spidx[buf * 32 + lane].x >= 0;  // the work list is padded to whole warps per k_pose block
         if (!__any_sync(full, valid)) continue;                    // a tile of padding only
         float R[9], t[3];
         if (valid) {
@@ -923,7 +946,8 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
             if (valid) {
                 // a pair none of whose terms is inside the cutoff contributes nothing: its record flag is cleared and
                 // no record is written (the reduction skips it)
-                const int pi = spidx[buf * 32 + lane];
+                const int4 pe = spidx[buf * 32 + lane];
+                const int pi = pe.x;
                 DEM_ASSERT(pi < a.npairs && slice < a.slices);
                 const size_t ri = (size_t)pi * a.slices + slice;
                 a.rflag[ri] = (unsigned char)(w.touched & 1u);
@@ -934,17 +958,15 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
                         F[k] = w.sacc[k * 32 + lane];
                         T[k] = w.sacc[(3 + k) * 32 + lane];
                     }
-                    const int c_ = c;
-                    const f4 p3 = a.pose[3 * plane + c_], p4 = a.pose[4 * plane + c_],
-                             p5 = a.pose[5 * plane + c_];
-                    const float Mi[9] = {p3.x, p3.y, p3.z, p3.w, p4.x, p4.y, p4.z, p4.w, p5.x};
+                    float Mi[9], dl[3];
+                    pose_tail(a.pos, a.quat, a.pos_double, a.box, make_int2(pe.y, pe.z), Mi, dl);
                     float out[10];
                     pair_finish<float>(Mi, t, F, T, w.sacc[6 * 32 + lane], out);
                     f4* rec = a.rec + DEM_REC * ri;
                     f4 r0, r1, r2;
                     r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
-                    r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = p5.y;
-                    r2.x = p5.z; r2.y = p5.w; r2.z = r2.w = 0.f;
+                    r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = dl[0];
+                    r2.x = dl[1]; r2.y = dl[2]; r2.z = r2.w = 0.f;
                     rec[0] = r0; rec[1] = r1; rec[2] = r2;
                 }
             }
@@ -976,7 +998,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
 // bytes of dynamic shared memory k_pair_fast needs in front of the staged tables
 static inline size_t fast_smem_header() {
     return 256 + sizeof(unsigned) * 4 * DEM_QCAP + sizeof(float) * 4 * 7 * 32 + sizeof(unsigned) * 16 +
-           sizeof(f4) * 4 * 2 * 3 * 32 + sizeof(int) * 4 * 2 * 32;
+           sizeof(f4) * 4 * 2 * 3 * 32 + sizeof(int4) * 4 * 2 * 32;
 }
 
 // ---- the kernel with exact per-feature culling (3D) ----------------------------------------------------------------------
@@ -1205,7 +1227,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     float* sacc_all = reinterpret_cast<float*>(queue + 4 * DEM_QCAP);      // 4 warps x 7 x 64
     unsigned* scnt_all = reinterpret_cast<unsigned*>(sacc_all + 4 * 7 * 64);  // 4 warps x 4
     f4* stage_pose = reinterpret_cast<f4*>(scnt_all + 16);                 // 4 warps x [3][64] float4 (R, t)
-    int* stage_pidx = reinterpret_cast<int*>(stage_pose + 4 * 3 * 64);      // 4 warps x [64]
+    int4* stage_pidx = reinterpret_cast<int4*>(stage_pose + 4 * 3 * 64);    // 4 warps x [64] (pair, i, j, 0)
     unsigned* items = reinterpret_cast<unsigned*>(stage_pidx + 4 * 64);     // 4 warps x DEM_IQCAP
     f4* sm = reinterpret_cast<f4*>(items + 4 * DEM_IQCAP);
     const bool same = SAME;
@@ -1217,7 +1239,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
     const int count = *a.count;  // a multiple of 64 (k_pose pads its block slices)
     const size_t plane = a.plane;
     f4* spose = stage_pose + warp * (3 * 64);
-    int* spidx = stage_pidx + warp * 64;
+    int4* spidx = stage_pidx + warp * 64;
     unsigned pm_e[2] = {0u, 0u}, pm_vj[2] = {0u, 0u}, pm_vi[2] = {0u, 0u};
     auto stage_tile = [&](int cbase_) {
 #pragma unroll
@@ -1227,7 +1249,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
             for (int k = 0; k < 3; ++k)  // R and t; R_i and d (planes 3-5) are fetched only by pairs that contribute
                 asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
                                  spose + k * 64 + own)), "l"(a.pose + k * plane + c_));
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(spidx + own)),
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(spidx + own)),
                          "l"(a.pidx + c_));
         }
         asm volatile("cp.async.commit_group;");
@@ -1287,8 +1309,8 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncwarp();
         bool valid[2];
-        valid[0] = spidx[lane] >= 0;  // the work list is padded to whole tiles per k_pose block (pidx = -1)
-        valid[1] = spidx[lane + 32] >= 0;
+        valid[0] = spidx[lane].x >= 0;  // the work list is padded to whole tiles per k_pose block (pidx = -1)
+        valid[1] = spidx[lane + 32].x >= 0;
         if (!__any_sync(full, valid[0] || valid[1])) continue;
         w.touched = 0u;
 #pragma unroll
@@ -1533,8 +1555,8 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
         for (int h = 0; h < 2; ++h) {
             if (!valid[h]) continue;
             const int own = lane + 32 * h;
-            DEM_ASSERT(spidx[own] < a.npairs && slice < a.slices);
-            const size_t ri = (size_t)spidx[own] * a.slices + slice;
+            DEM_ASSERT(spidx[own].x < a.npairs && slice < a.slices);
+            const size_t ri = (size_t)spidx[own].x * a.slices + slice;
             const bool hit = (w.touched >> h) & 1u;
             a.rflag[ri] = (unsigned char)hit;  // no contribution: no record is written, the reduction skips the pair
             if (!hit) continue;
@@ -1544,16 +1566,15 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
                 F[k] = w.sacc[k * 64 + own];
                 T[k] = w.sacc[(3 + k) * 64 + own];
             }
-            const int c_ = cbase + own;
-            const f4 p3 = a.pose[3 * plane + c_], p4 = a.pose[4 * plane + c_], p5 = a.pose[5 * plane + c_];
-            const float Mi[9] = {p3.x, p3.y, p3.z, p3.w, p4.x, p4.y, p4.z, p4.w, p5.x};
+            float Mi[9], dl[3];
+            pose_tail(a.pos, a.quat, a.pos_double, a.box, make_int2(spidx[own].y, spidx[own].z), Mi, dl);
             float out[10];
             pair_finish<float>(Mi, tq[h], F, T, w.sacc[6 * 64 + own], out);
             f4* rec = a.rec + DEM_REC * ri;
             f4 r0, r1, r2;
             r0.x = out[0]; r0.y = out[1]; r0.z = out[2]; r0.w = out[9];
-            r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = p5.y;
-            r2.x = p5.z; r2.y = p5.w; r2.z = r2.w = 0.f;
+            r1.x = out[3]; r1.y = out[4]; r1.z = out[5]; r1.w = dl[0];
+            r2.x = dl[1]; r2.y = dl[2]; r2.z = r2.w = 0.f;
             rec[0] = r0; rec[1] = r1; rec[2] = r2;
         }
     }
@@ -1579,7 +1600,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
 // bytes of dynamic shared memory k_pair_cull needs in front of the staged tables
 static inline size_t cull_smem_header() {
     return 256 + sizeof(unsigned) * 4 * DEM_QCAP + sizeof(float) * 4 * 7 * 64 + sizeof(unsigned) * 16 +
-           sizeof(f4) * 4 * 3 * 64 + sizeof(int) * 4 * 64 + sizeof(unsigned) * 4 * DEM_IQCAP;
+           sizeof(f4) * 4 * 3 * 64 + sizeof(int4) * 4 * 64 + sizeof(unsigned) * 4 * DEM_IQCAP;
 }
 
 }  // namespace dem

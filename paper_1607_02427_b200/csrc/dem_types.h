@@ -88,13 +88,14 @@ template <typename real> struct PairArgs {
                           //   (pair, slice) contributes nothing and its record was NOT written (the reduction skips it)
     const void* pos;
     const void* quat;
+    int pos_double;       // pos / quat are double[N][4] (else float[N][4])
     BoxDev box;
     double reach2;        // (R_a + R_b + 2^(1/6) sigma)^2 : beyond it no term can be inside the cutoff (exact, R10)
     PairConst<real> pc;
     real rc2_search;      // FP32 search kernel: squared candidate cutoff (WCA cutoff + slack, dem_fast.cuh)
     real cull_a2, cull_b2;  // culling kernel: (R_first + rc_search)^2, (R_second + rc_search)^2 (circumradii)
     const f4* pose;       // FP32 search kernel: this class's compacted pose records, pair indices and their number
-    const int* pidx;      //   (written by k_pose)
+    const int4* pidx;     //   (written by k_pose: pair index, its two particles, 0)
     const int* count;
     int* tile;            //   next tile to take (zero at launch), or null: tiles are dealt out by block and warp index
     size_t plane;         //   stride of the pose planes
@@ -113,7 +114,7 @@ struct PoseArgs {
     BoxDev box;
     double reach2;
     f4* pose;
-    int* pidx;
+    int4* pidx;  // (pair index or -1 for padding, first particle, second particle, 0)
     int* count;  // entries of this class's work list, padding included (zeroed before the launch)
     size_t plane;  // stride of the pose planes = capacity of the work list (pairs + 64 per k_pose block)
     int pad;       // entries per warp tile of the kernel that follows: 32 (k_pair_fast) or 64 (k_pair_cull)
