@@ -105,6 +105,11 @@ struct dem_ctx {
     int64_t last_terms = 0;
     int sm_count = 148;
     int* h_moved = nullptr;        // pinned host copy of dem_step's flags (moved, halt, steps completed)
+    // dem_step_host: positions and orientations are final before the last force evaluation of a call, so they travel back
+    // to the host (on copy_stream) while that evaluation runs
+    void* early_host[2] = {nullptr, nullptr};  // host destinations of pos and quat, or null (device-array calls)
+    bool early_done = false;
+    cudaEvent_t ev_early = nullptr;
     cudaStream_t copy_stream = nullptr;  // dem_step_host: second H2D stream (velocities, angular momenta)
     cudaEvent_t ev_copy = nullptr;
     bool ev_copy_pending = false;

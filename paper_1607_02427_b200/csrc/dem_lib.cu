@@ -411,6 +411,22 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
             const int out = pingpong && fa.mode == 2 ? c ^ 1 : c;
             fa.pos = xs[out];
             fa.quat = qs[out];
+            if (last && !th && ctx->early_host[0] && ctx->copy_stream) {
+                // the state this evaluation reads is the final one: send x and q on their way now
+                if (!ctx->ev_early) CU(cudaEventCreateWithFlags(&ctx->ev_early, cudaEventDisableTiming));
+                const size_t r4b = conv ? sizeof(f4) : sizeof(d4);
+                if (conv) {
+                    k_d4_to_f4<<<nblk(N, B), B, 0, st>>>(N, xs[c], static_cast<f4*>(pos));
+                    LAUNCHED(ctx);
+                    k_d4_to_f4<<<nblk(N, B), B, 0, st>>>(N, qs[c], static_cast<f4*>(quat));
+                    LAUNCHED(ctx);
+                }
+                CU(cudaEventRecord(ctx->ev_early, st));
+                CU(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_early, 0));
+                CU(cudaMemcpyAsync(ctx->early_host[0], conv ? pos : (void*)xs[c], r4b * N, cudaMemcpyDeviceToHost, ctx->copy_stream));
+                CU(cudaMemcpyAsync(ctx->early_host[1], conv ? quat : (void*)qs[c], r4b * N, cudaMemcpyDeviceToHost, ctx->copy_stream));
+                ctx->early_done = true;
+            }
             CHECK(evaluate(ctx, xs[c], qs[c], true, sid, N, F, T, nullptr, &fa));
             if (out != c) ++swaps;
             c = out;
@@ -442,7 +458,7 @@ template <typename real> int step_t(dem_ctx* ctx, void* pos, void* quat, void* v
     if (conv) {
         void* out[4] = {pos, quat, vel, ang};
         d4* in[4] = {xs[cur], qs[cur], v, L};
-        for (int k = 0; k < 4; ++k) {
+        for (int k = ctx->early_done ? 2 : 0; k < 4; ++k) {  // (x and q may be converted and on their way already)
             k_d4_to_f4<<<nblk(N, B), B, 0, st>>>(N, in[k], static_cast<f4*>(out[k]));
             LAUNCHED(ctx);
         }
@@ -601,7 +617,7 @@ template <typename real> int step_npt_t(dem_ctx* ctx, void* pos, void* quat, voi
     if (conv) {
         void* out[4] = {pos, quat, vel, ang};
         d4* in[4] = {x, q, v, L};
-        for (int k = 0; k < 4; ++k) {
+        for (int k = ctx->early_done ? 2 : 0; k < 4; ++k) {  // (x and q may be converted and on their way already)
             k_d4_to_f4<<<nblk(N, B), B, 0, st>>>(N, in[k], static_cast<f4*>(out[k]));
             LAUNCHED(ctx);
         }
@@ -673,6 +689,7 @@ int dem_destroy(dem_ctx* c) {
     if (c->h_moved) cudaFreeHost(c->h_moved);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->ev_copy) cudaEventDestroy(c->ev_copy);
+    if (c->ev_early) cudaEventDestroy(c->ev_early);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     for (int k = 0; k < 3; ++k) {
         if (c->class_stream[k]) cudaStreamDestroy(c->class_stream[k]);
@@ -915,17 +932,25 @@ int dem_step_host(dem_ctx* ctx, void* pos, void* quat, void* vel, void* angmom, 
     ctx->ev_copy_pending = true;
     CU(ctx->h_force.reserve(r4 * N));
     CU(ctx->h_torque.reserve(r4 * N));
+    ctx->early_host[0] = pos;
+    ctx->early_host[1] = quat;
+    ctx->early_done = false;
     const int rc = dem_step(ctx, ctx->h_pos.p, ctx->h_quat.p, ctx->h_vel.p, ctx->h_ang.p, ctx->h_sid.as<int32_t>(), N,
                             box, dt, nsteps, skin, ctx->h_force.p, ctx->h_torque.p);
+    const bool early = ctx->early_done;
+    ctx->early_host[0] = ctx->early_host[1] = nullptr;
+    ctx->early_done = false;
     if (rc != DEM_OK) {  // the caller's host arrays must not be in use by a copy when an error is returned
         cudaStreamSynchronize(ctx->copy_stream);
         ctx->ev_copy_pending = false;
         return rc;
     }
-    for (int k = 0; k < 4; ++k) CU(cudaMemcpyAsync(host[k], bufs[k]->p, r4 * N, cudaMemcpyDeviceToHost, st));
+    // (positions and orientations were final before the last evaluation: dem_step has sent them on copy_stream already)
+    for (int k = early ? 2 : 0; k < 4; ++k) CU(cudaMemcpyAsync(host[k], bufs[k]->p, r4 * N, cudaMemcpyDeviceToHost, st));
     if (force_energy) CU(cudaMemcpyAsync(force_energy, ctx->h_force.p, r4 * N, cudaMemcpyDeviceToHost, st));
     if (torque) CU(cudaMemcpyAsync(torque, ctx->h_torque.p, r4 * N, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    if (early) CU(cudaStreamSynchronize(ctx->copy_stream));
     return DEM_OK;
 }
 
