@@ -503,6 +503,20 @@ def main():
     e2e_value = aggregate_value(n, world, args.e2e_steps, max_over_ranks(e2e_s, world, "cuda") * 1e3)
     h2d = 4 * n * 16 + n * 4
     d2h = 5 * n * 16
+    # the same calls with the library's default pair kernel (exact culling on), when the headline arm switched it off
+    e2e_default = None
+    if searched and not particle2d and not args.cull:
+        dem.set_culling(True)
+        for _ in range(3):
+            dem.step_host(h["pos"], h["quat"], h["vel"], h["angmom"], hsid, st["box"], dt_step, 1, skin, hf, None)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            dem.step_host(h["pos"], h["quat"], h["vel"], h["angmom"], hsid, st["box"], dt_step, 1, skin, hf, None)
+        barrier()
+        e2e_default = aggregate_value(n, world, args.e2e_steps,
+                                      max_over_ranks(time.perf_counter() - t0, world, "cuda") * 1e3)
+        dem.set_culling(False)
 
     # ---- oracle on the host cores (rank 0, N = 1 only) ---------------------------------------------------------------
     cpu_baseline = None
@@ -532,7 +546,9 @@ def main():
             "roofline": roofline, "culled": culled, "every_term": every_term, "thermalised": thermal, "breakdown": detail,
             "cpu_baseline": cpu_baseline,
             "e2e": {"value": e2e_value, "unit": "particle-timesteps/s", "h2d_bytes_per_step": h2d,
-                    "d2h_bytes_per_step": d2h, "steps": args.e2e_steps},
+                    "d2h_bytes_per_step": d2h, "steps": args.e2e_steps,
+                    "pair_kernel": "as the headline arm (%s)" % ("culling on" if (args.cull or particle2d) else "every term swept"),
+                    "value_library_default": e2e_default},
             "gpu_launches": gpu_launches, "clocks": clocks,
             # the 160 MiB memset that flushes the L2 is inside every timed step above (value, culled, thermalised);
             # its own device time per step, from the breakdown pass, is given here for the reader, never subtracted
