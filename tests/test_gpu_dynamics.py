@@ -202,23 +202,27 @@ def test_parallel_edge_rule_energy_cost(pkg):
     assert worst < 2e-3, worst
 
 
-@pytest.mark.parametrize("precision,nsteps", [("f32", 20), ("f64", 20), ("f32", 1), ("f64", 1)])
-def test_step_host_matches_device(pkg, precision, nsteps):
+@pytest.mark.parametrize("precision,nsteps,skin", [("f32", 20, 0.3), ("f64", 20, 0.3), ("f32", 1, 0.3), ("f64", 1, 0.3),
+                                                   ("f32", 150, 0.01)])
+def test_step_host_matches_device(pkg, precision, nsteps, skin):
     """dem_step_host (positions and orientations travel back while the last evaluation still runs) against dem_step on
-    device arrays: the same bits, in both precisions, for one step and for many."""
+    device arrays: the same bits, in both precisions, for one step and for many, and with a skin so thin that the list
+    goes stale every few steps (also right before the last evaluation)."""
     import torch
 
     st = round_state(di.dense_state("cubes", 4), precision)
-    dev = _run(pkg, st, precision, 1e-3, nsteps, skin=0.3)
+    dev = _run(pkg, st, precision, 1e-3, nsteps, skin=skin)
     dem, _ = pkg.from_state(st, precision)
     dt_ = torch.float32 if precision == "f32" else torch.float64
     h = {k: torch.tensor(st[k], dtype=dt_).pin_memory() for k in ("pos", "quat", "vel", "angmom")}
     sid = torch.tensor(st["shape_id"], dtype=torch.int32).pin_memory()
     hf = torch.empty((st["N"], 4), dtype=dt_).pin_memory()
-    dem.step_host(h["pos"], h["quat"], h["vel"], h["angmom"], sid, st["box"], 1e-3, nsteps, 0.3, hf, None)
+    dem.step_host(h["pos"], h["quat"], h["vel"], h["angmom"], sid, st["box"], 1e-3, nsteps, skin, hf, None)
     for k in ("pos", "quat", "vel", "angmom"):
         assert np.array_equal(h[k].numpy().astype(np.float64), dev[k]), k
     assert np.array_equal(hf.numpy().astype(np.float64), dev["force"])
+    if skin < 0.1:
+        assert dev["launches"] > 4 * nsteps   # the device run did rebuild its list many times
     dem.close()
 
 
