@@ -83,7 +83,7 @@ __device__ __forceinline__ unsigned q_entry(int owner, int phase, int outer, int
 // ---- evaluate: up to 32 queued candidates, one per lane -----------------------------------------------------------------
 // q: this warp's queue (qn entries, the first cnt <= 32 are consumed and the rest moved to the front); sacc: this warp's
 // per-lane accumulators [7][32] = (F.xyz, T.xyz, u) in the owner's body frame; scnt: this warp's counters (active,
-// degenerate, parallel).  sp: the warp's staged pose records [6][32] (plane-major, indexed by owner lane); the
+// degenerate, parallel).  sp: the warp's staged pose records [3][nown] (plane-major, indexed by owner lane); the
 // evaluating lane reads its owner's pose from there.
 // Contributions are added to the owner in queue order, so the result does not depend on scheduling.  Returns, per lane,
 // which of its owner slots received a contribution (only those pairs get a result record).
@@ -741,7 +741,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_fast(const PairArgs<float> a
             DEM_ASSERT(c_ >= 0 && (size_t)count <= plane);
             if (c_ < count) {
 #pragma unroll
-                for (int k = 0; k < 3; ++k)  // R and t; R_i and d (planes 3-5) are fetched only by pairs that contribute
+                for (int k = 0; k < 3; ++k)  // R and t (R_i and d: pose_tail)
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
                                      spose + (buf * 3 + k) * 32 + lane)), "l"(a.pose + k * plane + c_));
                 asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
@@ -1246,7 +1246,7 @@ __global__ void __launch_bounds__(128, MINB) k_pair_cull(const PairArgs<float> a
         for (int h = 0; h < 2; ++h) {
             const int own = lane + 32 * h, c_ = cbase_ + own;
 #pragma unroll
-            for (int k = 0; k < 3; ++k)  // R and t; R_i and d (planes 3-5) are fetched only by pairs that contribute
+            for (int k = 0; k < 3; ++k)  // R and t (R_i and d: pose_tail)
                 asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(
                                  spose + k * 64 + own)), "l"(a.pose + k * plane + c_));
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(spidx + own)),
